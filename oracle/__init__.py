@@ -1,0 +1,186 @@
+"""ctypes binding of the CPU oracle (oracle/oracle.c).
+
+TEST INFRASTRUCTURE ONLY: imported by tests/, ``__graft_entry__.smoke()`` and the
+``cpu_baseline`` / ``--impl reference`` legs of bench.py.  Nothing under
+``paper_2107_05395_b200/`` imports this package and this package imports nothing from it.
+
+All routines are fp64 and take / return numpy arrays.  The pentadiagonal routines use the
+paper's diagonal names: a = 2nd sub-diagonal, b = sub-diagonal, c = main,
+d = super-diagonal, e = 2nd super-diagonal.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import subprocess
+from dataclasses import dataclass
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "oracle.c")
+_LIB = os.path.join(_HERE, "liboracle.so")
+
+_lib = None
+
+
+def build(force: bool = False) -> str:
+    """Compile oracle.c with gcc (-O2, FMA contraction off, OpenMP over systems)."""
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        tmp = _LIB + f".tmp{os.getpid()}"
+        cmd = ["gcc", "-std=c99", "-O2", "-ffp-contract=off", "-fopenmp", "-fPIC", "-shared",
+               "-fvisibility=hidden", "-Wall", "-Wextra", "-o", tmp, _SRC, "-lm"]
+        subprocess.run(cmd, check=True)
+        os.replace(tmp, _LIB)
+    return _LIB
+
+
+_dp = ctypes.POINTER(ctypes.c_double)
+_ll = ctypes.c_longlong
+
+
+def _load():
+    global _lib
+    if _lib is None:
+        lib = ctypes.CDLL(build())
+        lib.orc_tri_factor.argtypes = [ctypes.c_int, _dp, _dp, _dp]
+        lib.orc_tri_factor.restype = ctypes.c_int
+        lib.orc_tri_solve.argtypes = [ctypes.c_int, _dp, _dp, _dp, _dp]
+        lib.orc_tri_solve.restype = None
+        for name in ("orc_penta_factor", "orc_penta_factor_general"):
+            fn = getattr(lib, name)
+            fn.argtypes = [ctypes.c_int, _dp, _dp, _dp, _dp, _dp]
+            fn.restype = ctypes.c_int
+        lib.orc_penta_solve.argtypes = [ctypes.c_int, _dp, _dp, _dp, _dp, _dp, _dp]
+        lib.orc_penta_solve.restype = None
+        lib.orc_ch_rhs.argtypes = [ctypes.c_int, _dp, ctypes.c_double, _dp]
+        lib.orc_ch_rhs.restype = None
+        lib.orc_tri_solve_interleaved.argtypes = [ctypes.c_int, _dp, _dp, _dp, _dp, _ll, _ll, _ll,
+                                                  _ll, ctypes.c_int, ctypes.c_int]
+        lib.orc_tri_solve_interleaved.restype = ctypes.c_int
+        lib.orc_penta_solve_interleaved.argtypes = [ctypes.c_int, _dp, _dp, _dp, _dp, _dp, _dp, _ll,
+                                                    _ll, _ll, _ll, ctypes.c_int, ctypes.c_int]
+        lib.orc_penta_solve_interleaved.restype = ctypes.c_int
+        lib.orc_ch_step_interleaved.argtypes = [ctypes.c_int, _dp, _dp, _dp, _dp, _dp, _dp, _ll,
+                                                _ll, _ll, _ll, ctypes.c_double, ctypes.c_int,
+                                                ctypes.c_int]
+        lib.orc_ch_step_interleaved.restype = ctypes.c_int
+        _lib = lib
+    return _lib
+
+
+def _p(x: np.ndarray):
+    assert x.dtype == np.float64 and x.flags["C_CONTIGUOUS"]
+    return x.ctypes.data_as(_dp)
+
+
+def _f64(x) -> np.ndarray:
+    return np.ascontiguousarray(np.array(x, dtype=np.float64, copy=True))
+
+
+class FactorError(ArithmeticError):
+    """Zero / non-finite pivot; ``row`` is the 1-based row (the paper has no pivoting)."""
+
+    def __init__(self, row: int):
+        super().__init__(f"zero or non-finite pivot at row {row}")
+        self.row = row
+
+
+@dataclass
+class TriFactor:
+    n: int
+    a: np.ndarray   # untouched sub-diagonal
+    bh: np.ndarray  # b^  (eq. 2)
+    ch: np.ndarray  # c^  (eq. 1-2)
+
+
+@dataclass
+class PentaFactor:
+    n: int
+    eps: np.ndarray    # = a            (step 14)
+    beta: np.ndarray   # overwrote b
+    alpha: np.ndarray  # overwrote c
+    gamma: np.ndarray  # overwrote d
+    delta: np.ndarray  # overwrote e
+
+
+def tri_factor(a, b, c) -> TriFactor:
+    a, b, c = _f64(a), _f64(b), _f64(c)
+    n = b.size
+    assert a.size == n and c.size == n
+    rc = _load().orc_tri_factor(n, _p(a), _p(b), _p(c))
+    if rc:
+        raise FactorError(rc)
+    return TriFactor(n, a, b, c)
+
+
+def tri_solve(fac: TriFactor, d) -> np.ndarray:
+    """One contiguous system (length n); returns x."""
+    x = _f64(d)
+    assert x.shape == (fac.n,)
+    _load().orc_tri_solve(fac.n, _p(fac.a), _p(fac.bh), _p(fac.ch), _p(x))
+    return x
+
+
+def penta_factor(a, b, c, d, e, general: bool = False) -> PentaFactor:
+    a, b, c, d, e = (_f64(v) for v in (a, b, c, d, e))
+    n = c.size
+    assert all(v.size == n for v in (a, b, d, e))
+    fn = _load().orc_penta_factor_general if general else _load().orc_penta_factor
+    rc = fn(n, _p(a), _p(b), _p(c), _p(d), _p(e))
+    if rc:
+        raise FactorError(rc)
+    return PentaFactor(n, a, b, c, d, e)
+
+
+def penta_solve(fac: PentaFactor, f) -> np.ndarray:
+    x = _f64(f)
+    assert x.shape == (fac.n,)
+    _load().orc_penta_solve(fac.n, _p(fac.eps), _p(fac.beta), _p(fac.alpha), _p(fac.gamma),
+                            _p(fac.delta), _p(x))
+    return x
+
+
+def ch_rhs(c, alpha: float) -> np.ndarray:
+    c = _f64(c)
+    f = np.empty_like(c)
+    _load().orc_ch_rhs(c.size, _p(c), float(alpha), _p(f))
+    return f
+
+
+def _subset(M, subset):
+    jlo, jhi, jstride = (0, M, 1) if subset is None else subset
+    assert 0 <= jlo <= jhi <= M and jstride >= 1
+    return jlo, jhi, jstride
+
+
+def tri_solve_interleaved(fac: TriFactor, rhs: np.ndarray, nsteps: int = 1, subset=None,
+                          nthreads: int = 0) -> int:
+    """In place on ``rhs`` of shape (n, M) (element i of system j at rhs[i, j]).
+    ``subset=(jlo, jhi, jstride)`` restricts the systems touched.  Returns threads used."""
+    assert rhs.ndim == 2 and rhs.shape[0] == fac.n
+    M = rhs.shape[1]
+    jlo, jhi, js = _subset(M, subset)
+    return _load().orc_tri_solve_interleaved(fac.n, _p(fac.a), _p(fac.bh), _p(fac.ch), _p(rhs), M,
+                                             jlo, jhi, js, nsteps, nthreads)
+
+
+def penta_solve_interleaved(fac: PentaFactor, rhs: np.ndarray, nsteps: int = 1, subset=None,
+                            nthreads: int = 0) -> int:
+    assert rhs.ndim == 2 and rhs.shape[0] == fac.n
+    M = rhs.shape[1]
+    jlo, jhi, js = _subset(M, subset)
+    return _load().orc_penta_solve_interleaved(fac.n, _p(fac.eps), _p(fac.beta), _p(fac.alpha),
+                                               _p(fac.gamma), _p(fac.delta), _p(rhs), M, jlo, jhi,
+                                               js, nsteps, nthreads)
+
+
+def ch_step_interleaved(fac: PentaFactor, c: np.ndarray, alpha: float, nsteps: int = 1,
+                        subset=None, nthreads: int = 0) -> int:
+    """Config-5 stepper: nsteps x [f = c + alpha*D2(c^3-c); c = (I+sigma*D4)^-1 f], in place."""
+    assert c.ndim == 2 and c.shape[0] == fac.n
+    M = c.shape[1]
+    jlo, jhi, js = _subset(M, subset)
+    return _load().orc_ch_step_interleaved(fac.n, _p(fac.eps), _p(fac.beta), _p(fac.alpha),
+                                           _p(fac.gamma), _p(fac.delta), _p(c), M, jlo, jhi, js,
+                                           float(alpha), nsteps, nthreads)

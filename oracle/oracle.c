@@ -1,0 +1,269 @@
+/*
+ * oracle.c -- plain, slow, obviously-correct CPU reference ("the oracle") for the
+ * shared-LHS batched tridiagonal / pentadiagonal solves and the semi-implicit
+ * Cahn-Hilliard step of arxiv/paper_2107_05395.
+ *
+ * THIS IS TEST INFRASTRUCTURE, NOT PRODUCT CODE.  Only tests/, __graft_entry__.smoke()
+ * and bench.py's cpu_baseline / --impl reference legs may build, load or call it.
+ * It shares no code, header, table or helper with the CUDA library under
+ * paper_2107_05395_b200/csrc/, and neither side includes or imports the other.
+ *
+ * Everything is fp64, one system at a time, written in the paper's own order and
+ * notation (divisions kept, compiled with -ffp-contract=off so no FMA is formed):
+ *
+ *   orc_tri_factor      PAPER.md:87-93  (eq. 1-2),  555-566 (Alg. 1)
+ *   orc_tri_solve       PAPER.md:95-108 (eq. 3-6),  568-597 (Alg. 2)
+ *   orc_penta_factor    PAPER.md:219-256 (Sec. 4.1 steps 1-14), 601-637 (Alg. 3)
+ *   orc_penta_solve     PAPER.md:258-278 (Sec. 4.1), 639-676 (Alg. 4)
+ *   orc_ch_rhs          PAPER.md:365-392 (eq. 24, 25a, 26c)
+ *   *_interleaved       PAPER.md:69 (Sec. 2), Alg. 2 "rowID +- M": element i of
+ *                       system j lives at rhs[i*M + j]
+ *
+ * Readings of garbled / silent passages follow SURVEY.md 8(c) and are listed in
+ * DESIGN.md ("Readings"); each is marked [C-n] below.
+ *
+ * Parity pins (tests/test_oracle_*.py, all run without a GPU): exact rational Gaussian
+ * elimination on tiny systems, numpy dense solves, residuals, the closed-form
+ * eigenpairs of Toeplitz tri / penta (I + r T^2) matrices, exact modal decay over 100
+ * steps, L*R == A rebuilt densely, reductions (penta with zero outer bands == tri;
+ * tri with zero off-diagonals == scaling), a dense restatement of eq. 24 for the CH
+ * step and its discrete mass-balance identity.  No function here is "parity unpinned".
+ */
+#include <math.h>
+#include <stddef.h>
+#include <stdlib.h>
+#include <string.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+#define ORC_API __attribute__((visibility("default")))
+
+/* ------------------------------------------------------------------------------------
+ * Tridiagonal.  Row i (1-based, paper): a_i x_{i-1} + b_i x_i + c_i x_{i+1} = d_i.
+ * Arrays are 0-based here: a[i-1] holds a_i.  a[0] and c[n-1] are never read.
+ * ---------------------------------------------------------------------------------- */
+
+/* Alg. 1: overwrites b with b^, c with c^; a untouched.
+ * Returns 0, or the 1-based row whose pivot b^_i is zero / non-finite [C-14]. */
+ORC_API int orc_tri_factor(int n, const double *a, double *b, double *c)
+{
+    if (n < 1) return -1;
+    if (b[0] == 0.0 || !isfinite(b[0])) return 1;
+    if (n == 1) return 0;                        /* [C-13] nothing else to do         */
+    c[0] = c[0] / b[0];                          /* eq. 1:  c^_1 = c_1 / b_1          */
+    for (int i = 1; i <= n - 2; ++i) {           /* Alg. 1 line 3: i = 2 .. N-1       */
+        b[i] = b[i] - a[i] * c[i - 1];           /* eq. 2:  b^_i = b_i - a_i c^_{i-1} */
+        if (b[i] == 0.0 || !isfinite(b[i])) return i + 1;
+        c[i] = c[i] / b[i];                      /*         c^_i = c_i / b^_i         */
+    }
+    b[n - 1] = b[n - 1] - a[n - 1] * c[n - 2];   /* Alg. 1 line 7; c^_N unused [C-3]  */
+    if (b[n - 1] == 0.0 || !isfinite(b[n - 1])) return n;
+    return 0;
+}
+
+/* Alg. 2 for one contiguous system: d is overwritten by x. */
+ORC_API void orc_tri_solve(int n, const double *a, const double *bh, const double *ch, double *d)
+{
+    d[0] = d[0] / bh[0];                         /* eq. 3 (b^_1 = b_1 [C-2])          */
+    for (int i = 1; i < n; ++i)                  /* eq. 4                             */
+        d[i] = (d[i] - a[i] * d[i - 1]) / bh[i];
+    /* eq. 5: x_N = d^_N (already in place) */
+    for (int i = n - 2; i >= 0; --i)             /* eq. 6 as Alg. 2 line 10 [C-1]     */
+        d[i] = d[i] - ch[i] * d[i + 1];
+}
+
+/* ------------------------------------------------------------------------------------
+ * Pentadiagonal, paper naming: row i is
+ *   a_i x_{i-2} + b_i x_{i-1} + c_i x_i + d_i x_{i+1} + e_i x_{i+2} = f_i.
+ * 0-based arrays: a[i-1] holds a_i, etc.  Never read: a[0],a[1],b[0],d[n-1],e[n-2],e[n-1].
+ * After the factor: a = eps, b = beta, c = alpha, d = gamma, e = delta (step 14).
+ * ---------------------------------------------------------------------------------- */
+
+static int bad(double v) { return v == 0.0 || !isfinite(v); }
+
+/* General-row form used for N < 4 [C-13]: the same formulas as step 8 with every
+ * out-of-range gamma, delta taken as 0 and never-read diagonal entries ignored.
+ * tests/test_oracle_penta.py checks it is bit-identical to the literal steps for N >= 4. */
+ORC_API int orc_penta_factor_general(int n, const double *a, double *b, double *c, double *d, double *e)
+{
+    if (n < 1) return -1;
+    for (int i = 0; i < n; ++i) {
+        double gm1 = (i >= 1) ? d[i - 1] : 0.0, gm2 = (i >= 2) ? d[i - 2] : 0.0;
+        double dm1 = (i >= 1) ? e[i - 1] : 0.0, dm2 = (i >= 2) ? e[i - 2] : 0.0;
+        if (i >= 2) b[i] = b[i] - a[i] * gm2;                /* beta_i                 */
+        if (i >= 2) c[i] = c[i] - a[i] * dm2 - b[i] * gm1;   /* alpha_i                */
+        else if (i == 1) c[i] = c[i] - b[i] * gm1;
+        if (bad(c[i])) return i + 1;
+        if (i <= n - 2) d[i] = ((i >= 1) ? (d[i] - b[i] * dm1) : d[i]) / c[i]; /* gamma */
+        if (i <= n - 3) e[i] = e[i] / c[i];                                    /* delta */
+    }
+    return 0;
+}
+
+/* Sec. 4.1 steps 1-14 / Alg. 3, literally, for N >= 4; N < 4 goes to the general form. */
+ORC_API int orc_penta_factor(int n, const double *a, double *b, double *c, double *d, double *e)
+{
+    if (n < 4) return orc_penta_factor_general(n, a, b, c, d, e);
+    const int N = n;                         /* 1-based index i lives at [i-1]            */
+#define A_(i) a[(i) - 1]
+#define B_(i) b[(i) - 1]
+#define C_(i) c[(i) - 1]
+#define D_(i) d[(i) - 1]
+#define E_(i) e[(i) - 1]
+    if (bad(C_(1))) return 1;                /* 1. alpha_1 = c_1                          */
+    D_(1) = D_(1) / C_(1);                   /* 2. gamma_1 = d_1 / alpha_1                */
+    E_(1) = E_(1) / C_(1);                   /* 3. delta_1 = e_1 / alpha_1                */
+                                             /* 4. beta_2 = b_2                           */
+    C_(2) = C_(2) - B_(2) * D_(1);           /* 5. alpha_2 = c_2 - beta_2 gamma_1  [C-6]  */
+    if (bad(C_(2))) return 2;
+    D_(2) = (D_(2) - B_(2) * E_(1)) / C_(2); /* 6. gamma_2 = (d_2 - beta_2 delta_1)/alpha_2 [C-6] */
+    E_(2) = E_(2) / C_(2);                   /* 7. delta_2 = e_2 / alpha_2                */
+    for (int i = 3; i <= N - 2; ++i) {       /* 8. i = 3 .. N-2                           */
+        B_(i) = B_(i) - A_(i) * D_(i - 2);                       /* (a) [C-6]            */
+        C_(i) = C_(i) - A_(i) * E_(i - 2) - B_(i) * D_(i - 1);   /* (b) [C-6][C-9]       */
+        if (bad(C_(i))) return i;
+        D_(i) = (D_(i) - B_(i) * E_(i - 1)) / C_(i);             /* (c) [C-10]           */
+        E_(i) = E_(i) / C_(i);                                   /* (d) [C-7]            */
+    }
+    B_(N - 1) = B_(N - 1) - A_(N - 1) * D_(N - 3);                         /* 9.         */
+    C_(N - 1) = C_(N - 1) - A_(N - 1) * E_(N - 3) - B_(N - 1) * D_(N - 2); /* 10.        */
+    if (bad(C_(N - 1))) return N - 1;
+    D_(N - 1) = (D_(N - 1) - B_(N - 1) * E_(N - 2)) / C_(N - 1);           /* 11.        */
+    B_(N) = B_(N) - A_(N) * D_(N - 2);                                     /* 12. [C-11] */
+    C_(N) = C_(N) - A_(N) * E_(N - 2) - B_(N) * D_(N - 1);                 /* 13.        */
+    if (bad(C_(N))) return N;
+    /* 14. eps_i = a_i: a is untouched. */
+#undef A_
+#undef B_
+#undef C_
+#undef D_
+#undef E_
+    return 0;
+}
+
+/* Sec. 4.1 "steps to find g" + back-substitution / Alg. 4, one contiguous system;
+ * f is overwritten by x.  N < 4 uses the same formulas with out-of-range terms dropped
+ * [C-13] (for N >= 4 the guards below never fire except exactly where the paper
+ * special-cases rows 1, 2, N-1, N). */
+ORC_API void orc_penta_solve(int n, const double *eps, const double *beta, const double *alpha,
+                             const double *gamma, const double *delta, double *f)
+{
+    f[0] = f[0] / alpha[0];                                   /* 1. g_1                   */
+    if (n >= 2) f[1] = (f[1] - beta[1] * f[0]) / alpha[1];    /* 2. g_2                   */
+    for (int i = 2; i < n; ++i)                               /* 3. g_i, i = 3..N         */
+        f[i] = (f[i] - eps[i] * f[i - 2] - beta[i] * f[i - 1]) / alpha[i];
+    /* 1. x_N = g_N */
+    if (n >= 2) f[n - 2] = f[n - 2] - gamma[n - 2] * f[n - 1];            /* 2. x_{N-1}   */
+    for (int i = n - 3; i >= 0; --i)                                      /* 3. [C-8][C-12] */
+        f[i] = f[i] - gamma[i] * f[i + 1] - delta[i] * f[i + 2];
+}
+
+/* ------------------------------------------------------------------------------------
+ * Cahn-Hilliard explicit half (eq. 24 RHS with eq. 25a; eq. 26c with the C^n term
+ * restored [C-21]; truncated stencil, ghost values zero: w_0 = w_{N+1} = 0 [C-18]):
+ *   w_i = c_i^3 - c_i,   f_i = c_i + alpha (w_{i-1} - 2 w_i + w_{i+1}),  alpha = dt/dx^2.
+ * ---------------------------------------------------------------------------------- */
+ORC_API void orc_ch_rhs(int n, const double *c, double alpha, double *f)
+{
+    for (int i = 0; i < n; ++i) {
+        double wm = (i > 0) ? c[i - 1] * c[i - 1] * c[i - 1] - c[i - 1] : 0.0;
+        double w0 = c[i] * c[i] * c[i] - c[i];
+        double wp = (i < n - 1) ? c[i + 1] * c[i + 1] * c[i + 1] - c[i + 1] : 0.0;
+        f[i] = c[i] + alpha * (wm - 2.0 * w0 + wp);
+    }
+}
+
+/* ------------------------------------------------------------------------------------
+ * Interleaved batch drivers: gather column j -> contiguous, run the single-system
+ * routine nsteps times (RHS = previous solution), scatter back.
+ * Systems j = jlo, jlo+jstride, ... < jhi are processed; the rest are left untouched
+ * (lets a caller check / time a stated subset of a large batch).
+ * nthreads <= 0: all cores (OpenMP over systems); the arithmetic per system is serial.
+ * ---------------------------------------------------------------------------------- */
+static int set_threads(int nthreads)
+{
+#ifdef _OPENMP
+    if (nthreads > 0) omp_set_num_threads(nthreads);
+    else omp_set_num_threads(omp_get_num_procs());
+    int used = 1;
+#pragma omp parallel
+    {
+#pragma omp single
+        used = omp_get_num_threads();
+    }
+    return used;
+#else
+    (void)nthreads;
+    return 1;
+#endif
+}
+
+ORC_API int orc_tri_solve_interleaved(int n, const double *a, const double *bh, const double *ch,
+                                      double *rhs, long long M, long long jlo, long long jhi,
+                                      long long jstride, int nsteps, int nthreads)
+{
+    int used = set_threads(nthreads);
+#pragma omp parallel
+    {
+        double *col = (double *)malloc((size_t)n * sizeof(double));
+#pragma omp for schedule(static)
+        for (long long j = jlo; j < jhi; j += jstride) {
+            for (int i = 0; i < n; ++i) col[i] = rhs[(size_t)i * M + j];
+            for (int s = 0; s < nsteps; ++s) orc_tri_solve(n, a, bh, ch, col);
+            for (int i = 0; i < n; ++i) rhs[(size_t)i * M + j] = col[i];
+        }
+        free(col);
+    }
+    return used;
+}
+
+ORC_API int orc_penta_solve_interleaved(int n, const double *eps, const double *beta,
+                                        const double *alpha, const double *gamma,
+                                        const double *delta, double *rhs, long long M,
+                                        long long jlo, long long jhi, long long jstride,
+                                        int nsteps, int nthreads)
+{
+    int used = set_threads(nthreads);
+#pragma omp parallel
+    {
+        double *col = (double *)malloc((size_t)n * sizeof(double));
+#pragma omp for schedule(static)
+        for (long long j = jlo; j < jhi; j += jstride) {
+            for (int i = 0; i < n; ++i) col[i] = rhs[(size_t)i * M + j];
+            for (int s = 0; s < nsteps; ++s) orc_penta_solve(n, eps, beta, alpha, gamma, delta, col);
+            for (int i = 0; i < n; ++i) rhs[(size_t)i * M + j] = col[i];
+        }
+        free(col);
+    }
+    return used;
+}
+
+/* Config-5 stepper: for s in 1..nsteps: f = rhs(c) (eq. 24 explicit half); c = A^{-1} f
+ * with A = I + sigma*D4_trunc already factored into (eps..delta) by orc_penta_factor. */
+ORC_API int orc_ch_step_interleaved(int n, const double *eps, const double *beta,
+                                    const double *alpha, const double *gamma,
+                                    const double *delta, double *cbuf, long long M,
+                                    long long jlo, long long jhi, long long jstride,
+                                    double alpha_x, int nsteps, int nthreads)
+{
+    int used = set_threads(nthreads);
+#pragma omp parallel
+    {
+        double *col = (double *)malloc((size_t)n * sizeof(double));
+        double *f = (double *)malloc((size_t)n * sizeof(double));
+#pragma omp for schedule(static)
+        for (long long j = jlo; j < jhi; j += jstride) {
+            for (int i = 0; i < n; ++i) col[i] = cbuf[(size_t)i * M + j];
+            for (int s = 0; s < nsteps; ++s) {
+                orc_ch_rhs(n, col, alpha_x, f);
+                orc_penta_solve(n, eps, beta, alpha, gamma, delta, f);
+                memcpy(col, f, (size_t)n * sizeof(double));
+            }
+            for (int i = 0; i < n; ++i) cbuf[(size_t)i * M + j] = col[i];
+        }
+        free(col);
+        free(f);
+    }
+    return used;
+}
