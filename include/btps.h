@@ -1,0 +1,153 @@
+/*
+ * btps.h -- C-ABI of the B200-native batched shared-LHS tridiagonal / pentadiagonal solver
+ * (the hot path of arxiv/paper_2107_05395, "A Batched GPU Methodology for Numerical Solutions
+ * of PDEs").  One LHS matrix A is factored once on the host; every right-hand side of a huge
+ * batch then runs one forward-elimination and one back-substitution sweep, in place.
+ *
+ * Citations are PAPER.md:<line> (+ section / equation / algorithm).  Readings of garbled or
+ * silent passages are listed in DESIGN.md ("Readings", items C-n).
+ *
+ * Conventions shared by every call
+ * --------------------------------
+ *  - Layout (Sec. 2; Alg. 2 "rowID +- M"): a batch is ONE array of
+ *    n*batch values; element i (0-based row) of system j lives at  rhs[i*batch + j]
+ *    ("interleaved").  The solution overwrites the right-hand side.
+ *  - "host" pointers are ordinary CPU memory, "device" pointers are CUDA global memory of the
+ *    current device.  All pointers are borrowed for the duration of the call only.
+ *  - The `stream` argument is a cudaStream_t passed as void* (0 = legacy default stream), e.g.
+ *    torch.cuda.current_stream().cuda_stream.  Device-buffer calls only enqueue work on it:
+ *    no host synchronisation, no allocation, no host<->device copy.
+ *  - Handles are immutable after creation, own their device-side coefficient tables, may be
+ *    used from several streams at once, and must be destroyed by the matching *_destroy.
+ *  - Status codes: 0 = success, negative = BTPS_E_* below.  The failing call also records the
+ *    code (and, for factor failures, the 1-based row of the bad pivot) per host thread; read
+ *    it with btps_last_error().
+ *  - No pivoting (the paper has none): a zero or non-finite pivot makes the
+ *    factor call fail with BTPS_E_PIVOT.
+ *  - There is no CPU fallback anywhere: every call that touches a batch needs a CUDA device.
+ */
+#ifndef BTPS_H_
+#define BTPS_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#if defined(__GNUC__)
+#define BTPS_API __attribute__((visibility("default")))
+#else
+#define BTPS_API
+#endif
+
+#define BTPS_OK 0
+#define BTPS_E_ARG (-1)     /* null pointer, n < 1, batch < 1, nsteps < 0, bad handle            */
+#define BTPS_E_PIVOT (-2)   /* zero / non-finite pivot in the factorisation (row reported)        */
+#define BTPS_E_CUDA (-3)    /* a CUDA runtime call failed (cudaGetLastError text via btps_error_string) */
+#define BTPS_E_ALIGN (-4)   /* device pointer not aligned to sizeof(element)                      */
+
+typedef struct btps_tri_s *tri_handle_t;
+typedef struct btps_penta_s *penta_handle_t;
+
+/* ------------------------------------------------------------------------------------------
+ * (a1) Tridiagonal factor.  PAPER.md:87-93 (eq. 1-2), 555-566 (Alg. 1), run once on the host
+ * (PAPER.md:73).  Row i (0-based):  a[i]*x[i-1] + b[i]*x[i] + c[i]*x[i+1] = rhs[i]
+ * (paper's a, b, c).  a, b, c: host, length n; a[0] and c[n-1] are never read.
+ * Computes  c^_0 = c_0/b_0;  b^_i = b_i - a_i c^_{i-1};  c^_i = c_i/b^_i  in fp64, derives the
+ * sweep tables (reciprocal pivots, l_i = a_i/b^_i, partition response vectors -- DESIGN.md
+ * "Partitioned sweep") for fp64 and fp32, and uploads them once.
+ * Returns NULL on failure (see btps_last_error).
+ * ---------------------------------------------------------------------------------------- */
+BTPS_API tri_handle_t tri_factor(int n, const double *a, const double *b, const double *c);
+BTPS_API void tri_destroy(tri_handle_t h);
+
+/* ------------------------------------------------------------------------------------------
+ * (a3) Pentadiagonal factor A = L R.  PAPER.md:206-256 (Sec. 4.1 steps 1-14), 601-637 (Alg. 3).
+ * Row i:  e[i]*x[i-2] + a[i]*x[i-1] + d[i]*x[i] + c[i]*x[i+1] + f[i]*x[i+2] = rhs[i].
+ * NOTE the naming: BASELINE.json's (e,a,d,c,f) = the paper's (a,b,c,d,e) of PAPER.md:204.
+ * Host arrays of length n; never read: e[0], e[1], a[0], c[n-1], f[n-2], f[n-1].
+ * Computes (eps, beta, alpha, gamma, delta) in fp64 by the general-row form of step 8
+ * (identical to steps 1-14 for n >= 4, extends to n = 1..3; C-13).
+ * ---------------------------------------------------------------------------------------- */
+BTPS_API penta_handle_t penta_factor(int n, const double *e, const double *a, const double *d,
+                            const double *c, const double *f);
+BTPS_API void penta_destroy(penta_handle_t h);
+
+/* ------------------------------------------------------------------------------------------
+ * (a2)/(a4) Batched sweeps.  Tri: PAPER.md:95-108 (eq. 3-6), 568-597 (Alg. 2).
+ * Penta: PAPER.md:258-278 (Sec. 4.1 "g" steps + back-substitution), 639-676 (Alg. 4).
+ * d_rhs: DEVICE, n*batch elements, interleaved, solved in place.  Any batch >= 1.
+ * Asynchronous on `stream`.  HBM sees one read and one write per element (sweep intermediates
+ * stay in registers) unless n exceeds the on-chip plan limit (see btps_plan_info), in which
+ * case a two-pass kernel in the paper's own form (2 reads + 2 writes) is used.
+ * The *_f32 variants take float data and use the fp32-rounded tables of the same handle.
+ * ---------------------------------------------------------------------------------------- */
+BTPS_API int tri_solve_batched(tri_handle_t h, double *d_rhs, int64_t batch, void *stream);
+BTPS_API int tri_solve_batched_f32(tri_handle_t h, float *d_rhs, int64_t batch, void *stream);
+BTPS_API int penta_solve_batched(penta_handle_t h, double *d_rhs, int64_t batch, void *stream);
+BTPS_API int penta_solve_batched_f32(penta_handle_t h, float *d_rhs, int64_t batch, void *stream);
+
+/* ------------------------------------------------------------------------------------------
+ * (a6) Time-step driver: nsteps successive solves with RHS = previous solution (the paper
+ * times "just the time-stepping sections"; implicit diffusion / hyperdiffusion
+ * loops PAPER.md:120-136, 288-296, in BASELINE.json's backward-Euler form, C-22).
+ * Same arguments as the single solve; nsteps >= 0 launches are enqueued back to back on
+ * `stream` with no host synchronisation.
+ * ---------------------------------------------------------------------------------------- */
+BTPS_API int tri_solve_steps(tri_handle_t h, double *d_rhs, int64_t batch, int nsteps, void *stream);
+BTPS_API int penta_solve_steps(penta_handle_t h, double *d_rhs, int64_t batch, int nsteps, void *stream);
+
+/* ------------------------------------------------------------------------------------------
+ * (a5) Fused semi-implicit Cahn-Hilliard step.  PAPER.md:365-392 (eq. 24, 25a, 26a-c):
+ *   (I + sigma*D4) c^{n+1} = c^n + alpha * D2( (c^n)^3 - c^n ),   alpha = dt/dx^2,
+ * truncated (non-periodic) stencils, ghost values zero (BASELINE.json config 5; DESIGN.md
+ * C-18, C-21).  `h` is the caller's penta_factor of I + sigma*D4; d_c: DEVICE, n*batch fp64,
+ * interleaved, advanced nsteps steps in place.  One kernel per step builds the RHS in
+ * registers and sweeps; nothing but c^n in / c^{n+1} out crosses HBM.
+ * ---------------------------------------------------------------------------------------- */
+BTPS_API int ch_step_batched(penta_handle_t h, double *d_c, int64_t batch, double alpha, int nsteps,
+                    void *stream);
+
+/* ------------------------------------------------------------------------------------------
+ * End-to-end variants on HOST buffers (the call a user without device code makes).
+ * h_rhs / h_c: HOST, n*batch elements, interleaved; pinned memory is used at full speed,
+ * pageable memory works but copies slower.  The batch is cut into column chunks; each chunk
+ * is copied to the device (strided 2-D copy into its own interleaved buffer), advanced
+ * nsteps steps, and copied back, with copies and kernels of different chunks overlapped on
+ * internal streams.  Synchronous: returns when h_rhs holds the result.
+ * ---------------------------------------------------------------------------------------- */
+BTPS_API int tri_solve_batched_host(tri_handle_t h, double *h_rhs, int64_t batch, int nsteps);
+BTPS_API int penta_solve_batched_host(penta_handle_t h, double *h_rhs, int64_t batch, int nsteps);
+BTPS_API int ch_step_batched_host(penta_handle_t h, double *h_c, int64_t batch, double alpha, int nsteps);
+
+/* ------------------------------------------------------------------------------------------
+ * Introspection / tuning (used by tests, bench.py and ncu A/B runs; not needed by callers).
+ * ---------------------------------------------------------------------------------------- */
+
+/* Last status recorded on this host thread; *row (may be NULL) = 1-based pivot row or 0. */
+BTPS_API int btps_last_error(int *row);
+BTPS_API const char *btps_error_string(int code);
+
+/* Kernel plan of a handle for element size `elem_bytes` (8 or 4).  Writes 8 ints to out:
+ *   out[0] rows per thread (0 = two-pass kernel), out[1] partitions per system,
+ *   out[2] lanes (threads side by side on adjacent systems), out[3] systems per thread,
+ *   out[4] tiles per CTA, out[5] threads per CTA, out[6] dynamic shared memory bytes,
+ *   out[7] coefficient table bytes resident on the device for this plan.
+ * kind: 0 = tri handle, 1 = penta handle. */
+BTPS_API int btps_plan_info(int kind, const void *handle, int elem_bytes, int *out);
+
+/* Override the plan chosen at factor time (call BEFORE tri_factor / penta_factor; process
+ * global).  key is one of "rows" (rows per thread: 8, 16, 32), "lanes" (32, 16, 8, 4),
+ * "vec" (systems per thread: 1, 2), "tiles_per_cta", "force_two_pass" (0/1), "reverse"
+ * (0/1: alternate the tile order on successive steps of *_solve_steps / ch_step_batched so a
+ * step starts on the data the previous one left in L2).  value < 0 restores the default. */
+BTPS_API int btps_tune(const char *key, int value);
+
+/* Number of kernel launches issued by this library in this process (bench.py's gpu_launches). */
+BTPS_API int64_t btps_launch_count(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* BTPS_H_ */

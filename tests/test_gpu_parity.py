@@ -1,0 +1,365 @@
+"""GPU parity: the CUDA path (through the C-ABI binding) against the CPU oracle, element by element,
+on the same seeded inputs.  Tolerances are BASELINE.json's: max|gpu-oracle| / max|oracle| <= 1e-12
+(fp64 single solve), 1e-10 (fp64 after all time steps), 1e-5 (fp32 GPU vs fp64 oracle).
+"""
+import numpy as np
+import pytest
+
+import inputs
+import oracle
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+
+TOL_SINGLE = 1e-12
+TOL_STEPS = 1e-10
+TOL_F32 = 1e-5
+
+
+@pytest.fixture(scope="module")
+def lib():
+    if not torch.cuda.is_available():
+        pytest.fail("gpu tests need a CUDA device")
+    import paper_2107_05395_b200 as b
+    return b
+
+
+def rel_err(got, ref):
+    return float(np.max(np.abs(got - ref)) / max(np.max(np.abs(ref)), 1e-300))
+
+
+def dev(x):
+    return torch.from_numpy(x).cuda()
+
+
+def rand_tri(n, seed):
+    rng = np.random.default_rng(seed)
+    a = rng.uniform(-1, 1, n)
+    c = rng.uniform(-1, 1, n)
+    b = np.abs(a) + np.abs(c) + rng.uniform(0.5, 1.5, n)
+    b *= rng.choice([-1.0, 1.0], n)
+    return a, b, c
+
+
+def rand_penta(n, seed):
+    rng = np.random.default_rng(seed)
+    e, a, c, f = (rng.uniform(-1, 1, n) for _ in range(4))
+    d = np.abs(e) + np.abs(a) + np.abs(c) + np.abs(f) + rng.uniform(0.5, 1.5, n)
+    d *= rng.choice([-1.0, 1.0], n)
+    return e, a, d, c, f
+
+
+# ---- config 1 ----------------------------------------------------------------------------------
+
+def test_config1_tri_single_solve(lib):
+    n, batch = 64, 1024
+    a, b, c = inputs.tri_lhs(n, 0.5)
+    rhs = inputs.uniform_rhs(n, batch, seed=0)
+    ref = rhs.copy()
+    oracle.tri_solve_interleaved(oracle.tri_factor(a, b, c), ref)
+    h = lib.tri_factor(a, b, c)
+    d = dev(rhs)
+    lib.tri_solve_batched(h, d)
+    torch.cuda.synchronize()
+    assert rel_err(d.cpu().numpy(), ref) <= TOL_SINGLE
+
+
+# ---- general LHS, edge sizes, ragged batches ----------------------------------------------------
+
+SIZES = [1, 2, 3, 4, 5, 7, 8, 9, 16, 17, 31, 32, 33, 64, 100, 255, 256, 512, 777, 1024, 1500, 2048, 4096,
+         5000]
+
+
+@pytest.mark.parametrize("n", SIZES)
+def test_tri_general_lhs_sizes(lib, n):
+    a, b, c = rand_tri(n, 100 + n)
+    fac = oracle.tri_factor(a, b, c)
+    h = lib.tri_factor(a, b, c)
+    for batch in (1, 33, 257 if n > 1024 else 1000):
+        rhs = inputs.uniform_rhs(n, batch, seed=n)
+        ref = rhs.copy()
+        oracle.tri_solve_interleaved(fac, ref)
+        d = dev(rhs)
+        lib.tri_solve_batched(h, d)
+        assert rel_err(d.cpu().numpy(), ref) <= TOL_SINGLE, (n, batch, h.plan())
+
+
+@pytest.mark.parametrize("n", SIZES)
+def test_penta_general_lhs_sizes(lib, n):
+    e, a, d_, c, f = rand_penta(n, 200 + n)
+    fac = oracle.penta_factor(e, a, d_, c, f)
+    h = lib.penta_factor(e, a, d_, c, f)
+    for batch in (1, 33, 257 if n > 1024 else 1000):
+        rhs = inputs.uniform_rhs(n, batch, seed=n + 1)
+        ref = rhs.copy()
+        oracle.penta_solve_interleaved(fac, ref)
+        d = dev(rhs)
+        lib.penta_solve_batched(h, d)
+        assert rel_err(d.cpu().numpy(), ref) <= TOL_SINGLE, (n, batch, h.plan())
+
+
+@pytest.mark.parametrize("n", [1, 5, 33, 64, 256, 1024, 5000])
+def test_fp32_tri_and_penta(lib, n):
+    for kind in ("tri", "penta"):
+        if kind == "tri":
+            lhs = inputs.tri_lhs(n, 0.5)
+            fac, h = oracle.tri_factor(*lhs), lib.tri_factor(*lhs)
+        else:
+            lhs = inputs.penta_lhs(n, 0.5)
+            fac, h = oracle.penta_factor(*lhs), lib.penta_factor(*lhs)
+        for batch in (1, 31, 1000, 1001):   # odd batches take the scalar (unvectorised) kernel
+            rhs32 = inputs.uniform_rhs(n, batch, seed=3, dtype=np.float32)
+            ref = rhs32.astype(np.float64)
+            (oracle.tri_solve_interleaved if kind == "tri" else oracle.penta_solve_interleaved)(fac, ref)
+            d = dev(rhs32)
+            (lib.tri_solve_batched_f32 if kind == "tri" else lib.penta_solve_batched_f32)(h, d)
+            assert rel_err(d.cpu().numpy().astype(np.float64), ref) <= TOL_F32, (kind, n, batch)
+
+
+def test_unaligned_base_pointer_fp32(lib):
+    """A float buffer that starts 4 bytes off 8-byte alignment must take the scalar path."""
+    n, batch = 64, 512
+    lhs = inputs.tri_lhs(n, 0.5)
+    fac, h = oracle.tri_factor(*lhs), lib.tri_factor(*lhs)
+    rhs32 = inputs.uniform_rhs(n, batch, seed=5, dtype=np.float32)
+    ref = rhs32.astype(np.float64)
+    oracle.tri_solve_interleaved(fac, ref)
+    big = torch.empty(n * batch + 1, dtype=torch.float32, device="cuda")
+    view = big[1:]
+    view.copy_(torch.from_numpy(rhs32).reshape(-1))
+    lib.tri_solve_batched_f32(h, view)
+    assert rel_err(view.cpu().numpy().reshape(n, batch).astype(np.float64), ref) <= TOL_F32
+
+
+# ---- properties ----------------------------------------------------------------------------------
+
+def test_result_independent_of_batch_position(lib):
+    """A system's solution must not depend on where it sits in the batch or on the batch size
+    (bitwise: one code path per plan)."""
+    n = 512
+    lhs = inputs.penta_lhs(n, 0.5)
+    h = lib.penta_factor(*lhs)
+    full = inputs.uniform_rhs(n, 4096, seed=9)
+    d_full = dev(full)
+    lib.penta_solve_batched(h, d_full)
+    sub = np.ascontiguousarray(full[:, 1000:1777])
+    d_sub = dev(sub)
+    lib.penta_solve_batched(h, d_sub)
+    assert np.array_equal(d_full.cpu().numpy()[:, 1000:1777], d_sub.cpu().numpy())
+
+
+def test_handle_shared_by_two_streams(lib):
+    n, batch = 256, 8192
+    lhs = inputs.tri_lhs(n, 0.5)
+    h = lib.tri_factor(*lhs)
+    x1, x2 = dev(inputs.uniform_rhs(n, batch, seed=1)), dev(inputs.uniform_rhs(n, batch, seed=2))
+    ref1, ref2 = x1.clone(), x2.clone()
+    lib.tri_solve_batched(h, ref1)
+    lib.tri_solve_batched(h, ref2)
+    torch.cuda.synchronize()
+    s1, s2 = torch.cuda.Stream(), torch.cuda.Stream()
+    for _ in range(3):
+        y1, y2 = x1.clone(), x2.clone()
+        torch.cuda.synchronize()
+        lib.tri_solve_batched(h, y1, stream=s1.cuda_stream)
+        lib.tri_solve_batched(h, y2, stream=s2.cuda_stream)
+        torch.cuda.synchronize()
+        assert torch.equal(y1, ref1) and torch.equal(y2, ref2)
+
+
+def test_linearity(lib):
+    n, batch = 100, 64
+    lhs = rand_penta(n, 5)
+    h = lib.penta_factor(*lhs)
+    x, y = inputs.uniform_rhs(n, batch, seed=1), inputs.uniform_rhs(n, batch, seed=2)
+    dx, dy, dz = dev(x), dev(y), dev(2.0 * x - 3.0 * y)
+    for t in (dx, dy, dz):
+        lib.penta_solve_batched(h, t)
+    z = (2.0 * dx - 3.0 * dy).cpu().numpy()
+    assert rel_err(dz.cpu().numpy(), z) <= 1e-13
+
+
+def test_two_pass_kernel_matches(lib):
+    """The paper-form two-pass kernel (used beyond the on-chip limit) against the oracle at a size
+    the register-resident plan also covers."""
+    n, batch = 256, 1000
+    try:
+        lib.btps_tune("force_two_pass", 1)
+        lt, lp = inputs.tri_lhs(n), inputs.penta_lhs(n)
+        ht, hp = lib.tri_factor(*lt), lib.penta_factor(*lp)
+    finally:
+        lib.btps_tune("force_two_pass", -1)
+    assert ht.plan()["rows_per_thread"] == 0
+    rhs = inputs.uniform_rhs(n, batch, seed=4)
+    for h, fac, solve, osolve in ((ht, oracle.tri_factor(*lt), lib.tri_solve_batched, oracle.tri_solve_interleaved),
+                                  (hp, oracle.penta_factor(*lp), lib.penta_solve_batched,
+                                   oracle.penta_solve_interleaved)):
+        ref = rhs.copy()
+        osolve(fac, ref)
+        d = dev(rhs)
+        solve(h, d)
+        assert rel_err(d.cpu().numpy(), ref) <= TOL_SINGLE
+    sigma, alpha = inputs.ch_params(n)
+    c0 = 0.1 * inputs.uniform_rhs(n, batch, seed=6)
+    ref = c0.copy()
+    oracle.ch_step_interleaved(oracle.penta_factor(*inputs.ch_lhs(n)), ref, alpha, nsteps=20)
+    try:
+        lib.btps_tune("force_two_pass", 1)
+        hc = lib.penta_factor(*inputs.ch_lhs(n))
+    finally:
+        lib.btps_tune("force_two_pass", -1)
+    d = dev(c0)
+    lib.ch_step_batched(hc, d, alpha, 20)
+    assert rel_err(d.cpu().numpy(), ref) <= TOL_STEPS
+
+
+@pytest.mark.parametrize("rows,lanes,vec", [(8, 32, 1), (16, 32, 1), (16, 16, 2), (32, 16, 1), (32, 8, 1), (16, 4, 2)])
+def test_plan_variants(lib, rows, lanes, vec):
+    """Every (rows per thread, lanes, vector width) variant the tuner can pick gives the same answer."""
+    n, batch = 200, 600
+    lt, lp = rand_tri(n, 1), rand_penta(n, 2)
+    try:
+        lib.btps_tune("rows", rows)
+        lib.btps_tune("lanes", lanes)
+        lib.btps_tune("vec", vec)
+        ht, hp = lib.tri_factor(*lt), lib.penta_factor(*lp)
+    finally:
+        for k in ("rows", "lanes", "vec"):
+            lib.btps_tune(k, -1)
+    assert ht.plan()["rows_per_thread"] == rows
+    rhs = inputs.uniform_rhs(n, batch, seed=8)
+    ref = rhs.copy()
+    oracle.tri_solve_interleaved(oracle.tri_factor(*lt), ref)
+    d = dev(rhs)
+    lib.tri_solve_batched(h=ht, rhs=d)
+    assert rel_err(d.cpu().numpy(), ref) <= TOL_SINGLE
+    ref = rhs.copy()
+    oracle.penta_solve_interleaved(oracle.penta_factor(*lp), ref)
+    d = dev(rhs)
+    lib.penta_solve_batched(hp, d)
+    assert rel_err(d.cpu().numpy(), ref) <= TOL_SINGLE
+
+
+# ---- time stepping (configs 2, 3, 5) at reduced batch --------------------------------------------
+
+def test_config2_diffusion_100_steps(lib):
+    n, batch, steps = 512, 3000, 100
+    lhs = inputs.tri_lhs(n, 0.5)
+    u0, k, A = inputs.sine_modes_u0(n, batch, seed=0)
+    ref = u0.copy()
+    oracle.tri_solve_interleaved(oracle.tri_factor(*lhs), ref, nsteps=steps)
+    h = lib.tri_factor(*lhs)
+    d = dev(u0)
+    lib.tri_solve_steps(h, d, steps)
+    got = d.cpu().numpy()
+    assert rel_err(got, ref) <= TOL_STEPS
+    # exact modal decay (closed form, independent of both implementations)
+    x = np.arange(1, n + 1) / (n + 1)
+    lam = 1.0 + 4 * 0.5 * np.sin(k * np.pi / (2 * (n + 1))) ** 2
+    exact = sum((A[m] * lam[m] ** -steps)[None, :] * np.sin(np.pi * k[m][None, :] * x[:, None]) for m in range(4))
+    assert rel_err(got, exact) <= 1e-10
+
+
+def test_config3_hyperdiffusion_100_steps(lib):
+    n, batch, steps = 512, 3000, 100
+    lhs = inputs.penta_lhs(n, 0.5)
+    rhs = inputs.uniform_rhs(n, batch, seed=0)
+    ref = rhs.copy()
+    oracle.penta_solve_interleaved(oracle.penta_factor(*lhs), ref, nsteps=steps)
+    h = lib.penta_factor(*lhs)
+    d = dev(rhs)
+    lib.penta_solve_steps(h, d, steps)
+    assert rel_err(d.cpu().numpy(), ref) <= TOL_STEPS
+
+
+def test_config5_cahn_hilliard_1000_steps(lib):
+    n, batch, steps = 256, 1536, 1000
+    sigma, alpha = inputs.ch_params(n)
+    lhs = inputs.ch_lhs(n)
+    c0 = 0.1 * inputs.uniform_rhs(n, batch, seed=0)
+    ref = c0.copy()
+    oracle.ch_step_interleaved(oracle.penta_factor(*lhs), ref, alpha, nsteps=steps)
+    h = lib.penta_factor(*lhs)
+    d = dev(c0)
+    lib.ch_step_batched(h, d, alpha, steps)
+    assert rel_err(d.cpu().numpy(), ref) <= TOL_STEPS
+
+
+@pytest.mark.parametrize("n", [2, 3, 31, 33, 100, 777])
+def test_ch_step_edge_sizes(lib, n):
+    sigma, alpha = 0.7, 0.05
+    lhs = inputs.penta_lhs(n, sigma)
+    for batch in (1, 45, 600):
+        c0 = 0.5 * inputs.uniform_rhs(n, batch, seed=n)
+        ref = c0.copy()
+        oracle.ch_step_interleaved(oracle.penta_factor(*lhs), ref, alpha, nsteps=3)
+        h = lib.penta_factor(*lhs)
+        d = dev(c0)
+        lib.ch_step_batched(h, d, alpha, 3)
+        assert rel_err(d.cpu().numpy(), ref) <= 1e-12, (n, batch)
+
+
+def test_reverse_tile_order_same_result(lib):
+    n, batch, steps = 256, 5000, 6
+    lhs = inputs.penta_lhs(n, 0.5)
+    h = lib.penta_factor(*lhs)
+    rhs = inputs.uniform_rhs(n, batch, seed=11)
+    d0, d1 = dev(rhs), dev(rhs)
+    lib.penta_solve_steps(h, d0, steps)
+    try:
+        lib.btps_tune("reverse", 1)
+        lib.penta_solve_steps(h, d1, steps)
+    finally:
+        lib.btps_tune("reverse", -1)
+    assert torch.equal(d0, d1)
+
+
+# ---- host-buffer (end-to-end) calls ---------------------------------------------------------------
+
+def test_host_buffer_calls(lib):
+    n, batch = 256, 40000   # several chunks plus a ragged last one
+    lt, lp = inputs.tri_lhs(n), inputs.penta_lhs(n)
+    ht, hp = lib.tri_factor(*lt), lib.penta_factor(*lp)
+    rhs = inputs.uniform_rhs(n, batch, seed=12)
+    pinned = torch.from_numpy(rhs.copy()).pin_memory()
+    d = dev(rhs)
+    lib.tri_solve_steps(ht, d, 3)
+    lib.tri_solve_batched_host(ht, pinned, 3)
+    assert np.array_equal(pinned.numpy(), d.cpu().numpy())
+    pageable = rhs.copy()
+    d = dev(rhs)
+    lib.penta_solve_batched(hp, d)
+    lib.penta_solve_batched_host(hp, pageable, 1)
+    assert np.array_equal(pageable, d.cpu().numpy())
+    sigma, alpha = inputs.ch_params(n)
+    hc = lib.penta_factor(*inputs.ch_lhs(n))
+    c0 = 0.1 * rhs
+    d = dev(c0)
+    lib.ch_step_batched(hc, d, alpha, 5)
+    host = c0.copy()
+    lib.ch_step_batched_host(hc, host, alpha, 5)
+    assert np.array_equal(host, d.cpu().numpy())
+
+
+# ---- errors ---------------------------------------------------------------------------------------
+
+def test_error_paths(lib):
+    with pytest.raises(lib.BtpsError) as ei:
+        lib.tri_factor([0.0, 1.0, 1.0], [1.0, 1.0, 1.0], [1.0, 1.0, 0.0])   # b^_2 = 1 - 1*1 = 0
+    assert ei.value.code == -2 and ei.value.row == 2
+    with pytest.raises(lib.BtpsError):
+        lib.penta_factor([0.0] * 3, [0.0] * 3, [1.0, 0.0, 1.0], [0.0] * 3, [0.0] * 3)
+    h = lib.tri_factor(*inputs.tri_lhs(8))
+    with pytest.raises(ValueError):
+        lib.tri_solve_batched(h, torch.zeros(9, dtype=torch.float64, device="cuda"))
+    with pytest.raises(ValueError):
+        lib.tri_solve_batched(h, torch.zeros(8, dtype=torch.float32, device="cuda"))
+
+
+def test_inputs_device_generator_bitwise(lib):
+    for dtype, tdt in ((np.float64, torch.float64), (np.float32, torch.float32)):
+        n, batch = 37, 1001
+        host = inputs.uniform_rhs(n, batch, seed=42, scale=0.1, dtype=dtype)
+        t = torch.empty(n, batch, dtype=tdt, device="cuda")
+        inputs.fill_uniform_device(t, n, seed=42, scale=0.1)
+        assert np.array_equal(t.cpu().numpy(), host)
