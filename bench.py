@@ -1,0 +1,439 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the shared-LHS batched tri / penta / fused Cahn-Hilliard path on B200.
+
+Contract (driver): ``python bench.py --gpus N --steps K --warmup W`` prints ONE JSON line on rank 0.
+
+Workload: BASELINE.json configs[1] shape -- N=512 unknowns, batch=65536
+systems per GPU, fp64, interleaved.  One *step* is one pass of the whole hot path over that batch:
+  (a2) one tridiagonal sweep   (LHS of config 2: tridiag(-r, 1+2r, -r), r = 0.5; u0 = 4 sine modes)
+  (a4) one pentadiagonal sweep (LHS of config 3: I + r*[1,-4,6,-4,1];    rhs uniform[-1,1))
+  (a5) one fused Cahn-Hilliard step (LHS I + sigma*D4, RHS built in the kernel; c0 = 0.1*uniform)
+each on its own 256 MiB buffer (so 768 MiB rotate through the 126 MB L2: every launch is cold),
+advanced in place step after step (RHS = previous solution, the (a6) driver).  The factorisations
+(a1)/(a3) are done once before the loop, as the paper does ("pre-factorization step is not included
+in these timings"; "just the time-stepping sections"); their host time
+is reported as ``factor_ms``.
+
+value = system-solves per second, whole job (3 * batch * n_gpus per step).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import math
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+N_ROWS = 512
+BATCH = 65536
+METRIC = "systems solved/s (shared-LHS tri + penta + fused CH step, N=512, batch=65536/GPU, fp64)"
+UNIT = "systems/s"
+L2_BYTES = 126 * 1024 * 1024
+
+# dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full`
+# capture (profiles/r01_ncu_full_summary.md), keyed by kernel; None until a capture exists.
+NCU_TRAFFIC_BYTES = {"tri": None, "penta": None, "ch": None}
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--batch", type=int, default=BATCH, help="systems per GPU (default: config 2's 65536)")
+    ap.add_argument("--n", type=int, default=N_ROWS)
+    ap.add_argument("--seed", type=int, default=0)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-extra", action="store_true", help="skip the per-config table (configs 1-5)")
+    return ap.parse_args()
+
+
+def peaks():
+    """Measured HBM copy bandwidth (driver-written), else the profiling guide's fallback."""
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(path) as f:
+            return float(json.load(f)["hbm_gbs"]), "MEASURED_PEAKS.json hbm_gbs (of measured)"
+    except Exception:
+        return 6650.0, "B200_PROFILING.md fallback 6.65 TB/s (of fallback)"
+
+
+# ---------------------------------------------------------------------------------------------------
+# inputs (host, seeded; inputs/ holds no solver arithmetic)
+# ---------------------------------------------------------------------------------------------------
+def make_host_inputs(n, batch, seed, rank):
+    import numpy as np
+    import inputs
+    sys_ids = np.arange(rank * batch, (rank + 1) * batch, dtype=np.uint64)  # each rank: its own systems
+    u_tri, _, _ = inputs.sine_modes_u0(n, batch, seed=seed, systems=sys_ids)
+    u_penta = inputs.uniform_rhs(n, batch, seed=seed, systems=sys_ids)
+    c_ch = inputs.uniform_rhs(n, batch, seed=seed + 1, scale=0.1, systems=sys_ids)
+    return u_tri, u_penta, c_ch
+
+
+# ---------------------------------------------------------------------------------------------------
+# clocks sampler (nvidia-smi in the background during the timed region)
+# ---------------------------------------------------------------------------------------------------
+class ClockSampler:
+    FIELDS = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+              "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+              "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index = index
+        self.proc = None
+        self.path = None
+
+    def start(self):
+        try:
+            fd, self.path = tempfile.mkstemp(prefix="btps_clocks_", suffix=".csv")
+            os.close(fd)
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.FIELDS}",
+                 "--format=csv,noheader,nounits", "-lms", "50"],
+                stdout=open(self.path, "w"), stderr=subprocess.DEVNULL)
+        except Exception:
+            self.proc = None
+
+    def stop(self):
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        if self.proc is None:
+            return out
+        try:
+            self.proc.terminate()
+            self.proc.wait(timeout=5)
+        except Exception:
+            pass
+        try:
+            rows = [r.strip().split(",") for r in open(self.path) if r.strip()]
+            os.unlink(self.path)
+        except Exception:
+            return out
+        sm, reasons = [], set()
+        for r in rows:
+            if len(r) < 7:
+                continue
+            try:
+                sm.append(float(r[0]))
+                out["sm_max_mhz"] = float(r[1])
+            except ValueError:
+                continue
+            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), r[3:7]):
+                if v.strip().lower().startswith("active"):
+                    reasons.add(name)
+        if sm:
+            sm.sort()
+            out["sm_mhz"] = sm[len(sm) // 2]
+        out["reasons"] = sorted(reasons)
+        out["samples"] = len(sm)
+        return out
+
+
+# ---------------------------------------------------------------------------------------------------
+# oracle arm: one step = tri sweep + penta sweep + CH step on `sample` systems, on the host cores
+# ---------------------------------------------------------------------------------------------------
+def oracle_step_fn(n, sample, seed):
+    import numpy as np
+    import inputs
+    import oracle
+    ft = oracle.tri_factor(*inputs.tri_lhs(n, 0.5))
+    fp = oracle.penta_factor(*inputs.penta_lhs(n, 0.5))
+    sigma, alpha = inputs.ch_params(n)
+    fc = oracle.penta_factor(*inputs.ch_lhs(n))
+    ids = np.arange(sample, dtype=np.uint64)
+    u_tri, _, _ = inputs.sine_modes_u0(n, sample, seed=seed, systems=ids)
+    u_penta = inputs.uniform_rhs(n, sample, seed=seed, systems=ids)
+    c_ch = inputs.uniform_rhs(n, sample, seed=seed + 1, scale=0.1, systems=ids)
+    state = {"cores": 0}
+
+    def step():
+        c = oracle.tri_solve_interleaved(ft, u_tri)
+        oracle.penta_solve_interleaved(fp, u_penta)
+        oracle.ch_step_interleaved(fc, c_ch, alpha, nsteps=1)
+        state["cores"] = c
+    return step, state
+
+
+def run_reference(args):
+    """--impl reference: the oracle as it stands, on this box's host cores (rank 0 only)."""
+    if int(os.environ.get("RANK", "0")) != 0:
+        return
+    import oracle
+    oracle.build()
+    n, sample = args.n, min(args.batch, 16384)
+    step, state = oracle_step_fn(n, sample, args.seed)
+    for _ in range(max(args.warmup, 1)):
+        step()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        step()
+    dt = time.perf_counter() - t0
+    value = 3.0 * sample * args.steps / dt
+    desc = f"first {sample} systems of the N={n} batch per step (tri + penta + CH step)"
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+        "data": "synthetic (seeded; DESIGN.md input recipe)",
+        "config": {"workload": "BASELINE.json configs[1] shape: N=512, fp64, interleaved; bounded sample",
+                   "n": n, "sample_systems": sample},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": state["cores"], "kind": "oracle", "sample": desc},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+def cpu_baseline(n, batch, seed, budget_s=12.0):
+    """The oracle timed on this box's host cores on a bounded sample of the same workload."""
+    import oracle
+    oracle.build()
+    sample = min(batch, 65536)
+    step, state = oracle_step_fn(n, sample, seed)
+    step()  # warm-up (page faults, OpenMP team start)
+    t0 = time.perf_counter()
+    step()
+    t1 = time.perf_counter() - t0
+    reps = int(max(1, min(50, math.ceil(budget_s / max(t1, 1e-3)))))
+    t0 = time.perf_counter()
+    for _ in range(reps):
+        step()
+    dt = time.perf_counter() - t0
+    return {"value": 3.0 * sample * reps / dt, "unit": UNIT, "cores": state["cores"], "kind": "oracle",
+            "sample": f"{reps} steps x {sample} systems (N={n}; tri + penta + CH step per step), {dt:.1f} s of CPU work"}
+
+
+# ---------------------------------------------------------------------------------------------------
+# per-config table (BASELINE.json configs 1-5), reported under "configs"; not the headline
+# ---------------------------------------------------------------------------------------------------
+def time_launches(torch, fn_of_buf, bufs, launches, repeats=3):
+    """Median over `repeats` of the mean CUDA-event time (ms) of `launches` back-to-back calls,
+    rotating over `bufs` (so small working sets do not stay in L2)."""
+    ts = []
+    for _ in range(repeats):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        e0.record()
+        for i in range(launches):
+            fn_of_buf(bufs[i % len(bufs)])
+        e1.record()
+        torch.cuda.synchronize()
+        ts.append(e0.elapsed_time(e1) / launches)
+    ts.sort()
+    return ts[len(ts) // 2]
+
+
+def extra_table(torch, b, inputs, peak):
+    """Throughput at the other BASELINE.json configs: single launches, cold (rotating over
+    buffers whose total exceeds 4x L2 when one buffer would fit in L2)."""
+    out = []
+
+    def entry(name, kind, n, batch, elem, steps_per_call=1, launches=10):
+        dt = torch.float64 if elem == 8 else torch.float32
+        size = n * batch * elem
+        nbuf = 1 if size > 2 * L2_BYTES else int(min(64, math.ceil(4 * L2_BYTES / size)))
+        bufs = []
+        for k in range(nbuf):
+            t = torch.empty(n, batch, dtype=dt, device="cuda")
+            inputs.fill_uniform_device(t, n, seed=100 + k, scale=0.1 if kind == "ch" else 1.0)
+            bufs.append(t)
+        if kind == "tri":
+            h = b.tri_factor(*inputs.tri_lhs(n, 0.5))
+            one = b.tri_solve_batched if elem == 8 else b.tri_solve_batched_f32
+            fn = (lambda t: one(h, t)) if steps_per_call == 1 else (lambda t: b.tri_solve_steps(h, t, steps_per_call))
+        elif kind == "penta":
+            h = b.penta_factor(*inputs.penta_lhs(n, 0.5))
+            one = b.penta_solve_batched if elem == 8 else b.penta_solve_batched_f32
+            fn = (lambda t: one(h, t)) if steps_per_call == 1 else (lambda t: b.penta_solve_steps(h, t, steps_per_call))
+        else:
+            h = b.penta_factor(*inputs.ch_lhs(n))
+            _, alpha = inputs.ch_params(n)
+            fn = lambda t: b.ch_step_batched(h, t, alpha, steps_per_call)
+        fn(bufs[0])
+        ms = time_launches(torch, fn, bufs, launches) / steps_per_call
+        gbs = 2.0 * size / ms / 1e6
+        out.append({"config": name, "kind": kind, "n": n, "batch": batch, "dtype": "f64" if elem == 8 else "f32",
+                    "ms_per_solve": round(ms, 5), "systems_per_s": batch / ms * 1e3,
+                    "unknowns_per_s": n * batch / ms * 1e3, "hbm_gbs": round(gbs, 1),
+                    "frac_of_measured_peak": round(gbs / peak, 4),
+                    "cold": "rotating %d buffers" % nbuf if nbuf > 1 else "buffer > 2x L2",
+                    "plan": h.plan(elem)})
+        del bufs
+        torch.cuda.empty_cache()
+
+    entry("1 (latency-bound: 512 KiB)", "tri", 64, 1024, 8, launches=50)
+    entry("2 (100 steps per call)", "tri", 512, 65536, 8, steps_per_call=100, launches=2)
+    entry("3 (100 steps per call)", "penta", 512, 65536, 8, steps_per_call=100, launches=2)
+    entry("5 (1000 steps per call)", "ch", 256, 1 << 20, 8, steps_per_call=1000, launches=1)
+    for kind in ("tri", "penta"):
+        for elem in (8, 4):
+            for n in (64, 256, 1024):
+                for lb in (16, 20):
+                    entry("4 sweep", kind, n, 1 << lb, elem)
+    return out
+
+
+# ---------------------------------------------------------------------------------------------------
+# our arm
+# ---------------------------------------------------------------------------------------------------
+def run_ours(args):
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: the library has no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    import inputs
+    import paper_2107_05395_b200 as b  # raises if libbtps.so is missing
+
+    n, batch, K, W = args.n, args.batch, args.steps, max(args.warmup, 3)
+    peak, peak_src = peaks()
+
+    # ---- set-up: factor once (a1, a3), inputs on the host (pinned), resident copies in HBM -------
+    t0 = time.perf_counter()
+    h_tri = b.tri_factor(*inputs.tri_lhs(n, 0.5))
+    h_pen = b.penta_factor(*inputs.penta_lhs(n, 0.5))
+    h_ch = b.penta_factor(*inputs.ch_lhs(n))
+    factor_ms = 1e3 * (time.perf_counter() - t0)
+    _, alpha = inputs.ch_params(n)
+    host = [torch.from_numpy(x).pin_memory() for x in make_host_inputs(n, batch, args.seed, rank)]
+    dev = [x.cuda(non_blocking=True) for x in host]
+    torch.cuda.synchronize()
+    stream = torch.cuda.current_stream().cuda_stream
+
+    def step(ev=None):
+        if ev is not None:
+            ev[0].record()
+        b.tri_solve_batched(h_tri, dev[0], stream)
+        if ev is not None:
+            ev[1].record()
+        b.penta_solve_batched(h_pen, dev[1], stream)
+        if ev is not None:
+            ev[2].record()
+        b.ch_step_batched(h_ch, dev[2], alpha, 1, stream)
+        if ev is not None:
+            ev[3].record()
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(W):
+        step()
+    barrier()
+
+    # ---- timed region: exactly K steps ------------------------------------------------------------
+    evs = [[torch.cuda.Event(enable_timing=True) for _ in range(4)] for _ in range(K)]
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    sampler = ClockSampler(local)
+    sampler.start()
+    time.sleep(0.15)
+    launches0 = b.btps_launch_count()
+    barrier()
+    e0.record()
+    for k in range(K):
+        step(evs[k])
+    e1.record()
+    barrier()
+    launches = b.btps_launch_count() - launches0
+    total_ms = e0.elapsed_time(e1)
+    # keep the GPU busy a little longer so that nvidia-smi catches clocks under load
+    t_end = time.perf_counter() + 0.6
+    while time.perf_counter() < t_end:
+        step()
+    torch.cuda.synchronize()
+    clocks = sampler.stop()
+
+    if world > 1:
+        t = torch.tensor([total_ms], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        total_ms = float(t.item())
+    ms_per_step = total_ms / K
+    value = 3.0 * batch * world / (ms_per_step * 1e-3)
+
+    kern_ms = {name: float(np.mean([evs[k][i].elapsed_time(evs[k][i + 1]) for k in range(K)]))
+               for i, name in enumerate(("tri", "penta", "ch"))}
+    alg_bytes = 2.0 * n * batch * 8  # one read + one write of every element
+    kernels = {name: {"ms": round(ms, 5), "hbm_gbs": round(alg_bytes / ms / 1e6, 1),
+                      "frac": round(alg_bytes / ms / 1e6 / peak, 4), "plan": h.plan(8)}
+               for (name, ms), h in zip(kern_ms.items(), (h_tri, h_pen, h_ch))}
+    dom = max(kern_ms, key=kern_ms.get)
+    roofline = {"bound": "hbm", "kernel": dom, "achieved": kernels[dom]["hbm_gbs"], "peak": peak, "unit": "GB/s",
+                "frac": kernels[dom]["frac"], "traffic": NCU_TRAFFIC_BYTES[dom],
+                "algorithmic_bytes_per_launch": alg_bytes, "peak_source": peak_src,
+                "share_of_step": round(kern_ms[dom] / ms_per_step, 4)}
+
+    # ---- end to end through the host-buffer C-ABI calls (pinned host in, host out) ---------------
+    e2e = None
+    if not args.no_e2e:
+        Ke = min(K, 5)
+        b.tri_solve_batched_host(h_tri, host[0], 1)  # warm-up: allocates the staging buffers
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(Ke):
+            b.tri_solve_batched_host(h_tri, host[0], 1)
+            b.penta_solve_batched_host(h_pen, host[1], 1)
+            b.ch_step_batched_host(h_ch, host[2], alpha, 1)
+        torch.cuda.synchronize()
+        dt = time.perf_counter() - t0
+        if world > 1:
+            t = torch.tensor([dt], dtype=torch.float64, device="cuda")
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            dt = float(t.item())
+        e2e = {"value": 3.0 * batch * world * Ke / dt, "unit": UNIT, "h2d_bytes_per_step": int(3 * n * batch * 8),
+               "d2h_bytes_per_step": int(3 * n * batch * 8), "steps": Ke,
+               "api": "tri_solve_batched_host + penta_solve_batched_host + ch_step_batched_host (pinned host buffers)"}
+
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
+        "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic (seeded; DESIGN.md input recipe)",
+        "config": {"workload": "BASELINE.json configs[1] shape (N=512, batch=65536 per GPU, fp64, interleaved): "
+                               "per step one tri sweep + one penta sweep + one fused CH step",
+                   "n": n, "batch_per_gpu": batch, "l2": "inputs larger than L2 (3 x 256 MiB buffers per step)",
+                   "parallelism": f"dp{world} (independent shards, no collective)"},
+        "unknowns_per_s": value * n, "hbm_gbs_step": round(3 * alg_bytes / ms_per_step / 1e6, 1),
+        "frac_of_peak_step": round(3 * alg_bytes / ms_per_step / 1e6 / peak, 4),
+        "roofline": roofline, "kernels": kernels, "factor_ms": round(factor_ms, 3),
+        "gpu_launches": int(launches), "clocks": clocks, "e2e": e2e,
+    }
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        line["cpu_baseline"] = cpu_baseline(n, batch, args.seed)
+    if rank == 0 and world == 1 and not args.no_extra:
+        del dev
+        torch.cuda.empty_cache()
+        line["configs"] = extra_table(torch, b, inputs, peak)
+    if rank == 0:
+        print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+
+
+def main():
+    args = parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -340,6 +340,17 @@ size_t slot_smem(const DtypePlan &pl, int kind, int vec)
     return (size_t)pl.blob_bytes + xch;
 }
 
+// The partitioned plan keeps the whole coefficient image plus the exchange area in shared memory;
+// beyond the per-CTA limit of sm_100a (227 KB) the handle falls back to the two-pass kernel.
+constexpr size_t SMEM_LIMIT = 227 * 1024;
+
+void fit_plan(DtypePlan &pl, int handle_kind)
+{
+    if (pl.two_pass) return;
+    if (slot_smem(pl, handle_kind, pl.vec) > SMEM_LIMIT) pl.vec = 1;
+    if (slot_smem(pl, handle_kind, pl.vec) > SMEM_LIMIT) pl.two_pass = true;
+}
+
 void fill_slots(Handle *h)
 {
     for (int t = 0; t < 2; ++t) {
@@ -566,6 +577,7 @@ tri_handle_t tri_factor(int n, const double *a, const double *b, const double *c
             build_soa<float>({&inv, &nl, &nch}, n, soa);
         }
         pl.soa_bytes = soa.size();
+        fit_plan(pl, h->kind);
         if (upload(blob, &pl.d_blob) != BTPS_OK || upload(soa, &pl.d_soa) != BTPS_OK) {
             free_handle(h);
             return nullptr;
@@ -612,6 +624,7 @@ penta_handle_t penta_factor(int n, const double *e, const double *a, const doubl
             build_soa<float>({&inv, &nle, &nlb, &ngam, &ndel}, n, soa);
         }
         pl.soa_bytes = soa.size();
+        fit_plan(pl, h->kind);
         if (upload(blob, &pl.d_blob) != BTPS_OK || upload(soa, &pl.d_soa) != BTPS_OK) {
             free_handle(h);
             return nullptr;
