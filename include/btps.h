@@ -129,17 +129,20 @@ BTPS_API int ch_step_batched_host(penta_handle_t h, double *h_c, int64_t batch, 
 BTPS_API int btps_last_error(int *row);
 BTPS_API const char *btps_error_string(int code);
 
-/* Kernel plan of a handle for element size `elem_bytes` (8 or 4).  Writes 8 ints to out:
+/* Kernel plan of a handle for element size `elem_bytes` (8 or 4).  Writes 10 ints to out:
  *   out[0] rows per thread (0 = two-pass kernel), out[1] partitions per system,
  *   out[2] lanes (threads side by side on adjacent systems), out[3] systems per thread,
- *   out[4] tiles per CTA, out[5] threads per CTA, out[6] dynamic shared memory bytes,
- *   out[7] coefficient table bytes resident on the device for this plan.
- * kind: 0 = tri handle, 1 = penta handle. */
+ *   out[4] tile groups per CTA, out[5] threads per CTA, out[6] dynamic shared memory bytes,
+ *   out[7] coefficient table bytes resident on the device for this plan,
+ *   out[8] 1 if aligned batches are prefetched by TMA, out[9] 1 if carries use the warp scan.
+ * kind: 0 = tri handle, 1 = penta handle (solve kernels), 2 = penta handle (fused CH step kernels). */
 BTPS_API int btps_plan_info(int kind, const void *handle, int elem_bytes, int *out);
 
 /* Override the plan chosen at factor time (call BEFORE tri_factor / penta_factor; process
  * global).  key is one of "rows" (rows per thread: 8, 16, 32), "lanes" (32, 16, 8, 4),
- * "vec" (systems per thread: 1, 2), "tiles_per_cta", "force_two_pass" (0/1), "reverse"
+ * "vec" (systems per thread: 1, 2, 4), "tiles_per_cta", "force_two_pass" (0/1), "prefetch"
+ * (0: never use the TMA prefetch variant), "warp_scan" (0: serial carry walk), "pdl" (0: no
+ * programmatic dependent launch attribute), "reverse"
  * (0/1: alternate the tile order on successive steps of *_solve_steps / ch_step_batched so a
  * step starts on the data the previous one left in L2).  value < 0 restores the default. */
 BTPS_API int btps_tune(const char *key, int value);

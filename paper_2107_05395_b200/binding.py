@@ -130,6 +130,10 @@ class PentaHandle(_Handle):
     _destroy = staticmethod(lambda p: _lib.penta_destroy(p))
     kind = 1
 
+    def ch_plan(self, elem_bytes: int = 8) -> dict:
+        """Plan of the fused Cahn-Hilliard step kernels of this handle (btps_plan_info kind 2)."""
+        return btps_plan_info(self, elem_bytes, kind=2)
+
 
 def tri_factor(a, b, c) -> TriHandle:
     """btps.h tri_factor: host arrays a (sub), b (main), c (super), each length n."""
@@ -245,12 +249,12 @@ def btps_last_error():
 
 
 _PLAN_KEYS = ("rows_per_thread", "partitions", "lanes", "systems_per_thread", "tiles_per_cta",
-              "threads_per_cta", "smem_bytes", "table_bytes")
+              "threads_per_cta", "smem_bytes", "table_bytes", "tma_prefetch", "warp_scan")
 
 
-def btps_plan_info(h: _Handle, elem_bytes: int = 8) -> dict:
-    out = (ctypes.c_int * 8)()
-    _check(_lib.btps_plan_info(h.kind, h.ptr, elem_bytes, out))
+def btps_plan_info(h: _Handle, elem_bytes: int = 8, kind: int = None) -> dict:
+    out = (ctypes.c_int * 10)()
+    _check(_lib.btps_plan_info(h.kind if kind is None else kind, h.ptr, elem_bytes, out))
     return dict(zip(_PLAN_KEYS, list(out)))
 
 

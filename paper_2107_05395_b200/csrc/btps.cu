@@ -51,7 +51,8 @@ std::atomic<long long> g_launches{0};
 // tuning knobs (btps_tune)
 // ------------------------------------------------------------------------------------------------
 struct Tune {
-    int rows = -1, lanes = -1, vec = -1, tpc = -1, force_two_pass = -1, reverse = -1;
+    int rows = -1, lanes = -1, vec = -1, tpc = -1, force_two_pass = -1, reverse = -1, prefetch = -1, pdl = -1,
+        warp_scan = -1;
 };
 Tune g_tune;
 
@@ -59,22 +60,36 @@ Tune g_tune;
 // plans
 // ------------------------------------------------------------------------------------------------
 struct KernelSlot {
-    SweepEntry ent = {nullptr, nullptr};
+    SweepEntry ent = {nullptr, nullptr, 0};
     int vec = 1;
+    int tma = 0;       // 1: the TMA-prefetch variant (needs the ring in shared memory)
+    int xW = 1;        // padded exchange row length (elements)
     size_t smem = 0;
+    unsigned offX = 0, offM = 0, offR = 0;
+    unsigned box_rows = 0, nboxes = 0;
     int max_grid = 0;  // occupancy * SM count, resolved at first launch
+};
+
+// how one kernel family (solve / CH step) lays a tile over the threads of a CTA
+struct Shape {
+    int lanes = 32, lanes_log2 = 5, vec = 1, tpc = 1, threads = 0;
 };
 
 struct DtypePlan {
     int elem = 8;
-    int rows = 0, P = 0, lanes = 0, lanes_log2 = 0, vec = 1, tpc = 1, threads = 0;
+    int rows = 0, P = 0;
+    Shape shape[2];     // [0] solve (tri / penta), [1] fused CH step (penta handles)
+    int ws = 0;         // carries by the warp-shuffle scan
+    int scan_log2 = 0;  // log2 of the scan width
+    int tq = 32;        // partitions per scan-table row
     bool two_pass = false;
     void *d_blob = nullptr;  // partitioned-sweep coefficient image
-    unsigned blob_bytes = 0, offS = 0;
+    unsigned blob_bytes = 0, offT = 0;
     void *d_soa = nullptr;   // two-pass coefficient arrays
     size_t soa_bytes = 0;
-    // [kind slot][0 = vectorised, 1 = scalar tail-safe]; kind slot 0 = solve, 1 = CH (penta only)
-    KernelSlot k[2][2];
+    // [kind slot][vector mode: 0 = plan.vec, 1 = scalar tail-safe][0 = TMA prefetch, 1 = direct loads]
+    // kind slot 0 = solve, 1 = CH (penta handles only)
+    KernelSlot k[2][2][2];
 };
 
 constexpr int MAGIC_TRI = 0x74726931;    // "tri1"
@@ -96,29 +111,76 @@ int ilog2(int v)
     return l;
 }
 
-void choose_plan(int n, int elem, DtypePlan &pl)
+// Plan of the partitioned sweep: rows per thread, partitions, and per kernel
+// family the lanes, systems per thread and tile groups per CTA.  A thread keeps rows*vec elements
+// in registers: up to 64 registers' worth the kernels run 512 threads per CTA, above that 256.
+int thread_cap(int rows, int vec, int elem) { return (rows * vec * elem > 256) ? 256 : 512; }
+
+void choose_shape(int kind, int elem, int rows, int P, Shape &sh)
+{
+    // 16 bytes per thread and row (one LDS.128 / ST.128) for the solves; the CH step keeps one
+    // system per thread (its explicit half needs the registers)
+    int vec = g_tune.vec > 0 ? g_tune.vec : (kind == KIND_CH ? 1 : 16 / elem);
+    if (vec != 1 && vec != 2 && vec != 4) vec = 1;
+    if (vec * elem > 16) vec = 16 / elem;  // one vector access is at most 16 bytes
+    const int cap = thread_cap(rows, vec, elem);
+    int lanes = g_tune.lanes > 0 ? g_tune.lanes : ((P > 1 && (vec * elem == 16 || P >= 16)) ? 16 : 32);
+    if (lanes != 32 && lanes != 16 && lanes != 8 && lanes != 4) lanes = 32;
+    while (P * lanes > cap && lanes > 4) lanes >>= 1;
+    sh.lanes = lanes;
+    sh.lanes_log2 = ilog2(lanes);
+    sh.vec = vec;
+}
+
+void finish_shape(int elem, int rows, int P, Shape &sh)
+{
+    const int cap = thread_cap(rows, sh.vec, elem);
+    const int tpt = P * sh.lanes;
+    int tpc = g_tune.tpc > 0 ? g_tune.tpc : cap / tpt;
+    if (tpc < 1) tpc = 1;
+    while (tpc > 1 && tpc * tpt > cap) --tpc;
+    if (tpt % 32 != 0) tpc = 1;             // groups synchronise on whole warps
+    if (tpt != 32 && tpc > 15) tpc = 15;    // named barriers 1..15
+    if (tpc > 16) tpc = 16;                 // one mbarrier per group, 16 slots
+    sh.tpc = tpc;
+    sh.threads = tpc * tpt;
+}
+
+void choose_plan(int n, int elem, int handle_kind, DtypePlan &pl)
 {
     pl.elem = elem;
     int rows = g_tune.rows > 0 ? g_tune.rows : (n <= 8 ? 8 : (n <= 16 ? 16 : 32));
     if (rows != 8 && rows != 16 && rows != 32) rows = 32;
     int P = (n + rows - 1) / rows;
-    int lanes = g_tune.lanes > 0 ? g_tune.lanes : 32;
-    if (lanes != 32 && lanes != 16 && lanes != 8 && lanes != 4) lanes = 32;
-    while (P * lanes > 512 && lanes > 4) lanes >>= 1;
-    pl.two_pass = (P * lanes > 512) || (g_tune.force_two_pass > 0);
-    int vec = g_tune.vec > 0 ? g_tune.vec : (elem == 4 ? 2 : 1);
-    if (vec != 1 && vec != 2) vec = 1;
-    if (rows * vec * elem > 256) vec = 1;  // at most 64 data registers per thread
-    int tpc = g_tune.tpc > 0 ? g_tune.tpc : 256 / (P * lanes);
-    if (tpc < 1) tpc = 1;
-    while (tpc > 1 && tpc * P * lanes > 512) --tpc;
+    const int nshape = (handle_kind == KIND_TRI) ? 1 : 2;
+    for (int k = 0; k < nshape; ++k)
+        choose_shape(k == 0 ? handle_kind : KIND_CH, elem, rows, P, pl.shape[k]);
+    // the warp scan wants whole warps per group and at most 32 partitions: pad P with identity
+    // partitions where that makes every family's group a whole number of warps
+    int ws = (P > 1 && P <= 32 && g_tune.warp_scan != 0) ? 1 : 0;
+    if (ws) {
+        int Pp = P;
+        auto fits = [&](int q) {
+            for (int k = 0; k < nshape; ++k) {
+                const Shape &sh = pl.shape[k];
+                if ((q * sh.lanes) % 32 != 0 || q * sh.lanes > thread_cap(rows, sh.vec, elem)) return false;
+            }
+            return true;
+        };
+        while (Pp <= 32 && !fits(Pp)) ++Pp;
+        if (Pp <= 32) P = Pp;
+        else ws = 0;
+    }
+    pl.two_pass = (g_tune.force_two_pass > 0);
+    for (int k = 0; k < nshape; ++k) {
+        finish_shape(elem, rows, P, pl.shape[k]);
+        if (P * pl.shape[k].lanes > thread_cap(rows, pl.shape[k].vec, elem)) pl.two_pass = true;
+    }
     pl.rows = rows;
     pl.P = P;
-    pl.lanes = lanes;
-    pl.lanes_log2 = ilog2(lanes);
-    pl.vec = vec;
-    pl.tpc = tpc;
-    pl.threads = tpc * P * lanes;
+    pl.ws = ws;
+    pl.scan_log2 = ilog2(P);
+    pl.tq = P > SCAN_LANES ? P : SCAN_LANES;
 }
 
 template <typename T>
@@ -194,21 +256,87 @@ int factor_penta_host(int n, const double *e, const double *a, const double *d, 
 }
 
 // ------------------------------------------------------------------------------------------------
-// factor tables for the partitioned sweep; fp64 host arithmetic,
-// rounded to T when written into the blob.  Rows are padded to Np = P*rows with identity rows.
+// factor tables for the partitioned sweep; fp64 host arithmetic, rounded to
+// T when written into the blob.  Rows are padded to Np = P*rows with identity rows.
 // ------------------------------------------------------------------------------------------------
+
+// Carry-scan tables (sweep.cuh, RecLayout): slot 0 / 1 = forward / backward carry matrices of each
+// partition (Phi_q, Psi_q), slot 2 = chi at the partition's first rows, and for the warp scan the
+// Kogge-Stone multipliers of steps s >= 1 at slots 1+2s (forward) and 2+2s (backward):
+//   A^(s+1)_q = A^(s)_q A^(s)_{q-2^s}  (zero where q < 2^s),
+//   B^(s+1)_q = B^(s)_q B^(s)_{q+2^s}  (zero where q + 2^s >= P).
+// Matrices are NC x NC, row-major, stored [slot][entry][q] with tq partitions per row.
+struct Mat {
+    double m[4] = {0, 0, 0, 0};
+};
+
+Mat matmul(const Mat &x, const Mat &y, int nc)
+{
+    Mat r;
+    if (nc == 1) {
+        r.m[0] = x.m[0] * y.m[0];
+    } else {
+        r.m[0] = x.m[0] * y.m[0] + x.m[1] * y.m[2];
+        r.m[1] = x.m[0] * y.m[1] + x.m[1] * y.m[3];
+        r.m[2] = x.m[2] * y.m[0] + x.m[3] * y.m[2];
+        r.m[3] = x.m[2] * y.m[1] + x.m[3] * y.m[3];
+    }
+    return r;
+}
+
+template <typename T>
+void put_scan_tables(std::vector<unsigned char> &blob, const DtypePlan &pl, int nc, const std::vector<Mat> &Phi,
+                     const std::vector<Mat> &Psi, const std::vector<Mat> &Chi0)
+{
+    const int P = pl.P, tq = pl.tq, ne = nc * nc;
+    auto put_slot = [&](int slot, const std::vector<Mat> &v) {
+        for (int q = 0; q < P; ++q)
+            for (int m = 0; m < ne; ++m)
+                put<T>(blob, pl.offT + (((size_t)slot * ne + m) * tq + q) * sizeof(T), v[q].m[m]);
+    };
+    put_slot(0, Phi);
+    put_slot(1, Psi);
+    put_slot(2, Chi0);
+    if (!pl.ws) return;
+    std::vector<Mat> A = Phi, B = Psi;
+    const Mat zero;
+    // step 0 multipliers: no partner below / above the ends
+    A[0] = zero;
+    B[P - 1] = zero;
+    put_slot(0, A);
+    put_slot(1, B);
+    for (int st = 0; st + 1 < SCAN_STEPS; ++st) {
+        const int d = 1 << st;
+        std::vector<Mat> A2(P), B2(P);
+        for (int q = 0; q < P; ++q) {
+            A2[q] = (q >= 2 * d) ? matmul(A[q], A[q - d], nc) : zero;
+            B2[q] = (q + 2 * d < P) ? matmul(B[q], B[q + d], nc) : zero;
+        }
+        A.swap(A2);
+        B.swap(B2);
+        put_slot(1 + 2 * (st + 1), A);
+        put_slot(2 + 2 * (st + 1), B);
+    }
+}
+
+size_t scan_table_bytes(const DtypePlan &pl, int nc, size_t elem)
+{
+    const int slots = pl.ws ? (2 * SCAN_STEPS + 1) : 3;
+    return (size_t)slots * nc * nc * pl.tq * elem;
+}
+
 template <typename T>
 void build_blob_tri(int n, DtypePlan &pl, const std::vector<double> &inv, const std::vector<double> &nl,
                     const std::vector<double> &nch, std::vector<unsigned char> &blob)
 {
     const int MR = pl.rows, P = pl.P, Np = P * MR;
     constexpr int RT = 2 * RecLayout<KIND_TRI>::PAIRS;   // elements per row record
-    constexpr int STN = 2 * RecLayout<KIND_TRI>::SPAIRS;  // elements per partition entry
     auto at = [&](const std::vector<double> &v, int i, double pad) { return i < n ? v[i] : pad; };
-    pl.offS = (unsigned)align16((size_t)Np * RT * sizeof(T));
-    pl.blob_bytes = (unsigned)align16(pl.offS + (size_t)P * STN * sizeof(T));
+    pl.offT = (unsigned)align16((size_t)Np * RT * sizeof(T));
+    pl.blob_bytes = (unsigned)align16(pl.offT + scan_table_bytes(pl, 1, sizeof(T)));
     blob.assign(pl.blob_bytes, 0);
     std::vector<double> phi(MR), chi(MR), psi(MR);
+    std::vector<Mat> Phi(P), Psi(P), Chi0(P);
     for (int p = 0; p < P; ++p) {
         const int r0 = p * MR;
         double prev = 1.0;  // forward response to a unit incoming carry g_{r0-1} = 1
@@ -234,9 +362,11 @@ void build_blob_tri(int n, DtypePlan &pl, const std::vector<double> &inv, const 
             put<T>(blob, r + 4 * sizeof(T), chi[k]);
             put<T>(blob, r + 5 * sizeof(T), psi[k]);
         }
-        put<T>(blob, pl.offS + ((size_t)p * STN + 0) * sizeof(T), phi[MR - 1]);
-        put<T>(blob, pl.offS + ((size_t)p * STN + 1) * sizeof(T), 0.0);
+        Phi[p].m[0] = phi[MR - 1];
+        Psi[p].m[0] = psi[0];
+        Chi0[p].m[0] = chi[0];
     }
+    put_scan_tables<T>(blob, pl, 1, Phi, Psi, Chi0);
 }
 
 template <typename T>
@@ -246,10 +376,9 @@ void build_blob_penta(int n, DtypePlan &pl, const std::vector<double> &inv, cons
 {
     const int MR = pl.rows, P = pl.P, Np = P * MR;
     constexpr int RT = 2 * RecLayout<KIND_PENTA>::PAIRS;
-    constexpr int STN = 2 * RecLayout<KIND_PENTA>::SPAIRS;
     auto at = [&](const std::vector<double> &v, int i, double pad) { return i < n ? v[i] : pad; };
-    pl.offS = (unsigned)align16((size_t)Np * RT * sizeof(T));
-    pl.blob_bytes = (unsigned)align16(pl.offS + (size_t)P * STN * sizeof(T));
+    pl.offT = (unsigned)align16((size_t)Np * RT * sizeof(T));
+    pl.blob_bytes = (unsigned)align16(pl.offT + scan_table_bytes(pl, 2, sizeof(T)));
     blob.assign(pl.blob_bytes, 0);
     std::vector<double> phi[2], chi[2], psi[2];
     for (int t = 0; t < 2; ++t) {
@@ -257,6 +386,7 @@ void build_blob_penta(int n, DtypePlan &pl, const std::vector<double> &inv, cons
         chi[t].resize(MR);
         psi[t].resize(MR);
     }
+    std::vector<Mat> Phi(P), Psi(P), Chi0(P);
     for (int p = 0; p < P; ++p) {
         const int r0 = p * MR;
         for (int t = 0; t < 2; ++t) {
@@ -297,12 +427,22 @@ void build_blob_penta(int n, DtypePlan &pl, const std::vector<double> &inv, cons
             put<T>(blob, r + 8 * sizeof(T), psi[0][k]);
             put<T>(blob, r + 9 * sizeof(T), psi[1][k]);
         }
-        const size_t sOff = pl.offS + (size_t)p * STN * sizeof(T);
-        put<T>(blob, sOff + 0 * sizeof(T), phi[0][MR - 1]);
-        put<T>(blob, sOff + 1 * sizeof(T), phi[1][MR - 1]);
-        put<T>(blob, sOff + 2 * sizeof(T), phi[0][MR - 2]);
-        put<T>(blob, sOff + 3 * sizeof(T), phi[1][MR - 2]);
+        // carries: (g at the last row, g at the last-but-one row) forward; (x at the first row, x at
+        // the second row) backward
+        Phi[p].m[0] = phi[0][MR - 1];
+        Phi[p].m[1] = phi[1][MR - 1];
+        Phi[p].m[2] = phi[0][MR - 2];
+        Phi[p].m[3] = phi[1][MR - 2];
+        Psi[p].m[0] = psi[0][0];
+        Psi[p].m[1] = psi[1][0];
+        Psi[p].m[2] = psi[0][1];
+        Psi[p].m[3] = psi[1][1];
+        Chi0[p].m[0] = chi[0][0];
+        Chi0[p].m[1] = chi[1][0];
+        Chi0[p].m[2] = chi[0][1];
+        Chi0[p].m[3] = chi[1][1];
     }
+    put_scan_tables<T>(blob, pl, 2, Phi, Psi, Chi0);
 }
 
 template <typename T>
@@ -332,23 +472,63 @@ void free_handle(Handle *h)
     delete h;
 }
 
-size_t slot_smem(const DtypePlan &pl, int kind, int vec)
+// The partitioned plan keeps the whole coefficient image, the exchange area and (TMA variant) the
+// prefetch ring in shared memory; the per-CTA limit of sm_100a is 227 KB.
+constexpr size_t SMEM_LIMIT = 227 * 1024;
+
+size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+// shared-memory layout of one kernel variant: [blob][exchange][mbarriers][ring]
+void layout_slot(const DtypePlan &pl, const Shape &sh, int kind, KernelSlot &sl)
 {
     const int NC = (kind == KIND_TRI) ? 1 : 2;
-    const size_t W = (size_t)pl.lanes * vec;
-    const size_t xch = (pl.P > 1) ? (size_t)pl.tpc * 2 * pl.P * NC * W * pl.elem : 0;
-    return (size_t)pl.blob_bytes + xch;
+    const size_t W = (size_t)sh.lanes * sl.vec;
+    sl.xW = (int)(W | 1);  // odd row length: the scan lanes read a column without bank conflicts
+    const size_t xch = (pl.P > 1) ? (size_t)sh.tpc * 2 * NC * pl.P * sl.xW * pl.elem : 0;
+    sl.offX = (unsigned)align16(pl.blob_bytes);
+    sl.offM = (unsigned)align16(sl.offX + xch);
+    sl.offR = (unsigned)align_up(sl.offM + 16 * 8, 128);
+    // TMA boxes of whole partitions: the largest divisor g of P with g*rows <= 256 rows per box
+    const size_t Np = (size_t)pl.P * pl.rows;
+    int g = 256 / pl.rows < pl.P ? 256 / pl.rows : pl.P;
+    while (pl.P % g != 0) --g;
+    sl.box_rows = (unsigned)(g * pl.rows);
+    sl.nboxes = (unsigned)(pl.P / g);
+    const size_t ring = (size_t)sh.tpc * Np * W * pl.elem;
+    sl.smem = sl.tma ? sl.offR + ring : sl.offM;
 }
 
-// The partitioned plan keeps the whole coefficient image plus the exchange area in shared memory;
-// beyond the per-CTA limit of sm_100a (227 KB) the handle falls back to the two-pass kernel.
-constexpr size_t SMEM_LIMIT = 227 * 1024;
+bool tma_possible(const DtypePlan &pl, const Shape &sh, int vec)
+{
+    const size_t wb = (size_t)sh.lanes * vec * pl.elem;  // bytes of one tile row
+    if (g_tune.prefetch == 0) return false;
+    if (pl.P > 1 && !pl.ws) return false;       // the serial carry walk has no TMA variant
+    if (wb % 16 != 0 || sh.lanes * vec > 256) return false;
+    return true;
+}
+
+SweepEntry find_sweep(int kind, int elem_bytes, int vec, int rows, int single, int tma, int ws)
+{
+    if (elem_bytes == 8) {
+        if (kind == KIND_TRI) return find_sweep_tri_f64(vec, rows, single, tma, ws);
+        if (kind == KIND_PENTA) return find_sweep_penta_f64(vec, rows, single, tma, ws);
+        return find_sweep_ch_f64(vec, rows, single, tma, ws);
+    }
+    if (kind == KIND_TRI) return find_sweep_tri_f32(vec, rows, single, tma, ws);
+    if (kind == KIND_PENTA) return find_sweep_penta_f32(vec, rows, single, tma, ws);
+    return find_sweep_ch_f32(vec, rows, single, tma, ws);
+}
 
 void fit_plan(DtypePlan &pl, int handle_kind)
 {
     if (pl.two_pass) return;
-    if (slot_smem(pl, handle_kind, pl.vec) > SMEM_LIMIT) pl.vec = 1;
-    if (slot_smem(pl, handle_kind, pl.vec) > SMEM_LIMIT) pl.two_pass = true;
+    for (int k = 0; k < (handle_kind == KIND_TRI ? 1 : 2); ++k) {
+        KernelSlot probe;
+        probe.vec = 1;
+        probe.tma = 0;
+        layout_slot(pl, pl.shape[k], handle_kind, probe);
+        if (probe.smem > SMEM_LIMIT) pl.two_pass = true;
+    }
 }
 
 void fill_slots(Handle *h)
@@ -365,21 +545,26 @@ void fill_slots(Handle *h)
             } else {
                 kind = (ks == 0) ? KIND_PENTA : KIND_CH;
             }
+            const Shape &sh = pl.shape[ks];
             for (int s = 0; s < 2; ++s) {
-                const int vec = (s == 0) ? pl.vec : 1;
-                KernelSlot &sl = pl.k[ks][s];
-                sl.vec = vec;
-                if (kind == KIND_TRI) sl.ent = find_sweep_tri(pl.elem, vec, pl.rows, single);
-                else if (kind == KIND_PENTA) sl.ent = find_sweep_penta(pl.elem, vec, pl.rows, single);
-                else sl.ent = find_sweep_ch(pl.elem, vec, pl.rows, single);
-                sl.smem = slot_smem(pl, kind, vec);
-                sl.max_grid = 0;
+                for (int d = 0; d < 2; ++d) {
+                    KernelSlot &sl = pl.k[ks][s][d];
+                    sl.vec = (s == 0) ? sh.vec : 1;
+                    sl.tma = (d == 0) ? 1 : 0;
+                    sl.ent = SweepEntry{nullptr, nullptr, 0};
+                    sl.max_grid = 0;
+                    if (sl.tma && !tma_possible(pl, sh, sl.vec)) continue;
+                    layout_slot(pl, sh, kind, sl);
+                    if (sl.smem > SMEM_LIMIT) continue;
+                    sl.ent = find_sweep(kind, pl.elem, sl.vec, pl.rows, single, sl.tma, pl.ws);
+                    if (sl.ent.func && sl.ent.max_threads < sh.threads) sl.ent = SweepEntry{nullptr, nullptr, 0};
+                }
             }
         }
     }
 }
 
-int resolve_slot(Handle *h, const DtypePlan &pl, KernelSlot &sl)
+int resolve_slot(Handle *h, const Shape &sh, KernelSlot &sl)
 {
     std::lock_guard<std::mutex> lk(h->mu);
     if (sl.max_grid > 0) return BTPS_OK;
@@ -389,13 +574,58 @@ int resolve_slot(Handle *h, const DtypePlan &pl, KernelSlot &sl)
     int occ = 0, sms = 0, dev = 0;
     CU_TRY(cudaGetDevice(&dev));
     CU_TRY(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
-    CU_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, sl.ent.func, pl.threads, sl.smem));
+    CU_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, sl.ent.func, sh.threads, sl.smem));
     if (occ < 1) {
-        snprintf(tl_cuda_msg, sizeof(tl_cuda_msg), "kernel does not fit: %d threads, %zu B smem", pl.threads,
+        snprintf(tl_cuda_msg, sizeof(tl_cuda_msg), "kernel does not fit: %d threads, %zu B smem", sh.threads,
                  sl.smem);
         return set_err(BTPS_E_CUDA);
     }
     sl.max_grid = occ * sms;
+    return BTPS_OK;
+}
+
+// cuTensorMapEncodeTiled through the runtime's driver entry point (libcuda is not linked)
+typedef CUresult (*encode_tiled_fn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
+                                    const cuuint64_t *, const cuuint32_t *, const cuuint32_t *,
+                                    CUtensorMapInterleave, CUtensorMapSwizzle, CUtensorMapL2promotion,
+                                    CUtensorMapFloatOOBfill);
+
+encode_tiled_fn get_encode()
+{
+    static encode_tiled_fn fn = []() -> encode_tiled_fn {
+        void *p = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) != cudaSuccess ||
+            q != cudaDriverEntryPointSuccess)
+            return nullptr;
+        return (encode_tiled_fn)p;
+    }();
+    return fn;
+}
+
+// 2-D view of the interleaved batch for TMA: dim 0 = systems (contiguous), dim 1 = rows
+template <typename T>
+int make_tmap(CUtensorMap *tm, T *d_rhs, long long batch, int n, int W, unsigned box_rows)
+{
+    encode_tiled_fn enc = get_encode();
+    if (!enc) {
+        snprintf(tl_cuda_msg, sizeof(tl_cuda_msg), "cuTensorMapEncodeTiled is not available");
+        return set_err(BTPS_E_CUDA);
+    }
+    const cuuint64_t dims[2] = {(cuuint64_t)batch, (cuuint64_t)n};
+    const cuuint64_t strides[1] = {(cuuint64_t)batch * sizeof(T)};
+    const cuuint32_t box[2] = {(cuuint32_t)W, (cuuint32_t)box_rows};
+    const cuuint32_t estr[2] = {1, 1};
+    const CUresult r = enc(tm, sizeof(T) == 8 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2,
+                           (void *)d_rhs, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                           CU_TENSOR_MAP_SWIZZLE_NONE,
+                           (size_t)W * sizeof(T) >= 256 ? CU_TENSOR_MAP_L2_PROMOTION_L2_256B
+                                                        : CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+                           CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) {
+        snprintf(tl_cuda_msg, sizeof(tl_cuda_msg), "cuTensorMapEncodeTiled failed (%d)", (int)r);
+        return set_err(BTPS_E_CUDA);
+    }
     return BTPS_OK;
 }
 
@@ -418,36 +648,60 @@ int launch_one(Handle *h, int kind, T *d_rhs, long long batch, double alpha_x, i
         return BTPS_OK;
     }
     const int ks = (kind == KIND_CH) ? 1 : 0;
-    // the vectorised kernel needs whole vectors: batch % vec == 0 and an aligned base pointer
+    const Shape &sh = pl.shape[ks];
+    // the vectorised kernels need whole vectors: batch % vec == 0 and an aligned base pointer;
+    // TMA needs a 16-byte aligned base and row pitch
     int s = 0;
-    if (pl.vec > 1) {
-        const bool ok = (batch % pl.vec == 0) && (((uintptr_t)d_rhs % (sizeof(T) * pl.vec)) == 0);
+    if (sh.vec > 1) {
+        const bool ok = (batch % sh.vec == 0) && (((uintptr_t)d_rhs % (sizeof(T) * sh.vec)) == 0);
         if (!ok) s = 1;
     }
-    KernelSlot &sl = pl.k[ks][s];
+    const bool tma_ok = (((uintptr_t)d_rhs % 16) == 0) && ((((size_t)batch * sizeof(T)) % 16) == 0) &&
+                        (batch < (1ll << 31));
+    int d = (tma_ok && pl.k[ks][s][0].ent.func) ? 0 : 1;
+    if (!pl.k[ks][s][d].ent.func && s == 0) s = 1;  // e.g. the wide variant has no direct-load twin that fits
+    if (!pl.k[ks][s][d].ent.func) d = 1;
+    KernelSlot &sl = pl.k[ks][s][d];
+    if (!sl.ent.func) {
+        snprintf(tl_cuda_msg, sizeof(tl_cuda_msg), "no kernel variant for this plan");
+        return set_err(BTPS_E_CUDA);
+    }
     if (sl.max_grid == 0) {
-        const int rc = resolve_slot(h, pl, sl);
+        const int rc = resolve_slot(h, sh, sl);
         if (rc != BTPS_OK) return rc;
     }
     SweepArgs a;
     a.rhs = d_rhs;
     a.blob = pl.d_blob;
     a.batch = batch;
-    const long long W = (long long)pl.lanes * sl.vec;
+    const long long W = (long long)sh.lanes * sl.vec;
     a.num_tiles = (batch + W - 1) / W;
     a.alpha_x = alpha_x;
     a.n = h->n;
     a.P = pl.P;
-    a.lanes = pl.lanes;
-    a.lanes_log2 = pl.lanes_log2;
-    a.tpc = pl.tpc;
+    a.lanes = sh.lanes;
+    a.lanes_log2 = sh.lanes_log2;
+    a.tpc = sh.tpc;
     a.reverse = reverse;
+    a.scan_log2 = pl.scan_log2;
+    a.xW = sl.xW;
+    a.tq = pl.tq;
     a.blob_bytes = pl.blob_bytes;
-    a.offS = pl.offS;
-    a.offX = pl.blob_bytes;
-    long long grid = (a.num_tiles + pl.tpc - 1) / pl.tpc;
+    a.offT = pl.offT;
+    a.offX = sl.offX;
+    a.offM = sl.offM;
+    a.offR = sl.offR;
+    a.box_rows = sl.box_rows;
+    a.nboxes = sl.nboxes;
+    CUtensorMap tm;
+    memset(&tm, 0, sizeof(tm));
+    if (sl.tma) {
+        const int rc = make_tmap<T>(&tm, d_rhs, batch, h->n, (int)W, sl.box_rows);
+        if (rc != BTPS_OK) return rc;
+    }
+    long long grid = (a.num_tiles + sh.tpc - 1) / sh.tpc;
     if (grid > sl.max_grid) grid = sl.max_grid;
-    const cudaError_t e = sl.ent.launch(a, (int)grid, pl.threads, sl.smem, st);
+    const cudaError_t e = sl.ent.launch(a, tm, (int)grid, sh.threads, sl.smem, st, g_tune.pdl != 0);
     g_launches.fetch_add(1, std::memory_order_relaxed);
     if (e != cudaSuccess) return cuda_fail(e, "sweep launch");
     return BTPS_OK;
@@ -567,7 +821,7 @@ tri_handle_t tri_factor(int n, const double *a, const double *b, const double *c
     h->device = 0;
     for (int t = 0; t < 2; ++t) {
         DtypePlan &pl = h->plan[t];
-        choose_plan(n, t == 0 ? 8 : 4, pl);
+        choose_plan(n, t == 0 ? 8 : 4, h->kind, pl);
         std::vector<unsigned char> blob, soa;
         if (t == 0) {
             build_blob_tri<double>(n, pl, inv, nl, nch, blob);
@@ -614,7 +868,7 @@ penta_handle_t penta_factor(int n, const double *e, const double *a, const doubl
     h->device = 0;
     for (int t = 0; t < 2; ++t) {
         DtypePlan &pl = h->plan[t];
-        choose_plan(n, t == 0 ? 8 : 4, pl);
+        choose_plan(n, t == 0 ? 8 : 4, h->kind, pl);
         std::vector<unsigned char> blob, soa;
         if (t == 0) {
             build_blob_penta<double>(n, pl, inv, nle, nlb, ngam, ndel, blob);
@@ -704,16 +958,21 @@ const char *btps_error_string(int code)
 int btps_plan_info(int kind, const void *handle, int elem_bytes, int *out)
 {
     Handle *h = check(handle, kind == 0 ? MAGIC_TRI : MAGIC_PENTA);
-    if (!h || !out || (elem_bytes != 8 && elem_bytes != 4)) return set_err(BTPS_E_ARG);
+    if (!h || !out || (elem_bytes != 8 && elem_bytes != 4) || kind < 0 || kind > 2) return set_err(BTPS_E_ARG);
     const DtypePlan &pl = h->plan[elem_bytes == 8 ? 0 : 1];
+    const int ks = (kind == 2) ? 1 : 0;
+    const Shape &sh = pl.shape[ks];
+    const KernelSlot &sl = pl.k[ks][0][0].ent.func ? pl.k[ks][0][0] : pl.k[ks][0][1];
     out[0] = pl.two_pass ? 0 : pl.rows;
     out[1] = pl.two_pass ? 1 : pl.P;
-    out[2] = pl.two_pass ? 128 : pl.lanes;
-    out[3] = pl.two_pass ? 1 : pl.vec;
-    out[4] = pl.two_pass ? 1 : pl.tpc;
-    out[5] = pl.two_pass ? 128 : pl.threads;
-    out[6] = pl.two_pass ? 0 : (int)pl.k[0][0].smem;
+    out[2] = pl.two_pass ? 128 : sh.lanes;
+    out[3] = pl.two_pass ? 1 : sh.vec;
+    out[4] = pl.two_pass ? 1 : sh.tpc;
+    out[5] = pl.two_pass ? 128 : sh.threads;
+    out[6] = pl.two_pass ? 0 : (int)sl.smem;
     out[7] = pl.two_pass ? (int)pl.soa_bytes : (int)pl.blob_bytes;
+    out[8] = pl.two_pass ? 0 : sl.tma;
+    out[9] = pl.two_pass ? 0 : pl.ws;
     return set_err(BTPS_OK);
 }
 
@@ -726,6 +985,9 @@ int btps_tune(const char *key, int value)
     else if (!strcmp(key, "tiles_per_cta")) g_tune.tpc = value;
     else if (!strcmp(key, "force_two_pass")) g_tune.force_two_pass = value;
     else if (!strcmp(key, "reverse")) g_tune.reverse = value;
+    else if (!strcmp(key, "prefetch")) g_tune.prefetch = value;
+    else if (!strcmp(key, "pdl")) g_tune.pdl = value;
+    else if (!strcmp(key, "warp_scan")) g_tune.warp_scan = value;
     else return set_err(BTPS_E_ARG);
     return set_err(BTPS_OK);
 }

@@ -1,48 +1,71 @@
 // inst_common.cuh -- explicit-instantiation helper shared by the inst_*.cu units (one unit per
-// kind so that nvcc compiles them in parallel).
+// kind and element type so that nvcc compiles them in parallel).
 #pragma once
 #include "sweep.cuh"
 
 namespace btps {
 
-template <typename T, int V, int MR, bool SINGLE, int KIND>
+template <typename T, int V, int MR, bool SINGLE, int KIND, bool TMA, bool WS>
 static SweepEntry make_entry()
 {
     SweepEntry e;
-    e.launch = &launch_sweep<T, V, MR, SINGLE, KIND>;
-    e.func = reinterpret_cast<const void *>(&sweep_kernel<T, V, MR, SINGLE, KIND>);
+    e.launch = &launch_sweep<T, V, MR, SINGLE, KIND, TMA, WS>;
+    e.func = reinterpret_cast<const void *>(&sweep_kernel<T, V, MR, SINGLE, KIND, TMA, WS>);
+    e.max_threads = CtaShape<T, V, MR>::MAX_THREADS;
     return e;
 }
 
+// variants: single partition (no carries) with / without TMA; partitioned with the warp scan
+// (with / without TMA) or with the serial carry walk (direct loads only)
+template <typename T, int V, int MR, int KIND>
+static SweepEntry pick_variant(int single, int tma, int ws)
+{
+    if (single) return tma ? make_entry<T, V, MR, true, KIND, true, false>() : make_entry<T, V, MR, true, KIND, false, false>();
+    if (ws) return tma ? make_entry<T, V, MR, false, KIND, true, true>() : make_entry<T, V, MR, false, KIND, false, true>();
+    if (!tma) return make_entry<T, V, MR, false, KIND, false, false>();
+    SweepEntry none = {nullptr, nullptr, 0};
+    return none;
+}
+
 template <typename T, int V, int KIND>
-static SweepEntry pick_rows(int rows, int single)
+static SweepEntry pick_rows(int rows, int single, int tma, int ws)
 {
     switch (rows) {
-        case 8: return single ? make_entry<T, V, 8, true, KIND>() : make_entry<T, V, 8, false, KIND>();
-        case 16: return single ? make_entry<T, V, 16, true, KIND>() : make_entry<T, V, 16, false, KIND>();
-        case 32: return single ? make_entry<T, V, 32, true, KIND>() : make_entry<T, V, 32, false, KIND>();
+        case 8: return pick_variant<T, V, 8, KIND>(single, tma, ws);
+        case 16: return pick_variant<T, V, 16, KIND>(single, tma, ws);
+        case 32: return pick_variant<T, V, 32, KIND>(single, tma, ws);
         default: break;
     }
-    SweepEntry none = {nullptr, nullptr};
+    SweepEntry none = {nullptr, nullptr, 0};
     return none;
 }
 
 template <int KIND>
-static SweepEntry pick_all(int elem_bytes, int vec, int rows, int single)
+static SweepEntry pick_f64(int vec, int rows, int single, int tma, int ws)
 {
-    if (elem_bytes == 8) {
-        if (vec == 1) return pick_rows<double, 1, KIND>(rows, single);
-        if (vec == 2) return pick_rows<double, 2, KIND>(rows, single);
-    } else if (elem_bytes == 4) {
-        if (vec == 1) return pick_rows<float, 1, KIND>(rows, single);
-        if (vec == 2) return pick_rows<float, 2, KIND>(rows, single);
-    }
-    SweepEntry none = {nullptr, nullptr};
+    if (vec == 1) return pick_rows<double, 1, KIND>(rows, single, tma, ws);
+    if (vec == 2) return pick_rows<double, 2, KIND>(rows, single, tma, ws);
+    SweepEntry none = {nullptr, nullptr, 0};
     return none;
 }
 
-SweepEntry find_sweep_tri(int elem_bytes, int vec, int rows, int single);
-SweepEntry find_sweep_penta(int elem_bytes, int vec, int rows, int single);
-SweepEntry find_sweep_ch(int elem_bytes, int vec, int rows, int single);
+template <int KIND>
+static SweepEntry pick_f32(int vec, int rows, int single, int tma, int ws)
+{
+    if (vec == 1) return pick_rows<float, 1, KIND>(rows, single, tma, ws);
+    if (vec == 2) return pick_rows<float, 2, KIND>(rows, single, tma, ws);
+    if (vec == 4) return pick_rows<float, 4, KIND>(rows, single, tma, ws);
+    SweepEntry none = {nullptr, nullptr, 0};
+    return none;
+}
+
+// kind in {TRI, PENTA, CH}; elem_bytes 8: vec in {1, 2}; 4: vec in {1, 2, 4}; rows in {8, 16, 32}
+SweepEntry find_sweep(int kind, int elem_bytes, int vec, int rows, int single, int tma, int ws);
+SweepEntry find_sweep_tri_f64(int vec, int rows, int single, int tma, int ws);
+SweepEntry find_sweep_tri_f32(int vec, int rows, int single, int tma, int ws);
+SweepEntry find_sweep_penta_f64(int vec, int rows, int single, int tma, int ws);
+SweepEntry find_sweep_penta_f32(int vec, int rows, int single, int tma, int ws);
+SweepEntry find_sweep_ch_f64(int vec, int rows, int single, int tma, int ws);
+SweepEntry find_sweep_ch_f32(int vec, int rows, int single, int tma, int ws);
 
 }  // namespace btps

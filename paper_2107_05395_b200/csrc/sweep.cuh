@@ -8,23 +8,36 @@
 //   ch    : f_i = c_i + alpha_x (w_{i-1} - 2 w_i + w_{i+1}), w = c^3 - c, then the penta sweeps
 //           PAPER.md:365-392 (eq. 24, 25a, 26c), truncated stencil (C-18, C-21).
 //
-// How: the paper gives one thread a whole system and writes
-// g to global memory between the sweeps (2 reads + 2 writes per element).  Here a tile of W
-// adjacent systems is owned by P*lanes threads: thread (part, lane) keeps rows
-// [part*MR, part*MR+MR) of V adjacent systems in registers, so HBM sees one read and one
-// write per element.  Both recurrences are linear, so each partition sweeps locally with zero
-// incoming carries and the true carries are recovered by a short scan over partitions through
-// shared memory; because A is shared, the partition response vectors (Phi, chi, Psi) depend
-// on the LHS only and are part of the factor tables ("blob") staged into shared memory once
-// per CTA.  Divisions are replaced by factor-time reciprocals and the elimination multipliers
-// are pre-negated so that each row costs one multiply and FMAs (C-16).
+// How: the paper gives one thread a whole system and writes g to global
+// memory between the sweeps (2 reads + 2 writes per element).  Here a tile of W adjacent systems
+// is owned by a GROUP of P*lanes threads: thread (part, lane) keeps rows [part*MR, part*MR+MR) of
+// V adjacent systems in registers, so HBM sees one read and one write per element.  Both
+// recurrences are linear, so each partition sweeps locally with zero incoming carries; the true
+// carries across the P partitions follow from an affine scan  G_{q+1} = g^last_q + Phi_q G_q
+// (and its mirror image for the back substitution).  Because A is shared, Phi_q and all products
+// of Phi's depend on the LHS only: the scan is run as a log2(P)-step Kogge-Stone scan over the
+// lanes of one warp (__shfl) with multipliers precomputed at factor time, and the per-row
+// response vectors (chi, psi) that turn the carries into the final correction are part of the
+// factor tables ("blob") staged into shared memory once per CTA.  Divisions are replaced by
+// factor-time reciprocals and the elimination multipliers are pre-negated so that each row
+// costs one multiply and FMAs (C-16).
+//
+// Data movement: the NEXT tile of a group is fetched by TMA (cp.async.bulk.tensor.2d, one box of
+// [rows x W systems] per 256 rows, completion on an mbarrier) into a shared-memory ring while the
+// current tile is swept in registers; results are stored straight from registers (coalesced).
+// When the batch pitch or base pointer is not 16-byte aligned the same kernel body runs with
+// direct (non-prefetched) global loads instead.
 #pragma once
+#include <cuda.h>
 #include <cuda_runtime.h>
 #include <stdint.h>
 
 namespace btps {
 
 enum Kind { KIND_TRI = 0, KIND_PENTA = 1, KIND_CH = 2 };
+
+constexpr int SCAN_STEPS = 5;   // Kogge-Stone steps held in the tables (scan width <= 32)
+constexpr int SCAN_LANES = 32;
 
 struct SweepArgs {
     void *rhs;             // device, n*batch elements, interleaved
@@ -36,11 +49,18 @@ struct SweepArgs {
     int P;                 // partitions per system (rows padded to P*MR with identity rows)
     int lanes;             // threads side by side on adjacent systems (power of two <= 32)
     int lanes_log2;
-    int tpc;               // tiles processed concurrently by one CTA
+    int tpc;               // tile groups per CTA (each walks its own tiles)
     int reverse;           // 1: walk the tiles from the last to the first
+    int scan_log2;         // warp scan: log2 of the scan width (smallest power of two >= P)
+    int xW;                // padded (odd) row length of the exchange area, in elements
+    int tq;                // partitions per scan-table row (max(32, P))
     unsigned blob_bytes;   // multiple of 16
-    unsigned offS;         // byte offset of the per-partition table inside the blob (row records start at 0)
-    unsigned offX;         // byte offset of the exchange area in shared memory (after the blob)
+    unsigned offT;         // byte offset of the scan tables inside the blob (row records start at 0)
+    unsigned offX;         // byte offset of the exchange area in shared memory
+    unsigned offM;         // byte offset of the per-group mbarriers (TMA kernels)
+    unsigned offR;         // byte offset of the prefetch ring (TMA kernels), 128-B aligned
+    unsigned box_rows;     // rows per TMA box (<= 256)
+    unsigned nboxes;       // boxes per tile = ceil(P*MR / box_rows)
 };
 
 template <typename T, int N>
@@ -48,7 +68,7 @@ struct alignas((sizeof(T) * N) <= 16 ? (sizeof(T) * N) : 16) Tup {
     T v[N];
 };
 
-// ---- global memory access for V adjacent systems -------------------------------------------
+// ---- access to V adjacent systems (global or shared) ------------------------------------------
 template <typename T, int V>
 __device__ __forceinline__ void ld_sys(T (&d)[V], const T *p)
 {
@@ -92,23 +112,97 @@ __device__ __forceinline__ T ch_w(T c) { return fma_t<T>(c * c, c, -c); }
 //           sweeps to the incoming forward / backward carry
 //   penta record = 5 pairs: {inv, nle} {nlb, 0} {ngam, ndel} {chi1, chi2} {psi1, psi2}
 //           inv = 1/alpha_i, nle = -eps_i/alpha_i, nlb = -beta_i/alpha_i, ngam = -gamma_i, ndel = -delta_i
-// followed at offS by one entry per partition (forward response at the partition's last rows):
-//   tri   {phi_last, 0};   penta {phi1_last, phi2_last} {phi1_prev, phi2_prev}
+// followed at offT by the carry-scan tables, indexed [slot][m][q] with q = partition (32 entries),
+// m = entry of the NC x NC matrix (row-major), NC = 1 (tri) or 2 (penta):
+//   slot 2*s     : forward  multiplier of Kogge-Stone step s, A^(s)_q = Phi_q Phi_{q-1} ... (2^s factors),
+//                  zero where q < 2^s
+//   slot 2*s + 1 : backward multiplier of step s, B^(s)_q = Psi_q Psi_{q+1} ..., zero where q + 2^s >= P
+//   slot 2*SCAN_STEPS : chi at the partition's first NC rows (turns the forward carry into the
+//                  local back-substitution's value at those rows)
 template <int KIND>
 struct RecLayout {
     static constexpr int PAIRS = (KIND == KIND_TRI) ? 3 : 5;   // pairs per row record
-    static constexpr int SPAIRS = (KIND == KIND_TRI) ? 1 : 2;  // pairs per partition entry
+    static constexpr int NC = (KIND == KIND_TRI) ? 1 : 2;      // carries per direction
+    static constexpr int SCAN_SLOTS = 2 * SCAN_STEPS + 1;
+    static constexpr int SCAN_ELEMS = SCAN_SLOTS * NC * NC * SCAN_LANES;
 };
 
-template <typename T, int V, int MR, bool SINGLE, int KIND>
-__global__ void __launch_bounds__(512, 1) sweep_kernel(const SweepArgs a)
+// ---- TMA / mbarrier primitives (PTX) -------------------------------------------------------------
+__device__ __forceinline__ unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(unsigned bar, unsigned count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(unsigned bar, unsigned bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned bar, unsigned parity)
+{
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_%=:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra DONE_%=;\n"
+        "bra WAIT_%=;\n"
+        "DONE_%=:\n"
+        "}\n" ::"r"(bar), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void tma_load_2d(unsigned dst, const CUtensorMap *tm, int c0, int c1, unsigned bar)
+{
+    asm volatile(
+        "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];"
+        ::"r"(dst), "l"(tm), "r"(c0), "r"(c1), "r"(bar) : "memory");
+}
+
+// Barrier over the threads of one tile group.  A CTA hosts `tpc` groups that walk their tiles
+// independently of one another (so one group's arithmetic overlaps another group's waits); a
+// group of one warp synchronises with __syncwarp, one group per CTA with the CTA barrier, and
+// otherwise each group owns the named barrier 1 + sub.
+__device__ __forceinline__ void group_sync(int tpc, int sub, int count)
+{
+    if (count == 32) __syncwarp();
+    else if (tpc == 1) __syncthreads();
+    else asm volatile("bar.sync %0, %1;" ::"r"(sub + 1), "r"(count) : "memory");
+}
+
+// threads per CTA the kernel is compiled for: 128 registers per thread (512 threads) while the
+// tile rows of a thread fit in 64 registers, else 255 registers (256 threads)
+template <typename T, int V, int MR>
+struct CtaShape {
+    static constexpr bool WIDE = (sizeof(T) * V * MR > 256);
+    static constexpr int MAX_THREADS = WIDE ? 256 : 512;
+};
+
+// -----------------------------------------------------------------------------------------------
+// sweep_kernel<T, V, MR, SINGLE, KIND, TMA, WS>
+//   V      systems per thread (adjacent, one vector access)
+//   MR     rows per thread (= rows per partition)
+//   SINGLE P == 1: no carries to exchange
+//   TMA    next tile prefetched by TMA into the shared-memory ring (else direct global loads)
+//   WS     carries by the warp-shuffle scan (needs P <= 32 and whole-warp groups); else each
+//          thread walks the partitions before / after it serially (any P)
+// -----------------------------------------------------------------------------------------------
+template <typename T, int V, int MR, bool SINGLE, int KIND, bool TMA, bool WS>
+__global__ void __launch_bounds__(CtaShape<T, V, MR>::MAX_THREADS, 1)
+sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
 {
     constexpr bool TRI = (KIND == KIND_TRI);
-    constexpr int NC = TRI ? 1 : 2;  // carries per direction
+    constexpr int NC = RecLayout<KIND>::NC;
     constexpr int RP = RecLayout<KIND>::PAIRS;
-    constexpr int SP = RecLayout<KIND>::SPAIRS;
     using Pair = Tup<T, 2>;
-    extern __shared__ __align__(16) unsigned char smem[];
+    extern __shared__ __align__(128) unsigned char smem[];
+
+    const int W = a.lanes * V;
+    const int tpt = a.P * a.lanes;  // threads per tile group (SINGLE: P == 1)
+    const int sub = SINGLE ? (threadIdx.x >> a.lanes_log2) : (threadIdx.x / tpt);
+    const int lt = SINGLE ? (threadIdx.x & (a.lanes - 1)) : (threadIdx.x - sub * tpt);
+    const int part = SINGLE ? 0 : (lt >> a.lanes_log2);
+    const int sl = lt & (a.lanes - 1);
+    const int r0 = part * MR;
+    const long long batch = a.batch;
 
     // ---- stage the coefficient image once per CTA ------------------------------------------
     {
@@ -117,42 +211,80 @@ __global__ void __launch_bounds__(512, 1) sweep_kernel(const SweepArgs a)
         const unsigned nvec = a.blob_bytes >> 4;
         for (unsigned i = threadIdx.x; i < nvec; i += blockDim.x) dst[i] = __ldg(src + i);
     }
+    [[maybe_unused]] const unsigned mbar = smem_u32(smem + a.offM) + 8u * sub;
+    if constexpr (TMA) {
+        if (lt == 0) mbar_init(mbar, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
     __syncthreads();
+    // Programmatic dependent launch (time-step loops): everything above overlaps the tail of the
+    // previous launch on the stream; the batch itself is only touched after the wait.  Both
+    // instructions are no-ops for a launch without the attribute.
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+    asm volatile("griddepcontrol.wait;" ::: "memory");
 
-    const int W = a.lanes * V;
-    const int tpt = a.P * a.lanes;  // threads per tile
-    const int sub = SINGLE ? (threadIdx.x >> a.lanes_log2) : (threadIdx.x / tpt);
-    const int lt = SINGLE ? (threadIdx.x & (a.lanes - 1)) : (threadIdx.x - sub * tpt);
-    const int part = SINGLE ? 0 : (lt >> a.lanes_log2);
-    const int sl = lt & (a.lanes - 1);
-    const int r0 = part * MR;
-    const long long batch = a.batch;
+    // rows of this partition that exist
+    int nrow_part = a.n - r0;
+    nrow_part = nrow_part < 0 ? 0 : (nrow_part > MR ? MR : nrow_part);
 
-    const Pair *const Rall = reinterpret_cast<const Pair *>(smem);   // all row records
-    const Pair *const R = Rall + (size_t)r0 * RP;                    // this partition's records
-    const Pair *const S = reinterpret_cast<const Pair *>(smem + a.offS);
-    // exchange area: [tpc][2 (g-last | u-first)][P][NC][W]; this thread's column inside it
-    T *const xg = reinterpret_cast<T *>(smem + a.offX) + (size_t)sub * 2 * a.P * NC * W + sl * V;
-    const int xu_off = a.P * NC * W;
+    const Pair *const R = reinterpret_cast<const Pair *>(smem) + (size_t)r0 * RP;  // this partition's records
+    [[maybe_unused]] const Pair *const Rall = reinterpret_cast<const Pair *>(smem);
+    [[maybe_unused]] const T *const TAB = reinterpret_cast<const T *>(smem + a.offT);
+    // exchange area of this group: [2*NC values][P][xW]
+    [[maybe_unused]] T *const xb = reinterpret_cast<T *>(smem + a.offX) + (size_t)sub * 2 * NC * a.P * a.xW;
+    // prefetch ring of this group: [P*MR rows][W]
+    [[maybe_unused]] const unsigned ring_bytes = (unsigned)(a.P * MR * W) * (unsigned)sizeof(T);
+    [[maybe_unused]] T *const ring = reinterpret_cast<T *>(smem + a.offR + (size_t)sub * ring_bytes);
 
     const int ntiles = (int)a.num_tiles;
     const int stride_tiles = gridDim.x * a.tpc;
-    for (int base = blockIdx.x * a.tpc; base < ntiles; base += stride_tiles) {
-        int tile = base + sub;
-        const bool tile_ok = tile < ntiles;
-        if (a.reverse) tile = ntiles - 1 - tile;
-        const long long j = (long long)tile * W + (long long)sl * V;
-        const bool act = tile_ok && (j < batch);  // V > 1 requires batch % V == 0
-        // rows of this partition that exist and are touched by this thread
-        int nrow = a.n - r0;
-        nrow = nrow < 0 ? 0 : (nrow > MR ? MR : nrow);
-        if (!act) nrow = 0;
-        T *const p0 = reinterpret_cast<T *>(a.rhs) + (long long)r0 * batch + j;
+    T *const rhs0 = reinterpret_cast<T *>(a.rhs) + (long long)r0 * batch + (long long)sl * V;
 
-        // ---- load: all MR rows issued back to back (independent of the recurrence) ---------
-        // (one running row pointer: keeping MR separate 64-bit addresses alive would cost 2*MR registers)
+    // one thread of the group asks the TMA unit for tile `t` (walking order); columns beyond the
+    // batch and rows beyond n are zero-filled by the unit
+    auto tma_issue = [&](int t) {
+        const int tile = a.reverse ? ntiles - 1 - t : t;
+        mbar_expect_tx(mbar, ring_bytes);
+        const unsigned dst = smem_u32(ring);
+        const unsigned box_bytes = a.box_rows * (unsigned)W * (unsigned)sizeof(T);
+        for (unsigned b = 0; b < a.nboxes; ++b)
+            tma_load_2d(dst + b * box_bytes, &tmap, tile * W, (int)(b * a.box_rows), mbar);
+    };
+
+    int t = blockIdx.x * a.tpc + sub;
+    [[maybe_unused]] unsigned phase = 0;
+    if constexpr (TMA) {
+        if (lt == 0 && t < ntiles) tma_issue(t);
+    }
+    for (; t < ntiles; t += stride_tiles) {
+        const int tile = a.reverse ? ntiles - 1 - t : t;
+        const long long j = (long long)tile * W + (long long)sl * V;
+        const bool act = (j < batch);  // V > 1 requires batch % V == 0
+        const int nrow = act ? nrow_part : 0;  // rows stored by this thread
+        T *const p0 = rhs0 + (long long)tile * W;
+
         T v[MR][V];
-        {
+        [[maybe_unused]] T cm[V], cp[V];  // CH halo rows r0-1 and r0+MR (c^n)
+        if constexpr (TMA) {
+            // ---- take the prefetched tile out of the ring, then have it refilled ---------------
+            mbar_wait(mbar, phase);
+            phase ^= 1u;
+            const T *const rp = ring + (r0 * W + sl * V);
+#pragma unroll
+            for (int k = 0; k < MR; ++k) ld_sys<T, V>(v[k], rp + k * W);
+            if constexpr (KIND == KIND_CH) {
+#pragma unroll
+                for (int e = 0; e < V; ++e) cm[e] = cp[e] = T(0);
+                if constexpr (!SINGLE) {
+                    if (part > 0) ld_sys<T, V>(cm, rp - W);
+                    if (part + 1 < a.P) ld_sys<T, V>(cp, rp + MR * W);
+                }
+            }
+            group_sync(a.tpc, sub, tpt);  // every thread has drained the ring
+            if (lt == 0 && t + stride_tiles < ntiles) tma_issue(t + stride_tiles);
+        } else {
+            // ---- load: all MR rows issued back to back (independent of the recurrence) ---------
+            // (one running row pointer: keeping MR separate 64-bit addresses alive would cost 2*MR registers)
             const T *pl = p0;
 #pragma unroll
             for (int k = 0; k < MR; ++k) {
@@ -164,9 +296,17 @@ __global__ void __launch_bounds__(512, 1) sweep_kernel(const SweepArgs a)
                 }
                 pl += batch;
             }
+            if constexpr (KIND == KIND_CH) {
+                // halo rows come from the neighbouring partitions' rows in global memory (still
+                // c^n: nobody stores before the barriers below).
+#pragma unroll
+                for (int e = 0; e < V; ++e) cm[e] = cp[e] = T(0);
+                if (act && r0 > 0) ld_sys<T, V>(cm, p0 - batch);
+                if (act && (r0 + MR < a.n)) ld_sys<T, V>(cp, p0 + (long long)MR * batch);
+            }
         }
 
-        T glast2[V];  // penta: g at the partition's last-but-one row (overwritten by the backward sweep)
+        [[maybe_unused]] T glast2[V];  // penta: g at the partition's last-but-one row (overwritten by the backward sweep)
         if constexpr (TRI) {
             // ---- local forward sweep, zero incoming carry ---------------------------------
             T gp[V];
@@ -198,39 +338,28 @@ __global__ void __launch_bounds__(512, 1) sweep_kernel(const SweepArgs a)
 #pragma unroll
             for (int e = 0; e < V; ++e) g1[e] = g2[e] = T(0);
             if constexpr (KIND == KIND_CH) {
-                // explicit half: f_k = c_k + alpha_x (w_{k-1} - 2 w_k + w_{k+1}); halo rows come
-                // from the neighbouring partitions' rows in global memory (still c^n: nobody
-                // stores before the barriers below).
+                // explicit half: f_k = c_k + alpha_x (w_{k-1} - 2 w_k + w_{k+1}); cm / cp are the
+                // halo rows r0-1 and r0+MR fetched above (zero outside the system).
                 const T ax = (T)a.alpha_x;
-                T cm[V], cp[V], wm[V], wc[V];
-                if (act && r0 > 0) ld_sys<T, V>(cm, p0 - batch);
-                else {
-#pragma unroll
-                    for (int e = 0; e < V; ++e) cm[e] = T(0);
-                }
-                if (act && (r0 + MR < a.n)) ld_sys<T, V>(cp, p0 + (long long)MR * batch);
-                else {
-#pragma unroll
-                    for (int e = 0; e < V; ++e) cp[e] = T(0);
-                }
+                T wm[V], wc[V];
 #pragma unroll
                 for (int e = 0; e < V; ++e) { wm[e] = ch_w<T>(cm[e]); wc[e] = ch_w<T>(v[0][e]); }
 #pragma unroll
                 for (int k = 0; k < MR; ++k) {
                     const Pair cf = R[k * RP + 0];
                     const T nlb = R[k * RP + 1].v[0];
-                    const bool row_ok = (k < nrow);
+                    const bool row_ok = (k < nrow_part);
 #pragma unroll
                     for (int e = 0; e < V; ++e) {
                         const T wn = ch_w<T>((k + 1 < MR) ? v[(k + 1 < MR) ? k + 1 : k][e] : cp[e]);
                         T s = wm[e] + wn;
                         s = fma_t<T>(T(-2), wc[e], s);
                         T f = fma_t<T>(ax, s, v[k][e]);
-                        f = row_ok ? f : T(0);
+                        f = row_ok ? f : T(0);  // padding rows stay identity rows with zero RHS
                         wm[e] = wc[e];
                         wc[e] = wn;
-                        const T t = fma_t<T>(cf.v[1], g2[e], cf.v[0] * f);
-                        const T g = fma_t<T>(nlb, g1[e], t);
+                        const T t2 = fma_t<T>(cf.v[1], g2[e], cf.v[0] * f);
+                        const T g = fma_t<T>(nlb, g1[e], t2);
                         v[k][e] = g;
                         g2[e] = g1[e];
                         g1[e] = g;
@@ -243,8 +372,8 @@ __global__ void __launch_bounds__(512, 1) sweep_kernel(const SweepArgs a)
                     const T nlb = R[k * RP + 1].v[0];
 #pragma unroll
                     for (int e = 0; e < V; ++e) {
-                        const T t = fma_t<T>(cf.v[1], g2[e], cf.v[0] * v[k][e]);
-                        const T g = fma_t<T>(nlb, g1[e], t);
+                        const T t2 = fma_t<T>(cf.v[1], g2[e], cf.v[0] * v[k][e]);
+                        const T g = fma_t<T>(nlb, g1[e], t2);
                         v[k][e] = g;
                         g2[e] = g1[e];
                         g1[e] = g;
@@ -261,8 +390,8 @@ __global__ void __launch_bounds__(512, 1) sweep_kernel(const SweepArgs a)
                 const Pair cb = R[k * RP + 2];
 #pragma unroll
                 for (int e = 0; e < V; ++e) {
-                    const T t = fma_t<T>(cb.v[1], g2[e], v[k][e]);
-                    const T x = fma_t<T>(cb.v[0], g1[e], t);
+                    const T t2 = fma_t<T>(cb.v[1], g2[e], v[k][e]);
+                    const T x = fma_t<T>(cb.v[0], g1[e], t2);
                     v[k][e] = x;
                     g2[e] = g1[e];
                     g1[e] = x;
@@ -270,102 +399,189 @@ __global__ void __launch_bounds__(512, 1) sweep_kernel(const SweepArgs a)
             }
         }
 
+        // ---- carries across the partitions ----------------------------------------------------------
+        // exchange area xb[value][partition][column], value 0..NC-1: forward (g at the partition's
+        // last NC rows), NC..2NC-1: backward (x^ at its first NC rows); the scan overwrites them
+        // with the incoming carries G (forward) and X (backward) of that partition.
         if constexpr (!SINGLE) {
             const int P = a.P;
-            T *const xu = xg + xu_off;
-            // ---- publish the local forward result at the partition's end -------------------
-            if constexpr (TRI) {
-#pragma unroll
-                for (int e = 0; e < V; ++e) xg[part * W + e] = v[MR - 1][e];
-            } else {
+            const int xW = a.xW;
+            const int tq = a.tq;
+            T *const xc = xb + (size_t)part * xW + sl * V;  // this thread's column of its partition
+            const int vstr = P * xW;                        // elements between successive values
+            [[maybe_unused]] T G[NC][V], X[NC][V];
+            if constexpr (WS) {
 #pragma unroll
                 for (int e = 0; e < V; ++e) {
-                    xg[(part * 2 + 0) * W + e] = v[MR - 1][e];  // g_{last}  (x^ = g^ there)
-                    xg[(part * 2 + 1) * W + e] = glast2[e];     // g_{last-1}
+                    if constexpr (TRI) {
+                        xc[e] = v[MR - 1][e];
+                        xc[vstr + e] = v[0][e];
+                    } else {
+                        xc[e] = v[MR - 1][e];
+                        xc[vstr + e] = glast2[e];
+                        xc[2 * vstr + e] = v[0][e];
+                        xc[3 * vstr + e] = v[1][e];
+                    }
                 }
-            }
-            __syncthreads();
-            if constexpr (TRI) {
-                // ---- forward carry scan: G_{q+1} = g^last_q + phi_last_q G_q ----------------
-                T G[V], X[V];
+                group_sync(a.tpc, sub, tpt);
+                {
+                    // one scan job = one system: lane q of a `width`-lane segment holds partition q
+                    const int lane = lt & 31;
+                    const int wd = 1 << a.scan_log2;
+                    const int q = lane & (wd - 1);
+                    const int spw = 32 >> a.scan_log2;  // systems per warp pass
+                    const T *const tb = TAB + q;
+                    const int mstr = tq;                // elements between matrix entries
+                    const int sstr = NC * NC * tq;      // elements between table slots
+                    for (int s0 = (lt >> 5) * spw; s0 < W; s0 += (tpt >> 5) * spw) {
+                        const int col = s0 + (lane >> a.scan_log2);
+                        const bool ok = (q < P) && (col < W);
+                        T *const xs = xb + (size_t)q * xW + col;
+                        if constexpr (TRI) {
+                            T b = ok ? xs[0] : T(0);
+                            const T xf = ok ? xs[vstr] : T(0);
+                            for (int st = 0; st < a.scan_log2; ++st) {
+                                const T o = __shfl_up_sync(0xffffffffu, b, 1 << st, wd);
+                                b = fma_t<T>(tb[(st == 0 ? 0 : 1 + 2 * st) * sstr], o, b);
+                            }
+                            T g = __shfl_up_sync(0xffffffffu, b, 1, wd);
+                            g = (q == 0) ? T(0) : g;
+                            T c = fma_t<T>(tb[2 * sstr], g, xf);
+                            for (int st = 0; st < a.scan_log2; ++st) {
+                                const T o = __shfl_down_sync(0xffffffffu, c, 1 << st, wd);
+                                c = fma_t<T>(tb[(st == 0 ? 1 : 2 + 2 * st) * sstr], o, c);
+                            }
+                            T x = __shfl_down_sync(0xffffffffu, c, 1, wd);
+                            x = (q + 1 < P) ? x : T(0);
+                            if (ok) {
+                                xs[0] = g;
+                                xs[vstr] = x;
+                            }
+                        } else {
+                            T b1 = ok ? xs[0] : T(0), b2 = ok ? xs[vstr] : T(0);
+                            const T xf0 = ok ? xs[2 * vstr] : T(0), xf1 = ok ? xs[3 * vstr] : T(0);
+                            for (int st = 0; st < a.scan_log2; ++st) {
+                                const T *const m = tb + (st == 0 ? 0 : 1 + 2 * st) * sstr;
+                                const T o1 = __shfl_up_sync(0xffffffffu, b1, 1 << st, wd);
+                                const T o2 = __shfl_up_sync(0xffffffffu, b2, 1 << st, wd);
+                                b1 = fma_t<T>(m[mstr], o2, fma_t<T>(m[0], o1, b1));
+                                b2 = fma_t<T>(m[3 * mstr], o2, fma_t<T>(m[2 * mstr], o1, b2));
+                            }
+                            T g1 = __shfl_up_sync(0xffffffffu, b1, 1, wd);
+                            T g2 = __shfl_up_sync(0xffffffffu, b2, 1, wd);
+                            g1 = (q == 0) ? T(0) : g1;
+                            g2 = (q == 0) ? T(0) : g2;
+                            const T *const ch = tb + 2 * sstr;
+                            T c1 = fma_t<T>(ch[mstr], g2, fma_t<T>(ch[0], g1, xf0));
+                            T c2 = fma_t<T>(ch[3 * mstr], g2, fma_t<T>(ch[2 * mstr], g1, xf1));
+                            for (int st = 0; st < a.scan_log2; ++st) {
+                                const T *const m = tb + (st == 0 ? 1 : 2 + 2 * st) * sstr;
+                                const T o1 = __shfl_down_sync(0xffffffffu, c1, 1 << st, wd);
+                                const T o2 = __shfl_down_sync(0xffffffffu, c2, 1 << st, wd);
+                                c1 = fma_t<T>(m[mstr], o2, fma_t<T>(m[0], o1, c1));
+                                c2 = fma_t<T>(m[3 * mstr], o2, fma_t<T>(m[2 * mstr], o1, c2));
+                            }
+                            T x1 = __shfl_down_sync(0xffffffffu, c1, 1, wd);
+                            T x2 = __shfl_down_sync(0xffffffffu, c2, 1, wd);
+                            x1 = (q + 1 < P) ? x1 : T(0);
+                            x2 = (q + 1 < P) ? x2 : T(0);
+                            if (ok) {
+                                xs[0] = g1;
+                                xs[vstr] = g2;
+                                xs[2 * vstr] = x1;
+                                xs[3 * vstr] = x2;
+                            }
+                        }
+                    }
+                }
+                group_sync(a.tpc, sub, tpt);
 #pragma unroll
-                for (int e = 0; e < V; ++e) G[e] = T(0);
+                for (int e = 0; e < V; ++e) {
+#pragma unroll
+                    for (int c = 0; c < NC; ++c) {
+                        G[c][e] = xc[c * vstr + e];
+                        X[c][e] = xc[(NC + c) * vstr + e];
+                    }
+                }
+            } else {
+                // ---- serial form (any P): every thread walks the partitions before / after it ------
+                const T *const tb = TAB;
+                const int sstr = NC * NC * tq;
+#pragma unroll
+                for (int e = 0; e < V; ++e) {
+                    xc[e] = v[MR - 1][e];
+                    if constexpr (!TRI) xc[vstr + e] = glast2[e];
+                }
+                group_sync(a.tpc, sub, tpt);
+#pragma unroll
+                for (int e = 0; e < V; ++e)
+#pragma unroll
+                    for (int c = 0; c < NC; ++c) G[c][e] = X[c][e] = T(0);
                 for (int q = 0; q < part; ++q) {
-                    const T ph = S[q].v[0];
+                    const T *const xq = xb + (size_t)q * xW + sl * V;
+                    if constexpr (TRI) {
+                        const T ph = tb[q];
 #pragma unroll
-                    for (int e = 0; e < V; ++e) G[e] = fma_t<T>(ph, G[e], xg[q * W + e]);
+                        for (int e = 0; e < V; ++e) G[0][e] = fma_t<T>(ph, G[0][e], xq[e]);
+                    } else {
+                        const T m0 = tb[q], m1 = tb[tq + q], m2 = tb[2 * tq + q], m3 = tb[3 * tq + q];
+#pragma unroll
+                        for (int e = 0; e < V; ++e) {
+                            const T n1 = fma_t<T>(m1, G[1][e], fma_t<T>(m0, G[0][e], xq[e]));
+                            const T n2 = fma_t<T>(m3, G[1][e], fma_t<T>(m2, G[0][e], xq[vstr + e]));
+                            G[0][e] = n1;
+                            G[1][e] = n2;
+                        }
+                    }
                 }
                 {
-                    const T chi0 = R[2].v[0];
+                    const T *const ch = tb + 2 * sstr + part;
 #pragma unroll
-                    for (int e = 0; e < V; ++e) xu[part * W + e] = fma_t<T>(G[e], chi0, v[0][e]);
+                    for (int e = 0; e < V; ++e) {
+                        if constexpr (TRI) {
+                            xc[vstr + e] = fma_t<T>(ch[0], G[0][e], v[0][e]);
+                        } else {
+                            xc[2 * vstr + e] = fma_t<T>(ch[tq], G[1][e], fma_t<T>(ch[0], G[0][e], v[0][e]));
+                            xc[3 * vstr + e] = fma_t<T>(ch[3 * tq], G[1][e], fma_t<T>(ch[2 * tq], G[0][e], v[1][e]));
+                        }
+                    }
                 }
-                __syncthreads();
-                // ---- backward carry scan: X_{q-1} = u_q + psi_first_q X_q -------------------
-#pragma unroll
-                for (int e = 0; e < V; ++e) X[e] = T(0);
+                group_sync(a.tpc, sub, tpt);
                 for (int q = P - 1; q > part; --q) {
-                    const T ps = Rall[(size_t)q * MR * RP + 2].v[1];
+                    const T *const xq = xb + (size_t)q * xW + sl * V + NC * vstr;
+                    const T *const m = tb + sstr + q;
+                    if constexpr (TRI) {
+                        const T ps = m[0];
 #pragma unroll
-                    for (int e = 0; e < V; ++e) X[e] = fma_t<T>(ps, X[e], xu[q * W + e]);
+                        for (int e = 0; e < V; ++e) X[0][e] = fma_t<T>(ps, X[0][e], xq[e]);
+                    } else {
+                        const T m0 = m[0], m1 = m[tq], m2 = m[2 * tq], m3 = m[3 * tq];
+#pragma unroll
+                        for (int e = 0; e < V; ++e) {
+                            const T n1 = fma_t<T>(m1, X[1][e], fma_t<T>(m0, X[0][e], xq[e]));
+                            const T n2 = fma_t<T>(m3, X[1][e], fma_t<T>(m2, X[0][e], xq[vstr + e]));
+                            X[0][e] = n1;
+                            X[1][e] = n2;
+                        }
+                    }
                 }
-                // ---- correction ------------------------------------------------------------
+            }
+            // ---- correction: x_k = x^_k + chi_k . G + psi_k . X ------------------------------------
 #pragma unroll
-                for (int k = 0; k < MR; ++k) {
+            for (int k = 0; k < MR; ++k) {
+                if constexpr (TRI) {
                     const Pair cc = R[k * RP + 2];
 #pragma unroll
                     for (int e = 0; e < V; ++e)
-                        v[k][e] = fma_t<T>(X[e], cc.v[1], fma_t<T>(G[e], cc.v[0], v[k][e]));
-                }
-            } else {
-                T G1[V], G2[V], X1[V], X2[V];
-#pragma unroll
-                for (int e = 0; e < V; ++e) G1[e] = G2[e] = T(0);
-                for (int q = 0; q < part; ++q) {
-                    const Pair s0 = S[q * SP + 0], s1 = S[q * SP + 1];
-#pragma unroll
-                    for (int e = 0; e < V; ++e) {
-                        const T a1 = xg[(q * 2 + 0) * W + e];
-                        const T a2 = xg[(q * 2 + 1) * W + e];
-                        const T n1 = fma_t<T>(s0.v[1], G2[e], fma_t<T>(s0.v[0], G1[e], a1));
-                        const T n2 = fma_t<T>(s1.v[1], G2[e], fma_t<T>(s1.v[0], G1[e], a2));
-                        G1[e] = n1;
-                        G2[e] = n2;
-                    }
-                }
-                {
-                    const Pair c0 = R[3], c1 = R[RP + 3];  // chi pairs of the partition's rows 0, 1
-#pragma unroll
-                    for (int e = 0; e < V; ++e) {
-                        xu[(part * 2 + 0) * W + e] = fma_t<T>(G2[e], c0.v[1], fma_t<T>(G1[e], c0.v[0], v[0][e]));
-                        xu[(part * 2 + 1) * W + e] = fma_t<T>(G2[e], c1.v[1], fma_t<T>(G1[e], c1.v[0], v[1][e]));
-                    }
-                }
-                __syncthreads();
-#pragma unroll
-                for (int e = 0; e < V; ++e) X1[e] = X2[e] = T(0);
-                for (int q = P - 1; q > part; --q) {
-                    const Pair p0q = Rall[(size_t)q * MR * RP + 4];        // psi pair, row 0 of partition q
-                    const Pair p1q = Rall[(size_t)q * MR * RP + RP + 4];   // psi pair, row 1
-#pragma unroll
-                    for (int e = 0; e < V; ++e) {
-                        const T u1 = xu[(q * 2 + 0) * W + e];
-                        const T u2 = xu[(q * 2 + 1) * W + e];
-                        const T n1 = fma_t<T>(X2[e], p0q.v[1], fma_t<T>(X1[e], p0q.v[0], u1));
-                        const T n2 = fma_t<T>(X2[e], p1q.v[1], fma_t<T>(X1[e], p1q.v[0], u2));
-                        X1[e] = n1;
-                        X2[e] = n2;
-                    }
-                }
-#pragma unroll
-                for (int k = 0; k < MR; ++k) {
+                        v[k][e] = fma_t<T>(X[0][e], cc.v[1], fma_t<T>(G[0][e], cc.v[0], v[k][e]));
+                } else {
                     const Pair cc = R[k * RP + 3], cs = R[k * RP + 4];
 #pragma unroll
                     for (int e = 0; e < V; ++e) {
-                        T x = fma_t<T>(G1[e], cc.v[0], v[k][e]);
-                        x = fma_t<T>(G2[e], cc.v[1], x);
-                        x = fma_t<T>(X1[e], cs.v[0], x);
-                        v[k][e] = fma_t<T>(X2[e], cs.v[1], x);
+                        T x = fma_t<T>(G[0][e], cc.v[0], v[k][e]);
+                        x = fma_t<T>(G[1][e], cc.v[1], x);
+                        x = fma_t<T>(X[0][e], cs.v[0], x);
+                        v[k][e] = fma_t<T>(X[1][e], cs.v[1], x);
                     }
                 }
             }
@@ -383,7 +599,6 @@ __global__ void __launch_bounds__(512, 1) sweep_kernel(const SweepArgs a)
         }
     }
 }
-
 // -----------------------------------------------------------------------------------------------
 // Two-pass kernel in the paper's own form (Alg. 2 / Alg. 4: one thread per system, g written to
 // global memory by the forward loop and re-read by the backward loop).  Used only when n is too
@@ -450,22 +665,30 @@ __global__ void __launch_bounds__(128) two_pass_kernel(const T *__restrict__ co,
 }
 
 // launcher table entry (defined by the instantiation units)
-typedef cudaError_t (*sweep_launch_fn)(const SweepArgs &, int grid, int block, size_t smem, cudaStream_t);
-typedef const void *(*sweep_func_ptr)(void);
+typedef cudaError_t (*sweep_launch_fn)(const SweepArgs &, const CUtensorMap &, int grid, int block, size_t smem,
+                                       cudaStream_t, int pdl);
 
 struct SweepEntry {
     sweep_launch_fn launch;
     const void *func;  // for cudaFuncSetAttribute / occupancy queries
+    int max_threads;   // threads per CTA the kernel was compiled for
 };
 
-// kind in {TRI, PENTA, CH}, elem_bytes in {8, 4}, vec in {1, 2}, rows in {8, 16, 32}, single in {0,1}
-SweepEntry find_sweep(int kind, int elem_bytes, int vec, int rows, int single);
-
-template <typename T, int V, int MR, bool SINGLE, int KIND>
-cudaError_t launch_sweep(const SweepArgs &a, int grid, int block, size_t smem, cudaStream_t st)
+template <typename T, int V, int MR, bool SINGLE, int KIND, bool TMA, bool WS>
+cudaError_t launch_sweep(const SweepArgs &a, const CUtensorMap &tm, int grid, int block, size_t smem,
+                         cudaStream_t st, int pdl)
 {
-    sweep_kernel<T, V, MR, SINGLE, KIND><<<grid, block, smem, st>>>(a);
-    return cudaGetLastError();
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)grid);
+    cfg.blockDim = dim3((unsigned)block);
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = pdl ? 1 : 0;
+    return cudaLaunchKernelEx(&cfg, sweep_kernel<T, V, MR, SINGLE, KIND, TMA, WS>, a, tm);
 }
 
 }  // namespace btps
