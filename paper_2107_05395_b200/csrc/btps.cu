@@ -52,7 +52,7 @@ std::atomic<long long> g_launches{0};
 // ------------------------------------------------------------------------------------------------
 struct Tune {
     int rows = -1, lanes = -1, vec = -1, tpc = -1, force_two_pass = -1, reverse = -1, prefetch = -1, pdl = -1,
-        warp_scan = -1;
+        warp_scan = -1, grid = -1;
 };
 Tune g_tune;
 
@@ -63,7 +63,6 @@ struct KernelSlot {
     SweepEntry ent = {nullptr, nullptr, 0};
     int vec = 1;
     int tma = 0;       // 1: the TMA-prefetch variant (needs the ring in shared memory)
-    int xW = 1;        // padded exchange row length (elements)
     size_t smem = 0;
     unsigned offX = 0, offM = 0, offR = 0;
     unsigned box_rows = 0, nboxes = 0;
@@ -296,7 +295,6 @@ void put_scan_tables(std::vector<unsigned char> &blob, const DtypePlan &pl, int 
     };
     put_slot(0, Phi);
     put_slot(1, Psi);
-    put_slot(2, Chi0);
     if (!pl.ws) return;
     std::vector<Mat> A = Phi, B = Psi;
     const Mat zero;
@@ -314,14 +312,22 @@ void put_scan_tables(std::vector<unsigned char> &blob, const DtypePlan &pl, int 
         }
         A.swap(A2);
         B.swap(B2);
-        put_slot(1 + 2 * (st + 1), A);
-        put_slot(2 + 2 * (st + 1), B);
+        if (st + 1 < 4) {
+            put_slot(2 * (st + 1), A);
+            put_slot(2 * (st + 1) + 1, B);
+        } else {
+            // step 4: forward entries (q >= 16) and backward entries (q < 16) share slot 8
+            std::vector<Mat> AB(P);
+            for (int q = 0; q < P; ++q) AB[q] = (q >= 16) ? A[q] : B[q];
+            put_slot(8, AB);
+        }
     }
+    put_slot(9, Chi0);
 }
 
 size_t scan_table_bytes(const DtypePlan &pl, int nc, size_t elem)
 {
-    const int slots = pl.ws ? (2 * SCAN_STEPS + 1) : 3;
+    const int slots = pl.ws ? 2 * SCAN_STEPS : 2;  // ws: 8 step slots + merged step 4 + chi
     return (size_t)slots * nc * nc * pl.tq * elem;
 }
 
@@ -330,13 +336,16 @@ void build_blob_tri(int n, DtypePlan &pl, const std::vector<double> &inv, const 
                     const std::vector<double> &nch, std::vector<unsigned char> &blob)
 {
     const int MR = pl.rows, P = pl.P, Np = P * MR;
-    constexpr int RT = 2 * RecLayout<KIND_TRI>::PAIRS;   // elements per row record
+    constexpr int RT = RecLayout<KIND_TRI>::ELEMS;   // coefficient values per row
     auto at = [&](const std::vector<double> &v, int i, double pad) { return i < n ? v[i] : pad; };
     pl.offT = (unsigned)align16((size_t)Np * RT * sizeof(T));
     pl.blob_bytes = (unsigned)align16(pl.offT + scan_table_bytes(pl, 1, sizeof(T)));
     blob.assign(pl.blob_bytes, 0);
     std::vector<double> phi(MR), chi(MR), psi(MR);
     std::vector<Mat> Phi(P), Psi(P), Chi0(P);
+    auto putv = [&](int arr, int i, int j, double v) {  // array at element offset arr*Np, entry i, value j
+        put<T>(blob, ((size_t)arr * Np + (size_t)i * (arr == 2 ? 1 : 2) + j) * sizeof(T), v);
+    };
     for (int p = 0; p < P; ++p) {
         const int r0 = p * MR;
         double prev = 1.0;  // forward response to a unit incoming carry g_{r0-1} = 1
@@ -354,13 +363,11 @@ void build_blob_tri(int n, DtypePlan &pl, const std::vector<double> &inv, const 
         }
         for (int k = 0; k < MR; ++k) {
             const int i = r0 + k;
-            const size_t r = (size_t)i * RT * sizeof(T);
-            put<T>(blob, r + 0 * sizeof(T), at(inv, i, 1.0));
-            put<T>(blob, r + 1 * sizeof(T), at(nl, i, 0.0));
-            put<T>(blob, r + 2 * sizeof(T), at(nch, i, 0.0));
-            put<T>(blob, r + 3 * sizeof(T), 0.0);
-            put<T>(blob, r + 4 * sizeof(T), chi[k]);
-            put<T>(blob, r + 5 * sizeof(T), psi[k]);
+            putv(0, i, 0, at(inv, i, 1.0));
+            putv(0, i, 1, at(nl, i, 0.0));
+            putv(2, i, 0, at(nch, i, 0.0));
+            putv(3, i, 0, chi[k]);
+            putv(3, i, 1, psi[k]);
         }
         Phi[p].m[0] = phi[MR - 1];
         Psi[p].m[0] = psi[0];
@@ -375,7 +382,7 @@ void build_blob_penta(int n, DtypePlan &pl, const std::vector<double> &inv, cons
                       const std::vector<double> &ndel, std::vector<unsigned char> &blob)
 {
     const int MR = pl.rows, P = pl.P, Np = P * MR;
-    constexpr int RT = 2 * RecLayout<KIND_PENTA>::PAIRS;
+    constexpr int RT = RecLayout<KIND_PENTA>::ELEMS;
     auto at = [&](const std::vector<double> &v, int i, double pad) { return i < n ? v[i] : pad; };
     pl.offT = (unsigned)align16((size_t)Np * RT * sizeof(T));
     pl.blob_bytes = (unsigned)align16(pl.offT + scan_table_bytes(pl, 2, sizeof(T)));
@@ -387,6 +394,9 @@ void build_blob_penta(int n, DtypePlan &pl, const std::vector<double> &inv, cons
         psi[t].resize(MR);
     }
     std::vector<Mat> Phi(P), Psi(P), Chi0(P);
+    auto putv = [&](int arr, int i, int j, double v) {  // array at element offset arr*Np, entry i, value j
+        put<T>(blob, ((size_t)arr * Np + (size_t)i * (arr == 2 ? 1 : 2) + j) * sizeof(T), v);
+    };
     for (int p = 0; p < P; ++p) {
         const int r0 = p * MR;
         for (int t = 0; t < 2; ++t) {
@@ -415,17 +425,15 @@ void build_blob_penta(int n, DtypePlan &pl, const std::vector<double> &inv, cons
         }
         for (int k = 0; k < MR; ++k) {
             const int i = r0 + k;
-            const size_t r = (size_t)i * RT * sizeof(T);
-            put<T>(blob, r + 0 * sizeof(T), at(inv, i, 1.0));
-            put<T>(blob, r + 1 * sizeof(T), at(nle, i, 0.0));
-            put<T>(blob, r + 2 * sizeof(T), at(nlb, i, 0.0));
-            put<T>(blob, r + 3 * sizeof(T), 0.0);
-            put<T>(blob, r + 4 * sizeof(T), at(ngam, i, 0.0));
-            put<T>(blob, r + 5 * sizeof(T), at(ndel, i, 0.0));
-            put<T>(blob, r + 6 * sizeof(T), chi[0][k]);
-            put<T>(blob, r + 7 * sizeof(T), chi[1][k]);
-            put<T>(blob, r + 8 * sizeof(T), psi[0][k]);
-            put<T>(blob, r + 9 * sizeof(T), psi[1][k]);
+            putv(0, i, 0, at(inv, i, 1.0));
+            putv(0, i, 1, at(nle, i, 0.0));
+            putv(2, i, 0, at(nlb, i, 0.0));
+            putv(3, i, 0, at(ngam, i, 0.0));
+            putv(3, i, 1, at(ndel, i, 0.0));
+            putv(5, i, 0, chi[0][k]);
+            putv(5, i, 1, chi[1][k]);
+            putv(7, i, 0, psi[0][k]);
+            putv(7, i, 1, psi[1][k]);
         }
         // carries: (g at the last row, g at the last-but-one row) forward; (x at the first row, x at
         // the second row) backward
@@ -483,11 +491,10 @@ void layout_slot(const DtypePlan &pl, const Shape &sh, int kind, KernelSlot &sl)
 {
     const int NC = (kind == KIND_TRI) ? 1 : 2;
     const size_t W = (size_t)sh.lanes * sl.vec;
-    sl.xW = (int)(W | 1);  // odd row length: the scan lanes read a column without bank conflicts
-    const size_t xch = (pl.P > 1) ? (size_t)sh.tpc * 2 * NC * pl.P * sl.xW * pl.elem : 0;
+    const size_t xch = (pl.P > 1) ? (size_t)sh.tpc * 2 * NC * pl.P * W * pl.elem : 0;
     sl.offX = (unsigned)align16(pl.blob_bytes);
     sl.offM = (unsigned)align16(sl.offX + xch);
-    sl.offR = (unsigned)align_up(sl.offM + 16 * 8, 128);
+    sl.offR = (unsigned)align_up(sl.offM + 17 * 8, 128);
     // TMA boxes of whole partitions: the largest divisor g of P with g*rows <= 256 rows per box
     const size_t Np = (size_t)pl.P * pl.rows;
     int g = 256 / pl.rows < pl.P ? 256 / pl.rows : pl.P;
@@ -495,7 +502,7 @@ void layout_slot(const DtypePlan &pl, const Shape &sh, int kind, KernelSlot &sl)
     sl.box_rows = (unsigned)(g * pl.rows);
     sl.nboxes = (unsigned)(pl.P / g);
     const size_t ring = (size_t)sh.tpc * Np * W * pl.elem;
-    sl.smem = sl.tma ? sl.offR + ring : sl.offM;
+    sl.smem = sl.tma ? sl.offR + ring : sl.offM + 17 * 8;
 }
 
 bool tma_possible(const DtypePlan &pl, const Shape &sh, int vec)
@@ -684,7 +691,6 @@ int launch_one(Handle *h, int kind, T *d_rhs, long long batch, double alpha_x, i
     a.tpc = sh.tpc;
     a.reverse = reverse;
     a.scan_log2 = pl.scan_log2;
-    a.xW = sl.xW;
     a.tq = pl.tq;
     a.blob_bytes = pl.blob_bytes;
     a.offT = pl.offT;
@@ -701,6 +707,7 @@ int launch_one(Handle *h, int kind, T *d_rhs, long long batch, double alpha_x, i
     }
     long long grid = (a.num_tiles + sh.tpc - 1) / sh.tpc;
     if (grid > sl.max_grid) grid = sl.max_grid;
+    if (g_tune.grid > 0 && grid > g_tune.grid) grid = g_tune.grid;
     const cudaError_t e = sl.ent.launch(a, tm, (int)grid, sh.threads, sl.smem, st, g_tune.pdl != 0);
     g_launches.fetch_add(1, std::memory_order_relaxed);
     if (e != cudaSuccess) return cuda_fail(e, "sweep launch");
@@ -988,6 +995,7 @@ int btps_tune(const char *key, int value)
     else if (!strcmp(key, "prefetch")) g_tune.prefetch = value;
     else if (!strcmp(key, "pdl")) g_tune.pdl = value;
     else if (!strcmp(key, "warp_scan")) g_tune.warp_scan = value;
+    else if (!strcmp(key, "grid")) g_tune.grid = value;
     else return set_err(BTPS_E_ARG);
     return set_err(BTPS_OK);
 }

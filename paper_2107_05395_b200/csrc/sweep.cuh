@@ -52,7 +52,6 @@ struct SweepArgs {
     int tpc;               // tile groups per CTA (each walks its own tiles)
     int reverse;           // 1: walk the tiles from the last to the first
     int scan_log2;         // warp scan: log2 of the scan width (smallest power of two >= P)
-    int xW;                // padded (odd) row length of the exchange area, in elements
     int tq;                // partitions per scan-table row (max(32, P))
     unsigned blob_bytes;   // multiple of 16
     unsigned offT;         // byte offset of the scan tables inside the blob (row records start at 0)
@@ -106,25 +105,28 @@ template <typename T>
 __device__ __forceinline__ T ch_w(T c) { return fma_t<T>(c * c, c, -c); }
 
 // Coefficient image ("blob"), all in element type T, rows padded to Np = P*MR with identity rows.
-// One record per row, made of pairs {T,T} so that one LDS fetches what one phase of a row needs:
-//   tri   record = 3 pairs: {inv, nl} {nch, 0} {chi, psi}
+// Structure of arrays, one entry per row, pairs {T,T} where one phase of a row needs two values
+// (one LDS.128 in fp64); element offsets of the arrays in units of Np:
+//   tri   (5 Np): 0: {inv, nl}   2: nch    3: {chi, psi}
 //           inv = 1/b^_i, nl = -a_i/b^_i, nch = -c^_i; chi/psi = response of the finished local
 //           sweeps to the incoming forward / backward carry
-//   penta record = 5 pairs: {inv, nle} {nlb, 0} {ngam, ndel} {chi1, chi2} {psi1, psi2}
+//   penta (9 Np): 0: {inv, nle}  2: nlb    3: {ngam, ndel}   5: {chi1, chi2}   7: {psi1, psi2}
 //           inv = 1/alpha_i, nle = -eps_i/alpha_i, nlb = -beta_i/alpha_i, ngam = -gamma_i, ndel = -delta_i
-// followed at offT by the carry-scan tables, indexed [slot][m][q] with q = partition (32 entries),
+// followed at offT by the carry-scan tables, indexed [slot][m][q] with q = partition (tq entries),
 // m = entry of the NC x NC matrix (row-major), NC = 1 (tri) or 2 (penta):
-//   slot 2*s     : forward  multiplier of Kogge-Stone step s, A^(s)_q = Phi_q Phi_{q-1} ... (2^s factors),
+//   slot 2*s     : forward  multiplier of Kogge-Stone step s < 4, A^(s)_q = Phi_q Phi_{q-1} ... (2^s factors),
 //                  zero where q < 2^s
-//   slot 2*s + 1 : backward multiplier of step s, B^(s)_q = Psi_q Psi_{q+1} ..., zero where q + 2^s >= P
-//   slot 2*SCAN_STEPS : chi at the partition's first NC rows (turns the forward carry into the
-//                  local back-substitution's value at those rows)
+//   slot 2*s + 1 : backward multiplier of step s < 4, B^(s)_q = Psi_q Psi_{q+1} ..., zero where q + 2^s >= P
+//   slot 8       : step 4, both directions: A^(4)_q at q >= 16, B^(4)_q at q < 16 (each is zero on the
+//                  other half, so they share the slot and the reader masks)
+//   slot 9       : chi at the partition's first NC rows (turns the forward carry into the local
+//                  back-substitution's value at those rows)
+// (the serial carry walk keeps only slots 0 and 1, holding Phi_q and Psi_q themselves, and takes chi
+// from the row arrays).
 template <int KIND>
 struct RecLayout {
-    static constexpr int PAIRS = (KIND == KIND_TRI) ? 3 : 5;   // pairs per row record
+    static constexpr int ELEMS = (KIND == KIND_TRI) ? 5 : 9;   // coefficient values per row
     static constexpr int NC = (KIND == KIND_TRI) ? 1 : 2;      // carries per direction
-    static constexpr int SCAN_SLOTS = 2 * SCAN_STEPS + 1;
-    static constexpr int SCAN_ELEMS = SCAN_SLOTS * NC * NC * SCAN_LANES;
 };
 
 // ---- TMA / mbarrier primitives (PTX) -------------------------------------------------------------
@@ -149,6 +151,11 @@ __device__ __forceinline__ void mbar_wait(unsigned bar, unsigned parity)
         "bra WAIT_%=;\n"
         "DONE_%=:\n"
         "}\n" ::"r"(bar), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void bulk_load(unsigned dst, const void *src, unsigned bytes, unsigned bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(dst), "l"(src), "r"(bytes), "r"(bar) : "memory");
 }
 __device__ __forceinline__ void tma_load_2d(unsigned dst, const CUtensorMap *tm, int c0, int c1, unsigned bar)
 {
@@ -176,6 +183,20 @@ struct CtaShape {
     static constexpr int MAX_THREADS = WIDE ? 256 : 512;
 };
 
+// Loop over the Kogge-Stone steps.  In fp32 the loop is kept rolled and in fp64 left to the
+// compiler's own choice: measured with ptxas -v, that is what keeps the 255-register wide
+// variants from spilling their tile rows.
+template <bool ROLLED, typename F>
+__device__ __forceinline__ void scan_steps(int n, F &&f)
+{
+    if constexpr (ROLLED) {
+#pragma unroll 1
+        for (int st = 0; st < n; ++st) f(st);
+    } else {
+        for (int st = 0; st < n; ++st) f(st);
+    }
+}
+
 // -----------------------------------------------------------------------------------------------
 // sweep_kernel<T, V, MR, SINGLE, KIND, TMA, WS>
 //   V      systems per thread (adjacent, one vector access)
@@ -191,7 +212,6 @@ sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
 {
     constexpr bool TRI = (KIND == KIND_TRI);
     constexpr int NC = RecLayout<KIND>::NC;
-    constexpr int RP = RecLayout<KIND>::PAIRS;
     using Pair = Tup<T, 2>;
     extern __shared__ __align__(128) unsigned char smem[];
 
@@ -204,19 +224,20 @@ sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
     const int r0 = part * MR;
     const long long batch = a.batch;
 
-    // ---- stage the coefficient image once per CTA ------------------------------------------
-    {
-        const uint4 *src = reinterpret_cast<const uint4 *>(a.blob);
-        uint4 *dst = reinterpret_cast<uint4 *>(smem);
-        const unsigned nvec = a.blob_bytes >> 4;
-        for (unsigned i = threadIdx.x; i < nvec; i += blockDim.x) dst[i] = __ldg(src + i);
-    }
+    // ---- stage the coefficient image once per CTA: one asynchronous bulk copy ---------------------
+    // mbarrier slots at offM: 0..15 = the groups' prefetch rings, 16 = the coefficient image
     [[maybe_unused]] const unsigned mbar = smem_u32(smem + a.offM) + 8u * sub;
+    const unsigned bbar = smem_u32(smem + a.offM) + 8u * 16u;
+    if (threadIdx.x == 0) mbar_init(bbar, 1);
     if constexpr (TMA) {
         if (lt == 0) mbar_init(mbar, 1);
-        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     __syncthreads();
+    if (threadIdx.x == 0) {
+        mbar_expect_tx(bbar, a.blob_bytes);
+        bulk_load(smem_u32(smem), a.blob, a.blob_bytes, bbar);
+    }
     // Programmatic dependent launch (time-step loops): everything above overlaps the tail of the
     // previous launch on the stream; the batch itself is only touched after the wait.  Both
     // instructions are no-ops for a launch without the attribute.
@@ -227,11 +248,17 @@ sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
     int nrow_part = a.n - r0;
     nrow_part = nrow_part < 0 ? 0 : (nrow_part > MR ? MR : nrow_part);
 
-    const Pair *const R = reinterpret_cast<const Pair *>(smem) + (size_t)r0 * RP;  // this partition's records
-    [[maybe_unused]] const Pair *const Rall = reinterpret_cast<const Pair *>(smem);
+    // coefficient arrays of this partition's rows (RecLayout): Np = P*MR rows each
+    const int Np = a.P * MR;
+    const T *const cb = reinterpret_cast<const T *>(smem);
+    const Pair *const RA = reinterpret_cast<const Pair *>(cb) + r0;                        // {inv, nl | nle}
+    const T *const RB1 = cb + 2 * Np + r0;                                                 // nch | nlb
+    [[maybe_unused]] const Pair *const RBW = reinterpret_cast<const Pair *>(cb + 3 * Np) + r0;  // {chi, psi} | {ngam, ndel}
+    [[maybe_unused]] const Pair *const RC0 = reinterpret_cast<const Pair *>(cb + 5 * Np) + r0;  // penta {chi1, chi2}
+    [[maybe_unused]] const Pair *const RC1 = reinterpret_cast<const Pair *>(cb + 7 * Np) + r0;  // penta {psi1, psi2}
     [[maybe_unused]] const T *const TAB = reinterpret_cast<const T *>(smem + a.offT);
-    // exchange area of this group: [2*NC values][P][xW]
-    [[maybe_unused]] T *const xb = reinterpret_cast<T *>(smem + a.offX) + (size_t)sub * 2 * NC * a.P * a.xW;
+    // exchange area of this group: [2*NC values][P][W], columns XOR-swizzled with the partition index
+    [[maybe_unused]] T *const xb = reinterpret_cast<T *>(smem + a.offX) + (size_t)sub * 2 * NC * a.P * W;
     // prefetch ring of this group: [P*MR rows][W]
     [[maybe_unused]] const unsigned ring_bytes = (unsigned)(a.P * MR * W) * (unsigned)sizeof(T);
     [[maybe_unused]] T *const ring = reinterpret_cast<T *>(smem + a.offR + (size_t)sub * ring_bytes);
@@ -256,6 +283,7 @@ sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
     if constexpr (TMA) {
         if (lt == 0 && t < ntiles) tma_issue(t);
     }
+    mbar_wait(bbar, 0);  // coefficient image has landed
     for (; t < ntiles; t += stride_tiles) {
         const int tile = a.reverse ? ntiles - 1 - t : t;
         const long long j = (long long)tile * W + (long long)sl * V;
@@ -314,7 +342,7 @@ sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
             for (int e = 0; e < V; ++e) gp[e] = T(0);
 #pragma unroll
             for (int k = 0; k < MR; ++k) {
-                const Pair cf = R[k * RP + 0];
+                const Pair cf = RA[k];
 #pragma unroll
                 for (int e = 0; e < V; ++e) {
                     v[k][e] = fma_t<T>(cf.v[1], gp[e], cf.v[0] * v[k][e]);
@@ -326,7 +354,7 @@ sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
             for (int e = 0; e < V; ++e) gp[e] = T(0);
 #pragma unroll
             for (int k = MR - 1; k >= 0; --k) {
-                const T nch = R[k * RP + 1].v[0];
+                const T nch = RB1[k];
 #pragma unroll
                 for (int e = 0; e < V; ++e) {
                     v[k][e] = fma_t<T>(nch, gp[e], v[k][e]);
@@ -346,8 +374,8 @@ sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
                 for (int e = 0; e < V; ++e) { wm[e] = ch_w<T>(cm[e]); wc[e] = ch_w<T>(v[0][e]); }
 #pragma unroll
                 for (int k = 0; k < MR; ++k) {
-                    const Pair cf = R[k * RP + 0];
-                    const T nlb = R[k * RP + 1].v[0];
+                    const Pair cf = RA[k];
+                    const T nlb = RB1[k];
                     const bool row_ok = (k < nrow_part);
 #pragma unroll
                     for (int e = 0; e < V; ++e) {
@@ -368,8 +396,8 @@ sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
             } else {
 #pragma unroll
                 for (int k = 0; k < MR; ++k) {
-                    const Pair cf = R[k * RP + 0];
-                    const T nlb = R[k * RP + 1].v[0];
+                    const Pair cf = RA[k];
+                    const T nlb = RB1[k];
 #pragma unroll
                     for (int e = 0; e < V; ++e) {
                         const T t2 = fma_t<T>(cf.v[1], g2[e], cf.v[0] * v[k][e]);
@@ -387,11 +415,11 @@ sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
             for (int e = 0; e < V; ++e) g1[e] = g2[e] = T(0);  // x_{k+1}, x_{k+2}
 #pragma unroll
             for (int k = MR - 1; k >= 0; --k) {
-                const Pair cb = R[k * RP + 2];
+                const Pair cbw = RBW[k];
 #pragma unroll
                 for (int e = 0; e < V; ++e) {
-                    const T t2 = fma_t<T>(cb.v[1], g2[e], v[k][e]);
-                    const T x = fma_t<T>(cb.v[0], g1[e], t2);
+                    const T t2 = fma_t<T>(cbw.v[1], g2[e], v[k][e]);
+                    const T x = fma_t<T>(cbw.v[0], g1[e], t2);
                     v[k][e] = x;
                     g2[e] = g1[e];
                     g1[e] = x;
@@ -405,22 +433,25 @@ sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
         // with the incoming carries G (forward) and X (backward) of that partition.
         if constexpr (!SINGLE) {
             const int P = a.P;
-            const int xW = a.xW;
             const int tq = a.tq;
-            T *const xc = xb + (size_t)part * xW + sl * V;  // this thread's column of its partition
-            const int vstr = P * xW;                        // elements between successive values
+            const int wm = W - 1;
+            // this thread's columns of its partition: element e lives at xc[XI(e)]
+            T *const xc = xb + (size_t)part * W;
+            const int xsw = part & wm;
+#define XI(e) (((sl * V + (e)) ^ xsw))
+            const int vstr = P * W;  // elements between successive values
             [[maybe_unused]] T G[NC][V], X[NC][V];
             if constexpr (WS) {
 #pragma unroll
                 for (int e = 0; e < V; ++e) {
                     if constexpr (TRI) {
-                        xc[e] = v[MR - 1][e];
-                        xc[vstr + e] = v[0][e];
+                        xc[XI(e)] = v[MR - 1][e];
+                        xc[vstr + XI(e)] = v[0][e];
                     } else {
-                        xc[e] = v[MR - 1][e];
-                        xc[vstr + e] = glast2[e];
-                        xc[2 * vstr + e] = v[0][e];
-                        xc[3 * vstr + e] = v[1][e];
+                        xc[XI(e)] = v[MR - 1][e];
+                        xc[vstr + XI(e)] = glast2[e];
+                        xc[2 * vstr + XI(e)] = v[0][e];
+                        xc[3 * vstr + XI(e)] = v[1][e];
                     }
                 }
                 group_sync(a.tpc, sub, tpt);
@@ -433,24 +464,35 @@ sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
                     const T *const tb = TAB + q;
                     const int mstr = tq;                // elements between matrix entries
                     const int sstr = NC * NC * tq;      // elements between table slots
+                    // multipliers of step st: slots 2st (forward) / 2st+1 (backward); step 4 shares
+                    // slot 8: its forward entries are nonzero only at q >= 16, its backward ones only
+                    // at q < 16, and each reader masks the other half
+                    auto fwm = [&](int st, int m) -> T {
+                        const T val = tb[(st < 4 ? 2 * st : 8) * sstr + m * mstr];
+                        return (st < 4 || q >= 16) ? val : T(0);
+                    };
+                    auto bwm = [&](int st, int m) -> T {
+                        const T val = tb[(st < 4 ? 2 * st + 1 : 8) * sstr + m * mstr];
+                        return (st < 4 || q < 16) ? val : T(0);
+                    };
                     for (int s0 = (lt >> 5) * spw; s0 < W; s0 += (tpt >> 5) * spw) {
                         const int col = s0 + (lane >> a.scan_log2);
                         const bool ok = (q < P) && (col < W);
-                        T *const xs = xb + (size_t)q * xW + col;
+                        T *const xs = xb + (size_t)q * W + (col ^ (q & wm));
                         if constexpr (TRI) {
                             T b = ok ? xs[0] : T(0);
                             const T xf = ok ? xs[vstr] : T(0);
-                            for (int st = 0; st < a.scan_log2; ++st) {
+                            scan_steps<sizeof(T) == 4>(a.scan_log2, [&](int st) {
                                 const T o = __shfl_up_sync(0xffffffffu, b, 1 << st, wd);
-                                b = fma_t<T>(tb[(st == 0 ? 0 : 1 + 2 * st) * sstr], o, b);
-                            }
+                                b = fma_t<T>(fwm(st, 0), o, b);
+                            });
                             T g = __shfl_up_sync(0xffffffffu, b, 1, wd);
                             g = (q == 0) ? T(0) : g;
-                            T c = fma_t<T>(tb[2 * sstr], g, xf);
-                            for (int st = 0; st < a.scan_log2; ++st) {
+                            T c = fma_t<T>(tb[9 * sstr], g, xf);
+                            scan_steps<sizeof(T) == 4>(a.scan_log2, [&](int st) {
                                 const T o = __shfl_down_sync(0xffffffffu, c, 1 << st, wd);
-                                c = fma_t<T>(tb[(st == 0 ? 1 : 2 + 2 * st) * sstr], o, c);
-                            }
+                                c = fma_t<T>(bwm(st, 0), o, c);
+                            });
                             T x = __shfl_down_sync(0xffffffffu, c, 1, wd);
                             x = (q + 1 < P) ? x : T(0);
                             if (ok) {
@@ -460,27 +502,25 @@ sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
                         } else {
                             T b1 = ok ? xs[0] : T(0), b2 = ok ? xs[vstr] : T(0);
                             const T xf0 = ok ? xs[2 * vstr] : T(0), xf1 = ok ? xs[3 * vstr] : T(0);
-                            for (int st = 0; st < a.scan_log2; ++st) {
-                                const T *const m = tb + (st == 0 ? 0 : 1 + 2 * st) * sstr;
+                            scan_steps<sizeof(T) == 4>(a.scan_log2, [&](int st) {
                                 const T o1 = __shfl_up_sync(0xffffffffu, b1, 1 << st, wd);
                                 const T o2 = __shfl_up_sync(0xffffffffu, b2, 1 << st, wd);
-                                b1 = fma_t<T>(m[mstr], o2, fma_t<T>(m[0], o1, b1));
-                                b2 = fma_t<T>(m[3 * mstr], o2, fma_t<T>(m[2 * mstr], o1, b2));
-                            }
+                                b1 = fma_t<T>(fwm(st, 1), o2, fma_t<T>(fwm(st, 0), o1, b1));
+                                b2 = fma_t<T>(fwm(st, 3), o2, fma_t<T>(fwm(st, 2), o1, b2));
+                            });
                             T g1 = __shfl_up_sync(0xffffffffu, b1, 1, wd);
                             T g2 = __shfl_up_sync(0xffffffffu, b2, 1, wd);
                             g1 = (q == 0) ? T(0) : g1;
                             g2 = (q == 0) ? T(0) : g2;
-                            const T *const ch = tb + 2 * sstr;
+                            const T *const ch = tb + 9 * sstr;  // chi at the partition's first two rows
                             T c1 = fma_t<T>(ch[mstr], g2, fma_t<T>(ch[0], g1, xf0));
                             T c2 = fma_t<T>(ch[3 * mstr], g2, fma_t<T>(ch[2 * mstr], g1, xf1));
-                            for (int st = 0; st < a.scan_log2; ++st) {
-                                const T *const m = tb + (st == 0 ? 1 : 2 + 2 * st) * sstr;
+                            scan_steps<sizeof(T) == 4>(a.scan_log2, [&](int st) {
                                 const T o1 = __shfl_down_sync(0xffffffffu, c1, 1 << st, wd);
                                 const T o2 = __shfl_down_sync(0xffffffffu, c2, 1 << st, wd);
-                                c1 = fma_t<T>(m[mstr], o2, fma_t<T>(m[0], o1, c1));
-                                c2 = fma_t<T>(m[3 * mstr], o2, fma_t<T>(m[2 * mstr], o1, c2));
-                            }
+                                c1 = fma_t<T>(bwm(st, 1), o2, fma_t<T>(bwm(st, 0), o1, c1));
+                                c2 = fma_t<T>(bwm(st, 3), o2, fma_t<T>(bwm(st, 2), o1, c2));
+                            });
                             T x1 = __shfl_down_sync(0xffffffffu, c1, 1, wd);
                             T x2 = __shfl_down_sync(0xffffffffu, c2, 1, wd);
                             x1 = (q + 1 < P) ? x1 : T(0);
@@ -499,8 +539,8 @@ sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
                 for (int e = 0; e < V; ++e) {
 #pragma unroll
                     for (int c = 0; c < NC; ++c) {
-                        G[c][e] = xc[c * vstr + e];
-                        X[c][e] = xc[(NC + c) * vstr + e];
+                        G[c][e] = xc[c * vstr + XI(e)];
+                        X[c][e] = xc[(NC + c) * vstr + XI(e)];
                     }
                 }
             } else {
@@ -509,8 +549,8 @@ sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
                 const int sstr = NC * NC * tq;
 #pragma unroll
                 for (int e = 0; e < V; ++e) {
-                    xc[e] = v[MR - 1][e];
-                    if constexpr (!TRI) xc[vstr + e] = glast2[e];
+                    xc[XI(e)] = v[MR - 1][e];
+                    if constexpr (!TRI) xc[vstr + XI(e)] = glast2[e];
                 }
                 group_sync(a.tpc, sub, tpt);
 #pragma unroll
@@ -518,64 +558,67 @@ sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
 #pragma unroll
                     for (int c = 0; c < NC; ++c) G[c][e] = X[c][e] = T(0);
                 for (int q = 0; q < part; ++q) {
-                    const T *const xq = xb + (size_t)q * xW + sl * V;
+                    const T *const xq = xb + (size_t)q * W;
+                    const int qsw = q & wm;
                     if constexpr (TRI) {
                         const T ph = tb[q];
 #pragma unroll
-                        for (int e = 0; e < V; ++e) G[0][e] = fma_t<T>(ph, G[0][e], xq[e]);
+                        for (int e = 0; e < V; ++e) G[0][e] = fma_t<T>(ph, G[0][e], xq[(sl * V + e) ^ qsw]);
                     } else {
                         const T m0 = tb[q], m1 = tb[tq + q], m2 = tb[2 * tq + q], m3 = tb[3 * tq + q];
 #pragma unroll
                         for (int e = 0; e < V; ++e) {
-                            const T n1 = fma_t<T>(m1, G[1][e], fma_t<T>(m0, G[0][e], xq[e]));
-                            const T n2 = fma_t<T>(m3, G[1][e], fma_t<T>(m2, G[0][e], xq[vstr + e]));
+                            const T n1 = fma_t<T>(m1, G[1][e], fma_t<T>(m0, G[0][e], xq[(sl * V + e) ^ qsw]));
+                            const T n2 = fma_t<T>(m3, G[1][e], fma_t<T>(m2, G[0][e], xq[vstr + ((sl * V + e) ^ qsw)]));
                             G[0][e] = n1;
                             G[1][e] = n2;
                         }
                     }
                 }
                 {
-                    const T *const ch = tb + 2 * sstr + part;
 #pragma unroll
                     for (int e = 0; e < V; ++e) {
                         if constexpr (TRI) {
-                            xc[vstr + e] = fma_t<T>(ch[0], G[0][e], v[0][e]);
+                            xc[vstr + XI(e)] = fma_t<T>(RBW[0].v[0], G[0][e], v[0][e]);
                         } else {
-                            xc[2 * vstr + e] = fma_t<T>(ch[tq], G[1][e], fma_t<T>(ch[0], G[0][e], v[0][e]));
-                            xc[3 * vstr + e] = fma_t<T>(ch[3 * tq], G[1][e], fma_t<T>(ch[2 * tq], G[0][e], v[1][e]));
+                            const Pair ch0 = RC0[0], ch1 = RC0[1];  // chi at this partition's first two rows
+                            xc[2 * vstr + XI(e)] = fma_t<T>(ch0.v[1], G[1][e], fma_t<T>(ch0.v[0], G[0][e], v[0][e]));
+                            xc[3 * vstr + XI(e)] = fma_t<T>(ch1.v[1], G[1][e], fma_t<T>(ch1.v[0], G[0][e], v[1][e]));
                         }
                     }
                 }
                 group_sync(a.tpc, sub, tpt);
                 for (int q = P - 1; q > part; --q) {
-                    const T *const xq = xb + (size_t)q * xW + sl * V + NC * vstr;
+                    const T *const xq = xb + (size_t)q * W + NC * vstr;
+                    const int qsw = q & wm;
                     const T *const m = tb + sstr + q;
                     if constexpr (TRI) {
                         const T ps = m[0];
 #pragma unroll
-                        for (int e = 0; e < V; ++e) X[0][e] = fma_t<T>(ps, X[0][e], xq[e]);
+                        for (int e = 0; e < V; ++e) X[0][e] = fma_t<T>(ps, X[0][e], xq[(sl * V + e) ^ qsw]);
                     } else {
                         const T m0 = m[0], m1 = m[tq], m2 = m[2 * tq], m3 = m[3 * tq];
 #pragma unroll
                         for (int e = 0; e < V; ++e) {
-                            const T n1 = fma_t<T>(m1, X[1][e], fma_t<T>(m0, X[0][e], xq[e]));
-                            const T n2 = fma_t<T>(m3, X[1][e], fma_t<T>(m2, X[0][e], xq[vstr + e]));
+                            const T n1 = fma_t<T>(m1, X[1][e], fma_t<T>(m0, X[0][e], xq[(sl * V + e) ^ qsw]));
+                            const T n2 = fma_t<T>(m3, X[1][e], fma_t<T>(m2, X[0][e], xq[vstr + ((sl * V + e) ^ qsw)]));
                             X[0][e] = n1;
                             X[1][e] = n2;
                         }
                     }
                 }
             }
+#undef XI
             // ---- correction: x_k = x^_k + chi_k . G + psi_k . X ------------------------------------
 #pragma unroll
             for (int k = 0; k < MR; ++k) {
                 if constexpr (TRI) {
-                    const Pair cc = R[k * RP + 2];
+                    const Pair cc = RBW[k];
 #pragma unroll
                     for (int e = 0; e < V; ++e)
                         v[k][e] = fma_t<T>(X[0][e], cc.v[1], fma_t<T>(G[0][e], cc.v[0], v[k][e]));
                 } else {
-                    const Pair cc = R[k * RP + 3], cs = R[k * RP + 4];
+                    const Pair cc = RC0[k], cs = RC1[k];
 #pragma unroll
                     for (int e = 0; e < V; ++e) {
                         T x = fma_t<T>(G[0][e], cc.v[0], v[k][e]);
