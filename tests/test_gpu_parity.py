@@ -363,3 +363,135 @@ def test_inputs_device_generator_bitwise(lib):
         t = torch.empty(n, batch, dtype=tdt, device="cuda")
         inputs.fill_uniform_device(t, n, seed=42, scale=0.1)
         assert np.array_equal(t.cpu().numpy(), host)
+
+
+# ---- kernel variants: TMA prefetch / direct loads, warp scan / serial carry walk, vector widths --------
+
+def _solve_all(lib, n, batch, seed, f32=False):
+    """tri + penta + 2 CH steps through the current tune settings; returns [(got, ref, tol, tag)]."""
+    lt, lp = rand_tri(n, seed), rand_penta(n, seed + 1)
+    ht, hp = lib.tri_factor(*lt), lib.penta_factor(*lp)
+    dt = np.float32 if f32 else np.float64
+    rhs = inputs.uniform_rhs(n, batch, seed=seed).astype(dt)
+    out = []
+    ref = rhs.astype(np.float64)
+    oracle.tri_solve_interleaved(oracle.tri_factor(*lt), ref)
+    d = dev(rhs)
+    (lib.tri_solve_batched_f32 if f32 else lib.tri_solve_batched)(ht, d)
+    out.append((d.cpu().numpy(), ref, TOL_F32 if f32 else TOL_SINGLE, "tri"))
+    ref = rhs.astype(np.float64)
+    oracle.penta_solve_interleaved(oracle.penta_factor(*lp), ref)
+    d = dev(rhs)
+    (lib.penta_solve_batched_f32 if f32 else lib.penta_solve_batched)(hp, d)
+    out.append((d.cpu().numpy(), ref, TOL_F32 if f32 else TOL_SINGLE, "penta"))
+    if not f32:
+        lc = inputs.penta_lhs(n, 0.7)
+        hc = lib.penta_factor(*lc)
+        c0 = 0.5 * rhs
+        ref = c0.copy()
+        oracle.ch_step_interleaved(oracle.penta_factor(*lc), ref, 0.05, nsteps=2)
+        d = dev(c0)
+        lib.ch_step_batched(hc, d, 0.05, 2)
+        out.append((d.cpu().numpy(), ref, TOL_SINGLE, "ch"))
+    return out, ht.plan(4 if f32 else 8)
+
+
+@pytest.mark.parametrize("tune", [
+    dict(prefetch=0), dict(warp_scan=0), dict(prefetch=0, warp_scan=0), dict(vec=1), dict(vec=2), dict(vec=1, lanes=32),
+    dict(vec=2, lanes=32), dict(lanes=8), dict(tiles_per_cta=1), dict(rows=16), dict(rows=16, vec=2), dict(pdl=0),
+])
+@pytest.mark.parametrize("batch", [4096 + 64, 1001])  # 16-byte aligned pitch (TMA) / odd (direct loads, scalar tail)
+def test_kernel_variants_fp64(lib, tune, batch):
+    n = 300  # 10 partitions of 32 rows (padded), ragged last partition
+    try:
+        for k, v in tune.items():
+            lib.btps_tune(k, v)
+        res, plan = _solve_all(lib, n, batch, seed=21)
+    finally:
+        for k in tune:
+            lib.btps_tune(k, -1)
+    for got, ref, tol, tag in res:
+        assert rel_err(got, ref) <= tol, (tag, tune, batch, plan)
+
+
+@pytest.mark.parametrize("tune", [dict(), dict(vec=4), dict(vec=2), dict(vec=1), dict(prefetch=0), dict(warp_scan=0)])
+@pytest.mark.parametrize("batch", [2048 + 128, 999])
+def test_kernel_variants_fp32(lib, tune, batch):
+    n = 300
+    try:
+        for k, v in tune.items():
+            lib.btps_tune(k, v)
+        res, plan = _solve_all(lib, n, batch, seed=22, f32=True)
+    finally:
+        for k in tune:
+            lib.btps_tune(k, -1)
+    for got, ref, tol, tag in res:
+        assert rel_err(got, ref) <= tol, (tag, tune, batch, plan)
+
+
+@pytest.mark.parametrize("n", [530, 545, 1000, 1024, 1500, 2500])
+def test_partition_padding_and_serial_walk(lib, n):
+    """n = 530/545: odd partition counts are padded so groups are whole warps; 1000/1024: 32 partitions
+    (5-step scan, merged step-4 table slot); 1500/2500: more than 32 partitions -> serial carry walk."""
+    for batch in (515, 2048):
+        res, plan = _solve_all(lib, n, batch, seed=n)
+        for got, ref, tol, tag in res:
+            assert rel_err(got, ref) <= tol, (tag, n, batch, plan)
+    if n <= 1024:
+        assert plan["warp_scan"] == 1
+    else:
+        assert plan["warp_scan"] == 0
+
+
+def test_plan_reports_tma_and_ch_shape(lib):
+    h = lib.penta_factor(*inputs.penta_lhs(512, 0.5))
+    p, c = h.plan(8), h.ch_plan(8)
+    assert p["tma_prefetch"] == 1 and c["tma_prefetch"] == 1
+    assert p["partitions"] == c["partitions"] == 16
+    assert p["smem_bytes"] <= 227 * 1024 and c["smem_bytes"] <= 227 * 1024
+    big = lib.penta_factor(*inputs.penta_lhs(1024, 0.5))
+    assert big.plan(8)["tma_prefetch"] == 1 and big.plan(8)["smem_bytes"] <= 227 * 1024
+
+
+# ---- BASELINE.json's full sizes, in the launch configuration bench.py times: sampled systems ---------
+
+def _sample_ids(batch):
+    ids = np.concatenate([np.arange(0, 96), np.arange(batch - 96, batch),
+                          np.arange(97, batch - 96, max(1, batch // 257))])
+    return np.unique(ids).astype(np.int64)
+
+
+@pytest.mark.parametrize("kind,n,lb,f32", [("tri", 512, 16, False), ("penta", 512, 16, False), ("ch", 256, 20, False),
+                                           ("tri", 64, 20, False), ("penta", 1024, 18, False), ("tri", 1024, 18, True),
+                                           ("penta", 256, 20, True)])
+def test_full_size_sampled(lib, kind, n, lb, f32):
+    batch = 1 << lb
+    dtype = torch.float32 if f32 else torch.float64
+    scale = 0.1 if kind == "ch" else 1.0
+    d = torch.empty(n, batch, dtype=dtype, device="cuda")
+    inputs.fill_uniform_device(d, n, seed=5, scale=scale)
+    ids = _sample_ids(batch)
+    # the oracle regenerates its subset on the host (generator keyed on (system, row), bit-identical)
+    ref = inputs.uniform_rhs(n, len(ids), seed=5, scale=scale, systems=ids.astype(np.uint64))
+    if f32:
+        ref = ref.astype(np.float32).astype(np.float64)
+    assert np.array_equal(d[:, torch.from_numpy(ids).cuda()].cpu().numpy().astype(np.float64), ref)
+    if kind == "tri":
+        lhs = inputs.tri_lhs(n, 0.5)
+        h = lib.tri_factor(*lhs)
+        (lib.tri_solve_batched_f32 if f32 else lib.tri_solve_batched)(h, d)
+        oracle.tri_solve_interleaved(oracle.tri_factor(*lhs), ref)
+    elif kind == "penta":
+        lhs = inputs.penta_lhs(n, 0.5)
+        h = lib.penta_factor(*lhs)
+        (lib.penta_solve_batched_f32 if f32 else lib.penta_solve_batched)(h, d)
+        oracle.penta_solve_interleaved(oracle.penta_factor(*lhs), ref)
+    else:
+        lhs = inputs.ch_lhs(n)
+        _, alpha = inputs.ch_params(n)
+        h = lib.penta_factor(*lhs)
+        lib.ch_step_batched(h, d, alpha, 3)
+        oracle.ch_step_interleaved(oracle.penta_factor(*lhs), ref, alpha, nsteps=3)
+    got = d[:, torch.from_numpy(ids).cuda()].cpu().numpy().astype(np.float64)
+    assert rel_err(got, ref) <= (TOL_F32 if f32 else TOL_SINGLE), (kind, n, batch, h.plan(4 if f32 else 8))
+    assert bool(torch.isfinite(d).all())
