@@ -73,7 +73,9 @@ def peaks():
 def make_host_inputs(n, batch, seed, rank):
     import numpy as np
     import inputs
-    sys_ids = np.arange(rank * batch, (rank + 1) * batch, dtype=np.uint64)  # each rank: its own systems
+    from paper_2107_05395_b200 import sharding
+    j0, j1 = sharding.weak_shard(batch, rank)  # each rank: its own systems, no exchange
+    sys_ids = np.arange(j0, j1, dtype=np.uint64)
     u_tri, _, _ = inputs.sine_modes_u0(n, batch, seed=seed, systems=sys_ids)
     u_penta = inputs.uniform_rhs(n, batch, seed=seed, systems=sys_ids)
     c_ch = inputs.uniform_rhs(n, batch, seed=seed + 1, scale=0.1, systems=sys_ids)
