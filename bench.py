@@ -263,7 +263,22 @@ def extra_table(torch, b, inputs, peak):
         fn(bufs[0])
         ms = time_launches(torch, fn, bufs, launches) / steps_per_call
         gbs = 2.0 * size / ms / 1e6
+        extra = {}
+        if steps_per_call > 1:
+            # time loops advance up to 8 steps per launch while a tile is on chip (btps_tune "fuse_steps"):
+            # HBM then moves 2*N*M*sizeof(T) per 8 steps, so the per-step figure below is an EFFECTIVE rate
+            # (it may exceed the HBM peak); the same loop with one launch per step is timed beside it.
+            b.btps_tune("fuse_steps", 1)
+            try:
+                ms1 = time_launches(torch, fn, bufs, launches) / steps_per_call
+            finally:
+                b.btps_tune("fuse_steps", -1)
+            extra = {"fused_steps_per_launch": 8, "ms_per_solve_one_step_per_launch": round(ms1, 5),
+                     "hbm_gbs_one_step_per_launch": round(2.0 * size / ms1 / 1e6, 1),
+                     "frac_one_step_per_launch": round(2.0 * size / ms1 / 1e6 / peak, 4),
+                     "note": "hbm_gbs / frac_of_measured_peak are effective (per-step algorithmic bytes / time)"}
         out.append({"config": name, "kind": kind, "n": n, "batch": batch, "dtype": "f64" if elem == 8 else "f32",
+                    **extra,
                     "ms_per_solve": round(ms, 5), "systems_per_s": batch / ms * 1e3,
                     "unknowns_per_s": n * batch / ms * 1e3, "hbm_gbs": round(gbs, 1),
                     "frac_of_measured_peak": round(gbs / peak, 4),

@@ -142,7 +142,9 @@ BTPS_API int btps_plan_info(int kind, const void *handle, int elem_bytes, int *o
  * global).  key is one of "rows" (rows per thread: 8, 16, 32), "lanes" (32, 16, 8, 4),
  * "vec" (systems per thread: 1, 2, 4), "tiles_per_cta", "force_two_pass" (0/1), "prefetch"
  * (0: never use the TMA prefetch variant), "warp_scan" (0: serial carry walk), "pdl" (0: no
- * programmatic dependent launch attribute), "reverse"
+ * programmatic dependent launch attribute), "fuse_steps" (time steps advanced per launch while a tile
+ * is on chip in *_solve_steps / ch_step_batched: default 8, 1 = one launch per step), "grid" (cap on
+ * the number of CTAs), "reverse"
  * (0/1: alternate the tile order on successive steps of *_solve_steps / ch_step_batched so a
  * step starts on the data the previous one left in L2).  value < 0 restores the default. */
 BTPS_API int btps_tune(const char *key, int value);

@@ -52,7 +52,7 @@ std::atomic<long long> g_launches{0};
 // ------------------------------------------------------------------------------------------------
 struct Tune {
     int rows = -1, lanes = -1, vec = -1, tpc = -1, force_two_pass = -1, reverse = -1, prefetch = -1, pdl = -1,
-        warp_scan = -1, grid = -1;
+        warp_scan = -1, grid = -1, fuse = -1;
 };
 Tune g_tune;
 
@@ -61,8 +61,11 @@ Tune g_tune;
 // ------------------------------------------------------------------------------------------------
 struct KernelSlot {
     SweepEntry ent = {nullptr, nullptr, 0};
+    SweepEntry fused = {nullptr, nullptr, 0};  // multi-step form of the same variant (TMA variants)
+    int fused_ready = 0;
     int vec = 1;
     int tma = 0;       // 1: the TMA-prefetch variant (needs the ring in shared memory)
+    int xvals = 2;     // exchange values per (partition, system)
     size_t smem = 0;
     unsigned offX = 0, offM = 0, offR = 0;
     unsigned box_rows = 0, nboxes = 0;
@@ -487,11 +490,12 @@ constexpr size_t SMEM_LIMIT = 227 * 1024;
 size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
 // shared-memory layout of one kernel variant: [blob][exchange][mbarriers][ring]
-void layout_slot(const DtypePlan &pl, const Shape &sh, int kind, KernelSlot &sl)
+void layout_slot(const DtypePlan &pl, const Shape &sh, int kind, KernelSlot &sl, bool halo = true)
 {
     const int NC = (kind == KIND_TRI) ? 1 : 2;
     const size_t W = (size_t)sh.lanes * sl.vec;
-    const size_t xch = (pl.P > 1) ? (size_t)sh.tpc * 2 * NC * pl.P * W * pl.elem : 0;
+    sl.xvals = 2 * NC + ((kind == KIND_CH && halo) ? 2 : 0);  // CH: + the halo rows exchanged between fused steps
+    const size_t xch = (pl.P > 1) ? (size_t)sh.tpc * sl.xvals * pl.P * W * pl.elem : 0;
     sl.offX = (unsigned)align16(pl.blob_bytes);
     sl.offM = (unsigned)align16(sl.offX + xch);
     sl.offR = (unsigned)align_up(sl.offM + 17 * 8, 128);
@@ -514,16 +518,16 @@ bool tma_possible(const DtypePlan &pl, const Shape &sh, int vec)
     return true;
 }
 
-SweepEntry find_sweep(int kind, int elem_bytes, int vec, int rows, int single, int tma, int ws)
+SweepEntry find_sweep(int kind, int elem_bytes, int vec, int rows, int single, int tma, int ws, int fuse)
 {
     if (elem_bytes == 8) {
-        if (kind == KIND_TRI) return find_sweep_tri_f64(vec, rows, single, tma, ws);
-        if (kind == KIND_PENTA) return find_sweep_penta_f64(vec, rows, single, tma, ws);
-        return find_sweep_ch_f64(vec, rows, single, tma, ws);
+        if (kind == KIND_TRI) return find_sweep_tri_f64(vec, rows, single, tma, ws, fuse);
+        if (kind == KIND_PENTA) return find_sweep_penta_f64(vec, rows, single, tma, ws, fuse);
+        return find_sweep_ch_f64(vec, rows, single, tma, ws, fuse);
     }
-    if (kind == KIND_TRI) return find_sweep_tri_f32(vec, rows, single, tma, ws);
-    if (kind == KIND_PENTA) return find_sweep_penta_f32(vec, rows, single, tma, ws);
-    return find_sweep_ch_f32(vec, rows, single, tma, ws);
+    if (kind == KIND_TRI) return find_sweep_tri_f32(vec, rows, single, tma, ws, fuse);
+    if (kind == KIND_PENTA) return find_sweep_penta_f32(vec, rows, single, tma, ws, fuse);
+    return find_sweep_ch_f32(vec, rows, single, tma, ws, fuse);
 }
 
 void fit_plan(DtypePlan &pl, int handle_kind)
@@ -562,9 +566,17 @@ void fill_slots(Handle *h)
                     sl.max_grid = 0;
                     if (sl.tma && !tma_possible(pl, sh, sl.vec)) continue;
                     layout_slot(pl, sh, kind, sl);
+                    bool can_fuse = true;
+                    if (sl.smem > SMEM_LIMIT && kind == KIND_CH) {
+                        // tight fit (N = 1024 fp64): drop the halo exchange rows, one step per launch
+                        layout_slot(pl, sh, kind, sl, false);
+                        can_fuse = false;
+                    }
                     if (sl.smem > SMEM_LIMIT) continue;
-                    sl.ent = find_sweep(kind, pl.elem, sl.vec, pl.rows, single, sl.tma, pl.ws);
+                    sl.ent = find_sweep(kind, pl.elem, sl.vec, pl.rows, single, sl.tma, pl.ws, 0);
                     if (sl.ent.func && sl.ent.max_threads < sh.threads) sl.ent = SweepEntry{nullptr, nullptr, 0};
+                    sl.fused = SweepEntry{nullptr, nullptr, 0};
+                    if (sl.ent.func && sl.tma && can_fuse) sl.fused = find_sweep(kind, pl.elem, sl.vec, pl.rows, single, 1, pl.ws, 1);
                 }
             }
         }
@@ -578,6 +590,8 @@ int resolve_slot(Handle *h, const Shape &sh, KernelSlot &sl)
     if (!sl.ent.func) return set_err(BTPS_E_ARG);
     if (sl.smem > 48 * 1024)
         CU_TRY(cudaFuncSetAttribute(sl.ent.func, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sl.smem));
+    if (sl.fused.func && sl.smem > 48 * 1024)
+        CU_TRY(cudaFuncSetAttribute(sl.fused.func, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sl.smem));
     int occ = 0, sms = 0, dev = 0;
     CU_TRY(cudaGetDevice(&dev));
     CU_TRY(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
@@ -638,7 +652,8 @@ int make_tmap(CUtensorMap *tm, T *d_rhs, long long batch, int n, int W, unsigned
 
 // one sweep launch (kind = KIND_TRI / KIND_PENTA / KIND_CH) on a device buffer
 template <typename T>
-int launch_one(Handle *h, int kind, T *d_rhs, long long batch, double alpha_x, int reverse, cudaStream_t st)
+int launch_one(Handle *h, int kind, T *d_rhs, long long batch, double alpha_x, int reverse, int ksteps,
+               cudaStream_t st)
 {
     DtypePlan &pl = h->plan[sizeof(T) == 8 ? 0 : 1];
     if (pl.two_pass) {
@@ -652,7 +667,7 @@ int launch_one(Handle *h, int kind, T *d_rhs, long long batch, double alpha_x, i
             two_pass_kernel<T, KIND_CH><<<(unsigned)grid, block, 0, st>>>((const T *)pl.d_soa, d_rhs, batch, h->n, alpha_x);
         g_launches.fetch_add(1, std::memory_order_relaxed);
         CU_TRY(cudaGetLastError());
-        return BTPS_OK;
+        return BTPS_OK;  // fuse_limit() keeps ksteps == 1 for this plan
     }
     const int ks = (kind == KIND_CH) ? 1 : 0;
     const Shape &sh = pl.shape[ks];
@@ -692,6 +707,8 @@ int launch_one(Handle *h, int kind, T *d_rhs, long long batch, double alpha_x, i
     a.reverse = reverse;
     a.scan_log2 = pl.scan_log2;
     a.tq = pl.tq;
+    a.ksteps = ksteps;
+    a.xvals = sl.xvals;
     a.blob_bytes = pl.blob_bytes;
     a.offT = pl.offT;
     a.offX = sl.offX;
@@ -708,10 +725,27 @@ int launch_one(Handle *h, int kind, T *d_rhs, long long batch, double alpha_x, i
     long long grid = (a.num_tiles + sh.tpc - 1) / sh.tpc;
     if (grid > sl.max_grid) grid = sl.max_grid;
     if (g_tune.grid > 0 && grid > g_tune.grid) grid = g_tune.grid;
-    const cudaError_t e = sl.ent.launch(a, tm, (int)grid, sh.threads, sl.smem, st, g_tune.pdl != 0);
-    g_launches.fetch_add(1, std::memory_order_relaxed);
-    if (e != cudaSuccess) return cuda_fail(e, "sweep launch");
+    // several steps per launch need the fused instantiation; without one (direct-load variants)
+    // the steps are launched one by one
+    const bool fused = (ksteps > 1) && sl.fused.func;
+    const int nlaunch = fused ? 1 : ksteps;
+    a.ksteps = fused ? ksteps : 1;
+    for (int l = 0; l < nlaunch; ++l) {
+        const cudaError_t e = (fused ? sl.fused : sl.ent).launch(a, tm, (int)grid, sh.threads, sl.smem, st, g_tune.pdl != 0);
+        g_launches.fetch_add(1, std::memory_order_relaxed);
+        if (e != cudaSuccess) return cuda_fail(e, "sweep launch");
+    }
     return BTPS_OK;
+}
+
+// Time steps advanced per launch while a tile is on chip: systems never interact, so
+// the RHS = previous solution loop can run on the registers; HBM then sees one read
+// and one write per `fuse` steps.  The two-pass kernel advances one step per launch.
+int fuse_limit(const DtypePlan &pl)
+{
+    if (pl.two_pass) return 1;
+    const int k = g_tune.fuse > 0 ? g_tune.fuse : 8;
+    return k < 1 ? 1 : (k > 64 ? 64 : k);
 }
 
 Handle *check(const void *hv, int magic)
@@ -729,9 +763,12 @@ int solve_steps(const void *hv, int magic, int kind, T *d_rhs, int64_t batch, do
     if (!h || !d_rhs || batch < 1 || nsteps < 0) return set_err(BTPS_E_ARG);
     if ((uintptr_t)d_rhs % sizeof(T)) return set_err(BTPS_E_ALIGN);
     const bool rev = g_tune.reverse > 0;
-    for (int s = 0; s < nsteps; ++s) {
-        const int rc = launch_one<T>(h, kind, d_rhs, batch, alpha_x, rev ? (s & 1) : 0, (cudaStream_t)stream);
+    const int kmax = fuse_limit(h->plan[sizeof(T) == 8 ? 0 : 1]);
+    for (int s = 0, l = 0; s < nsteps; ++l) {
+        const int k = (nsteps - s < kmax) ? (nsteps - s) : kmax;
+        const int rc = launch_one<T>(h, kind, d_rhs, batch, alpha_x, rev ? (l & 1) : 0, k, (cudaStream_t)stream);
         if (rc != BTPS_OK) return rc;
+        s += k;
     }
     return set_err(BTPS_OK);
 }
@@ -791,9 +828,12 @@ int solve_host(const void *hv, int magic, int kind, T *h_rhs, int64_t batch, dou
         T *d = (T *)g_pipe.buf[b];
         CU_TRY(cudaMemcpy2DAsync(d, (size_t)w * sizeof(T), h_rhs + j0, (size_t)batch * sizeof(T),
                                  (size_t)w * sizeof(T), (size_t)n, cudaMemcpyHostToDevice, st));
-        for (int s = 0; s < nsteps; ++s) {
-            rc = launch_one<T>(h, kind, d, w, alpha_x, rev ? (s & 1) : 0, st);
+        const int kmax = fuse_limit(h->plan[sizeof(T) == 8 ? 0 : 1]);
+        for (int s = 0, l = 0; s < nsteps; ++l) {
+            const int k = (nsteps - s < kmax) ? (nsteps - s) : kmax;
+            rc = launch_one<T>(h, kind, d, w, alpha_x, rev ? (l & 1) : 0, k, st);
             if (rc != BTPS_OK) return rc;
+            s += k;
         }
         CU_TRY(cudaMemcpy2DAsync(h_rhs + j0, (size_t)batch * sizeof(T), d, (size_t)w * sizeof(T),
                                  (size_t)w * sizeof(T), (size_t)n, cudaMemcpyDeviceToHost, st));
@@ -996,6 +1036,7 @@ int btps_tune(const char *key, int value)
     else if (!strcmp(key, "pdl")) g_tune.pdl = value;
     else if (!strcmp(key, "warp_scan")) g_tune.warp_scan = value;
     else if (!strcmp(key, "grid")) g_tune.grid = value;
+    else if (!strcmp(key, "fuse_steps")) g_tune.fuse = value;
     else return set_err(BTPS_E_ARG);
     return set_err(BTPS_OK);
 }

@@ -2,8 +2,8 @@
 #include "inst_common.cuh"
 
 namespace btps {
-SweepEntry find_sweep_ch_f64(int vec, int rows, int single, int tma, int ws)
+SweepEntry find_sweep_ch_f64(int vec, int rows, int single, int tma, int ws, int fuse)
 {
-    return pick_f64<KIND_CH>(vec, rows, single, tma, ws);
+    return pick_f64<KIND_CH>(vec, rows, single, tma, ws, fuse);
 }
 }  // namespace btps

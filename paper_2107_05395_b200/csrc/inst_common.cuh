@@ -5,21 +5,28 @@
 
 namespace btps {
 
-template <typename T, int V, int MR, bool SINGLE, int KIND, bool TMA, bool WS>
+template <typename T, int V, int MR, bool SINGLE, int KIND, bool TMA, bool WS, bool FUSE = false>
 static SweepEntry make_entry()
 {
     SweepEntry e;
-    e.launch = &launch_sweep<T, V, MR, SINGLE, KIND, TMA, WS>;
-    e.func = reinterpret_cast<const void *>(&sweep_kernel<T, V, MR, SINGLE, KIND, TMA, WS>);
+    e.launch = &launch_sweep<T, V, MR, SINGLE, KIND, TMA, WS, FUSE>;
+    e.func = reinterpret_cast<const void *>(&sweep_kernel<T, V, MR, SINGLE, KIND, TMA, WS, FUSE>);
     e.max_threads = CtaShape<T, V, MR>::MAX_THREADS;
     return e;
 }
 
 // variants: single partition (no carries) with / without TMA; partitioned with the warp scan
-// (with / without TMA) or with the serial carry walk (direct loads only)
+// (with / without TMA) or with the serial carry walk (direct loads only); the fused multi-step
+// form exists for the TMA variants
 template <typename T, int V, int MR, int KIND>
-static SweepEntry pick_variant(int single, int tma, int ws)
+static SweepEntry pick_variant(int single, int tma, int ws, int fuse)
 {
+    if (fuse) {
+        if (!tma) return SweepEntry{nullptr, nullptr, 0};
+        if (single) return make_entry<T, V, MR, true, KIND, true, false, true>();
+        if (ws) return make_entry<T, V, MR, false, KIND, true, true, true>();
+        return SweepEntry{nullptr, nullptr, 0};
+    }
     if (single) return tma ? make_entry<T, V, MR, true, KIND, true, false>() : make_entry<T, V, MR, true, KIND, false, false>();
     if (ws) return tma ? make_entry<T, V, MR, false, KIND, true, true>() : make_entry<T, V, MR, false, KIND, false, true>();
     if (!tma) return make_entry<T, V, MR, false, KIND, false, false>();
@@ -28,12 +35,12 @@ static SweepEntry pick_variant(int single, int tma, int ws)
 }
 
 template <typename T, int V, int KIND>
-static SweepEntry pick_rows(int rows, int single, int tma, int ws)
+static SweepEntry pick_rows(int rows, int single, int tma, int ws, int fuse)
 {
     switch (rows) {
-        case 8: return pick_variant<T, V, 8, KIND>(single, tma, ws);
-        case 16: return pick_variant<T, V, 16, KIND>(single, tma, ws);
-        case 32: return pick_variant<T, V, 32, KIND>(single, tma, ws);
+        case 8: return pick_variant<T, V, 8, KIND>(single, tma, ws, fuse);
+        case 16: return pick_variant<T, V, 16, KIND>(single, tma, ws, fuse);
+        case 32: return pick_variant<T, V, 32, KIND>(single, tma, ws, fuse);
         default: break;
     }
     SweepEntry none = {nullptr, nullptr, 0};
@@ -41,31 +48,31 @@ static SweepEntry pick_rows(int rows, int single, int tma, int ws)
 }
 
 template <int KIND>
-static SweepEntry pick_f64(int vec, int rows, int single, int tma, int ws)
+static SweepEntry pick_f64(int vec, int rows, int single, int tma, int ws, int fuse)
 {
-    if (vec == 1) return pick_rows<double, 1, KIND>(rows, single, tma, ws);
-    if (vec == 2) return pick_rows<double, 2, KIND>(rows, single, tma, ws);
+    if (vec == 1) return pick_rows<double, 1, KIND>(rows, single, tma, ws, fuse);
+    if (vec == 2) return pick_rows<double, 2, KIND>(rows, single, tma, ws, fuse);
     SweepEntry none = {nullptr, nullptr, 0};
     return none;
 }
 
 template <int KIND>
-static SweepEntry pick_f32(int vec, int rows, int single, int tma, int ws)
+static SweepEntry pick_f32(int vec, int rows, int single, int tma, int ws, int fuse)
 {
-    if (vec == 1) return pick_rows<float, 1, KIND>(rows, single, tma, ws);
-    if (vec == 2) return pick_rows<float, 2, KIND>(rows, single, tma, ws);
-    if (vec == 4) return pick_rows<float, 4, KIND>(rows, single, tma, ws);
+    if (vec == 1) return pick_rows<float, 1, KIND>(rows, single, tma, ws, fuse);
+    if (vec == 2) return pick_rows<float, 2, KIND>(rows, single, tma, ws, fuse);
+    if (vec == 4) return pick_rows<float, 4, KIND>(rows, single, tma, ws, fuse);
     SweepEntry none = {nullptr, nullptr, 0};
     return none;
 }
 
 // kind in {TRI, PENTA, CH}; elem_bytes 8: vec in {1, 2}; 4: vec in {1, 2, 4}; rows in {8, 16, 32}
-SweepEntry find_sweep(int kind, int elem_bytes, int vec, int rows, int single, int tma, int ws);
-SweepEntry find_sweep_tri_f64(int vec, int rows, int single, int tma, int ws);
-SweepEntry find_sweep_tri_f32(int vec, int rows, int single, int tma, int ws);
-SweepEntry find_sweep_penta_f64(int vec, int rows, int single, int tma, int ws);
-SweepEntry find_sweep_penta_f32(int vec, int rows, int single, int tma, int ws);
-SweepEntry find_sweep_ch_f64(int vec, int rows, int single, int tma, int ws);
-SweepEntry find_sweep_ch_f32(int vec, int rows, int single, int tma, int ws);
+SweepEntry find_sweep(int kind, int elem_bytes, int vec, int rows, int single, int tma, int ws, int fuse);
+SweepEntry find_sweep_tri_f64(int vec, int rows, int single, int tma, int ws, int fuse);
+SweepEntry find_sweep_tri_f32(int vec, int rows, int single, int tma, int ws, int fuse);
+SweepEntry find_sweep_penta_f64(int vec, int rows, int single, int tma, int ws, int fuse);
+SweepEntry find_sweep_penta_f32(int vec, int rows, int single, int tma, int ws, int fuse);
+SweepEntry find_sweep_ch_f64(int vec, int rows, int single, int tma, int ws, int fuse);
+SweepEntry find_sweep_ch_f32(int vec, int rows, int single, int tma, int ws, int fuse);
 
 }  // namespace btps

@@ -53,6 +53,8 @@ struct SweepArgs {
     int reverse;           // 1: walk the tiles from the last to the first
     int scan_log2;         // warp scan: log2 of the scan width (smallest power of two >= P)
     int tq;                // partitions per scan-table row (max(32, P))
+    int ksteps;            // time steps advanced per tile while it is on chip (>= 1)
+    int xvals;             // values per (partition, system) in the exchange area: 2*NC (+2 halo rows, CH)
     unsigned blob_bytes;   // multiple of 16
     unsigned offT;         // byte offset of the scan tables inside the blob (row records start at 0)
     unsigned offX;         // byte offset of the exchange area in shared memory
@@ -205,8 +207,10 @@ __device__ __forceinline__ void scan_steps(int n, F &&f)
 //   TMA    next tile prefetched by TMA into the shared-memory ring (else direct global loads)
 //   WS     carries by the warp-shuffle scan (needs P <= 32 and whole-warp groups); else each
 //          thread walks the partitions before / after it serially (any P)
+//   FUSE   a.ksteps time steps per tile (separate instantiation: the step loop costs registers, so
+//          single-step launches run the FUSE = false kernel)
 // -----------------------------------------------------------------------------------------------
-template <typename T, int V, int MR, bool SINGLE, int KIND, bool TMA, bool WS>
+template <typename T, int V, int MR, bool SINGLE, int KIND, bool TMA, bool WS, bool FUSE>
 __global__ void __launch_bounds__(CtaShape<T, V, MR>::MAX_THREADS, 1)
 sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
 {
@@ -258,7 +262,7 @@ sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
     [[maybe_unused]] const Pair *const RC1 = reinterpret_cast<const Pair *>(cb + 7 * Np) + r0;  // penta {psi1, psi2}
     [[maybe_unused]] const T *const TAB = reinterpret_cast<const T *>(smem + a.offT);
     // exchange area of this group: [2*NC values][P][W], columns XOR-swizzled with the partition index
-    [[maybe_unused]] T *const xb = reinterpret_cast<T *>(smem + a.offX) + (size_t)sub * 2 * NC * a.P * W;
+    [[maybe_unused]] T *const xb = reinterpret_cast<T *>(smem + a.offX) + (size_t)sub * a.xvals * a.P * W;
     // prefetch ring of this group: [P*MR rows][W]
     [[maybe_unused]] const unsigned ring_bytes = (unsigned)(a.P * MR * W) * (unsigned)sizeof(T);
     [[maybe_unused]] T *const ring = reinterpret_cast<T *>(smem + a.offR + (size_t)sub * ring_bytes);
@@ -334,6 +338,22 @@ sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
             }
         }
 
+        // ---- ksteps time steps on the tile while it is on chip (RHS = previous solution) ----
+        const int nks = FUSE ? a.ksteps : 1;
+        for (int ks = 0; ks < nks; ++ks) {
+        if constexpr (KIND == KIND_CH && !SINGLE) {
+            if (ks > 0) {
+                // halo rows of c^{n+ks}: the neighbouring partitions' first / last rows, published to
+                // exchange values 2NC (first row) and 2NC+1 (last row) at the end of the previous step
+                group_sync(a.tpc, sub, tpt);
+                const int hv = a.P * W, hm = W - 1;
+#pragma unroll
+                for (int e = 0; e < V; ++e) {
+                    cm[e] = (part > 0) ? xb[(2 * NC + 1) * hv + (part - 1) * W + ((sl * V + e) ^ ((part - 1) & hm))] : T(0);
+                    cp[e] = (part + 1 < a.P) ? xb[2 * NC * hv + (part + 1) * W + ((sl * V + e) ^ ((part + 1) & hm))] : T(0);
+                }
+            }
+        }
         [[maybe_unused]] T glast2[V];  // penta: g at the partition's last-but-one row (overwritten by the backward sweep)
         if constexpr (TRI) {
             // ---- local forward sweep, zero incoming carry ---------------------------------
@@ -608,7 +628,6 @@ sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
                     }
                 }
             }
-#undef XI
             // ---- correction: x_k = x^_k + chi_k . G + psi_k . X ------------------------------------
 #pragma unroll
             for (int k = 0; k < MR; ++k) {
@@ -628,7 +647,18 @@ sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
                     }
                 }
             }
+            if constexpr (KIND == KIND_CH) {
+                if (ks + 1 < nks) {  // publish this partition's first / last rows for the next step
+#pragma unroll
+                    for (int e = 0; e < V; ++e) {
+                        xc[2 * NC * vstr + XI(e)] = v[0][e];
+                        xc[(2 * NC + 1) * vstr + XI(e)] = v[MR - 1][e];
+                    }
+                }
+            }
+#undef XI
         }
+        }  // ksteps
 
         // ---- store ---------------------------------------------------------------------------
         {
@@ -717,7 +747,7 @@ struct SweepEntry {
     int max_threads;   // threads per CTA the kernel was compiled for
 };
 
-template <typename T, int V, int MR, bool SINGLE, int KIND, bool TMA, bool WS>
+template <typename T, int V, int MR, bool SINGLE, int KIND, bool TMA, bool WS, bool FUSE>
 cudaError_t launch_sweep(const SweepArgs &a, const CUtensorMap &tm, int grid, int block, size_t smem,
                          cudaStream_t st, int pdl)
 {
@@ -731,7 +761,7 @@ cudaError_t launch_sweep(const SweepArgs &a, const CUtensorMap &tm, int grid, in
     attr[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = attr;
     cfg.numAttrs = pdl ? 1 : 0;
-    return cudaLaunchKernelEx(&cfg, sweep_kernel<T, V, MR, SINGLE, KIND, TMA, WS>, a, tm);
+    return cudaLaunchKernelEx(&cfg, sweep_kernel<T, V, MR, SINGLE, KIND, TMA, WS, FUSE>, a, tm);
 }
 
 }  // namespace btps

@@ -495,3 +495,46 @@ def test_full_size_sampled(lib, kind, n, lb, f32):
     got = d[:, torch.from_numpy(ids).cuda()].cpu().numpy().astype(np.float64)
     assert rel_err(got, ref) <= (TOL_F32 if f32 else TOL_SINGLE), (kind, n, batch, h.plan(4 if f32 else 8))
     assert bool(torch.isfinite(d).all())
+
+
+# ---- fused time steps (several steps per launch while the tile is on chip) ---------------------------
+
+@pytest.mark.parametrize("n,batch", [(300, 2048 + 32), (20, 640), (512, 1024), (1000, 512)])
+def test_fused_steps_equal_single_step_launches(lib, n, batch):
+    """tri/penta_solve_steps and ch_step_batched advance up to 8 steps per launch; the arithmetic per
+    step is the same as one launch per step, so the results must be bitwise equal -- and both must
+    match the oracle's step-by-step loop."""
+    steps = 11  # one launch of 8 + one of 3
+    lt, lp, lc = inputs.tri_lhs(n, 0.5), inputs.penta_lhs(n, 0.5), inputs.penta_lhs(n, 0.7)
+    rhs = inputs.uniform_rhs(n, batch, seed=31)
+    c0 = 0.5 * rhs
+    outs = {}
+    for fuse in (1, -1, 3):
+        try:
+            lib.btps_tune("fuse_steps", fuse)
+            ht, hp, hc = lib.tri_factor(*lt), lib.penta_factor(*lp), lib.penta_factor(*lc)
+            n0 = lib.btps_launch_count()
+            dt_, dp_, dc_ = dev(rhs), dev(rhs), dev(c0)
+            lib.tri_solve_steps(ht, dt_, steps)
+            lib.penta_solve_steps(hp, dp_, steps)
+            lib.ch_step_batched(hc, dc_, 0.05, steps)
+            outs[fuse] = (dt_.cpu().numpy(), dp_.cpu().numpy(), dc_.cpu().numpy(), lib.btps_launch_count() - n0)
+        finally:
+            lib.btps_tune("fuse_steps", -1)
+    # 11 steps: 11 launches unfused, 2 (8 + 3) by default, 4 with fuse_steps = 3; a variant without a
+    # fused form (CH at n = 1000: no room for the halo exchange rows) falls back to one launch per step
+    assert outs[1][3] == 3 * steps and 3 * 2 <= outs[-1][3] <= outs[3][3] < 3 * steps
+    if n <= 512:
+        assert outs[-1][3] == 3 * 2 and outs[3][3] == 3 * 4
+    for k in (-1, 3):
+        for a, b_ in zip(outs[1][:3], outs[k][:3]):
+            assert np.array_equal(a, b_)
+    ref = rhs.copy()
+    oracle.tri_solve_interleaved(oracle.tri_factor(*lt), ref, nsteps=steps)
+    assert rel_err(outs[-1][0], ref) <= TOL_STEPS
+    ref = rhs.copy()
+    oracle.penta_solve_interleaved(oracle.penta_factor(*lp), ref, nsteps=steps)
+    assert rel_err(outs[-1][1], ref) <= TOL_STEPS
+    ref = c0.copy()
+    oracle.ch_step_interleaved(oracle.penta_factor(*lc), ref, 0.05, nsteps=steps)
+    assert rel_err(outs[-1][2], ref) <= TOL_STEPS
