@@ -346,8 +346,9 @@ void build_blob_tri(int n, DtypePlan &pl, const std::vector<double> &inv, const 
     blob.assign(pl.blob_bytes, 0);
     std::vector<double> phi(MR), chi(MR), psi(MR);
     std::vector<Mat> Phi(P), Psi(P), Chi0(P);
-    auto putv = [&](int arr, int i, int j, double v) {  // array at element offset arr*Np, entry i, value j
-        put<T>(blob, ((size_t)arr * Np + (size_t)i * (arr == 2 ? 1 : 2) + j) * sizeof(T), v);
+    auto putv = [&](int arr, int i, int j, double v) {  // partition block, array at offset arr*MR, row i, value j
+        const size_t blk = (size_t)(i / MR) * RT * MR;
+        put<T>(blob, (blk + (size_t)arr * MR + (size_t)(i % MR) * (arr == 2 ? 1 : 2) + j) * sizeof(T), v);
     };
     for (int p = 0; p < P; ++p) {
         const int r0 = p * MR;
@@ -397,8 +398,9 @@ void build_blob_penta(int n, DtypePlan &pl, const std::vector<double> &inv, cons
         psi[t].resize(MR);
     }
     std::vector<Mat> Phi(P), Psi(P), Chi0(P);
-    auto putv = [&](int arr, int i, int j, double v) {  // array at element offset arr*Np, entry i, value j
-        put<T>(blob, ((size_t)arr * Np + (size_t)i * (arr == 2 ? 1 : 2) + j) * sizeof(T), v);
+    auto putv = [&](int arr, int i, int j, double v) {  // partition block, array at offset arr*MR, row i, value j
+        const size_t blk = (size_t)(i / MR) * RT * MR;
+        put<T>(blob, (blk + (size_t)arr * MR + (size_t)(i % MR) * (arr == 2 ? 1 : 2) + j) * sizeof(T), v);
     };
     for (int p = 0; p < P; ++p) {
         const int r0 = p * MR;

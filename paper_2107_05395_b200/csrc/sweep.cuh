@@ -107,12 +107,13 @@ template <typename T>
 __device__ __forceinline__ T ch_w(T c) { return fma_t<T>(c * c, c, -c); }
 
 // Coefficient image ("blob"), all in element type T, rows padded to Np = P*MR with identity rows.
-// Structure of arrays, one entry per row, pairs {T,T} where one phase of a row needs two values
-// (one LDS.128 in fp64); element offsets of the arrays in units of Np:
-//   tri   (5 Np): 0: {inv, nl}   2: nch    3: {chi, psi}
+// One block per partition (MR rows), inside it a structure of arrays with one entry per row, pairs
+// {T,T} where one phase of a row needs two values (one LDS.128 in fp64), so that a thread addresses
+// everything as one base + compile-time offsets; element offsets of the arrays in units of MR:
+//   tri   (5 MR): 0: {inv, nl}   2: nch    3: {chi, psi}
 //           inv = 1/b^_i, nl = -a_i/b^_i, nch = -c^_i; chi/psi = response of the finished local
 //           sweeps to the incoming forward / backward carry
-//   penta (9 Np): 0: {inv, nle}  2: nlb    3: {ngam, ndel}   5: {chi1, chi2}   7: {psi1, psi2}
+//   penta (9 MR): 0: {inv, nle}  2: nlb    3: {ngam, ndel}   5: {chi1, chi2}   7: {psi1, psi2}
 //           inv = 1/alpha_i, nle = -eps_i/alpha_i, nlb = -beta_i/alpha_i, ngam = -gamma_i, ndel = -delta_i
 // followed at offT by the carry-scan tables, indexed [slot][m][q] with q = partition (tq entries),
 // m = entry of the NC x NC matrix (row-major), NC = 1 (tri) or 2 (penta):
@@ -252,14 +253,14 @@ sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
     int nrow_part = a.n - r0;
     nrow_part = nrow_part < 0 ? 0 : (nrow_part > MR ? MR : nrow_part);
 
-    // coefficient arrays of this partition's rows (RecLayout): Np = P*MR rows each
-    const int Np = a.P * MR;
-    const T *const cb = reinterpret_cast<const T *>(smem);
-    const Pair *const RA = reinterpret_cast<const Pair *>(cb) + r0;                        // {inv, nl | nle}
-    const T *const RB1 = cb + 2 * Np + r0;                                                 // nch | nlb
-    [[maybe_unused]] const Pair *const RBW = reinterpret_cast<const Pair *>(cb + 3 * Np) + r0;  // {chi, psi} | {ngam, ndel}
-    [[maybe_unused]] const Pair *const RC0 = reinterpret_cast<const Pair *>(cb + 5 * Np) + r0;  // penta {chi1, chi2}
-    [[maybe_unused]] const Pair *const RC1 = reinterpret_cast<const Pair *>(cb + 7 * Np) + r0;  // penta {psi1, psi2}
+    // coefficient arrays of this partition's rows (RecLayout): one base address, the arrays at
+    // compile-time offsets from it
+    const T *const cb = reinterpret_cast<const T *>(smem) + (size_t)part * (RecLayout<KIND>::ELEMS * MR);
+    const Pair *const RA = reinterpret_cast<const Pair *>(cb);                             // {inv, nl | nle}
+    const T *const RB1 = cb + 2 * MR;                                                      // nch | nlb
+    [[maybe_unused]] const Pair *const RBW = reinterpret_cast<const Pair *>(cb + 3 * MR);  // {chi, psi} | {ngam, ndel}
+    [[maybe_unused]] const Pair *const RC0 = reinterpret_cast<const Pair *>(cb + 5 * MR);  // penta {chi1, chi2}
+    [[maybe_unused]] const Pair *const RC1 = reinterpret_cast<const Pair *>(cb + 7 * MR);  // penta {psi1, psi2}
     [[maybe_unused]] const T *const TAB = reinterpret_cast<const T *>(smem + a.offT);
     // exchange area of this group: [2*NC values][P][W], columns XOR-swizzled with the partition index
     [[maybe_unused]] T *const xb = reinterpret_cast<T *>(smem + a.offX) + (size_t)sub * a.xvals * a.P * W;
@@ -301,7 +302,8 @@ sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
             // ---- take the prefetched tile out of the ring, then have it refilled ---------------
             mbar_wait(mbar, phase);
             phase ^= 1u;
-            const T *const rp = ring + (r0 * W + sl * V);
+            const T *rp = ring + (r0 * W + sl * V);
+            asm volatile("" : "+l"(rp));  // recompute the MR row addresses per tile: hoisted out of the loop they spill
 #pragma unroll
             for (int k = 0; k < MR; ++k) ld_sys<T, V>(v[k], rp + k * W);
             if constexpr (KIND == KIND_CH) {
@@ -456,7 +458,8 @@ sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
             const int tq = a.tq;
             const int wm = W - 1;
             // this thread's columns of its partition: element e lives at xc[XI(e)]
-            T *const xc = xb + (size_t)part * W;
+            T *xc = xb + (size_t)part * W;
+            if constexpr (FUSE) asm volatile("" : "+l"(xc));
             const int xsw = part & wm;
 #define XI(e) (((sl * V + (e)) ^ xsw))
             const int vstr = P * W;  // elements between successive values
@@ -476,12 +479,13 @@ sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
                 }
                 group_sync(a.tpc, sub, tpt);
                 {
-                    // one scan job = one system: lane q of a `width`-lane segment holds partition q
+                    // lane q of a `width`-lane segment holds partition q
                     const int lane = lt & 31;
                     const int wd = 1 << a.scan_log2;
                     const int q = lane & (wd - 1);
-                    const int spw = 32 >> a.scan_log2;  // systems per warp pass
-                    const T *const tb = TAB + q;
+                    const int spw = 32 >> a.scan_log2;  // jobs per warp pass
+                    const T *tb = TAB + q;
+                    if constexpr (FUSE) asm volatile("" : "+l"(tb));
                     const int mstr = tq;                // elements between matrix entries
                     const int sstr = NC * NC * tq;      // elements between table slots
                     // multipliers of step st: slots 2st (forward) / 2st+1 (backward); step 4 shares
@@ -495,63 +499,88 @@ sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
                         const T val = tb[(st < 4 ? 2 * st + 1 : 8) * sstr + m * mstr];
                         return (st < 4 || q < 16) ? val : T(0);
                     };
-                    for (int s0 = (lt >> 5) * spw; s0 < W; s0 += (tpt >> 5) * spw) {
-                        const int col = s0 + (lane >> a.scan_log2);
-                        const bool ok = (q < P) && (col < W);
-                        T *const xs = xb + (size_t)q * W + (col ^ (q & wm));
-                        if constexpr (TRI) {
-                            T b = ok ? xs[0] : T(0);
-                            const T xf = ok ? xs[vstr] : T(0);
-                            scan_steps<sizeof(T) == 4>(a.scan_log2, [&](int st) {
-                                const T o = __shfl_up_sync(0xffffffffu, b, 1 << st, wd);
-                                b = fma_t<T>(fwm(st, 0), o, b);
-                            });
-                            T g = __shfl_up_sync(0xffffffffu, b, 1, wd);
-                            g = (q == 0) ? T(0) : g;
-                            T c = fma_t<T>(tb[9 * sstr], g, xf);
-                            scan_steps<sizeof(T) == 4>(a.scan_log2, [&](int st) {
-                                const T o = __shfl_down_sync(0xffffffffu, c, 1 << st, wd);
-                                c = fma_t<T>(bwm(st, 0), o, c);
-                            });
-                            T x = __shfl_down_sync(0xffffffffu, c, 1, wd);
-                            x = (q + 1 < P) ? x : T(0);
-                            if (ok) {
-                                xs[0] = g;
-                                xs[vstr] = x;
+                    // job = the V systems of one owner thread column sg: V independent chains per lane
+                    for (int s0 = (lt >> 5) * spw; s0 < a.lanes; s0 += (tpt >> 5) * spw) {
+                        const int sg = s0 + (lane >> a.scan_log2);
+                        const bool ok = (q < P) && (sg < a.lanes);
+                        T *xs = xb + (size_t)q * W;
+                        if constexpr (FUSE) asm volatile("" : "+l"(xs));  // (as for rp: hoisted out of the step loop it spills)
+                        const int qsw = q & wm;
+                        T fb[NC][V], bb[NC][V];  // forward / backward scan state (then the carries G / X)
+#pragma unroll
+                        for (int c = 0; c < NC; ++c)
+#pragma unroll
+                            for (int e = 0; e < V; ++e) {
+                                const int ix = (sg * V + e) ^ qsw;
+                                fb[c][e] = ok ? xs[c * vstr + ix] : T(0);
+                                bb[c][e] = ok ? xs[(NC + c) * vstr + ix] : T(0);
                             }
-                        } else {
-                            T b1 = ok ? xs[0] : T(0), b2 = ok ? xs[vstr] : T(0);
-                            const T xf0 = ok ? xs[2 * vstr] : T(0), xf1 = ok ? xs[3 * vstr] : T(0);
-                            scan_steps<sizeof(T) == 4>(a.scan_log2, [&](int st) {
-                                const T o1 = __shfl_up_sync(0xffffffffu, b1, 1 << st, wd);
-                                const T o2 = __shfl_up_sync(0xffffffffu, b2, 1 << st, wd);
-                                b1 = fma_t<T>(fwm(st, 1), o2, fma_t<T>(fwm(st, 0), o1, b1));
-                                b2 = fma_t<T>(fwm(st, 3), o2, fma_t<T>(fwm(st, 2), o1, b2));
-                            });
-                            T g1 = __shfl_up_sync(0xffffffffu, b1, 1, wd);
-                            T g2 = __shfl_up_sync(0xffffffffu, b2, 1, wd);
-                            g1 = (q == 0) ? T(0) : g1;
-                            g2 = (q == 0) ? T(0) : g2;
-                            const T *const ch = tb + 9 * sstr;  // chi at the partition's first two rows
-                            T c1 = fma_t<T>(ch[mstr], g2, fma_t<T>(ch[0], g1, xf0));
-                            T c2 = fma_t<T>(ch[3 * mstr], g2, fma_t<T>(ch[2 * mstr], g1, xf1));
-                            scan_steps<sizeof(T) == 4>(a.scan_log2, [&](int st) {
-                                const T o1 = __shfl_down_sync(0xffffffffu, c1, 1 << st, wd);
-                                const T o2 = __shfl_down_sync(0xffffffffu, c2, 1 << st, wd);
-                                c1 = fma_t<T>(bwm(st, 1), o2, fma_t<T>(bwm(st, 0), o1, c1));
-                                c2 = fma_t<T>(bwm(st, 3), o2, fma_t<T>(bwm(st, 2), o1, c2));
-                            });
-                            T x1 = __shfl_down_sync(0xffffffffu, c1, 1, wd);
-                            T x2 = __shfl_down_sync(0xffffffffu, c2, 1, wd);
-                            x1 = (q + 1 < P) ? x1 : T(0);
-                            x2 = (q + 1 < P) ? x2 : T(0);
-                            if (ok) {
-                                xs[0] = g1;
-                                xs[vstr] = g2;
-                                xs[2 * vstr] = x1;
-                                xs[3 * vstr] = x2;
+                        scan_steps<sizeof(T) == 4>(a.scan_log2, [&](int st) {
+                            T m[NC * NC];
+#pragma unroll
+                            for (int i = 0; i < NC * NC; ++i) m[i] = fwm(st, i);
+#pragma unroll
+                            for (int e = 0; e < V; ++e) {
+                                T o[NC];
+#pragma unroll
+                                for (int c = 0; c < NC; ++c) o[c] = __shfl_up_sync(0xffffffffu, fb[c][e], 1 << st, wd);
+                                if constexpr (TRI) {
+                                    fb[0][e] = fma_t<T>(m[0], o[0], fb[0][e]);
+                                } else {
+                                    fb[0][e] = fma_t<T>(m[1], o[1], fma_t<T>(m[0], o[0], fb[0][e]));
+                                    fb[1][e] = fma_t<T>(m[3], o[1], fma_t<T>(m[2], o[0], fb[1][e]));
+                                }
+                            }
+                        });
+                        {
+                            // carry INTO partition q = inclusive result of partition q-1; then the local
+                            // back-substitution's first rows given that carry: u = x^_first + chi G
+                            T ch[NC * NC];
+#pragma unroll
+                            for (int i = 0; i < NC * NC; ++i) ch[i] = tb[9 * sstr + i * mstr];
+#pragma unroll
+                            for (int e = 0; e < V; ++e) {
+#pragma unroll
+                                for (int c = 0; c < NC; ++c) {
+                                    const T g = __shfl_up_sync(0xffffffffu, fb[c][e], 1, wd);
+                                    fb[c][e] = (q == 0) ? T(0) : g;
+                                }
+                                if constexpr (TRI) {
+                                    bb[0][e] = fma_t<T>(ch[0], fb[0][e], bb[0][e]);
+                                } else {
+                                    bb[0][e] = fma_t<T>(ch[1], fb[1][e], fma_t<T>(ch[0], fb[0][e], bb[0][e]));
+                                    bb[1][e] = fma_t<T>(ch[3], fb[1][e], fma_t<T>(ch[2], fb[0][e], bb[1][e]));
+                                }
                             }
                         }
+                        scan_steps<sizeof(T) == 4>(a.scan_log2, [&](int st) {
+                            T m[NC * NC];
+#pragma unroll
+                            for (int i = 0; i < NC * NC; ++i) m[i] = bwm(st, i);
+#pragma unroll
+                            for (int e = 0; e < V; ++e) {
+                                T o[NC];
+#pragma unroll
+                                for (int c = 0; c < NC; ++c) o[c] = __shfl_down_sync(0xffffffffu, bb[c][e], 1 << st, wd);
+                                if constexpr (TRI) {
+                                    bb[0][e] = fma_t<T>(m[0], o[0], bb[0][e]);
+                                } else {
+                                    bb[0][e] = fma_t<T>(m[1], o[1], fma_t<T>(m[0], o[0], bb[0][e]));
+                                    bb[1][e] = fma_t<T>(m[3], o[1], fma_t<T>(m[2], o[0], bb[1][e]));
+                                }
+                            }
+                        });
+#pragma unroll
+                        for (int c = 0; c < NC; ++c)
+#pragma unroll
+                            for (int e = 0; e < V; ++e) {
+                                const T x = __shfl_down_sync(0xffffffffu, bb[c][e], 1, wd);
+                                const int ix = (sg * V + e) ^ qsw;
+                                if (ok) {
+                                    xs[c * vstr + ix] = fb[c][e];
+                                    xs[(NC + c) * vstr + ix] = (q + 1 < P) ? x : T(0);
+                                }
+                            }
                     }
                 }
                 group_sync(a.tpc, sub, tpt);
