@@ -120,9 +120,8 @@ int thread_cap(int rows, int vec, int elem) { return (rows * vec * elem > 256) ?
 
 void choose_shape(int kind, int elem, int rows, int P, Shape &sh)
 {
-    // 16 bytes per thread and row (one LDS.128 / ST.128) for the solves; the CH step keeps one
-    // system per thread (its explicit half needs the registers)
-    int vec = g_tune.vec > 0 ? g_tune.vec : (kind == KIND_CH ? 1 : 16 / elem);
+    // 16 bytes per thread and row (one LDS.128 / ST.128)
+    int vec = g_tune.vec > 0 ? g_tune.vec : 16 / elem;
     if (vec != 1 && vec != 2 && vec != 4) vec = 1;
     if (vec * elem > 16) vec = 16 / elem;  // one vector access is at most 16 bytes
     const int cap = thread_cap(rows, vec, elem);
