@@ -65,6 +65,15 @@ def _load():
                                                 _ll, _ll, _ll, ctypes.c_double, ctypes.c_int,
                                                 ctypes.c_int]
         lib.orc_ch_step_interleaved.restype = ctypes.c_int
+        lib.orc_tri_periodic_factor.argtypes = [ctypes.c_int, _dp, _dp, _dp, _dp, _dp, _dp]
+        lib.orc_tri_periodic_factor.restype = ctypes.c_int
+        lib.orc_tri_periodic_solve.argtypes = [ctypes.c_int, _dp, _dp, _dp, _dp, ctypes.c_double,
+                                               ctypes.c_double, _dp]
+        lib.orc_tri_periodic_solve.restype = None
+        lib.orc_tri_periodic_solve_interleaved.argtypes = [ctypes.c_int, _dp, _dp, _dp, _dp,
+                                                           ctypes.c_double, ctypes.c_double, _dp, _ll,
+                                                           _ll, _ll, _ll, ctypes.c_int, ctypes.c_int]
+        lib.orc_tri_periodic_solve_interleaved.restype = ctypes.c_int
         _lib = lib
     return _lib
 
@@ -184,3 +193,46 @@ def ch_step_interleaved(fac: PentaFactor, c: np.ndarray, alpha: float, nsteps: i
     return _load().orc_ch_step_interleaved(fac.n, _p(fac.eps), _p(fac.beta), _p(fac.alpha),
                                            _p(fac.gamma), _p(fac.delta), _p(c), M, jlo, jhi, js,
                                            float(alpha), nsteps, nthreads)
+
+
+# ---- periodic tridiagonal (eq. 12-15) ---------------------------------------------
+
+@dataclass
+class TriPeriodicFactor:
+    n: int
+    a: np.ndarray   # sub-diagonal; a[0] was the corner entry (row 1, column N)
+    bh: np.ndarray  # b^ of A' (eq. 13b)
+    ch: np.ndarray  # c^ of A'
+    z: np.ndarray   # A'^{-1} u (eq. 14)
+    vN: float       # last entry of v (eq. 13a)
+    den: float      # 1 + v.z (eq. 15)
+
+
+def tri_periodic_factor(a, b, c) -> TriPeriodicFactor:
+    """Cyclic tridiagonal matrix: row i is a[i] x[i-1] + b[i] x[i] + c[i] x[i+1] with indices mod n,
+    i.e. a[0] multiplies x[n-1] and c[n-1] multiplies x[0]."""
+    a, b, c = _f64(a), _f64(b), _f64(c)
+    n = b.size
+    assert a.size == n and c.size == n
+    z = np.zeros(n)
+    vN, den = ctypes.c_double(0.0), ctypes.c_double(0.0)
+    rc = _load().orc_tri_periodic_factor(n, _p(a), _p(b), _p(c), _p(z), ctypes.byref(vN), ctypes.byref(den))
+    if rc:
+        raise FactorError(rc)
+    return TriPeriodicFactor(n, a, b, c, z, vN.value, den.value)
+
+
+def tri_periodic_solve(fac: TriPeriodicFactor, d) -> np.ndarray:
+    x = _f64(d)
+    assert x.shape == (fac.n,)
+    _load().orc_tri_periodic_solve(fac.n, _p(fac.a), _p(fac.bh), _p(fac.ch), _p(fac.z), fac.vN, fac.den, _p(x))
+    return x
+
+
+def tri_periodic_solve_interleaved(fac: TriPeriodicFactor, rhs: np.ndarray, nsteps: int = 1, subset=None,
+                                   nthreads: int = 0) -> int:
+    assert rhs.ndim == 2 and rhs.shape[0] == fac.n
+    M = rhs.shape[1]
+    jlo, jhi, js = _subset(M, subset)
+    return _load().orc_tri_periodic_solve_interleaved(fac.n, _p(fac.a), _p(fac.bh), _p(fac.ch), _p(fac.z),
+                                                      fac.vN, fac.den, _p(rhs), M, jlo, jhi, js, nsteps, nthreads)

@@ -16,6 +16,7 @@
  *   orc_penta_factor    PAPER.md:219-256 (Sec. 4.1 steps 1-14), 601-637 (Alg. 3)
  *   orc_penta_solve     PAPER.md:258-278 (Sec. 4.1), 639-676 (Alg. 4)
  *   orc_ch_rhs          PAPER.md:365-392 (eq. 24, 25a, 26c)
+ *   orc_tri_periodic_*  PAPER.md:140-164 (Sec. 3.3, eq. 12-15: Sherman-Morrison)
  *   *_interleaved       PAPER.md:69 (Sec. 2), Alg. 2 "rowID +- M": element i of
  *                       system j lives at rhs[i*M + j]
  *
@@ -27,7 +28,9 @@
  * eigenpairs of Toeplitz tri / penta (I + r T^2) matrices, exact modal decay over 100
  * steps, L*R == A rebuilt densely, reductions (penta with zero outer bands == tri;
  * tri with zero off-diagonals == scaling), a dense restatement of eq. 24 for the CH
- * step and its discrete mass-balance identity.  No function here is "parity unpinned".
+ * step and its discrete mass-balance identity; for the periodic solve the splitting
+ * A' + u (x) v == A entrywise, dense solves of the cyclic matrix, the circulant eigenpairs and
+ * conservation of the column sum.  No function here is "parity unpinned".
  */
 #include <math.h>
 #include <stddef.h>
@@ -264,6 +267,66 @@ ORC_API int orc_ch_step_interleaved(int n, const double *eps, const double *beta
         }
         free(col);
         free(f);
+    }
+    return used;
+}
+
+/* ------------------------------------------------------------------------------------
+ * Periodic tridiagonal, PAPER.md:140-164 (Sec. 3.3, eq. 12-15): Sherman-Morrison.
+ *   A = A' + u (x) v,  u = (-b_1, 0, ..., 0, c_N)^T,  v = (1, 0, ..., 0, -a_1/b_1)^T  (13a)
+ *   A' = A without its two corner entries, with diagonal ends 2 b_1 and b_N + a_1 c_N / b_1  (13b)
+ *   A' y = d,  A' z = u (once),  x = y - (v.y)/(1 + v.z) z                               (14, 15)
+ * The paper writes constant diagonals a, b, c; with general diagonals the corner entries are
+ * a_1 (row 1, column N) and c_N (row N, column 1): a[0] and c[n-1] of the arrays.  n >= 3.
+ * orc_tri_periodic_factor overwrites b, c with the Thomas factors of A' (Alg. 1) and returns
+ * z (length n), vN = -a_1/b_1 and den = 1 + v.z.  Returns 0, a 1-based bad pivot row, or -1.
+ * ---------------------------------------------------------------------------------- */
+ORC_API int orc_tri_periodic_factor(int n, const double *a, double *b, double *c, double *z,
+                                    double *vN, double *den)
+{
+    if (n < 3) return -1;
+    if (b[0] == 0.0 || !isfinite(b[0])) return 1;
+    const double b1 = b[0], a1 = a[0], cN = c[n - 1];
+    for (int i = 0; i < n; ++i) z[i] = 0.0;
+    z[0] = -b1;                                  /* u, eq. 13a                        */
+    z[n - 1] = cN;
+    *vN = -a1 / b1;                              /* v_N, eq. 13a                      */
+    b[0] = 2.0 * b1;                             /* A', eq. 13b                       */
+    b[n - 1] = b[n - 1] + a1 * cN / b1;
+    const int rc = orc_tri_factor(n, a, b, c);   /* Alg. 1 on A'                      */
+    if (rc) return rc;
+    orc_tri_solve(n, a, b, c, z);                /* A' z = u, eq. 14                  */
+    *den = 1.0 + (z[0] + (*vN) * z[n - 1]);      /* 1 + v.z, eq. 15                   */
+    if (*den == 0.0 || !isfinite(*den)) return n;
+    return 0;
+}
+
+/* One contiguous system: d is overwritten by x (eq. 14-15). */
+ORC_API void orc_tri_periodic_solve(int n, const double *a, const double *bh, const double *ch,
+                                    const double *z, double vN, double den, double *d)
+{
+    orc_tri_solve(n, a, bh, ch, d);                          /* A' y = d              */
+    const double fac = (d[0] + vN * d[n - 1]) / den;         /* (v.y)/(1 + v.z)       */
+    for (int i = 0; i < n; ++i) d[i] = d[i] - fac * z[i];    /* eq. 15                */
+}
+
+ORC_API int orc_tri_periodic_solve_interleaved(int n, const double *a, const double *bh,
+                                               const double *ch, const double *z, double vN,
+                                               double den, double *rhs, long long M, long long jlo,
+                                               long long jhi, long long jstride, int nsteps,
+                                               int nthreads)
+{
+    int used = set_threads(nthreads);
+#pragma omp parallel
+    {
+        double *col = (double *)malloc((size_t)n * sizeof(double));
+#pragma omp for schedule(static)
+        for (long long j = jlo; j < jhi; j += jstride) {
+            for (int i = 0; i < n; ++i) col[i] = rhs[(size_t)i * M + j];
+            for (int s = 0; s < nsteps; ++s) orc_tri_periodic_solve(n, a, bh, ch, z, vN, den, col);
+            for (int i = 0; i < n; ++i) rhs[(size_t)i * M + j] = col[i];
+        }
+        free(col);
     }
     return used;
 }
