@@ -248,8 +248,9 @@ def extra_table(torch, b, inputs, peak):
             t = torch.empty(n, batch, dtype=dt, device="cuda")
             inputs.fill_uniform_device(t, n, seed=100 + k, scale=0.1 if kind == "ch" else 1.0)
             bufs.append(t)
-        if kind == "tri":
-            h = b.tri_factor(*inputs.tri_lhs(n, 0.5))
+        if kind in ("tri", "tri_periodic"):
+            h = b.tri_factor(*inputs.tri_lhs(n, 0.5)) if kind == "tri" else \
+                b.tri_factor_periodic([-0.5] * n, [2.0] * n, [-0.5] * n)
             one = b.tri_solve_batched if elem == 8 else b.tri_solve_batched_f32
             fn = (lambda t: one(h, t)) if steps_per_call == 1 else (lambda t: b.tri_solve_steps(h, t, steps_per_call))
         elif kind == "penta":
@@ -291,6 +292,12 @@ def extra_table(torch, b, inputs, peak):
     entry("2 (100 steps per call)", "tri", 512, 65536, 8, steps_per_call=100, launches=2)
     entry("3 (100 steps per call)", "penta", 512, 65536, 8, steps_per_call=100, launches=2)
     entry("5 (1000 steps per call)", "ch", 256, 1 << 20, 8, steps_per_call=1000, launches=1)
+    # periodic BCs by Sherman-Morrison, the form the paper's own
+    # diffusion benchmark solves (Table 1 shapes: M = 2^16, N = 64 / 256 / 1024; 1000 steps)
+    entry("f1 periodic (single solve)", "tri_periodic", 512, 65536, 8)
+    for n in (64, 256, 1024):
+        entry("f1 periodic, Table 1 shape (1000 steps per call)", "tri_periodic", n, 65536, 8, steps_per_call=1000,
+              launches=1)
     for kind in ("tri", "penta"):
         for elem in (8, 4):
             for n in (64, 256, 1024):

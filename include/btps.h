@@ -63,6 +63,20 @@ BTPS_API tri_handle_t tri_factor(int n, const double *a, const double *b, const 
 BTPS_API void tri_destroy(tri_handle_t h);
 
 /* ------------------------------------------------------------------------------------------
+ * Periodic (cyclic) tridiagonal factor.  PAPER.md:140-164 (Sec. 3.3, eq. 12-15): the matrix of
+ * tri_factor plus the two corner entries a[0] (row 0, column n-1) and c[n-1] (row n-1, column 0),
+ * i.e. row i is  a[i]*x[(i-1) mod n] + b[i]*x[i] + c[i]*x[(i+1) mod n] = rhs[i].  n >= 3.
+ * Sherman-Morrison: A = A' + u (x) v with u = (-b_0, 0, ..., c_{n-1})^T, v = (1, 0, ..., -a_0/b_0)^T;
+ * A' (diagonal ends 2 b_0 and b_{n-1} + a_0 c_{n-1} / b_0) is factored as in tri_factor and
+ * z = A'^{-1} u is solved once on the host.  The returned handle is used with the same
+ * tri_solve_batched[_f32] / tri_solve_steps / tri_solve_batched_host calls: each solve runs the sweeps
+ * for A' y = rhs and finishes in the same kernel with x = y - (v.y)/(1 + v.z) z (eq. 15), so HBM still
+ * sees one read and one write per element.  Fails with BTPS_E_PIVOT if b_0, a pivot of A' or 1 + v.z
+ * is zero / non-finite.
+ * ---------------------------------------------------------------------------------------- */
+BTPS_API tri_handle_t tri_factor_periodic(int n, const double *a, const double *b, const double *c);
+
+/* ------------------------------------------------------------------------------------------
  * (a3) Pentadiagonal factor A = L R.  PAPER.md:206-256 (Sec. 4.1 steps 1-14), 601-637 (Alg. 3).
  * Row i:  e[i]*x[i-2] + a[i]*x[i-1] + d[i]*x[i] + c[i]*x[i+1] + f[i]*x[i+2] = rhs[i].
  * NOTE the naming: BASELINE.json's (e,a,d,c,f) = the paper's (a,b,c,d,e) of PAPER.md:204.

@@ -11,7 +11,7 @@ _LIB_PATH = os.path.join(_HERE, "libbtps.so")
 
 # every symbol include/btps.h declares (tests check the library exports each of them)
 EXPORTS = [
-    "tri_factor", "tri_destroy", "penta_factor", "penta_destroy",
+    "tri_factor", "tri_factor_periodic", "tri_destroy", "penta_factor", "penta_destroy",
     "tri_solve_batched", "tri_solve_batched_f32", "penta_solve_batched", "penta_solve_batched_f32",
     "tri_solve_steps", "penta_solve_steps", "ch_step_batched",
     "tri_solve_batched_host", "penta_solve_batched_host", "ch_step_batched_host",
@@ -40,6 +40,8 @@ def _load() -> ctypes.CDLL:
         ctypes.c_int64, ctypes.c_int
     lib.tri_factor.argtypes = [ci, dp, dp, dp]
     lib.tri_factor.restype = vp
+    lib.tri_factor_periodic.argtypes = [ci, dp, dp, dp]
+    lib.tri_factor_periodic.restype = vp
     lib.tri_destroy.argtypes = [vp]
     lib.tri_destroy.restype = None
     lib.penta_factor.argtypes = [ci, dp, dp, dp, dp, dp]
@@ -142,6 +144,19 @@ def tri_factor(a, b, c) -> TriHandle:
     if a.size != n or c.size != n:
         raise ValueError("a, b, c must have the same length")
     ptr = _lib.tri_factor(n, _dptr(a), _dptr(b), _dptr(c))
+    if not ptr:
+        _raise_last()
+    return TriHandle(ptr, n)
+
+
+def tri_factor_periodic(a, b, c) -> TriHandle:
+    """btps.h tri_factor_periodic: cyclic tridiagonal matrix (a[0] and c[n-1] are the corner entries);
+    the handle is used with the same tri_solve_* calls."""
+    a, b, c = _host64(a), _host64(b), _host64(c)
+    n = b.size
+    if a.size != n or c.size != n:
+        raise ValueError("a, b, c must have the same length")
+    ptr = _lib.tri_factor_periodic(n, _dptr(a), _dptr(b), _dptr(c))
     if not ptr:
         _raise_last()
     return TriHandle(ptr, n)

@@ -100,6 +100,8 @@ constexpr int MAGIC_PENTA = 0x70656e31;  // "pen1"
 struct Handle {
     int magic;
     int kind;  // KIND_TRI / KIND_PENTA
+    bool periodic = false;                    // tri: cyclic matrix solved by Sherman-Morrison (KIND_TRIP kernels)
+    double per_vN = 0.0, per_invden = 0.0;    // eq. 13a / 15 scalars of the periodic solve
     int n;
     int device;
     DtypePlan plan[2];  // 0: fp64, 1: fp32
@@ -335,10 +337,12 @@ size_t scan_table_bytes(const DtypePlan &pl, int nc, size_t elem)
 
 template <typename T>
 void build_blob_tri(int n, DtypePlan &pl, const std::vector<double> &inv, const std::vector<double> &nl,
-                    const std::vector<double> &nch, std::vector<unsigned char> &blob)
+                    const std::vector<double> &nch, std::vector<unsigned char> &blob,
+                    const std::vector<double> *z = nullptr)
 {
     const int MR = pl.rows, P = pl.P, Np = P * MR;
-    constexpr int RT = RecLayout<KIND_TRI>::ELEMS;   // coefficient values per row
+    // coefficient values per row: the periodic form carries z = A'^{-1} u as a sixth array
+    const int RT = z ? RecLayout<KIND_TRIP>::ELEMS : RecLayout<KIND_TRI>::ELEMS;
     auto at = [&](const std::vector<double> &v, int i, double pad) { return i < n ? v[i] : pad; };
     pl.offT = (unsigned)align16((size_t)Np * RT * sizeof(T));
     pl.blob_bytes = (unsigned)align16(pl.offT + scan_table_bytes(pl, 1, sizeof(T)));
@@ -371,6 +375,7 @@ void build_blob_tri(int n, DtypePlan &pl, const std::vector<double> &inv, const 
             putv(2, i, 0, at(nch, i, 0.0));
             putv(3, i, 0, chi[k]);
             putv(3, i, 1, psi[k]);
+            if (z) put<T>(blob, ((size_t)(i / MR) * RT * MR + (size_t)5 * MR + (i % MR)) * sizeof(T), at(*z, i, 0.0));
         }
         Phi[p].m[0] = phi[MR - 1];
         Psi[p].m[0] = psi[0];
@@ -493,9 +498,10 @@ size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 // shared-memory layout of one kernel variant: [blob][exchange][mbarriers][ring]
 void layout_slot(const DtypePlan &pl, const Shape &sh, int kind, KernelSlot &sl, bool halo = true)
 {
-    const int NC = (kind == KIND_TRI) ? 1 : 2;
+    const int NC = (kind == KIND_TRI || kind == KIND_TRIP) ? 1 : 2;
     const size_t W = (size_t)sh.lanes * sl.vec;
-    sl.xvals = 2 * NC + ((kind == KIND_CH && halo) ? 2 : 0);  // CH: + the halo rows exchanged between fused steps
+    // CH: + the halo rows exchanged between fused steps; periodic tri: + y_1 and y_N of eq. 15
+    sl.xvals = 2 * NC + ((kind == KIND_CH && halo) ? 2 : 0) + (kind == KIND_TRIP ? 2 : 0);
     const size_t xch = (pl.P > 1) ? (size_t)sh.tpc * sl.xvals * pl.P * W * pl.elem : 0;
     sl.offX = (unsigned)align16(pl.blob_bytes);
     sl.offM = (unsigned)align16(sl.offX + xch);
@@ -523,10 +529,12 @@ SweepEntry find_sweep(int kind, int elem_bytes, int vec, int rows, int single, i
 {
     if (elem_bytes == 8) {
         if (kind == KIND_TRI) return find_sweep_tri_f64(vec, rows, single, tma, ws, fuse);
+        if (kind == KIND_TRIP) return find_sweep_trip_f64(vec, rows, single, tma, ws, fuse);
         if (kind == KIND_PENTA) return find_sweep_penta_f64(vec, rows, single, tma, ws, fuse);
         return find_sweep_ch_f64(vec, rows, single, tma, ws, fuse);
     }
     if (kind == KIND_TRI) return find_sweep_tri_f32(vec, rows, single, tma, ws, fuse);
+    if (kind == KIND_TRIP) return find_sweep_trip_f32(vec, rows, single, tma, ws, fuse);
     if (kind == KIND_PENTA) return find_sweep_penta_f32(vec, rows, single, tma, ws, fuse);
     return find_sweep_ch_f32(vec, rows, single, tma, ws, fuse);
 }
@@ -553,7 +561,7 @@ void fill_slots(Handle *h)
             int kind;
             if (h->kind == KIND_TRI) {
                 if (ks == 1) continue;
-                kind = KIND_TRI;
+                kind = h->periodic ? KIND_TRIP : KIND_TRI;
             } else {
                 kind = (ks == 0) ? KIND_PENTA : KIND_CH;
             }
@@ -660,7 +668,10 @@ int launch_one(Handle *h, int kind, T *d_rhs, long long batch, double alpha_x, i
     if (pl.two_pass) {
         const int block = 128;
         const long long grid = (batch + block - 1) / block;
-        if (kind == KIND_TRI)
+        if (kind == KIND_TRI && h->periodic)
+            two_pass_kernel<T, KIND_TRIP><<<(unsigned)grid, block, 0, st>>>((const T *)pl.d_soa, d_rhs, batch, h->n,
+                                                                            h->per_vN, h->per_invden);
+        else if (kind == KIND_TRI)
             two_pass_kernel<T, KIND_TRI><<<(unsigned)grid, block, 0, st>>>((const T *)pl.d_soa, d_rhs, batch, h->n, 0.0);
         else if (kind == KIND_PENTA)
             two_pass_kernel<T, KIND_PENTA><<<(unsigned)grid, block, 0, st>>>((const T *)pl.d_soa, d_rhs, batch, h->n, 0.0);
@@ -700,6 +711,10 @@ int launch_one(Handle *h, int kind, T *d_rhs, long long batch, double alpha_x, i
     const long long W = (long long)sh.lanes * sl.vec;
     a.num_tiles = (batch + W - 1) / W;
     a.alpha_x = alpha_x;
+    a.per_vN = h->per_vN;
+    a.per_invden = h->per_invden;
+    a.last_part = (h->n - 1) / pl.rows;
+    a.last_k = (h->n - 1) % pl.rows;
     a.n = h->n;
     a.P = pl.P;
     a.lanes = sh.lanes;
@@ -850,6 +865,44 @@ int solve_host(const void *hv, int magic, int kind, T *h_rhs, int64_t batch, dou
 // ================================================================================================
 extern "C" {
 
+// shared by tri_factor and tri_factor_periodic: tables + upload for a factored (possibly modified) matrix
+static tri_handle_t make_tri_handle(int n, const std::vector<double> &inv, const std::vector<double> &nl,
+                                    const std::vector<double> &nch, const std::vector<double> *z, double vN,
+                                    double invden)
+{
+    Handle *h = new Handle();
+    h->magic = MAGIC_TRI;
+    h->kind = KIND_TRI;
+    h->periodic = (z != nullptr);
+    h->per_vN = vN;
+    h->per_invden = invden;
+    h->n = n;
+    h->device = 0;
+    for (int t = 0; t < 2; ++t) {
+        DtypePlan &pl = h->plan[t];
+        choose_plan(n, t == 0 ? 8 : 4, h->kind, pl);
+        std::vector<unsigned char> blob, soa;
+        std::vector<const std::vector<double> *> arrs = {&inv, &nl, &nch};
+        if (z) arrs.push_back(z);
+        if (t == 0) {
+            build_blob_tri<double>(n, pl, inv, nl, nch, blob, z);
+            build_soa<double>(arrs, n, soa);
+        } else {
+            build_blob_tri<float>(n, pl, inv, nl, nch, blob, z);
+            build_soa<float>(arrs, n, soa);
+        }
+        pl.soa_bytes = soa.size();
+        fit_plan(pl, h->periodic ? KIND_TRIP : KIND_TRI);
+        if (upload(blob, &pl.d_blob) != BTPS_OK || upload(soa, &pl.d_soa) != BTPS_OK) {
+            free_handle(h);
+            return nullptr;
+        }
+    }
+    fill_slots(h);
+    set_err(BTPS_OK);
+    return (tri_handle_t)h;
+}
+
 tri_handle_t tri_factor(int n, const double *a, const double *b, const double *c)
 {
     if (n < 1 || !a || !b || !c) {
@@ -862,32 +915,48 @@ tri_handle_t tri_factor(int n, const double *a, const double *b, const double *c
         set_err(BTPS_E_PIVOT, row);
         return nullptr;
     }
-    Handle *h = new Handle();
-    h->magic = MAGIC_TRI;
-    h->kind = KIND_TRI;
-    h->n = n;
-    h->device = 0;
-    for (int t = 0; t < 2; ++t) {
-        DtypePlan &pl = h->plan[t];
-        choose_plan(n, t == 0 ? 8 : 4, h->kind, pl);
-        std::vector<unsigned char> blob, soa;
-        if (t == 0) {
-            build_blob_tri<double>(n, pl, inv, nl, nch, blob);
-            build_soa<double>({&inv, &nl, &nch}, n, soa);
-        } else {
-            build_blob_tri<float>(n, pl, inv, nl, nch, blob);
-            build_soa<float>({&inv, &nl, &nch}, n, soa);
-        }
-        pl.soa_bytes = soa.size();
-        fit_plan(pl, h->kind);
-        if (upload(blob, &pl.d_blob) != BTPS_OK || upload(soa, &pl.d_soa) != BTPS_OK) {
-            free_handle(h);
-            return nullptr;
-        }
+    return make_tri_handle(n, inv, nl, nch, nullptr, 0.0, 0.0);
+}
+
+// Periodic (cyclic) tridiagonal matrix, PAPER.md:140-164 (Sec. 3.3): A = A' + u (x) v with
+// u = (-b_1, 0, ..., c_N)^T, v = (1, 0, ..., -a_1/b_1)^T (eq. 13a) and A' = A without its corners, diagonal
+// ends 2 b_1 and b_N + a_1 c_N / b_1 (eq. 13b).  A' is factored as in tri_factor, z = A'^{-1} u is
+// solved once here (eq. 14) and stored with the tables; the kernels finish each solve with eq. 15.
+tri_handle_t tri_factor_periodic(int n, const double *a, const double *b, const double *c)
+{
+    if (n < 3 || !a || !b || !c) {
+        set_err(BTPS_E_ARG);
+        return nullptr;
     }
-    fill_slots(h);
-    set_err(BTPS_OK);
-    return (tri_handle_t)h;
+    if (b[0] == 0.0 || !std::isfinite(b[0])) {
+        set_err(BTPS_E_PIVOT, 1);
+        return nullptr;
+    }
+    std::vector<double> bp(b, b + n);
+    bp[0] = 2.0 * b[0];
+    bp[n - 1] = b[n - 1] + a[0] * c[n - 1] / b[0];
+    std::vector<double> inv, nl, nch;
+    int row = 0;
+    if (factor_tri_host(n, a, bp.data(), c, inv, nl, nch, &row) != BTPS_OK) {
+        set_err(BTPS_E_PIVOT, row);
+        return nullptr;
+    }
+    std::vector<double> z(n, 0.0);
+    z[0] = -b[0];
+    z[n - 1] = c[n - 1];
+    double g = 0.0;
+    for (int i = 0; i < n; ++i) {  // forward sweep of A' z = u with the sweep multipliers
+        g = nl[i] * g + inv[i] * z[i];
+        z[i] = g;
+    }
+    for (int i = n - 2; i >= 0; --i) z[i] = z[i] + nch[i] * z[i + 1];
+    const double vN = -a[0] / b[0];
+    const double den = 1.0 + z[0] + vN * z[n - 1];
+    if (den == 0.0 || !std::isfinite(den)) {
+        set_err(BTPS_E_PIVOT, n);
+        return nullptr;
+    }
+    return make_tri_handle(n, inv, nl, nch, &z, vN, 1.0 / den);
 }
 
 void tri_destroy(tri_handle_t hv)

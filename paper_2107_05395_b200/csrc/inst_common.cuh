@@ -74,5 +74,7 @@ SweepEntry find_sweep_penta_f64(int vec, int rows, int single, int tma, int ws, 
 SweepEntry find_sweep_penta_f32(int vec, int rows, int single, int tma, int ws, int fuse);
 SweepEntry find_sweep_ch_f64(int vec, int rows, int single, int tma, int ws, int fuse);
 SweepEntry find_sweep_ch_f32(int vec, int rows, int single, int tma, int ws, int fuse);
+SweepEntry find_sweep_trip_f64(int vec, int rows, int single, int tma, int ws, int fuse);
+SweepEntry find_sweep_trip_f32(int vec, int rows, int single, int tma, int ws, int fuse);
 
 }  // namespace btps

@@ -5,6 +5,8 @@
 //           backward x_i = g_i - c^_i x_{i+1}                  PAPER.md:101-108 (eq. 5-6), Alg. 2
 //   penta : forward  g_i = (f_i - eps_i g_{i-2} - beta_i g_{i-1}) / alpha_i
 //           backward x_i = g_i - gamma_i x_{i+1} - delta_i x_{i+2}            PAPER.md:268-278, Alg. 4
+//   periodic tri : A = A' + u (x) v (Sherman-Morrison, eq. 12-15): y = A'^{-1} d by the
+//           sweeps above, then x = y - (v.y)/(1 + v.z) z with z = A'^{-1} u from the factor tables
 //   ch    : f_i = c_i + alpha_x (w_{i-1} - 2 w_i + w_{i+1}), w = c^3 - c, then the penta sweeps
 //           PAPER.md:365-392 (eq. 24, 25a, 26c), truncated stencil (C-18, C-21).
 //
@@ -34,7 +36,7 @@
 
 namespace btps {
 
-enum Kind { KIND_TRI = 0, KIND_PENTA = 1, KIND_CH = 2 };
+enum Kind { KIND_TRI = 0, KIND_PENTA = 1, KIND_CH = 2, KIND_TRIP = 3 };  // TRIP: periodic tridiagonal
 
 constexpr int SCAN_STEPS = 5;   // Kogge-Stone steps held in the tables (scan width <= 32)
 constexpr int SCAN_LANES = 32;
@@ -45,6 +47,9 @@ struct SweepArgs {
     long long batch;
     long long num_tiles;   // ceil(batch / (lanes*V))
     double alpha_x;        // CH only: dt/dx^2
+    double per_vN;         // periodic tri: last entry of v, eq. 13a (-a_1/b_1)
+    double per_invden;     // periodic tri: 1 / (1 + v.z), eq. 15
+    int last_part, last_k; // periodic tri: partition and local row of row n-1
     int n;                 // true number of rows
     int P;                 // partitions per system (rows padded to P*MR with identity rows)
     int lanes;             // threads side by side on adjacent systems (power of two <= 32)
@@ -113,6 +118,7 @@ __device__ __forceinline__ T ch_w(T c) { return fma_t<T>(c * c, c, -c); }
 //   tri   (5 MR): 0: {inv, nl}   2: nch    3: {chi, psi}
 //           inv = 1/b^_i, nl = -a_i/b^_i, nch = -c^_i; chi/psi = response of the finished local
 //           sweeps to the incoming forward / backward carry
+//   periodic tri (6 MR): as tri, plus 5: z = A'^{-1} u of the Sherman-Morrison splitting
 //   penta (9 MR): 0: {inv, nle}  2: nlb    3: {ngam, ndel}   5: {chi1, chi2}   7: {psi1, psi2}
 //           inv = 1/alpha_i, nle = -eps_i/alpha_i, nlb = -beta_i/alpha_i, ngam = -gamma_i, ndel = -delta_i
 // followed at offT by the carry-scan tables, indexed [slot][m][q] with q = partition (tq entries),
@@ -128,8 +134,9 @@ __device__ __forceinline__ T ch_w(T c) { return fma_t<T>(c * c, c, -c); }
 // from the row arrays).
 template <int KIND>
 struct RecLayout {
-    static constexpr int ELEMS = (KIND == KIND_TRI) ? 5 : 9;   // coefficient values per row
-    static constexpr int NC = (KIND == KIND_TRI) ? 1 : 2;      // carries per direction
+    static constexpr bool TRI = (KIND == KIND_TRI || KIND == KIND_TRIP);
+    static constexpr int ELEMS = (KIND == KIND_TRI) ? 5 : (KIND == KIND_TRIP ? 6 : 9);  // coefficient values per row
+    static constexpr int NC = TRI ? 1 : 2;                     // carries per direction
 };
 
 // ---- TMA / mbarrier primitives (PTX) -------------------------------------------------------------
@@ -215,7 +222,7 @@ template <typename T, int V, int MR, bool SINGLE, int KIND, bool TMA, bool WS, b
 __global__ void __launch_bounds__(CtaShape<T, V, MR>::MAX_THREADS, 1)
 sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
 {
-    constexpr bool TRI = (KIND == KIND_TRI);
+    constexpr bool TRI = RecLayout<KIND>::TRI;
     constexpr int NC = RecLayout<KIND>::NC;
     using Pair = Tup<T, 2>;
     extern __shared__ __align__(128) unsigned char smem[];
@@ -687,6 +694,44 @@ sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
             }
 #undef XI
         }
+        if constexpr (KIND == KIND_TRIP) {
+            // ---- eq. 15: x = y - (v.y)/(1 + v.z) z,  v.y = y_1 + v_N y_N ------------------------------
+            T y0[V], yN[V];
+#pragma unroll
+            for (int e = 0; e < V; ++e) { y0[e] = v[0][e]; yN[e] = T(0); }
+#pragma unroll
+            for (int k = 0; k < MR; ++k)
+                if (k == a.last_k) {
+#pragma unroll
+                    for (int e = 0; e < V; ++e) yN[e] = v[k][e];
+                }
+            if constexpr (!SINGLE) {
+                // y_1 lives in partition 0, y_N in partition last_part: two more exchange planes
+                T *const pz = xb + (size_t)2 * NC * a.P * W + sl * V;
+                if (part == 0) {
+#pragma unroll
+                    for (int e = 0; e < V; ++e) pz[e] = y0[e];
+                }
+                if (part == a.last_part) {
+#pragma unroll
+                    for (int e = 0; e < V; ++e) pz[a.P * W + e] = yN[e];
+                }
+                group_sync(a.tpc, sub, tpt);
+#pragma unroll
+                for (int e = 0; e < V; ++e) { y0[e] = pz[e]; yN[e] = pz[a.P * W + e]; }
+            }
+            const T vN = (T)a.per_vN, invden = (T)a.per_invden;
+            T nfac[V];
+#pragma unroll
+            for (int e = 0; e < V; ++e) nfac[e] = -(fma_t<T>(vN, yN[e], y0[e]) * invden);
+            const T *const RZ = cb + 5 * MR;
+#pragma unroll
+            for (int k = 0; k < MR; ++k) {
+                const T zk = RZ[k];
+#pragma unroll
+                for (int e = 0; e < V; ++e) v[k][e] = fma_t<T>(nfac[e], zk, v[k][e]);
+            }
+        }
         }  // ksteps
 
         // ---- store ---------------------------------------------------------------------------
@@ -712,12 +757,12 @@ sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
 // -----------------------------------------------------------------------------------------------
 template <typename T, int KIND>
 __global__ void __launch_bounds__(128) two_pass_kernel(const T *__restrict__ co, T *rhs, long long batch,
-                                                       int n, double alpha_x)
+                                                       int n, double alpha_x, double alpha_y = 0.0)
 {
     const long long j = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (j >= batch) return;
     T *p = rhs + j;
-    if constexpr (KIND == KIND_TRI) {
+    if constexpr (KIND == KIND_TRI || KIND == KIND_TRIP) {
         const T *inv = co, *nl = co + n, *nch = co + 2 * (size_t)n;
         T g = T(0);
         for (int i = 0; i < n; ++i) {
@@ -728,6 +773,12 @@ __global__ void __launch_bounds__(128) two_pass_kernel(const T *__restrict__ co,
         for (int i = n - 2; i >= 0; --i) {
             x = fma_t<T>(__ldg(nch + i), x, p[(long long)i * batch]);
             p[(long long)i * batch] = x;
+        }
+        if constexpr (KIND == KIND_TRIP) {
+            // eq. 15: alpha_x carries v_N, alpha_y 1/(1 + v.z); z follows nch in co
+            const T *z = co + 3 * (size_t)n;
+            const T nfac = -(fma_t<T>((T)alpha_x, g, x) * (T)alpha_y);  // x = y_1, g = y_N here
+            for (int i = 0; i < n; ++i) p[(long long)i * batch] = fma_t<T>(nfac, __ldg(z + i), p[(long long)i * batch]);
         }
     } else {
         const T *inv = co, *nle = co + n, *nlb = co + 2 * (size_t)n, *ngam = co + 3 * (size_t)n,

@@ -538,3 +538,73 @@ def test_fused_steps_equal_single_step_launches(lib, n, batch):
     ref = c0.copy()
     oracle.ch_step_interleaved(oracle.penta_factor(*lc), ref, 0.05, nsteps=steps)
     assert rel_err(outs[-1][2], ref) <= TOL_STEPS
+
+
+# ---- periodic tridiagonal (Sherman-Morrison) ---------------------------------------
+
+def rand_cyclic(n, seed):
+    rng = np.random.default_rng(seed)
+    a, c = rng.uniform(-1, 1, n), rng.uniform(-1, 1, n)
+    b = np.abs(a) + np.abs(c) + rng.uniform(0.5, 1.5, n)
+    return a, b, c
+
+
+@pytest.mark.parametrize("n", [3, 4, 31, 32, 33, 64, 300, 512, 1000, 1024, 1500, 5000])
+def test_tri_periodic_sizes(lib, n):
+    lhs = rand_cyclic(n, n)
+    fo = oracle.tri_periodic_factor(*lhs)
+    h = lib.tri_factor_periodic(*lhs)
+    for batch in (1, 33, 1024 + 32, 1001):
+        rhs = inputs.uniform_rhs(n, batch, seed=n + batch)
+        ref = rhs.copy()
+        oracle.tri_periodic_solve_interleaved(fo, ref)
+        d = dev(rhs)
+        lib.tri_solve_batched(h, d)
+        assert rel_err(d.cpu().numpy(), ref) <= TOL_SINGLE, (n, batch, h.plan())
+    rhs = inputs.uniform_rhs(n, 512, seed=3).astype(np.float32)
+    ref = rhs.astype(np.float64)
+    oracle.tri_periodic_solve_interleaved(fo, ref)
+    d = dev(rhs)
+    lib.tri_solve_batched_f32(h, d)
+    assert rel_err(d.cpu().numpy(), ref) <= TOL_F32, (n, h.plan(4))
+
+
+@pytest.mark.parametrize("tune", [dict(), dict(prefetch=0), dict(warp_scan=0), dict(vec=1), dict(force_two_pass=1),
+                                  dict(fuse_steps=1)])
+def test_tri_periodic_diffusion_steps_and_mass(lib, tune):
+    """Periodic implicit diffusion (the paper's own benchmark form, PAPER.md:120-136 in BASELINE.json's
+    backward-Euler reading): 20 steps against the oracle, conservation of each system's sum
+    (PAPER.md:339-348 holds for periodic BCs) and the exact decay of a cosine mode."""
+    n, batch, r, steps = 256, 2048 + 64, 0.5, 20
+    lhs = ([-r] * n, [1 + 2 * r] * n, [-r] * n)
+    try:
+        for k, v in tune.items():
+            lib.btps_tune(k, v)
+        h = lib.tri_factor_periodic(*lhs)
+    finally:
+        for k in tune:
+            lib.btps_tune(k, -1)
+    rhs = inputs.uniform_rhs(n, batch, seed=17)
+    rhs[:, 0] = np.cos(2 * np.pi * 3 * np.arange(n) / n)
+    ref = rhs.copy()
+    oracle.tri_periodic_solve_interleaved(oracle.tri_periodic_factor(*lhs), ref, nsteps=steps)
+    d = dev(rhs)
+    try:
+        for k, v in tune.items():
+            lib.btps_tune(k, v)
+        lib.tri_solve_steps(h, d, steps)
+    finally:
+        for k in tune:
+            lib.btps_tune(k, -1)
+    got = d.cpu().numpy()
+    assert rel_err(got, ref) <= TOL_STEPS, (tune, h.plan())
+    assert np.max(np.abs(got.sum(axis=0) - rhs.sum(axis=0))) <= 1e-11
+    lam = 1 + 4 * r * np.sin(np.pi * 3 / n) ** 2
+    assert np.max(np.abs(got[:, 0] - rhs[:, 0] * lam ** -steps)) <= 1e-12
+
+
+def test_tri_periodic_errors(lib):
+    with pytest.raises(lib.BtpsError):
+        lib.tri_factor_periodic([1.0, 1.0], [2.0, 2.0], [1.0, 1.0])          # n < 3
+    with pytest.raises(lib.BtpsError):
+        lib.tri_factor_periodic([1.0] * 4, [0.0, 2.0, 2.0, 2.0], [1.0] * 4)  # b_0 = 0
