@@ -74,6 +74,15 @@ def _load():
                                                            ctypes.c_double, ctypes.c_double, _dp, _ll,
                                                            _ll, _ll, _ll, ctypes.c_int, ctypes.c_int]
         lib.orc_tri_periodic_solve_interleaved.restype = ctypes.c_int
+        lib.orc_penta_periodic_factor.argtypes = [ctypes.c_int, _dp, _dp, _dp, _dp, _dp, _dp, _dp, _dp]
+        lib.orc_penta_periodic_factor.restype = ctypes.c_int
+        lib.orc_penta_periodic_solve.argtypes = [ctypes.c_int] + [_dp] * 9
+        lib.orc_penta_periodic_solve.restype = None
+        lib.orc_ch_rhs_periodic.argtypes = [ctypes.c_int, _dp, ctypes.c_double, _dp]
+        lib.orc_ch_rhs_periodic.restype = None
+        lib.orc_penta_periodic_interleaved.argtypes = [ctypes.c_int] + [_dp] * 9 + [_ll, _ll, _ll, _ll, ctypes.c_int,
+                                                                                    ctypes.c_double, ctypes.c_int, ctypes.c_int]
+        lib.orc_penta_periodic_interleaved.restype = ctypes.c_int
         _lib = lib
     return _lib
 
@@ -236,3 +245,65 @@ def tri_periodic_solve_interleaved(fac: TriPeriodicFactor, rhs: np.ndarray, nste
     jlo, jhi, js = _subset(M, subset)
     return _load().orc_tri_periodic_solve_interleaved(fac.n, _p(fac.a), _p(fac.bh), _p(fac.ch), _p(fac.z),
                                                       fac.vN, fac.den, _p(rhs), M, jlo, jhi, js, nsteps, nthreads)
+
+
+# ---- periodic pentadiagonal (eq. 26a; Woodbury, C-31) and periodic CH step ------
+
+@dataclass
+class PentaPeriodicFactor:
+    n: int
+    eps: np.ndarray
+    beta: np.ndarray
+    alpha: np.ndarray
+    gamma: np.ndarray
+    delta: np.ndarray
+    Z: np.ndarray    # (n, 4) = A'^{-1} U
+    H: np.ndarray    # (4, 4) = (I + V^T Z)^{-1}
+    w6: np.ndarray   # the six wrap-around entries
+
+
+def penta_periodic_factor(a, b, c, d, e) -> PentaPeriodicFactor:
+    """Cyclic pentadiagonal matrix, paper naming: row i is a[i] x[i-2] + b[i] x[i-1] + c[i] x[i] +
+    d[i] x[i+1] + e[i] x[i+2] with indices mod n."""
+    a, b, c, d, e = (_f64(v) for v in (a, b, c, d, e))
+    n = c.size
+    assert all(v.size == n for v in (a, b, d, e))
+    Z, H, w6 = np.zeros((n, 4)), np.zeros((4, 4)), np.zeros(6)
+    rc = _load().orc_penta_periodic_factor(n, _p(a), _p(b), _p(c), _p(d), _p(e), _p(Z), _p(H), _p(w6))
+    if rc:
+        raise FactorError(rc)
+    return PentaPeriodicFactor(n, a, b, c, d, e, Z, H, w6)
+
+
+def penta_periodic_solve(fac: PentaPeriodicFactor, f) -> np.ndarray:
+    x = _f64(f)
+    assert x.shape == (fac.n,)
+    _load().orc_penta_periodic_solve(fac.n, _p(fac.eps), _p(fac.beta), _p(fac.alpha), _p(fac.gamma), _p(fac.delta),
+                                     _p(fac.Z), _p(fac.H), _p(fac.w6), _p(x))
+    return x
+
+
+def ch_rhs_periodic(c, alpha: float) -> np.ndarray:
+    c = _f64(c)
+    f = np.zeros_like(c)
+    _load().orc_ch_rhs_periodic(c.size, _p(c), alpha, _p(f))
+    return f
+
+
+def _penta_periodic_interleaved(fac, buf, mode, alpha_x, nsteps, subset, nthreads):
+    assert buf.ndim == 2 and buf.shape[0] == fac.n
+    M = buf.shape[1]
+    jlo, jhi, js = _subset(M, subset)
+    return _load().orc_penta_periodic_interleaved(fac.n, _p(fac.eps), _p(fac.beta), _p(fac.alpha), _p(fac.gamma),
+                                                  _p(fac.delta), _p(fac.Z), _p(fac.H), _p(fac.w6), _p(buf), M, jlo,
+                                                  jhi, js, mode, alpha_x, nsteps, nthreads)
+
+
+def penta_periodic_solve_interleaved(fac: PentaPeriodicFactor, rhs: np.ndarray, nsteps: int = 1, subset=None,
+                                     nthreads: int = 0) -> int:
+    return _penta_periodic_interleaved(fac, rhs, 0, 0.0, nsteps, subset, nthreads)
+
+
+def ch_periodic_step_interleaved(fac: PentaPeriodicFactor, c: np.ndarray, alpha: float, nsteps: int = 1,
+                                 subset=None, nthreads: int = 0) -> int:
+    return _penta_periodic_interleaved(fac, c, 1, alpha, nsteps, subset, nthreads)

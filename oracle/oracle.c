@@ -330,3 +330,125 @@ ORC_API int orc_tri_periodic_solve_interleaved(int n, const double *a, const dou
     }
     return used;
 }
+
+/* ------------------------------------------------------------------------------------
+ * Periodic (cyclic) pentadiagonal, PAPER.md:380 (eq. 26a).  The paper solves it "following
+ * [24,4,25]" without writing the method out (SURVEY 8(c) / DESIGN.md reading C-31): the result is
+ * defined as x = A^{-1} f for the cyclic matrix, reached here by the Woodbury identity on the
+ * same pattern as Sec. 3.3:  A = A' + U V^T,  A' = A without its six wrap-around entries
+ * (pentadiagonal, factored by Sec. 4.1),  U = unit columns at rows 1, 2, N-1, N,  V^T = the
+ * wrap-around entries:
+ *     row 1:  a_1 at column N-1, b_1 at column N        row 2:  a_2 at column N
+ *     row N-1: e_{N-1} at column 1                       row N:  d_N at column 1, e_N at column 2
+ *   y = A'^{-1} f,  Z = A'^{-1} U (once),  H = (I_4 + V^T Z)^{-1} (once),  x = y - Z H (V^T y).
+ * Paper naming (a,b,c,d,e = offsets -2,-1,0,+1,+2), 0-based arrays.  n >= 5.
+ * orc_penta_periodic_factor overwrites b..e with the factors of A' and returns Z (n x 4, row-major),
+ * H (4 x 4, row-major) and w6 = (a_1, b_1, a_2, e_{N-1}, d_N, e_N).  Returns 0, a bad pivot row, or -1.
+ * ---------------------------------------------------------------------------------- */
+static int inv4(const double *A, double *H)
+{
+    double M[4][8];
+    for (int i = 0; i < 4; ++i)
+        for (int j = 0; j < 4; ++j) { M[i][j] = A[i * 4 + j]; M[i][4 + j] = (i == j) ? 1.0 : 0.0; }
+    for (int k = 0; k < 4; ++k) {                /* Gauss-Jordan with partial pivoting   */
+        int p = k;
+        for (int r = k + 1; r < 4; ++r) if (fabs(M[r][k]) > fabs(M[p][k])) p = r;
+        if (M[p][k] == 0.0 || !isfinite(M[p][k])) return 1;
+        for (int j = 0; j < 8; ++j) { double t = M[k][j]; M[k][j] = M[p][j]; M[p][j] = t; }
+        double piv = M[k][k];
+        for (int j = 0; j < 8; ++j) M[k][j] /= piv;
+        for (int r = 0; r < 4; ++r) if (r != k) {
+            double m = M[r][k];
+            for (int j = 0; j < 8; ++j) M[r][j] -= m * M[k][j];
+        }
+    }
+    for (int i = 0; i < 4; ++i) for (int j = 0; j < 4; ++j) H[i * 4 + j] = M[i][4 + j];
+    return 0;
+}
+
+ORC_API int orc_penta_periodic_factor(int n, const double *a, double *b, double *c, double *d,
+                                      double *e, double *Z, double *H, double *w6)
+{
+    if (n < 5) return -1;
+    w6[0] = a[0]; w6[1] = b[0]; w6[2] = a[1]; w6[3] = e[n - 2]; w6[4] = d[n - 1]; w6[5] = e[n - 1];
+    const int rc = orc_penta_factor_general(n, a, b, c, d, e);   /* A' (never reads the corners) */
+    if (rc) return rc;
+    double *col = (double *)malloc((size_t)n * sizeof(double));
+    const int urow[4] = {0, 1, n - 2, n - 1};
+    for (int m = 0; m < 4; ++m) {                                /* Z = A'^{-1} U              */
+        for (int i = 0; i < n; ++i) col[i] = 0.0;
+        col[urow[m]] = 1.0;
+        orc_penta_solve(n, a, b, c, d, e, col);
+        for (int i = 0; i < n; ++i) Z[(size_t)i * 4 + m] = col[i];
+    }
+    free(col);
+    double S[16];                                                /* I + V^T Z                  */
+    for (int m = 0; m < 4; ++m) {
+        S[0 * 4 + m] = w6[0] * Z[(size_t)(n - 2) * 4 + m] + w6[1] * Z[(size_t)(n - 1) * 4 + m];
+        S[1 * 4 + m] = w6[2] * Z[(size_t)(n - 1) * 4 + m];
+        S[2 * 4 + m] = w6[3] * Z[m];
+        S[3 * 4 + m] = w6[4] * Z[m] + w6[5] * Z[4 + m];
+    }
+    for (int m = 0; m < 4; ++m) S[m * 4 + m] += 1.0;
+    if (inv4(S, H)) return n;
+    return 0;
+}
+
+ORC_API void orc_penta_periodic_solve(int n, const double *eps, const double *beta, const double *alpha,
+                                      const double *gamma, const double *delta, const double *Z,
+                                      const double *H, const double *w6, double *f)
+{
+    orc_penta_solve(n, eps, beta, alpha, gamma, delta, f);       /* A' y = f                   */
+    double t[4], w[4];
+    t[0] = w6[0] * f[n - 2] + w6[1] * f[n - 1];                  /* V^T y                      */
+    t[1] = w6[2] * f[n - 1];
+    t[2] = w6[3] * f[0];
+    t[3] = w6[4] * f[0] + w6[5] * f[1];
+    for (int i = 0; i < 4; ++i) w[i] = H[i * 4] * t[0] + H[i * 4 + 1] * t[1] + H[i * 4 + 2] * t[2] + H[i * 4 + 3] * t[3];
+    for (int i = 0; i < n; ++i)                                  /* x = y - Z w                */
+        f[i] = f[i] - (Z[(size_t)i * 4] * w[0] + Z[(size_t)i * 4 + 1] * w[1] + Z[(size_t)i * 4 + 2] * w[2] +
+                       Z[(size_t)i * 4 + 3] * w[3]);
+}
+
+/* Explicit half of eq. 24 with PERIODIC differences (the paper's own boundary conditions,
+ * PAPER.md:337, 365-392): f_i = c_i + alpha (w_{i-1} - 2 w_i + w_{i+1}), w = c^3 - c, indices mod n. */
+ORC_API void orc_ch_rhs_periodic(int n, const double *c, double alpha, double *f)
+{
+    for (int i = 0; i < n; ++i) {
+        const int im = (i + n - 1) % n, ip = (i + 1) % n;
+        double wm = c[im] * c[im] * c[im] - c[im];
+        double w0 = c[i] * c[i] * c[i] - c[i];
+        double wp = c[ip] * c[ip] * c[ip] - c[ip];
+        f[i] = c[i] + alpha * (wm - 2.0 * w0 + wp);
+    }
+}
+
+/* mode 0: nsteps periodic penta solves (RHS = previous solution); mode 1: nsteps periodic CH steps. */
+ORC_API int orc_penta_periodic_interleaved(int n, const double *eps, const double *beta, const double *alpha,
+                                           const double *gamma, const double *delta, const double *Z,
+                                           const double *H, const double *w6, double *buf, long long M,
+                                           long long jlo, long long jhi, long long jstride, int mode,
+                                           double alpha_x, int nsteps, int nthreads)
+{
+    int used = set_threads(nthreads);
+#pragma omp parallel
+    {
+        double *col = (double *)malloc((size_t)n * sizeof(double));
+        double *f = (double *)malloc((size_t)n * sizeof(double));
+#pragma omp for schedule(static)
+        for (long long j = jlo; j < jhi; j += jstride) {
+            for (int i = 0; i < n; ++i) col[i] = buf[(size_t)i * M + j];
+            for (int s = 0; s < nsteps; ++s) {
+                if (mode == 1) {
+                    orc_ch_rhs_periodic(n, col, alpha_x, f);
+                    memcpy(col, f, (size_t)n * sizeof(double));
+                }
+                orc_penta_periodic_solve(n, eps, beta, alpha, gamma, delta, Z, H, w6, col);
+            }
+            for (int i = 0; i < n; ++i) buf[(size_t)i * M + j] = col[i];
+        }
+        free(col);
+        free(f);
+    }
+    return used;
+}
