@@ -246,19 +246,20 @@ def extra_table(torch, b, inputs, peak):
         bufs = []
         for k in range(nbuf):
             t = torch.empty(n, batch, dtype=dt, device="cuda")
-            inputs.fill_uniform_device(t, n, seed=100 + k, scale=0.1 if kind == "ch" else 1.0)
+            inputs.fill_uniform_device(t, n, seed=100 + k, scale=0.1 if kind.startswith("ch") else 1.0)
             bufs.append(t)
         if kind in ("tri", "tri_periodic"):
             h = b.tri_factor(*inputs.tri_lhs(n, 0.5)) if kind == "tri" else \
                 b.tri_factor_periodic([-0.5] * n, [2.0] * n, [-0.5] * n)
             one = b.tri_solve_batched if elem == 8 else b.tri_solve_batched_f32
             fn = (lambda t: one(h, t)) if steps_per_call == 1 else (lambda t: b.tri_solve_steps(h, t, steps_per_call))
-        elif kind == "penta":
-            h = b.penta_factor(*inputs.penta_lhs(n, 0.5))
+        elif kind in ("penta", "penta_periodic"):
+            h = b.penta_factor(*inputs.penta_lhs(n, 0.5)) if kind == "penta" else \
+                b.penta_factor_periodic(*inputs.penta_lhs(n, 0.5))
             one = b.penta_solve_batched if elem == 8 else b.penta_solve_batched_f32
             fn = (lambda t: one(h, t)) if steps_per_call == 1 else (lambda t: b.penta_solve_steps(h, t, steps_per_call))
         else:
-            h = b.penta_factor(*inputs.ch_lhs(n))
+            h = b.penta_factor(*inputs.ch_lhs(n)) if kind == "ch" else b.penta_factor_periodic(*inputs.ch_lhs(n))
             _, alpha = inputs.ch_params(n)
             fn = lambda t: b.ch_step_batched(h, t, alpha, steps_per_call)
         fn(bufs[0])
@@ -284,7 +285,7 @@ def extra_table(torch, b, inputs, peak):
                     "unknowns_per_s": n * batch / ms * 1e3, "hbm_gbs": round(gbs, 1),
                     "frac_of_measured_peak": round(gbs / peak, 4),
                     "cold": "rotating %d buffers" % nbuf if nbuf > 1 else "buffer > 2x L2",
-                    "plan": h.ch_plan(elem) if kind == "ch" else h.plan(elem)})
+                    "plan": h.ch_plan(elem) if kind.startswith("ch") else h.plan(elem)})
         del bufs
         torch.cuda.empty_cache()
 
@@ -295,6 +296,11 @@ def extra_table(torch, b, inputs, peak):
     # periodic BCs by Sherman-Morrison, the form the paper's own
     # diffusion benchmark solves (Table 1 shapes: M = 2^16, N = 64 / 256 / 1024; 1000 steps)
     entry("f1 periodic (single solve)", "tri_periodic", 512, 65536, 8)
+    entry("f1 periodic (single solve)", "penta_periodic", 512, 65536, 8)
+    entry("f1 periodic (single step)", "ch_periodic", 512, 65536, 8)
+    # the paper's Cahn-Hilliard setting: periodic, N = 256, 2^20 independent runs
+    entry("f1 periodic CH, 2^20 runs (1000 steps per call)", "ch_periodic", 256, 1 << 20, 8, steps_per_call=1000,
+          launches=1)
     for n in (64, 256, 1024):
         entry("f1 periodic, Table 1 shape (1000 steps per call)", "tri_periodic", n, 65536, 8, steps_per_call=1000,
               launches=1)

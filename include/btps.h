@@ -89,6 +89,21 @@ BTPS_API penta_handle_t penta_factor(int n, const double *e, const double *a, co
 BTPS_API void penta_destroy(penta_handle_t h);
 
 /* ------------------------------------------------------------------------------------------
+ * Periodic (cyclic) pentadiagonal factor (eq. 26a): the matrix of penta_factor plus
+ * its six wrap-around entries, i.e. row i is  e[i]*x[i-2] + a[i]*x[i-1] + d[i]*x[i] + c[i]*x[i+1] +
+ * f[i]*x[i+2]  with indices mod n (e[0], e[1], a[0], c[n-1], f[n-2], f[n-1] ARE read here).  n >= 5.
+ * The paper cites [24,4,25] for the method; this library uses the Woodbury identity on the pattern of
+ * its Sec. 3.3 (C-31): A = A' + U V^T, Z = A'^{-1} U (4 columns) and H = (I + V^T Z)^{-1}
+ * computed once on the host; every solve runs the sweeps for A' y = rhs and finishes in the same kernel
+ * with x = y - Z H (V^T y).  The handle is used with penta_solve_batched[_f32], penta_solve_steps,
+ * penta_solve_batched_host and with ch_step_batched / ch_step_batched_host, where the explicit half then
+ * uses periodic differences too (the paper's own Cahn-Hilliard setting; total mass is
+ * conserved, eq. 21-22).
+ * ---------------------------------------------------------------------------------------- */
+BTPS_API penta_handle_t penta_factor_periodic(int n, const double *e, const double *a, const double *d,
+                                     const double *c, const double *f);
+
+/* ------------------------------------------------------------------------------------------
  * (a2)/(a4) Batched sweeps.  Tri: PAPER.md:95-108 (eq. 3-6), 568-597 (Alg. 2).
  * Penta: PAPER.md:258-278 (Sec. 4.1 "g" steps + back-substitution), 639-676 (Alg. 4).
  * d_rhs: DEVICE, n*batch elements, interleaved, solved in place.  Any batch >= 1.

@@ -9,7 +9,7 @@ ImportError.  (The binding is resolved on first attribute access so that the bui
 this package can be run before the library exists.)
 """
 _NAMES = (
-    "BtpsError", "TriHandle", "PentaHandle", "tri_factor", "tri_factor_periodic", "penta_factor",
+    "BtpsError", "TriHandle", "PentaHandle", "tri_factor", "tri_factor_periodic", "penta_factor", "penta_factor_periodic",
     "tri_solve_batched", "tri_solve_batched_f32", "penta_solve_batched", "penta_solve_batched_f32",
     "tri_solve_steps", "penta_solve_steps", "ch_step_batched",
     "tri_solve_batched_host", "penta_solve_batched_host", "ch_step_batched_host",

@@ -11,7 +11,7 @@ _LIB_PATH = os.path.join(_HERE, "libbtps.so")
 
 # every symbol include/btps.h declares (tests check the library exports each of them)
 EXPORTS = [
-    "tri_factor", "tri_factor_periodic", "tri_destroy", "penta_factor", "penta_destroy",
+    "tri_factor", "tri_factor_periodic", "tri_destroy", "penta_factor", "penta_factor_periodic", "penta_destroy",
     "tri_solve_batched", "tri_solve_batched_f32", "penta_solve_batched", "penta_solve_batched_f32",
     "tri_solve_steps", "penta_solve_steps", "ch_step_batched",
     "tri_solve_batched_host", "penta_solve_batched_host", "ch_step_batched_host",
@@ -46,6 +46,8 @@ def _load() -> ctypes.CDLL:
     lib.tri_destroy.restype = None
     lib.penta_factor.argtypes = [ci, dp, dp, dp, dp, dp]
     lib.penta_factor.restype = vp
+    lib.penta_factor_periodic.argtypes = [ci, dp, dp, dp, dp, dp]
+    lib.penta_factor_periodic.restype = vp
     lib.penta_destroy.argtypes = [vp]
     lib.penta_destroy.restype = None
     for name in ("tri_solve_batched", "tri_solve_batched_f32", "penta_solve_batched",
@@ -169,6 +171,18 @@ def penta_factor(e, a, d, c, f) -> PentaHandle:
     if any(v.size != n for v in (e, a, c, f)):
         raise ValueError("e, a, d, c, f must have the same length")
     ptr = _lib.penta_factor(n, _dptr(e), _dptr(a), _dptr(d), _dptr(c), _dptr(f))
+    if not ptr:
+        _raise_last()
+    return PentaHandle(ptr, n)
+
+
+def penta_factor_periodic(e, a, d, c, f) -> PentaHandle:
+    """btps.h penta_factor: host arrays e (2nd sub), a (sub), d (main), c (super), f (2nd super)."""
+    e, a, d, c, f = (_host64(v) for v in (e, a, d, c, f))
+    n = d.size
+    if any(v.size != n for v in (e, a, c, f)):
+        raise ValueError("e, a, d, c, f must have the same length")
+    ptr = _lib.penta_factor_periodic(n, _dptr(e), _dptr(a), _dptr(d), _dptr(c), _dptr(f))
     if not ptr:
         _raise_last()
     return PentaHandle(ptr, n)

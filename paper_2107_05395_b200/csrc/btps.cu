@@ -7,6 +7,7 @@
 #include "../../include/btps.h"
 #include "inst_common.cuh"
 
+#include <algorithm>
 #include <atomic>
 #include <cmath>
 #include <cstdio>
@@ -66,6 +67,7 @@ struct KernelSlot {
     int vec = 1;
     int tma = 0;       // 1: the TMA-prefetch variant (needs the ring in shared memory)
     int xvals = 2;     // exchange values per (partition, system)
+    int xstride = 0, xper = 0;  // exchange elements per group; offset of the periodic-penta values in it
     size_t smem = 0;
     unsigned offX = 0, offM = 0, offR = 0;
     unsigned box_rows = 0, nboxes = 0;
@@ -102,6 +104,7 @@ struct Handle {
     int kind;  // KIND_TRI / KIND_PENTA
     bool periodic = false;                    // tri: cyclic matrix solved by Sherman-Morrison (KIND_TRIP kernels)
     double per_vN = 0.0, per_invden = 0.0;    // eq. 13a / 15 scalars of the periodic solve
+    PerPenta pp = {};                         // periodic penta: Woodbury scalars (H, wrap-around entries)
     int n;
     int device;
     DtypePlan plan[2];  // 0: fp64, 1: fp32
@@ -387,10 +390,12 @@ void build_blob_tri(int n, DtypePlan &pl, const std::vector<double> &inv, const 
 template <typename T>
 void build_blob_penta(int n, DtypePlan &pl, const std::vector<double> &inv, const std::vector<double> &nle,
                       const std::vector<double> &nlb, const std::vector<double> &ngam,
-                      const std::vector<double> &ndel, std::vector<unsigned char> &blob)
+                      const std::vector<double> &ndel, std::vector<unsigned char> &blob,
+                      const std::vector<double> *Z = nullptr)
 {
     const int MR = pl.rows, P = pl.P, Np = P * MR;
-    constexpr int RT = RecLayout<KIND_PENTA>::ELEMS;
+    // coefficient values per row: the periodic form carries the rows of Z = A'^{-1} U (n x 4, row-major)
+    const int RT = Z ? RecLayout<KIND_PENTAP>::ELEMS : RecLayout<KIND_PENTA>::ELEMS;
     auto at = [&](const std::vector<double> &v, int i, double pad) { return i < n ? v[i] : pad; };
     pl.offT = (unsigned)align16((size_t)Np * RT * sizeof(T));
     pl.blob_bytes = (unsigned)align16(pl.offT + scan_table_bytes(pl, 2, sizeof(T)));
@@ -443,6 +448,8 @@ void build_blob_penta(int n, DtypePlan &pl, const std::vector<double> &inv, cons
             putv(5, i, 1, chi[1][k]);
             putv(7, i, 0, psi[0][k]);
             putv(7, i, 1, psi[1][k]);
+            if (Z)
+                for (int m = 0; m < 4; ++m) putv(m < 2 ? 9 : 11, i, m & 1, i < n ? (*Z)[(size_t)i * 4 + m] : 0.0);
         }
         // carries: (g at the last row, g at the last-but-one row) forward; (x at the first row, x at
         // the second row) backward
@@ -499,10 +506,13 @@ size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 void layout_slot(const DtypePlan &pl, const Shape &sh, int kind, KernelSlot &sl, bool halo = true)
 {
     const int NC = (kind == KIND_TRI || kind == KIND_TRIP) ? 1 : 2;
+    const bool is_ch = (kind == KIND_CH || kind == KIND_CHP), wood = (kind == KIND_PENTAP || kind == KIND_CHP);
     const size_t W = (size_t)sh.lanes * sl.vec;
     // CH: + the halo rows exchanged between fused steps; periodic tri: + y_1 and y_N of eq. 15
-    sl.xvals = 2 * NC + ((kind == KIND_CH && halo) ? 2 : 0) + (kind == KIND_TRIP ? 2 : 0);
-    const size_t xch = (pl.P > 1) ? (size_t)sh.tpc * sl.xvals * pl.P * W * pl.elem : 0;
+    sl.xvals = 2 * NC + ((is_ch && halo) ? 2 : 0) + (kind == KIND_TRIP ? 2 : 0);
+    sl.xper = (int)(sl.xvals * pl.P * W);
+    sl.xstride = sl.xper + (wood ? (int)(4 * W) : 0);  // cyclic penta: y at rows 0, 1, n-2, n-1
+    const size_t xch = (pl.P > 1) ? (size_t)sh.tpc * sl.xstride * pl.elem : 0;
     sl.offX = (unsigned)align16(pl.blob_bytes);
     sl.offM = (unsigned)align16(sl.offX + xch);
     sl.offR = (unsigned)align_up(sl.offM + 17 * 8, 128);
@@ -530,11 +540,15 @@ SweepEntry find_sweep(int kind, int elem_bytes, int vec, int rows, int single, i
     if (elem_bytes == 8) {
         if (kind == KIND_TRI) return find_sweep_tri_f64(vec, rows, single, tma, ws, fuse);
         if (kind == KIND_TRIP) return find_sweep_trip_f64(vec, rows, single, tma, ws, fuse);
+        if (kind == KIND_PENTAP) return find_sweep_pentap_f64(vec, rows, single, tma, ws, fuse);
+        if (kind == KIND_CHP) return find_sweep_chp_f64(vec, rows, single, tma, ws, fuse);
         if (kind == KIND_PENTA) return find_sweep_penta_f64(vec, rows, single, tma, ws, fuse);
         return find_sweep_ch_f64(vec, rows, single, tma, ws, fuse);
     }
     if (kind == KIND_TRI) return find_sweep_tri_f32(vec, rows, single, tma, ws, fuse);
     if (kind == KIND_TRIP) return find_sweep_trip_f32(vec, rows, single, tma, ws, fuse);
+    if (kind == KIND_PENTAP) return find_sweep_pentap_f32(vec, rows, single, tma, ws, fuse);
+    if (kind == KIND_CHP) return find_sweep_chp_f32(vec, rows, single, tma, ws, fuse);
     if (kind == KIND_PENTA) return find_sweep_penta_f32(vec, rows, single, tma, ws, fuse);
     return find_sweep_ch_f32(vec, rows, single, tma, ws, fuse);
 }
@@ -563,7 +577,10 @@ void fill_slots(Handle *h)
                 if (ks == 1) continue;
                 kind = h->periodic ? KIND_TRIP : KIND_TRI;
             } else {
-                kind = (ks == 0) ? KIND_PENTA : KIND_CH;
+                kind = (ks == 0) ? (h->periodic ? KIND_PENTAP : KIND_PENTA) : (h->periodic ? KIND_CHP : KIND_CH);
+                // the periodic CH kernels need whole partitions and at least two of them (halo wrap);
+                // other sizes run the two-pass form
+                if (kind == KIND_CHP && (h->n % pl.rows != 0 || pl.P < 2 || pl.P * pl.rows != h->n)) continue;
             }
             const Shape &sh = pl.shape[ks];
             for (int s = 0; s < 2; ++s) {
@@ -576,7 +593,7 @@ void fill_slots(Handle *h)
                     if (sl.tma && !tma_possible(pl, sh, sl.vec)) continue;
                     layout_slot(pl, sh, kind, sl);
                     bool can_fuse = true;
-                    if (sl.smem > SMEM_LIMIT && kind == KIND_CH) {
+                    if (sl.smem > SMEM_LIMIT && (kind == KIND_CH || kind == KIND_CHP)) {
                         // tight fit (N = 1024 fp64): drop the halo exchange rows, one step per launch
                         layout_slot(pl, sh, kind, sl, false);
                         can_fuse = false;
@@ -665,22 +682,31 @@ int launch_one(Handle *h, int kind, T *d_rhs, long long batch, double alpha_x, i
                cudaStream_t st)
 {
     DtypePlan &pl = h->plan[sizeof(T) == 8 ? 0 : 1];
-    if (pl.two_pass) {
+    // the paper's own 2R+2W form (Alg. 2 / 4), ksteps launches: plans too large for the on-chip tables,
+    // and periodic CH shapes the partitioned kernels do not cover (n not a multiple of the rows per thread)
+    auto two_pass = [&]() -> int {
         const int block = 128;
         const long long grid = (batch + block - 1) / block;
-        if (kind == KIND_TRI && h->periodic)
-            two_pass_kernel<T, KIND_TRIP><<<(unsigned)grid, block, 0, st>>>((const T *)pl.d_soa, d_rhs, batch, h->n,
-                                                                            h->per_vN, h->per_invden);
-        else if (kind == KIND_TRI)
-            two_pass_kernel<T, KIND_TRI><<<(unsigned)grid, block, 0, st>>>((const T *)pl.d_soa, d_rhs, batch, h->n, 0.0);
-        else if (kind == KIND_PENTA)
-            two_pass_kernel<T, KIND_PENTA><<<(unsigned)grid, block, 0, st>>>((const T *)pl.d_soa, d_rhs, batch, h->n, 0.0);
-        else
-            two_pass_kernel<T, KIND_CH><<<(unsigned)grid, block, 0, st>>>((const T *)pl.d_soa, d_rhs, batch, h->n, alpha_x);
-        g_launches.fetch_add(1, std::memory_order_relaxed);
-        CU_TRY(cudaGetLastError());
-        return BTPS_OK;  // fuse_limit() keeps ksteps == 1 for this plan
-    }
+        const T *co = (const T *)pl.d_soa;
+        for (int l = 0; l < ksteps; ++l) {
+            if (kind == KIND_TRI && h->periodic)
+                two_pass_kernel<T, KIND_TRIP><<<(unsigned)grid, block, 0, st>>>(co, d_rhs, batch, h->n, h->per_vN, h->per_invden, h->pp);
+            else if (kind == KIND_TRI)
+                two_pass_kernel<T, KIND_TRI><<<(unsigned)grid, block, 0, st>>>(co, d_rhs, batch, h->n, 0.0, 0.0, h->pp);
+            else if (kind == KIND_PENTA && h->periodic)
+                two_pass_kernel<T, KIND_PENTAP><<<(unsigned)grid, block, 0, st>>>(co, d_rhs, batch, h->n, 0.0, 0.0, h->pp);
+            else if (kind == KIND_PENTA)
+                two_pass_kernel<T, KIND_PENTA><<<(unsigned)grid, block, 0, st>>>(co, d_rhs, batch, h->n, 0.0, 0.0, h->pp);
+            else if (h->periodic)
+                two_pass_kernel<T, KIND_CHP><<<(unsigned)grid, block, 0, st>>>(co, d_rhs, batch, h->n, alpha_x, 0.0, h->pp);
+            else
+                two_pass_kernel<T, KIND_CH><<<(unsigned)grid, block, 0, st>>>(co, d_rhs, batch, h->n, alpha_x, 0.0, h->pp);
+            g_launches.fetch_add(1, std::memory_order_relaxed);
+            CU_TRY(cudaGetLastError());
+        }
+        return BTPS_OK;
+    };
+    if (pl.two_pass) return two_pass();
     const int ks = (kind == KIND_CH) ? 1 : 0;
     const Shape &sh = pl.shape[ks];
     // the vectorised kernels need whole vectors: batch % vec == 0 and an aligned base pointer;
@@ -696,10 +722,7 @@ int launch_one(Handle *h, int kind, T *d_rhs, long long batch, double alpha_x, i
     if (!pl.k[ks][s][d].ent.func && s == 0) s = 1;  // e.g. the wide variant has no direct-load twin that fits
     if (!pl.k[ks][s][d].ent.func) d = 1;
     KernelSlot &sl = pl.k[ks][s][d];
-    if (!sl.ent.func) {
-        snprintf(tl_cuda_msg, sizeof(tl_cuda_msg), "no kernel variant for this plan");
-        return set_err(BTPS_E_CUDA);
-    }
+    if (!sl.ent.func) return two_pass();
     if (sl.max_grid == 0) {
         const int rc = resolve_slot(h, sh, sl);
         if (rc != BTPS_OK) return rc;
@@ -715,6 +738,17 @@ int launch_one(Handle *h, int kind, T *d_rhs, long long batch, double alpha_x, i
     a.per_invden = h->per_invden;
     a.last_part = (h->n - 1) / pl.rows;
     a.last_k = (h->n - 1) % pl.rows;
+    for (int i = 0; i < 16; ++i) a.per_H[i] = h->pp.H[i];
+    for (int i = 0; i < 6; ++i) a.per_w6[i] = h->pp.w6[i];
+    {
+        const int wr[4] = {0, h->n > 1 ? 1 : 0, h->n > 2 ? h->n - 2 : 0, h->n - 1};
+        for (int i = 0; i < 4; ++i) {
+            a.wrow_part[i] = wr[i] / pl.rows;
+            a.wrow_k[i] = wr[i] % pl.rows;
+        }
+    }
+    a.xstride = sl.xstride;
+    a.xper = sl.xper;
     a.n = h->n;
     a.P = pl.P;
     a.lanes = sh.lanes;
@@ -965,6 +999,51 @@ void tri_destroy(tri_handle_t hv)
     if (h) free_handle(h);
 }
 
+// shared by penta_factor and penta_factor_periodic: tables + upload for a factored matrix
+static penta_handle_t make_penta_handle(int n, const std::vector<double> &inv, const std::vector<double> &nle,
+                                        const std::vector<double> &nlb, const std::vector<double> &ngam,
+                                        const std::vector<double> &ndel, const std::vector<double> *Z,
+                                        const PerPenta *pp)
+{
+    Handle *h = new Handle();
+    h->magic = MAGIC_PENTA;
+    h->kind = KIND_PENTA;
+    h->periodic = (Z != nullptr);
+    if (pp) h->pp = *pp;
+    h->n = n;
+    h->device = 0;
+    std::vector<double> zc[4];
+    std::vector<const std::vector<double> *> arrs = {&inv, &nle, &nlb, &ngam, &ndel};
+    if (Z) {
+        for (int m = 0; m < 4; ++m) {
+            zc[m].resize(n);
+            for (int i = 0; i < n; ++i) zc[m][i] = (*Z)[(size_t)i * 4 + m];
+            arrs.push_back(&zc[m]);
+        }
+    }
+    for (int t = 0; t < 2; ++t) {
+        DtypePlan &pl = h->plan[t];
+        choose_plan(n, t == 0 ? 8 : 4, h->kind, pl);
+        std::vector<unsigned char> blob, soa;
+        if (t == 0) {
+            build_blob_penta<double>(n, pl, inv, nle, nlb, ngam, ndel, blob, Z);
+            build_soa<double>(arrs, n, soa);
+        } else {
+            build_blob_penta<float>(n, pl, inv, nle, nlb, ngam, ndel, blob, Z);
+            build_soa<float>(arrs, n, soa);
+        }
+        pl.soa_bytes = soa.size();
+        fit_plan(pl, Z ? KIND_PENTAP : KIND_PENTA);
+        if (upload(blob, &pl.d_blob) != BTPS_OK || upload(soa, &pl.d_soa) != BTPS_OK) {
+            free_handle(h);
+            return nullptr;
+        }
+    }
+    fill_slots(h);
+    set_err(BTPS_OK);
+    return (penta_handle_t)h;
+}
+
 penta_handle_t penta_factor(int n, const double *e, const double *a, const double *d, const double *c,
                             const double *f)
 {
@@ -978,32 +1057,79 @@ penta_handle_t penta_factor(int n, const double *e, const double *a, const doubl
         set_err(BTPS_E_PIVOT, row);
         return nullptr;
     }
-    Handle *h = new Handle();
-    h->magic = MAGIC_PENTA;
-    h->kind = KIND_PENTA;
-    h->n = n;
-    h->device = 0;
-    for (int t = 0; t < 2; ++t) {
-        DtypePlan &pl = h->plan[t];
-        choose_plan(n, t == 0 ? 8 : 4, h->kind, pl);
-        std::vector<unsigned char> blob, soa;
-        if (t == 0) {
-            build_blob_penta<double>(n, pl, inv, nle, nlb, ngam, ndel, blob);
-            build_soa<double>({&inv, &nle, &nlb, &ngam, &ndel}, n, soa);
-        } else {
-            build_blob_penta<float>(n, pl, inv, nle, nlb, ngam, ndel, blob);
-            build_soa<float>({&inv, &nle, &nlb, &ngam, &ndel}, n, soa);
+    return make_penta_handle(n, inv, nle, nlb, ngam, ndel, nullptr, nullptr);
+}
+
+// Periodic (cyclic) pentadiagonal matrix (eq. 26a).  The paper cites [24,4,25] for the
+// method; here (C-31) A = A' + U V^T with A' the matrix without its six wrap-around entries
+// (factored as in penta_factor), U = unit columns at rows 0, 1, n-2, n-1 and V^T the wrap-around
+// entries; Z = A'^{-1} U and H = (I + V^T Z)^{-1} are computed once here, the kernels finish each solve
+// with x = y - Z H (V^T y).
+penta_handle_t penta_factor_periodic(int n, const double *e, const double *a, const double *d, const double *c,
+                                     const double *f)
+{
+    if (n < 5 || !e || !a || !d || !c || !f) {
+        set_err(BTPS_E_ARG);
+        return nullptr;
+    }
+    std::vector<double> inv, nle, nlb, ngam, ndel;
+    int row = 0;
+    if (factor_penta_host(n, e, a, d, c, f, inv, nle, nlb, ngam, ndel, &row) != BTPS_OK) {
+        set_err(BTPS_E_PIVOT, row);
+        return nullptr;
+    }
+    PerPenta pp = {};
+    const double w6[6] = {e[0], a[0], e[1], f[n - 2], c[n - 1], f[n - 1]};
+    for (int i = 0; i < 6; ++i) pp.w6[i] = w6[i];
+    // Z = A'^{-1} U with the sweep multipliers (forward: g_i = inv_i r_i + nle_i g_{i-2} + nlb_i g_{i-1};
+    // backward: x_i = g_i + ngam_i x_{i+1} + ndel_i x_{i+2})
+    std::vector<double> Z((size_t)n * 4, 0.0), col(n);
+    const int urow[4] = {0, 1, n - 2, n - 1};
+    for (int m = 0; m < 4; ++m) {
+        std::fill(col.begin(), col.end(), 0.0);
+        col[urow[m]] = 1.0;
+        for (int i = 0; i < n; ++i)
+            col[i] = inv[i] * col[i] + (i >= 2 ? nle[i] * col[i - 2] : 0.0) + (i >= 1 ? nlb[i] * col[i - 1] : 0.0);
+        for (int i = n - 2; i >= 0; --i)
+            col[i] = col[i] + ngam[i] * col[i + 1] + (i + 2 < n ? ndel[i] * col[i + 2] : 0.0);
+        for (int i = 0; i < n; ++i) Z[(size_t)i * 4 + m] = col[i];
+    }
+    // S = I + V^T Z, H = S^{-1}: solve S H = I column by column (Gaussian elimination, partial pivoting)
+    double S[4][4];
+    for (int m = 0; m < 4; ++m) {
+        S[0][m] = w6[0] * Z[(size_t)(n - 2) * 4 + m] + w6[1] * Z[(size_t)(n - 1) * 4 + m];
+        S[1][m] = w6[2] * Z[(size_t)(n - 1) * 4 + m];
+        S[2][m] = w6[3] * Z[m];
+        S[3][m] = w6[4] * Z[m] + w6[5] * Z[4 + m];
+    }
+    for (int m = 0; m < 4; ++m) S[m][m] += 1.0;
+    double aug[4][8];
+    for (int i = 0; i < 4; ++i)
+        for (int j = 0; j < 4; ++j) {
+            aug[i][j] = S[i][j];
+            aug[i][4 + j] = (i == j) ? 1.0 : 0.0;
         }
-        pl.soa_bytes = soa.size();
-        fit_plan(pl, h->kind);
-        if (upload(blob, &pl.d_blob) != BTPS_OK || upload(soa, &pl.d_soa) != BTPS_OK) {
-            free_handle(h);
+    for (int k = 0; k < 4; ++k) {
+        int pr = k;
+        for (int r = k + 1; r < 4; ++r)
+            if (std::fabs(aug[r][k]) > std::fabs(aug[pr][k])) pr = r;
+        if (aug[pr][k] == 0.0 || !std::isfinite(aug[pr][k])) {
+            set_err(BTPS_E_PIVOT, n);
             return nullptr;
         }
+        for (int j = 0; j < 8; ++j) std::swap(aug[k][j], aug[pr][j]);
+        for (int r = k + 1; r < 4; ++r) {
+            const double mlt = aug[r][k] / aug[k][k];
+            for (int j = k; j < 8; ++j) aug[r][j] -= mlt * aug[k][j];
+        }
     }
-    fill_slots(h);
-    set_err(BTPS_OK);
-    return (penta_handle_t)h;
+    for (int j = 0; j < 4; ++j)          // back substitution for each column of H
+        for (int i = 3; i >= 0; --i) {
+            double v = aug[i][4 + j];
+            for (int r = i + 1; r < 4; ++r) v -= aug[i][r] * pp.H[r * 4 + j];
+            pp.H[i * 4 + j] = v / aug[i][i];
+        }
+    return make_penta_handle(n, inv, nle, nlb, ngam, ndel, &Z, &pp);
 }
 
 void penta_destroy(penta_handle_t hv)

@@ -76,5 +76,9 @@ SweepEntry find_sweep_ch_f64(int vec, int rows, int single, int tma, int ws, int
 SweepEntry find_sweep_ch_f32(int vec, int rows, int single, int tma, int ws, int fuse);
 SweepEntry find_sweep_trip_f64(int vec, int rows, int single, int tma, int ws, int fuse);
 SweepEntry find_sweep_trip_f32(int vec, int rows, int single, int tma, int ws, int fuse);
+SweepEntry find_sweep_pentap_f64(int vec, int rows, int single, int tma, int ws, int fuse);
+SweepEntry find_sweep_pentap_f32(int vec, int rows, int single, int tma, int ws, int fuse);
+SweepEntry find_sweep_chp_f64(int vec, int rows, int single, int tma, int ws, int fuse);
+SweepEntry find_sweep_chp_f32(int vec, int rows, int single, int tma, int ws, int fuse);
 
 }  // namespace btps

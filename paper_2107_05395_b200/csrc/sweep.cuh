@@ -36,7 +36,8 @@
 
 namespace btps {
 
-enum Kind { KIND_TRI = 0, KIND_PENTA = 1, KIND_CH = 2, KIND_TRIP = 3 };  // TRIP: periodic tridiagonal
+// TRIP / PENTAP / CHP: the periodic (cyclic) forms of TRI / PENTA / CH
+enum Kind { KIND_TRI = 0, KIND_PENTA = 1, KIND_CH = 2, KIND_TRIP = 3, KIND_PENTAP = 4, KIND_CHP = 5 };
 
 constexpr int SCAN_STEPS = 5;   // Kogge-Stone steps held in the tables (scan width <= 32)
 constexpr int SCAN_LANES = 32;
@@ -50,6 +51,11 @@ struct SweepArgs {
     double per_vN;         // periodic tri: last entry of v, eq. 13a (-a_1/b_1)
     double per_invden;     // periodic tri: 1 / (1 + v.z), eq. 15
     int last_part, last_k; // periodic tri: partition and local row of row n-1
+    double per_H[16];      // periodic penta: (I + V^T Z)^{-1}, row-major (Woodbury)
+    double per_w6[6];      // periodic penta: wrap-around entries e_0, a_0, e_1, f_{n-2}, c_{n-1}, f_{n-1}
+    int wrow_part[4], wrow_k[4];  // periodic penta: partition / local row of rows 0, 1, n-2, n-1
+    int xstride;           // elements of exchange area per group
+    int xper;              // element offset (inside a group's area) of the 4 x W periodic-penta values
     int n;                 // true number of rows
     int P;                 // partitions per system (rows padded to P*MR with identity rows)
     int lanes;             // threads side by side on adjacent systems (power of two <= 32)
@@ -119,6 +125,7 @@ __device__ __forceinline__ T ch_w(T c) { return fma_t<T>(c * c, c, -c); }
 //           inv = 1/b^_i, nl = -a_i/b^_i, nch = -c^_i; chi/psi = response of the finished local
 //           sweeps to the incoming forward / backward carry
 //   periodic tri (6 MR): as tri, plus 5: z = A'^{-1} u of the Sherman-Morrison splitting
+//   periodic penta (13 MR): as penta, plus 9: {z0, z1}  11: {z2, z3}, the rows of Z = A'^{-1} U (Woodbury)
 //   penta (9 MR): 0: {inv, nle}  2: nlb    3: {ngam, ndel}   5: {chi1, chi2}   7: {psi1, psi2}
 //           inv = 1/alpha_i, nle = -eps_i/alpha_i, nlb = -beta_i/alpha_i, ngam = -gamma_i, ndel = -delta_i
 // followed at offT by the carry-scan tables, indexed [slot][m][q] with q = partition (tq entries),
@@ -135,7 +142,8 @@ __device__ __forceinline__ T ch_w(T c) { return fma_t<T>(c * c, c, -c); }
 template <int KIND>
 struct RecLayout {
     static constexpr bool TRI = (KIND == KIND_TRI || KIND == KIND_TRIP);
-    static constexpr int ELEMS = (KIND == KIND_TRI) ? 5 : (KIND == KIND_TRIP ? 6 : 9);  // coefficient values per row
+    static constexpr bool WOOD = (KIND == KIND_PENTAP || KIND == KIND_CHP);  // rank-4 Woodbury correction
+    static constexpr int ELEMS = (KIND == KIND_TRI) ? 5 : (KIND == KIND_TRIP ? 6 : (WOOD ? 13 : 9));  // values per row
     static constexpr int NC = TRI ? 1 : 2;                     // carries per direction
 };
 
@@ -223,6 +231,9 @@ __global__ void __launch_bounds__(CtaShape<T, V, MR>::MAX_THREADS, 1)
 sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
 {
     constexpr bool TRI = RecLayout<KIND>::TRI;
+    constexpr bool ISCH = (KIND == KIND_CH || KIND == KIND_CHP);  // explicit Cahn-Hilliard half fused in
+    constexpr bool WRAP = (KIND == KIND_CHP);                     // ... with periodic differences
+    constexpr bool WOOD = RecLayout<KIND>::WOOD;
     constexpr int NC = RecLayout<KIND>::NC;
     using Pair = Tup<T, 2>;
     extern __shared__ __align__(128) unsigned char smem[];
@@ -270,7 +281,7 @@ sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
     [[maybe_unused]] const Pair *const RC1 = reinterpret_cast<const Pair *>(cb + 7 * MR);  // penta {psi1, psi2}
     [[maybe_unused]] const T *const TAB = reinterpret_cast<const T *>(smem + a.offT);
     // exchange area of this group: [2*NC values][P][W], columns XOR-swizzled with the partition index
-    [[maybe_unused]] T *const xb = reinterpret_cast<T *>(smem + a.offX) + (size_t)sub * a.xvals * a.P * W;
+    [[maybe_unused]] T *const xb = reinterpret_cast<T *>(smem + a.offX) + (size_t)sub * a.xstride;
     // prefetch ring of this group: [P*MR rows][W]
     [[maybe_unused]] const unsigned ring_bytes = (unsigned)(a.P * MR * W) * (unsigned)sizeof(T);
     [[maybe_unused]] T *const ring = reinterpret_cast<T *>(smem + a.offR + (size_t)sub * ring_bytes);
@@ -313,12 +324,15 @@ sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
             asm volatile("" : "+l"(rp));  // recompute the MR row addresses per tile: hoisted out of the loop they spill
 #pragma unroll
             for (int k = 0; k < MR; ++k) ld_sys<T, V>(v[k], rp + k * W);
-            if constexpr (KIND == KIND_CH) {
+            if constexpr (ISCH) {
 #pragma unroll
                 for (int e = 0; e < V; ++e) cm[e] = cp[e] = T(0);
                 if constexpr (!SINGLE) {
+                    // periodic form (n a multiple of MR): row -1 is row n-1, row n is row 0
                     if (part > 0) ld_sys<T, V>(cm, rp - W);
+                    else if (WRAP) ld_sys<T, V>(cm, ring + ((a.n - 1) * W + sl * V));
                     if (part + 1 < a.P) ld_sys<T, V>(cp, rp + MR * W);
+                    else if (WRAP) ld_sys<T, V>(cp, ring + sl * V);
                 }
             }
             group_sync(a.tpc, sub, tpt);  // every thread has drained the ring
@@ -337,20 +351,22 @@ sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
                 }
                 pl += batch;
             }
-            if constexpr (KIND == KIND_CH) {
+            if constexpr (ISCH) {
                 // halo rows come from the neighbouring partitions' rows in global memory (still
                 // c^n: nobody stores before the barriers below).
 #pragma unroll
                 for (int e = 0; e < V; ++e) cm[e] = cp[e] = T(0);
                 if (act && r0 > 0) ld_sys<T, V>(cm, p0 - batch);
+                else if (WRAP && act) ld_sys<T, V>(cm, p0 + (long long)(a.n - 1) * batch);   // r0 == 0: row n-1
                 if (act && (r0 + MR < a.n)) ld_sys<T, V>(cp, p0 + (long long)MR * batch);
+                else if (WRAP && act) ld_sys<T, V>(cp, p0 - (long long)r0 * batch);          // row 0
             }
         }
 
         // ---- ksteps time steps on the tile while it is on chip (RHS = previous solution) ----
         const int nks = FUSE ? a.ksteps : 1;
         for (int ks = 0; ks < nks; ++ks) {
-        if constexpr (KIND == KIND_CH && !SINGLE) {
+        if constexpr (ISCH && !SINGLE) {
             if (ks > 0) {
                 // halo rows of c^{n+ks}: the neighbouring partitions' first / last rows, published to
                 // exchange values 2NC (first row) and 2NC+1 (last row) at the end of the previous step
@@ -358,8 +374,10 @@ sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
                 const int hv = a.P * W, hm = W - 1;
 #pragma unroll
                 for (int e = 0; e < V; ++e) {
-                    cm[e] = (part > 0) ? xb[(2 * NC + 1) * hv + (part - 1) * W + ((sl * V + e) ^ ((part - 1) & hm))] : T(0);
-                    cp[e] = (part + 1 < a.P) ? xb[2 * NC * hv + (part + 1) * W + ((sl * V + e) ^ ((part + 1) & hm))] : T(0);
+                    const int pm = (part > 0) ? part - 1 : (WRAP ? a.P - 1 : -1);
+                    const int pp = (part + 1 < a.P) ? part + 1 : (WRAP ? 0 : -1);
+                    cm[e] = (pm >= 0) ? xb[(2 * NC + 1) * hv + pm * W + ((sl * V + e) ^ (pm & hm))] : T(0);
+                    cp[e] = (pp >= 0) ? xb[2 * NC * hv + pp * W + ((sl * V + e) ^ (pp & hm))] : T(0);
                 }
             }
         }
@@ -394,7 +412,7 @@ sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
             T g1[V], g2[V];  // g_{k-1}, g_{k-2}
 #pragma unroll
             for (int e = 0; e < V; ++e) g1[e] = g2[e] = T(0);
-            if constexpr (KIND == KIND_CH) {
+            if constexpr (ISCH) {
                 // explicit half: f_k = c_k + alpha_x (w_{k-1} - 2 w_k + w_{k+1}); cm / cp are the
                 // halo rows r0-1 and r0+MR fetched above (zero outside the system).
                 const T ax = (T)a.alpha_x;
@@ -683,15 +701,6 @@ sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
                     }
                 }
             }
-            if constexpr (KIND == KIND_CH) {
-                if (ks + 1 < nks) {  // publish this partition's first / last rows for the next step
-#pragma unroll
-                    for (int e = 0; e < V; ++e) {
-                        xc[2 * NC * vstr + XI(e)] = v[0][e];
-                        xc[(2 * NC + 1) * vstr + XI(e)] = v[MR - 1][e];
-                    }
-                }
-            }
 #undef XI
         }
         if constexpr (KIND == KIND_TRIP) {
@@ -732,6 +741,73 @@ sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
                 for (int e = 0; e < V; ++e) v[k][e] = fma_t<T>(nfac[e], zk, v[k][e]);
             }
         }
+        if constexpr (WOOD) {
+            // ---- cyclic pentadiagonal: x = y - Z H (V^T y)  (Woodbury; C-31) ------------------
+            // V^T y needs y at rows 0, 1, n-2, n-1; their owners publish them to 4 x W exchange values
+            T yr[4][V];
+#pragma unroll
+            for (int m = 0; m < 4; ++m) {
+#pragma unroll
+                for (int e = 0; e < V; ++e) yr[m][e] = T(0);
+                if (SINGLE || part == a.wrow_part[m]) {
+#pragma unroll
+                    for (int k = 0; k < MR; ++k)
+                        if (k == a.wrow_k[m]) {
+#pragma unroll
+                            for (int e = 0; e < V; ++e) yr[m][e] = v[k][e];
+                        }
+                }
+            }
+            if constexpr (!SINGLE) {
+                T *const pw = xb + a.xper + sl * V;
+#pragma unroll
+                for (int m = 0; m < 4; ++m)
+                    if (part == a.wrow_part[m]) {
+#pragma unroll
+                        for (int e = 0; e < V; ++e) pw[m * W + e] = yr[m][e];
+                    }
+                group_sync(a.tpc, sub, tpt);
+#pragma unroll
+                for (int m = 0; m < 4; ++m)
+#pragma unroll
+                    for (int e = 0; e < V; ++e) yr[m][e] = pw[m * W + e];
+            }
+            T nw[4][V];
+#pragma unroll
+            for (int e = 0; e < V; ++e) {
+                const T t0 = fma_t<T>((T)a.per_w6[1], yr[3][e], (T)a.per_w6[0] * yr[2][e]);
+                const T t1 = (T)a.per_w6[2] * yr[3][e];
+                const T t2 = (T)a.per_w6[3] * yr[0][e];
+                const T t3 = fma_t<T>((T)a.per_w6[5], yr[1][e], (T)a.per_w6[4] * yr[0][e]);
+#pragma unroll
+                for (int m = 0; m < 4; ++m)
+                    nw[m][e] = -fma_t<T>((T)a.per_H[m * 4 + 3], t3, fma_t<T>((T)a.per_H[m * 4 + 2], t2,
+                                          fma_t<T>((T)a.per_H[m * 4 + 1], t1, (T)a.per_H[m * 4] * t0)));
+            }
+            const Pair *const Z01 = reinterpret_cast<const Pair *>(cb + 9 * MR);
+            const Pair *const Z23 = reinterpret_cast<const Pair *>(cb + 11 * MR);
+#pragma unroll
+            for (int k = 0; k < MR; ++k) {
+                const Pair za = Z01[k], zb = Z23[k];
+#pragma unroll
+                for (int e = 0; e < V; ++e) {
+                    T x = fma_t<T>(nw[0][e], za.v[0], v[k][e]);
+                    x = fma_t<T>(nw[1][e], za.v[1], x);
+                    x = fma_t<T>(nw[2][e], zb.v[0], x);
+                    v[k][e] = fma_t<T>(nw[3][e], zb.v[1], x);
+                }
+            }
+        }
+        if constexpr (ISCH && !SINGLE) {
+            if (ks + 1 < nks) {  // publish this partition's first / last rows: the neighbours' halo of the next step
+                const int hv = a.P * W, hx = part & (W - 1);
+#pragma unroll
+                for (int e = 0; e < V; ++e) {
+                    xb[2 * NC * hv + part * W + ((sl * V + e) ^ hx)] = v[0][e];
+                    xb[(2 * NC + 1) * hv + part * W + ((sl * V + e) ^ hx)] = v[MR - 1][e];
+                }
+            }
+        }
         }  // ksteps
 
         // ---- store ---------------------------------------------------------------------------
@@ -755,9 +831,14 @@ sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
 //   tri   : co[0..n) inv, co[n..2n) nl, co[2n..3n) nch
 //   penta : inv, nle, nlb, ngam, ndel
 // -----------------------------------------------------------------------------------------------
+struct PerPenta {  // scalars of the cyclic pentadiagonal (Woodbury) correction
+    double H[16];  // (I + V^T Z)^{-1}, row-major
+    double w6[6];  // wrap-around entries e_0, a_0, e_1, f_{n-2}, c_{n-1}, f_{n-1}
+};
+
 template <typename T, int KIND>
 __global__ void __launch_bounds__(128) two_pass_kernel(const T *__restrict__ co, T *rhs, long long batch,
-                                                       int n, double alpha_x, double alpha_y = 0.0)
+                                                       int n, double alpha_x, double alpha_y, const PerPenta pp)
 {
     const long long j = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (j >= batch) return;
@@ -784,11 +865,13 @@ __global__ void __launch_bounds__(128) two_pass_kernel(const T *__restrict__ co,
         const T *inv = co, *nle = co + n, *nlb = co + 2 * (size_t)n, *ngam = co + 3 * (size_t)n,
                 *ndel = co + 4 * (size_t)n;
         T g1 = T(0), g2 = T(0);
-        if constexpr (KIND == KIND_CH) {
+        if constexpr (KIND == KIND_CH || KIND == KIND_CHP) {
+            constexpr bool WRAPS = (KIND == KIND_CHP);  // periodic differences: row -1 = row n-1, row n = row 0
             const T ax = (T)alpha_x;
-            T wm = T(0), cc = p[0], wc = ch_w<T>(cc);
+            const T c_first = p[0];
+            T wm = WRAPS ? ch_w<T>(p[(long long)(n - 1) * batch]) : T(0), cc = c_first, wc = ch_w<T>(cc);
             for (int i = 0; i < n; ++i) {
-                const T cn = (i + 1 < n) ? p[(long long)(i + 1) * batch] : T(0);
+                const T cn = (i + 1 < n) ? p[(long long)(i + 1) * batch] : (WRAPS ? c_first : T(0));
                 const T wn = ch_w<T>(cn);
                 T s = wm + wn;
                 s = fma_t<T>(T(-2), wc, s);
@@ -813,6 +896,23 @@ __global__ void __launch_bounds__(128) two_pass_kernel(const T *__restrict__ co,
             const T x = fma_t<T>(__ldg(ngam + i), x1, t);
             p[(long long)i * batch] = x;
             x2 = x1; x1 = x;
+        }
+        if constexpr (KIND == KIND_PENTAP || KIND == KIND_CHP) {
+            // cyclic matrix: x = y - Z H (V^T y) (Woodbury, C-31); Z's four columns follow ndel in co
+            const T y0 = p[0], y1 = p[batch], yn2 = p[(long long)(n - 2) * batch], yn1 = p[(long long)(n - 1) * batch];
+            const T t0 = fma_t<T>((T)pp.w6[1], yn1, (T)pp.w6[0] * yn2), t1 = (T)pp.w6[2] * yn1, t2 = (T)pp.w6[3] * y0;
+            const T t3 = fma_t<T>((T)pp.w6[5], y1, (T)pp.w6[4] * y0);
+            T nw[4];
+            for (int m = 0; m < 4; ++m)
+                nw[m] = -fma_t<T>((T)pp.H[m * 4 + 3], t3, fma_t<T>((T)pp.H[m * 4 + 2], t2,
+                                  fma_t<T>((T)pp.H[m * 4 + 1], t1, (T)pp.H[m * 4] * t0)));
+            const T *z0 = co + 5 * (size_t)n, *z1 = co + 6 * (size_t)n, *z2 = co + 7 * (size_t)n, *z3 = co + 8 * (size_t)n;
+            for (int i = 0; i < n; ++i) {
+                T x = fma_t<T>(nw[0], __ldg(z0 + i), p[(long long)i * batch]);
+                x = fma_t<T>(nw[1], __ldg(z1 + i), x);
+                x = fma_t<T>(nw[2], __ldg(z2 + i), x);
+                p[(long long)i * batch] = fma_t<T>(nw[3], __ldg(z3 + i), x);
+            }
         }
     }
 }

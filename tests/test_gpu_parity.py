@@ -608,3 +608,68 @@ def test_tri_periodic_errors(lib):
         lib.tri_factor_periodic([1.0, 1.0], [2.0, 2.0], [1.0, 1.0])          # n < 3
     with pytest.raises(lib.BtpsError):
         lib.tri_factor_periodic([1.0] * 4, [0.0, 2.0, 2.0, 2.0], [1.0] * 4)  # b_0 = 0
+
+
+# ---- periodic pentadiagonal (Woodbury, C-31) and periodic Cahn-Hilliard --------------------
+
+def rand_cyclic_penta(n, seed):
+    rng = np.random.default_rng(seed)
+    e, a, c, f = (rng.uniform(-1, 1, n) for _ in range(4))
+    d = np.abs(e) + np.abs(a) + np.abs(c) + np.abs(f) + rng.uniform(0.5, 1.5, n)
+    return e, a, d, c, f
+
+
+@pytest.mark.parametrize("n", [5, 6, 31, 32, 33, 64, 300, 512, 1000, 1024, 1500, 5000])
+def test_penta_periodic_sizes(lib, n):
+    lhs = rand_cyclic_penta(n, n)
+    fo = oracle.penta_periodic_factor(*lhs)   # paper naming (a,b,c,d,e) = API (e,a,d,c,f)
+    h = lib.penta_factor_periodic(*lhs)
+    for batch in (1, 33, 1024 + 32, 1001):
+        rhs = inputs.uniform_rhs(n, batch, seed=n + batch)
+        ref = rhs.copy()
+        oracle.penta_periodic_solve_interleaved(fo, ref)
+        d = dev(rhs)
+        lib.penta_solve_batched(h, d)
+        assert rel_err(d.cpu().numpy(), ref) <= TOL_SINGLE, (n, batch, h.plan())
+    rhs = inputs.uniform_rhs(n, 512, seed=3).astype(np.float32)
+    ref = rhs.astype(np.float64)
+    oracle.penta_periodic_solve_interleaved(fo, ref)
+    d = dev(rhs)
+    lib.penta_solve_batched_f32(h, d)
+    assert rel_err(d.cpu().numpy(), ref) <= TOL_F32, (n, h.plan(4))
+
+
+@pytest.mark.parametrize("tune", [dict(), dict(prefetch=0), dict(warp_scan=0), dict(vec=1), dict(force_two_pass=1),
+                                  dict(fuse_steps=1)])
+@pytest.mark.parametrize("n", [256, 200])  # 200: not a multiple of the rows per thread -> two-pass form
+def test_periodic_cahn_hilliard_steps_and_mass(lib, tune, n):
+    """The paper's own Cahn-Hilliard setting (periodic): 40 steps against the oracle,
+    exact conservation of every run's mass (eq. 21-22), and the periodic penta time loop."""
+    batch, steps = 2048 + 64, 40
+    sigma, alpha = inputs.ch_params(256)
+    st = ([sigma] * n, [-4 * sigma] * n, [1 + 6 * sigma] * n, [-4 * sigma] * n, [sigma] * n)
+    try:
+        for k, v in tune.items():
+            lib.btps_tune(k, v)
+        h = lib.penta_factor_periodic(*st)
+        c0 = 0.1 * inputs.uniform_rhs(n, batch, seed=23)
+        d, d2 = dev(c0), dev(c0)
+        lib.ch_step_batched(h, d, alpha, steps)
+        lib.penta_solve_steps(h, d2, 11)
+    finally:
+        for k in tune:
+            lib.btps_tune(k, -1)
+    fo = oracle.penta_periodic_factor(*st)
+    ref = c0.copy()
+    oracle.ch_periodic_step_interleaved(fo, ref, alpha, nsteps=steps)
+    got = d.cpu().numpy()
+    assert rel_err(got, ref) <= TOL_STEPS, (tune, n, h.ch_plan())
+    assert np.max(np.abs(got.sum(axis=0) - c0.sum(axis=0))) <= 1e-13
+    ref = c0.copy()
+    oracle.penta_periodic_solve_interleaved(fo, ref, nsteps=11)
+    assert rel_err(d2.cpu().numpy(), ref) <= TOL_STEPS, (tune, n, h.plan())
+
+
+def test_penta_periodic_errors(lib):
+    with pytest.raises(lib.BtpsError):
+        lib.penta_factor_periodic(*([[1.0] * 4] * 5))  # n < 5
