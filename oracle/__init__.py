@@ -83,6 +83,8 @@ def _load():
         lib.orc_penta_periodic_interleaved.argtypes = [ctypes.c_int] + [_dp] * 9 + [_ll, _ll, _ll, _ll, ctypes.c_int,
                                                                                     ctypes.c_double, ctypes.c_int, ctypes.c_int]
         lib.orc_penta_periodic_interleaved.restype = ctypes.c_int
+        lib.orc_lbar_interleaved.argtypes = [ctypes.c_int, _dp, _ll]
+        lib.orc_lbar_interleaved.restype = ctypes.c_double
         _lib = lib
     return _lib
 
@@ -307,3 +309,23 @@ def penta_periodic_solve_interleaved(fac: PentaPeriodicFactor, rhs: np.ndarray, 
 def ch_periodic_step_interleaved(fac: PentaPeriodicFactor, c: np.ndarray, alpha: float, nsteps: int = 1,
                                  subset=None, nthreads: int = 0) -> int:
     return _penta_periodic_interleaved(fac, c, 1, alpha, nsteps, subset, nthreads)
+
+
+# ---- coarsening statistic (eq. 30) ---------------------------------------------------
+
+def lbar_interleaved(c: np.ndarray) -> float:
+    """Mean over the runs (columns) of 1 / (1 - <C^2>), <C^2> = mean over the rows of C^2."""
+    assert c.ndim == 2 and c.dtype == np.float64 and c.flags.c_contiguous
+    return float(_load().orc_lbar_interleaved(c.shape[0], _p(c), c.shape[1]))
+
+
+def ch_steps_with_lbar(fac, c: np.ndarray, alpha: float, nsteps: int, periodic: bool = True) -> np.ndarray:
+    """Advance ``c`` in place ``nsteps`` steps, returning lbar after every step (eq. 30 "at every time-step")."""
+    out = np.zeros(nsteps)
+    for s in range(nsteps):
+        if periodic:
+            ch_periodic_step_interleaved(fac, c, alpha, nsteps=1)
+        else:
+            ch_step_interleaved(fac, c, alpha, nsteps=1)
+        out[s] = lbar_interleaved(c)
+    return out

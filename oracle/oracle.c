@@ -452,3 +452,20 @@ ORC_API int orc_penta_periodic_interleaved(int n, const double *eps, const doubl
     }
     return used;
 }
+
+/* ------------------------------------------------------------------------------------
+ * Coarsening statistic, PAPER.md:433-439 (eq. 30): l = 1 / (1 - <C^2>), <C^2> = (1/L) int C^2 dx,
+ * evaluated on the uniform periodic grid as the mean of C_i^2 over the N points of a run, then averaged
+ * over the M independent runs of the batch ("captured for each simulation ... then averaged across
+ * simulations").  Serial, in index order.
+ * ---------------------------------------------------------------------------------- */
+ORC_API double orc_lbar_interleaved(int n, const double *c, long long M)
+{
+    double acc = 0.0;
+    for (long long j = 0; j < M; ++j) {
+        double s2 = 0.0;
+        for (int i = 0; i < n; ++i) s2 += c[(size_t)i * M + j] * c[(size_t)i * M + j];
+        acc += 1.0 / (1.0 - s2 / (double)n);
+    }
+    return acc / (double)M;
+}

@@ -129,3 +129,21 @@ def test_subset_and_threads():
     np.testing.assert_array_equal(sub[:, cols], full[:, cols])
     rest = [j for j in range(M) if j not in cols]
     np.testing.assert_array_equal(sub[:, rest], c[:, rest])
+
+
+# ---- coarsening statistic (eq. 30) ---------------------------------------------------
+
+def test_lbar_closed_forms():
+    """<C^2> of a constant c0 is c0^2; of A*cos(2 pi k x / L) on the periodic grid it is A^2 / 2 exactly
+    (0 < k < N/2); the batch value is the mean of 1/(1 - <C^2>) over the runs."""
+    import oracle
+    n = 64
+    j = np.arange(n)
+    cols = [np.full(n, 0.3), 0.8 * np.cos(2 * np.pi * 5 * j / n), 0.5 * np.sin(2 * np.pi * 3 * j / n), np.zeros(n)]
+    c = np.ascontiguousarray(np.stack(cols, axis=1))
+    expect = np.mean([1 / (1 - 0.09), 1 / (1 - 0.32), 1 / (1 - 0.125), 1.0])
+    assert abs(oracle.lbar_interleaved(c) - expect) <= 1e-15
+    # a single run; and invariance under a permutation of the rows (it is a mean over the grid)
+    one = np.ascontiguousarray(c[:, 1:2])
+    assert abs(oracle.lbar_interleaved(one) - 1 / (1 - 0.32)) <= 1e-15
+    assert abs(oracle.lbar_interleaved(np.ascontiguousarray(one[::-1])) - 1 / (1 - 0.32)) <= 1e-15
