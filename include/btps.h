@@ -139,6 +139,18 @@ BTPS_API int ch_step_batched(penta_handle_t h, double *d_c, int64_t batch, doubl
                     void *stream);
 
 /* ------------------------------------------------------------------------------------------
+ * The same steps, recording the coarsening statistic of PAPER.md:433-439 (eq. 30) after every step:
+ *   d_lbar[s] = (1/batch) * sum over the runs j of  1 / (1 - <C_j^2>),  <C_j^2> = (1/n) sum_i c[i*batch+j]^2
+ * for s = 0 .. nsteps-1 ("captured for each simulation at every time-step and then averaged across
+ * simulations").  d_lbar: DEVICE, nsteps doubles, overwritten (zeroed on the stream, then accumulated
+ * with atomic adds: the summation order over the runs is not fixed, results agree to rounding).  The sums
+ * are formed inside the fused step kernels from the registers that hold c^{n+1}; where no fused kernel
+ * runs (unaligned batches, two-pass plans) a separate read pass computes them.
+ * ---------------------------------------------------------------------------------------- */
+BTPS_API int ch_step_batched_stat(penta_handle_t h, double *d_c, int64_t batch, double alpha, int nsteps,
+                         double *d_lbar, void *stream);
+
+/* ------------------------------------------------------------------------------------------
  * End-to-end variants on HOST buffers (the call a user without device code makes).
  * h_rhs / h_c: HOST, n*batch elements, interleaved; pinned memory is used at full speed,
  * pageable memory works but copies slower.  The batch is cut into column chunks; each chunk

@@ -13,7 +13,7 @@ _LIB_PATH = os.path.join(_HERE, "libbtps.so")
 EXPORTS = [
     "tri_factor", "tri_factor_periodic", "tri_destroy", "penta_factor", "penta_factor_periodic", "penta_destroy",
     "tri_solve_batched", "tri_solve_batched_f32", "penta_solve_batched", "penta_solve_batched_f32",
-    "tri_solve_steps", "penta_solve_steps", "ch_step_batched",
+    "tri_solve_steps", "penta_solve_steps", "ch_step_batched", "ch_step_batched_stat",
     "tri_solve_batched_host", "penta_solve_batched_host", "ch_step_batched_host",
     "btps_last_error", "btps_error_string", "btps_plan_info", "btps_tune", "btps_launch_count",
 ]
@@ -61,6 +61,8 @@ def _load() -> ctypes.CDLL:
         fn.restype = ci
     lib.ch_step_batched.argtypes = [vp, vp, i64, ctypes.c_double, ci, vp]
     lib.ch_step_batched.restype = ci
+    lib.ch_step_batched_stat.argtypes = [vp, vp, i64, ctypes.c_double, ci, vp, vp]
+    lib.ch_step_batched_stat.restype = ci
     for name in ("tri_solve_batched_host", "penta_solve_batched_host"):
         fn = getattr(lib, name)
         fn.argtypes = [vp, vp, i64, ci]
@@ -239,6 +241,14 @@ def penta_solve_steps(h: PentaHandle, rhs, nsteps: int, stream=None):
 def ch_step_batched(h: PentaHandle, c, alpha: float, nsteps: int = 1, stream=None):
     p, batch = _dev_args(h, c, 8)
     _check(_lib.ch_step_batched(h.ptr, p, batch, float(alpha), int(nsteps), _stream(stream)))
+
+
+def ch_step_batched_stat(h: PentaHandle, c, alpha: float, nsteps: int, lbar, stream=None):
+    """btps.h ch_step_batched_stat: ``lbar`` is a CUDA float64 tensor of nsteps elements (overwritten)."""
+    p, batch = _dev_args(h, c, 8)
+    if not (lbar.is_cuda and lbar.is_contiguous() and lbar.element_size() == 8 and lbar.numel() >= int(nsteps)):
+        raise ValueError("lbar must be a contiguous CUDA float64 tensor with at least nsteps elements")
+    _check(_lib.ch_step_batched_stat(h.ptr, p, batch, float(alpha), int(nsteps), lbar.data_ptr(), _stream(stream)))
 
 
 def _host_args(h: _Handle, x):

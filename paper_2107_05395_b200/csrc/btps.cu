@@ -679,7 +679,7 @@ int make_tmap(CUtensorMap *tm, T *d_rhs, long long batch, int n, int W, unsigned
 // one sweep launch (kind = KIND_TRI / KIND_PENTA / KIND_CH) on a device buffer
 template <typename T>
 int launch_one(Handle *h, int kind, T *d_rhs, long long batch, double alpha_x, int reverse, int ksteps,
-               cudaStream_t st)
+               cudaStream_t st, double *stat = nullptr)
 {
     DtypePlan &pl = h->plan[sizeof(T) == 8 ? 0 : 1];
     // the paper's own 2R+2W form (Alg. 2 / 4), ksteps launches: plans too large for the on-chip tables,
@@ -703,6 +703,11 @@ int launch_one(Handle *h, int kind, T *d_rhs, long long batch, double alpha_x, i
                 two_pass_kernel<T, KIND_CH><<<(unsigned)grid, block, 0, st>>>(co, d_rhs, batch, h->n, alpha_x, 0.0, h->pp);
             g_launches.fetch_add(1, std::memory_order_relaxed);
             CU_TRY(cudaGetLastError());
+            if (stat) {
+                lbar_kernel<T><<<(unsigned)grid, block, 0, st>>>(d_rhs, batch, h->n, stat + l, 1.0 / (double)batch);
+                g_launches.fetch_add(1, std::memory_order_relaxed);
+                CU_TRY(cudaGetLastError());
+            }
         }
         return BTPS_OK;
     };
@@ -777,13 +782,23 @@ int launch_one(Handle *h, int kind, T *d_rhs, long long batch, double alpha_x, i
     if (g_tune.grid > 0 && grid > g_tune.grid) grid = g_tune.grid;
     // several steps per launch need the fused instantiation; without one (direct-load variants)
     // the steps are launched one by one
-    const bool fused = (ksteps > 1) && sl.fused.func;
+    // (the statistic of eq. 30 is computed inside the fused kernels; elsewhere by a pass of its own)
+    const bool fused = (ksteps > 1 || stat) && sl.fused.func;
     const int nlaunch = fused ? 1 : ksteps;
     a.ksteps = fused ? ksteps : 1;
+    a.stat = fused ? stat : nullptr;
+    a.stat_scale = 1.0 / (double)batch;
     for (int l = 0; l < nlaunch; ++l) {
         const cudaError_t e = (fused ? sl.fused : sl.ent).launch(a, tm, (int)grid, sh.threads, sl.smem, st, g_tune.pdl != 0);
         g_launches.fetch_add(1, std::memory_order_relaxed);
         if (e != cudaSuccess) return cuda_fail(e, "sweep launch");
+        if (stat && !fused) {
+            const int block = 128;
+            lbar_kernel<T><<<(unsigned)((batch + block - 1) / block), block, 0, st>>>(d_rhs, batch, h->n, stat + l,
+                                                                                      1.0 / (double)batch);
+            g_launches.fetch_add(1, std::memory_order_relaxed);
+            CU_TRY(cudaGetLastError());
+        }
     }
     return BTPS_OK;
 }
@@ -807,7 +822,7 @@ Handle *check(const void *hv, int magic)
 
 template <typename T>
 int solve_steps(const void *hv, int magic, int kind, T *d_rhs, int64_t batch, double alpha_x, int nsteps,
-                void *stream)
+                void *stream, double *d_stat = nullptr)
 {
     Handle *h = check(hv, magic);
     if (!h || !d_rhs || batch < 1 || nsteps < 0) return set_err(BTPS_E_ARG);
@@ -816,7 +831,8 @@ int solve_steps(const void *hv, int magic, int kind, T *d_rhs, int64_t batch, do
     const int kmax = fuse_limit(h->plan[sizeof(T) == 8 ? 0 : 1]);
     for (int s = 0, l = 0; s < nsteps; ++l) {
         const int k = (nsteps - s < kmax) ? (nsteps - s) : kmax;
-        const int rc = launch_one<T>(h, kind, d_rhs, batch, alpha_x, rev ? (l & 1) : 0, k, (cudaStream_t)stream);
+        const int rc = launch_one<T>(h, kind, d_rhs, batch, alpha_x, rev ? (l & 1) : 0, k, (cudaStream_t)stream,
+                                     d_stat ? d_stat + s : nullptr);
         if (rc != BTPS_OK) return rc;
         s += k;
     }
@@ -1165,6 +1181,17 @@ int penta_solve_steps(penta_handle_t h, double *d_rhs, int64_t batch, int nsteps
 int ch_step_batched(penta_handle_t h, double *d_c, int64_t batch, double alpha, int nsteps, void *stream)
 {
     return solve_steps<double>(h, MAGIC_PENTA, KIND_CH, d_c, batch, alpha, nsteps, stream);
+}
+
+int ch_step_batched_stat(penta_handle_t h, double *d_c, int64_t batch, double alpha, int nsteps, double *d_lbar,
+                         void *stream)
+{
+    if (!d_lbar || nsteps < 0) return set_err(BTPS_E_ARG);
+    if (nsteps > 0) {
+        const cudaError_t e = cudaMemsetAsync(d_lbar, 0, (size_t)nsteps * sizeof(double), (cudaStream_t)stream);
+        if (e != cudaSuccess) return cuda_fail(e, "cudaMemsetAsync");
+    }
+    return solve_steps<double>(h, MAGIC_PENTA, KIND_CH, d_c, batch, alpha, nsteps, stream, d_lbar);
 }
 
 int tri_solve_batched_host(tri_handle_t h, double *h_rhs, int64_t batch, int nsteps)

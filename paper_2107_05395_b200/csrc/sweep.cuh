@@ -56,6 +56,9 @@ struct SweepArgs {
     int wrow_part[4], wrow_k[4];  // periodic penta: partition / local row of rows 0, 1, n-2, n-1
     int xstride;           // elements of exchange area per group
     int xper;              // element offset (inside a group's area) of the 4 x W periodic-penta values
+    double *stat;          // CH, fused kernels: device array, stat[ks] += stat_scale * sum over this launch's runs of
+                           // 1 / (1 - <C^2>) after step ks (eq. 30); nullptr: no statistic
+    double stat_scale;     // 1 / batch
     int n;                 // true number of rows
     int P;                 // partitions per system (rows padded to P*MR with identity rows)
     int lanes;             // threads side by side on adjacent systems (power of two <= 32)
@@ -798,6 +801,42 @@ sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
                 }
             }
         }
+        if constexpr (ISCH && FUSE) {
+            if (a.stat != nullptr) {
+                // ---- eq. 30: l = 1 / (1 - <C^2>) of every run after this step, summed over the tile ------
+                T s2[V];
+#pragma unroll
+                for (int e = 0; e < V; ++e) s2[e] = T(0);
+#pragma unroll
+                for (int k = 0; k < MR; ++k)
+#pragma unroll
+                    for (int e = 0; e < V; ++e) s2[e] = fma_t<T>(v[k][e], v[k][e], s2[e]);  // padding rows are zero
+                double lsum = 0.0;
+                const double invn = 1.0 / (double)a.n;
+                if constexpr (SINGLE) {
+#pragma unroll
+                    for (int e = 0; e < V; ++e)
+                        if (j + e < batch) lsum += 1.0 / (1.0 - (double)s2[e] * invn);
+                } else {
+                    // partial sums of the partitions through exchange value 0 (its carries have been consumed)
+                    const int hx = part & (W - 1);
+#pragma unroll
+                    for (int e = 0; e < V; ++e) xb[part * W + ((sl * V + e) ^ hx)] = s2[e];
+                    group_sync(a.tpc, sub, tpt);
+                    if (part == 0) {
+#pragma unroll
+                        for (int e = 0; e < V; ++e) {
+                            T tot = T(0);
+                            for (int q = 0; q < a.P; ++q) tot += xb[q * W + ((sl * V + e) ^ (q & (W - 1)))];
+                            if (j + e < batch) lsum += 1.0 / (1.0 - (double)tot * invn);
+                        }
+                    }
+                }
+#pragma unroll
+                for (int o = 16; o > 0; o >>= 1) lsum += __shfl_xor_sync(0xffffffffu, lsum, o);
+                if ((threadIdx.x & 31) == 0 && lsum != 0.0) atomicAdd(a.stat + ks, lsum * a.stat_scale);
+            }
+        }
         if constexpr (ISCH && !SINGLE) {
             if (ks + 1 < nks) {  // publish this partition's first / last rows: the neighbours' halo of the next step
                 const int hv = a.P * W, hx = part & (W - 1);
@@ -915,6 +954,27 @@ __global__ void __launch_bounds__(128) two_pass_kernel(const T *__restrict__ co,
             }
         }
     }
+}
+
+// Coarsening statistic from the state in global memory (one extra read pass; used where no fused CH
+// kernel runs: misaligned batches, two-pass plans): stat[0] += scale * sum_j 1 / (1 - mean_i c_ij^2).
+template <typename T>
+__global__ void __launch_bounds__(128) lbar_kernel(const T *__restrict__ c, long long batch, int n, double *stat,
+                                                   double scale)
+{
+    const long long j = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    double l = 0.0;
+    if (j < batch) {
+        T s2 = T(0);
+        for (int i = 0; i < n; ++i) {
+            const T x = c[(long long)i * batch + j];
+            s2 = fma_t<T>(x, x, s2);
+        }
+        l = 1.0 / (1.0 - (double)s2 / (double)n);
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) l += __shfl_xor_sync(0xffffffffu, l, o);
+    if ((threadIdx.x & 31) == 0 && l != 0.0) atomicAdd(stat, l * scale);
 }
 
 // launcher table entry (defined by the instantiation units)

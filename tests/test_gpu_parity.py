@@ -673,3 +673,36 @@ def test_periodic_cahn_hilliard_steps_and_mass(lib, tune, n):
 def test_penta_periodic_errors(lib):
     with pytest.raises(lib.BtpsError):
         lib.penta_factor_periodic(*([[1.0] * 4] * 5))  # n < 5
+
+
+# ---- coarsening statistic (eq. 30) ---------------------------------------------------
+
+@pytest.mark.parametrize("periodic,n,batch,tune", [
+    (True, 256, 4096 + 32, {}), (True, 256, 1001, {}), (True, 200, 2048, {}), (False, 256, 4096, {}),
+    (True, 64, 8192, {}), (True, 256, 2048, dict(force_two_pass=1)), (True, 32, 640, {}),
+])
+def test_coarsening_statistic(lib, periodic, n, batch, tune):
+    steps = 13
+    sigma, alpha = inputs.ch_params(256)
+    st = ([sigma] * n, [-4 * sigma] * n, [1 + 6 * sigma] * n, [-4 * sigma] * n, [sigma] * n)
+    c0 = 0.3 * inputs.uniform_rhs(n, batch, seed=29)
+    try:
+        for k, v in tune.items():
+            lib.btps_tune(k, v)
+        h = lib.penta_factor_periodic(*st) if periodic else lib.penta_factor(*st)
+        d = dev(c0)
+        lbar = torch.full((steps,), -1.0, dtype=torch.float64, device="cuda")
+        lib.ch_step_batched_stat(h, d, alpha, steps, lbar)
+        d_plain = dev(c0)
+        lib.ch_step_batched(h, d_plain, alpha, steps)
+    finally:
+        for k in tune:
+            lib.btps_tune(k, -1)
+    fo = oracle.penta_periodic_factor(*st) if periodic else oracle.penta_factor(*st)
+    ref = c0.copy()
+    ref_l = oracle.ch_steps_with_lbar(fo, ref, alpha, steps, periodic=periodic)
+    assert torch.equal(d, d_plain)                      # recording the statistic does not change the state
+    assert rel_err(d.cpu().numpy(), ref) <= TOL_STEPS
+    got_l = lbar.cpu().numpy()
+    assert np.max(np.abs(got_l - ref_l) / ref_l) <= TOL_STEPS, (got_l, ref_l)
+    assert np.all(got_l > 1.0)
