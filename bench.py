@@ -38,8 +38,8 @@ UNIT = "systems/s"
 L2_BYTES = 126 * 1024 * 1024
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full`
-# capture (profiles/r01b_ncu_full_summary.md), keyed by kernel.
-NCU_TRAFFIC_BYTES = {"tri": 268665088 + 210626560, "penta": 268559616 + 211135488, "ch": 268530688 + 213692416}
+# capture (profiles/r01c_ncu_full_summary.md), keyed by kernel.
+NCU_TRAFFIC_BYTES = {"tri": 268508160 + 209617408, "penta": 268541440 + 210829056, "ch": 268547840 + 209697536}
 
 
 def parse_args():
