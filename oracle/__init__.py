@@ -85,6 +85,13 @@ def _load():
         lib.orc_penta_periodic_interleaved.restype = ctypes.c_int
         lib.orc_lbar_interleaved.argtypes = [ctypes.c_int, _dp, _ll]
         lib.orc_lbar_interleaved.restype = ctypes.c_double
+        lib.orc_tri_explicit.argtypes = [ctypes.c_int, _dp, ctypes.c_double, ctypes.c_double, ctypes.c_double,
+                                         ctypes.c_int, _dp]
+        lib.orc_tri_explicit.restype = None
+        lib.orc_tri_cn_step_interleaved.argtypes = [ctypes.c_int, _dp, _dp, _dp, _dp, ctypes.c_double, ctypes.c_double,
+                                                    ctypes.c_int, ctypes.c_double, ctypes.c_double, ctypes.c_double, _dp,
+                                                    _ll, _ll, _ll, _ll, ctypes.c_int, ctypes.c_int]
+        lib.orc_tri_cn_step_interleaved.restype = ctypes.c_int
         _lib = lib
     return _lib
 
@@ -329,3 +336,25 @@ def ch_steps_with_lbar(fac, c: np.ndarray, alpha: float, nsteps: int, periodic: 
             ch_step_interleaved(fac, c, alpha, nsteps=1)
         out[s] = lbar_interleaved(c)
     return out
+
+
+# ---- Crank-Nicolson diffusion step (eq. 9-11) -----------------------------------------
+
+def tri_explicit(c, xa: float, xb: float, xc: float, periodic: bool) -> np.ndarray:
+    c = _f64(c)
+    f = np.zeros_like(c)
+    _load().orc_tri_explicit(c.size, _p(c), xa, xb, xc, int(periodic), _p(f))
+    return f
+
+
+def tri_cn_step_interleaved(fac, u: np.ndarray, xa: float, xb: float, xc: float, nsteps: int = 1, subset=None,
+                            nthreads: int = 0) -> int:
+    """``fac``: TriFactor (truncated) or TriPeriodicFactor (periodic).  In place on ``u`` (n, M)."""
+    assert u.ndim == 2 and u.shape[0] == fac.n
+    M = u.shape[1]
+    jlo, jhi, js = _subset(M, subset)
+    per = isinstance(fac, TriPeriodicFactor)
+    z = fac.z if per else np.zeros(1)
+    return _load().orc_tri_cn_step_interleaved(fac.n, _p(fac.a), _p(fac.bh), _p(fac.ch), _p(z),
+                                               fac.vN if per else 0.0, fac.den if per else 1.0, int(per), xa, xb, xc,
+                                               _p(u), M, jlo, jhi, js, nsteps, nthreads)

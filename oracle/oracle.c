@@ -469,3 +469,48 @@ ORC_API double orc_lbar_interleaved(int n, const double *c, long long M)
     }
     return acc / (double)M;
 }
+
+/* ------------------------------------------------------------------------------------
+ * Crank-Nicolson diffusion step, PAPER.md:120-136 (eq. 9-11): the right-hand side is the explicit
+ * three-point stencil of the previous state,
+ *     f_i = xa C_{i-1} + xb C_i + xc C_{i+1}      (eq. 9: xa = xc = sigma_x, xb = 1 - 2 sigma_x),
+ * followed by the tridiagonal solve with a = c = -sigma_x, b = 1 + 2 sigma_x (eq. 11).
+ * periodic != 0: indices mod n and the Sherman-Morrison solve of Sec. 3.3 (the paper's setting);
+ * periodic == 0: ghost values zero and the plain Thomas solve (BASELINE.json's truncated reading, C-18).
+ * z / vN / den are only read in the periodic case.
+ * ---------------------------------------------------------------------------------- */
+ORC_API void orc_tri_explicit(int n, const double *c, double xa, double xb, double xc, int periodic, double *f)
+{
+    for (int i = 0; i < n; ++i) {
+        double cm = (i > 0) ? c[i - 1] : (periodic ? c[n - 1] : 0.0);
+        double cp = (i < n - 1) ? c[i + 1] : (periodic ? c[0] : 0.0);
+        f[i] = xa * cm + xb * c[i] + xc * cp;
+    }
+}
+
+ORC_API int orc_tri_cn_step_interleaved(int n, const double *a, const double *bh, const double *ch,
+                                        const double *z, double vN, double den, int periodic, double xa,
+                                        double xb, double xc, double *buf, long long M, long long jlo,
+                                        long long jhi, long long jstride, int nsteps, int nthreads)
+{
+    int used = set_threads(nthreads);
+#pragma omp parallel
+    {
+        double *col = (double *)malloc((size_t)n * sizeof(double));
+        double *f = (double *)malloc((size_t)n * sizeof(double));
+#pragma omp for schedule(static)
+        for (long long j = jlo; j < jhi; j += jstride) {
+            for (int i = 0; i < n; ++i) col[i] = buf[(size_t)i * M + j];
+            for (int s = 0; s < nsteps; ++s) {
+                orc_tri_explicit(n, col, xa, xb, xc, periodic, f);
+                if (periodic) orc_tri_periodic_solve(n, a, bh, ch, z, vN, den, f);
+                else orc_tri_solve(n, a, bh, ch, f);
+                memcpy(col, f, (size_t)n * sizeof(double));
+            }
+            for (int i = 0; i < n; ++i) buf[(size_t)i * M + j] = col[i];
+        }
+        free(col);
+        free(f);
+    }
+    return used;
+}

@@ -108,3 +108,45 @@ def test_bad_inputs():
         oracle.tri_periodic_factor([1.0, 1.0], [2.0, 2.0], [1.0, 1.0])  # n < 3
     with pytest.raises(oracle.FactorError):
         oracle.tri_periodic_factor([1.0] * 4, [0.0, 2.0, 2.0, 2.0], [1.0] * 4)  # b_1 = 0
+
+
+# ---- Crank-Nicolson diffusion step (eq. 9-11) -----------------------------------------
+
+def test_cn_periodic_modal_amplification_and_mass():
+    """Periodic CN: the mode cos(2 pi k j / N) is multiplied per step by
+    (1 - 4 s sin^2(pi k / N)) / (1 + 4 s sin^2(pi k / N)), s = sigma_x (von Neumann factor of eq. 9); the
+    sum over the grid is conserved (column sums of both stencils are 1)."""
+    n, M, s, steps = 64, 5, 0.7, 30
+    j = np.arange(n)
+    u = np.zeros((n, M))
+    ks = [0, 1, 3, 7, 31]
+    for m, k in enumerate(ks):
+        u[:, m] = np.cos(2 * np.pi * k * j / n)
+    u0 = u.copy()
+    f = oracle.tri_periodic_factor([-s] * n, [1 + 2 * s] * n, [-s] * n)
+    oracle.tri_cn_step_interleaved(f, u, s, 1 - 2 * s, s, nsteps=steps)
+    for m, k in enumerate(ks):
+        q = 4 * s * np.sin(np.pi * k / n) ** 2
+        assert np.max(np.abs(u[:, m] - u0[:, m] * ((1 - q) / (1 + q)) ** steps)) <= 1e-13
+    rng = np.random.default_rng(4)
+    w = rng.uniform(-1, 1, (n, 3))
+    w0 = w.copy()
+    oracle.tri_cn_step_interleaved(f, w, s, 1 - 2 * s, s, nsteps=steps)
+    assert np.max(np.abs(w.sum(axis=0) - w0.sum(axis=0))) <= 1e-13
+
+
+@pytest.mark.parametrize("periodic", [False, True])
+def test_cn_step_dense_restatement(periodic):
+    """One step against numpy: (I - s L) u' = (I + s L) u with L the (periodic | truncated) second difference."""
+    n, s = 12, 0.4
+    I = np.eye(n)
+    L = -2 * I + np.diag(np.ones(n - 1), 1) + np.diag(np.ones(n - 1), -1)
+    if periodic:
+        L[0, -1] = L[-1, 0] = 1.0
+    rng = np.random.default_rng(5)
+    u = rng.uniform(-1, 1, (n, 4))
+    ref = np.linalg.solve(I - s * L, (I + s * L) @ u)
+    f = (oracle.tri_periodic_factor if periodic else oracle.tri_factor)([-s] * n, [1 + 2 * s] * n, [-s] * n)
+    assert np.max(np.abs(oracle.tri_explicit(u[:, 0], s, 1 - 2 * s, s, periodic) - ((I + s * L) @ u)[:, 0])) <= 1e-15
+    oracle.tri_cn_step_interleaved(f, u, s, 1 - 2 * s, s)
+    assert np.max(np.abs(u - ref)) <= 1e-14
