@@ -234,6 +234,30 @@ def time_launches(torch, fn_of_buf, bufs, launches, repeats=3):
     return ts[len(ts) // 2]
 
 
+# The paper's own benchmark (Table 1): periodic 1-D diffusion, Crank-Nicolson, 1000 time
+# steps, fp64 assumed (the paper does not state the precision); its numbers are a V100's, for the whole step
+# including a separate stencil pass: context, not a target.
+PAPER_TABLE1_V100_S = {(6, 64): 0.097, (6, 256): 0.161, (6, 1024): 0.510, (12, 64): 0.101, (12, 256): 0.255,
+                       (12, 1024): 1.020, (16, 64): 1.278, (16, 256): 5.015, (16, 1024): 20.268}
+
+
+def paper_table1(torch, b, inputs, sigma=0.5, steps=1000):
+    rows = []
+    for (lb, n), paper_s in sorted(PAPER_TABLE1_V100_S.items()):
+        batch = 1 << lb
+        h = b.tri_factor_periodic([-sigma] * n, [1 + 2 * sigma] * n, [-sigma] * n)
+        u = torch.empty(n, batch, dtype=torch.float64, device="cuda")
+        inputs.fill_uniform_device(u, n, seed=7)
+        fn = lambda t: b.tri_cn_step_batched(h, t, sigma, 1 - 2 * sigma, sigma, steps)
+        fn(u)
+        ms = time_launches(torch, fn, [u], 1)
+        rows.append({"batch": batch, "n": n, "seconds_1000_steps": round(ms * 1e-3, 6),
+                     "paper_v100_seconds": paper_s, "plan": h.cn_plan(8)})
+        del u
+    return {"workload": "periodic Crank-Nicolson diffusion, 1000 steps (tri_cn_step_batched, fused 8 steps per launch)",
+            "note": "paper's numbers: Tesla V100, whole step incl. a separate stencil pass; context only", "rows": rows}
+
+
 def extra_table(torch, b, inputs, peak):
     """Throughput at the other BASELINE.json configs: single launches, cold (rotating over
     buffers whose total exceeds 4x L2 when one buffer would fit in L2)."""
@@ -304,6 +328,7 @@ def extra_table(torch, b, inputs, peak):
     for n in (64, 256, 1024):
         entry("f1 periodic, Table 1 shape (1000 steps per call)", "tri_periodic", n, 65536, 8, steps_per_call=1000,
               launches=1)
+    out.append({"paper_table1": paper_table1(torch, b, inputs)})
     for kind in ("tri", "penta"):
         for elem in (8, 4):
             for n in (64, 256, 1024):

@@ -128,6 +128,17 @@ BTPS_API int tri_solve_steps(tri_handle_t h, double *d_rhs, int64_t batch, int n
 BTPS_API int penta_solve_steps(penta_handle_t h, double *d_rhs, int64_t batch, int nsteps, void *stream);
 
 /* ------------------------------------------------------------------------------------------
+ * Fused Crank-Nicolson diffusion step.  PAPER.md:120-136 (eq. 9-11): per step the right-hand side
+ *   f_i = xa*u[i-1] + xb*u[i] + xc*u[i+1]      (eq. 9: xa = xc = sigma_x, xb = 1 - 2*sigma_x)
+ * is built in registers and the tridiagonal system of `h` (eq. 11: a = c = -sigma_x, b = 1 + 2*sigma_x,
+ * factored by the caller) is solved in the same kernel; nsteps steps, in place, fp64.  With a
+ * tri_factor_periodic handle both the stencil and the solve are periodic (the paper's benchmark of
+ * Table 1); with a tri_factor handle ghost values are zero.  Same conventions as ch_step_batched.
+ * ---------------------------------------------------------------------------------------- */
+BTPS_API int tri_cn_step_batched(tri_handle_t h, double *d_u, int64_t batch, double xa, double xb, double xc,
+                        int nsteps, void *stream);
+
+/* ------------------------------------------------------------------------------------------
  * (a5) Fused semi-implicit Cahn-Hilliard step.  PAPER.md:365-392 (eq. 24, 25a, 26a-c):
  *   (I + sigma*D4) c^{n+1} = c^n + alpha * D2( (c^n)^3 - c^n ),   alpha = dt/dx^2,
  * truncated (non-periodic) stencils, ghost values zero (BASELINE.json config 5; DESIGN.md
@@ -176,7 +187,8 @@ BTPS_API const char *btps_error_string(int code);
  *   out[4] tile groups per CTA, out[5] threads per CTA, out[6] dynamic shared memory bytes,
  *   out[7] coefficient table bytes resident on the device for this plan,
  *   out[8] 1 if aligned batches are prefetched by TMA, out[9] 1 if carries use the warp scan.
- * kind: 0 = tri handle, 1 = penta handle (solve kernels), 2 = penta handle (fused CH step kernels). */
+ * kind: 0 = tri handle, 1 = penta handle (solve kernels), 2 = penta handle (fused CH step kernels),
+ * 3 = tri handle (fused Crank-Nicolson step kernels). */
 BTPS_API int btps_plan_info(int kind, const void *handle, int elem_bytes, int *out);
 
 /* Override the plan chosen at factor time (call BEFORE tri_factor / penta_factor; process

@@ -13,7 +13,7 @@ _LIB_PATH = os.path.join(_HERE, "libbtps.so")
 EXPORTS = [
     "tri_factor", "tri_factor_periodic", "tri_destroy", "penta_factor", "penta_factor_periodic", "penta_destroy",
     "tri_solve_batched", "tri_solve_batched_f32", "penta_solve_batched", "penta_solve_batched_f32",
-    "tri_solve_steps", "penta_solve_steps", "ch_step_batched", "ch_step_batched_stat",
+    "tri_solve_steps", "penta_solve_steps", "ch_step_batched", "ch_step_batched_stat", "tri_cn_step_batched",
     "tri_solve_batched_host", "penta_solve_batched_host", "ch_step_batched_host",
     "btps_last_error", "btps_error_string", "btps_plan_info", "btps_tune", "btps_launch_count",
 ]
@@ -61,6 +61,8 @@ def _load() -> ctypes.CDLL:
         fn.restype = ci
     lib.ch_step_batched.argtypes = [vp, vp, i64, ctypes.c_double, ci, vp]
     lib.ch_step_batched.restype = ci
+    lib.tri_cn_step_batched.argtypes = [vp, vp, i64, ctypes.c_double, ctypes.c_double, ctypes.c_double, ci, vp]
+    lib.tri_cn_step_batched.restype = ci
     lib.ch_step_batched_stat.argtypes = [vp, vp, i64, ctypes.c_double, ci, vp, vp]
     lib.ch_step_batched_stat.restype = ci
     for name in ("tri_solve_batched_host", "penta_solve_batched_host"):
@@ -130,6 +132,10 @@ class _Handle:
 class TriHandle(_Handle):
     _destroy = staticmethod(lambda p: _lib.tri_destroy(p))
     kind = 0
+
+    def cn_plan(self, elem_bytes: int = 8) -> dict:
+        """Plan of the fused Crank-Nicolson step kernels of this handle (btps_plan_info kind 3)."""
+        return btps_plan_info(self, elem_bytes, kind=3)
 
 
 class PentaHandle(_Handle):
@@ -241,6 +247,11 @@ def penta_solve_steps(h: PentaHandle, rhs, nsteps: int, stream=None):
 def ch_step_batched(h: PentaHandle, c, alpha: float, nsteps: int = 1, stream=None):
     p, batch = _dev_args(h, c, 8)
     _check(_lib.ch_step_batched(h.ptr, p, batch, float(alpha), int(nsteps), _stream(stream)))
+
+
+def tri_cn_step_batched(h: TriHandle, u, xa: float, xb: float, xc: float, nsteps: int = 1, stream=None):
+    p, batch = _dev_args(h, u, 8)
+    _check(_lib.tri_cn_step_batched(h.ptr, p, batch, float(xa), float(xb), float(xc), int(nsteps), _stream(stream)))
 
 
 def ch_step_batched_stat(h: PentaHandle, c, alpha: float, nsteps: int, lbar, stream=None):

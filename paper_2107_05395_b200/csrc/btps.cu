@@ -158,9 +158,9 @@ void choose_plan(int n, int elem, int handle_kind, DtypePlan &pl)
     int rows = g_tune.rows > 0 ? g_tune.rows : (n <= 8 ? 8 : (n <= 16 ? 16 : 32));
     if (rows != 8 && rows != 16 && rows != 32) rows = 32;
     int P = (n + rows - 1) / rows;
-    const int nshape = (handle_kind == KIND_TRI) ? 1 : 2;
+    const int nshape = 2;  // [0] solves, [1] fused explicit-half steps (CH for penta handles, Crank-Nicolson for tri)
     for (int k = 0; k < nshape; ++k)
-        choose_shape(k == 0 ? handle_kind : KIND_CH, elem, rows, P, pl.shape[k]);
+        choose_shape(k == 0 ? handle_kind : (handle_kind == KIND_TRI ? KIND_TRICN : KIND_CH), elem, rows, P, pl.shape[k]);
     // the warp scan wants whole warps per group and at most 32 partitions: pad P with identity
     // partitions where that makes every family's group a whole number of warps
     int ws = (P > 1 && P <= 32 && g_tune.warp_scan != 0) ? 1 : 0;
@@ -505,11 +505,14 @@ size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 // shared-memory layout of one kernel variant: [blob][exchange][mbarriers][ring]
 void layout_slot(const DtypePlan &pl, const Shape &sh, int kind, KernelSlot &sl, bool halo = true)
 {
-    const int NC = (kind == KIND_TRI || kind == KIND_TRIP) ? 1 : 2;
-    const bool is_ch = (kind == KIND_CH || kind == KIND_CHP), wood = (kind == KIND_PENTAP || kind == KIND_CHP);
+    const bool tri = (kind == KIND_TRI || kind == KIND_TRIP || kind == KIND_TRICN || kind == KIND_TRICNP);
+    const int NC = tri ? 1 : 2;
+    // kinds with an explicit half need one halo row on each side between fused steps
+    const bool is_ch = (kind == KIND_CH || kind == KIND_CHP || kind == KIND_TRICN || kind == KIND_TRICNP);
+    const bool wood = (kind == KIND_PENTAP || kind == KIND_CHP), pert = (kind == KIND_TRIP || kind == KIND_TRICNP);
     const size_t W = (size_t)sh.lanes * sl.vec;
     // CH: + the halo rows exchanged between fused steps; periodic tri: + y_1 and y_N of eq. 15
-    sl.xvals = 2 * NC + ((is_ch && halo) ? 2 : 0) + (kind == KIND_TRIP ? 2 : 0);
+    sl.xvals = 2 * NC + ((is_ch && halo) ? 2 : 0) + (pert ? 2 : 0);
     sl.xper = (int)(sl.xvals * pl.P * W);
     sl.xstride = sl.xper + (wood ? (int)(4 * W) : 0);  // cyclic penta: y at rows 0, 1, n-2, n-1
     const size_t xch = (pl.P > 1) ? (size_t)sh.tpc * sl.xstride * pl.elem : 0;
@@ -542,6 +545,8 @@ SweepEntry find_sweep(int kind, int elem_bytes, int vec, int rows, int single, i
         if (kind == KIND_TRIP) return find_sweep_trip_f64(vec, rows, single, tma, ws, fuse);
         if (kind == KIND_PENTAP) return find_sweep_pentap_f64(vec, rows, single, tma, ws, fuse);
         if (kind == KIND_CHP) return find_sweep_chp_f64(vec, rows, single, tma, ws, fuse);
+        if (kind == KIND_TRICN) return find_sweep_tricn_f64(vec, rows, single, tma, ws, fuse);
+        if (kind == KIND_TRICNP) return find_sweep_tricnp_f64(vec, rows, single, tma, ws, fuse);
         if (kind == KIND_PENTA) return find_sweep_penta_f64(vec, rows, single, tma, ws, fuse);
         return find_sweep_ch_f64(vec, rows, single, tma, ws, fuse);
     }
@@ -549,6 +554,7 @@ SweepEntry find_sweep(int kind, int elem_bytes, int vec, int rows, int single, i
     if (kind == KIND_TRIP) return find_sweep_trip_f32(vec, rows, single, tma, ws, fuse);
     if (kind == KIND_PENTAP) return find_sweep_pentap_f32(vec, rows, single, tma, ws, fuse);
     if (kind == KIND_CHP) return find_sweep_chp_f32(vec, rows, single, tma, ws, fuse);
+    if (kind == KIND_TRICN || kind == KIND_TRICNP) return SweepEntry{nullptr, nullptr, 0};  // fp64 only
     if (kind == KIND_PENTA) return find_sweep_penta_f32(vec, rows, single, tma, ws, fuse);
     return find_sweep_ch_f32(vec, rows, single, tma, ws, fuse);
 }
@@ -556,7 +562,7 @@ SweepEntry find_sweep(int kind, int elem_bytes, int vec, int rows, int single, i
 void fit_plan(DtypePlan &pl, int handle_kind)
 {
     if (pl.two_pass) return;
-    for (int k = 0; k < (handle_kind == KIND_TRI ? 1 : 2); ++k) {
+    for (int k = 0; k < 2; ++k) {
         KernelSlot probe;
         probe.vec = 1;
         probe.tma = 0;
@@ -574,13 +580,15 @@ void fill_slots(Handle *h)
         for (int ks = 0; ks < 2; ++ks) {
             int kind;
             if (h->kind == KIND_TRI) {
-                if (ks == 1) continue;
-                kind = h->periodic ? KIND_TRIP : KIND_TRI;
+                kind = (ks == 0) ? (h->periodic ? KIND_TRIP : KIND_TRI) : (h->periodic ? KIND_TRICNP : KIND_TRICN);
+                if (ks == 1 && pl.elem != 8) continue;  // the Crank-Nicolson step is fp64 only
+                // periodic explicit halves need whole partitions and at least two of them (halo wrap)
+                if (kind == KIND_TRICNP && (pl.P < 2 || pl.P * pl.rows != h->n)) continue;
             } else {
                 kind = (ks == 0) ? (h->periodic ? KIND_PENTAP : KIND_PENTA) : (h->periodic ? KIND_CHP : KIND_CH);
                 // the periodic CH kernels need whole partitions and at least two of them (halo wrap);
                 // other sizes run the two-pass form
-                if (kind == KIND_CHP && (h->n % pl.rows != 0 || pl.P < 2 || pl.P * pl.rows != h->n)) continue;
+                if (kind == KIND_CHP && (pl.P < 2 || pl.P * pl.rows != h->n)) continue;
             }
             const Shape &sh = pl.shape[ks];
             for (int s = 0; s < 2; ++s) {
@@ -593,7 +601,7 @@ void fill_slots(Handle *h)
                     if (sl.tma && !tma_possible(pl, sh, sl.vec)) continue;
                     layout_slot(pl, sh, kind, sl);
                     bool can_fuse = true;
-                    if (sl.smem > SMEM_LIMIT && (kind == KIND_CH || kind == KIND_CHP)) {
+                    if (sl.smem > SMEM_LIMIT && (kind == KIND_CH || kind == KIND_CHP || kind == KIND_TRICN || kind == KIND_TRICNP)) {
                         // tight fit (N = 1024 fp64): drop the halo exchange rows, one step per launch
                         layout_slot(pl, sh, kind, sl, false);
                         can_fuse = false;
@@ -679,7 +687,7 @@ int make_tmap(CUtensorMap *tm, T *d_rhs, long long batch, int n, int W, unsigned
 // one sweep launch (kind = KIND_TRI / KIND_PENTA / KIND_CH) on a device buffer
 template <typename T>
 int launch_one(Handle *h, int kind, T *d_rhs, long long batch, double alpha_x, int reverse, int ksteps,
-               cudaStream_t st, double *stat = nullptr)
+               cudaStream_t st, double *stat = nullptr, const double *ex = nullptr)
 {
     DtypePlan &pl = h->plan[sizeof(T) == 8 ? 0 : 1];
     // the paper's own 2R+2W form (Alg. 2 / 4), ksteps launches: plans too large for the on-chip tables,
@@ -688,11 +696,17 @@ int launch_one(Handle *h, int kind, T *d_rhs, long long batch, double alpha_x, i
         const int block = 128;
         const long long grid = (batch + block - 1) / block;
         const T *co = (const T *)pl.d_soa;
+        PerPenta ppx = h->pp;
+        for (int i = 0; i < 3; ++i) ppx.ex[i] = ex ? ex[i] : 0.0;
         for (int l = 0; l < ksteps; ++l) {
             if (kind == KIND_TRI && h->periodic)
                 two_pass_kernel<T, KIND_TRIP><<<(unsigned)grid, block, 0, st>>>(co, d_rhs, batch, h->n, h->per_vN, h->per_invden, h->pp);
             else if (kind == KIND_TRI)
                 two_pass_kernel<T, KIND_TRI><<<(unsigned)grid, block, 0, st>>>(co, d_rhs, batch, h->n, 0.0, 0.0, h->pp);
+            else if (kind == KIND_TRICN && h->periodic)
+                two_pass_kernel<T, KIND_TRICNP><<<(unsigned)grid, block, 0, st>>>(co, d_rhs, batch, h->n, h->per_vN, h->per_invden, ppx);
+            else if (kind == KIND_TRICN)
+                two_pass_kernel<T, KIND_TRICN><<<(unsigned)grid, block, 0, st>>>(co, d_rhs, batch, h->n, 0.0, 0.0, ppx);
             else if (kind == KIND_PENTA && h->periodic)
                 two_pass_kernel<T, KIND_PENTAP><<<(unsigned)grid, block, 0, st>>>(co, d_rhs, batch, h->n, 0.0, 0.0, h->pp);
             else if (kind == KIND_PENTA)
@@ -712,7 +726,7 @@ int launch_one(Handle *h, int kind, T *d_rhs, long long batch, double alpha_x, i
         return BTPS_OK;
     };
     if (pl.two_pass) return two_pass();
-    const int ks = (kind == KIND_CH) ? 1 : 0;
+    const int ks = (kind == KIND_CH || kind == KIND_TRICN) ? 1 : 0;
     const Shape &sh = pl.shape[ks];
     // the vectorised kernels need whole vectors: batch % vec == 0 and an aligned base pointer;
     // TMA needs a 16-byte aligned base and row pitch
@@ -743,6 +757,7 @@ int launch_one(Handle *h, int kind, T *d_rhs, long long batch, double alpha_x, i
     a.per_invden = h->per_invden;
     a.last_part = (h->n - 1) / pl.rows;
     a.last_k = (h->n - 1) % pl.rows;
+    for (int i = 0; i < 3; ++i) a.ex[i] = ex ? ex[i] : 0.0;
     for (int i = 0; i < 16; ++i) a.per_H[i] = h->pp.H[i];
     for (int i = 0; i < 6; ++i) a.per_w6[i] = h->pp.w6[i];
     {
@@ -822,7 +837,7 @@ Handle *check(const void *hv, int magic)
 
 template <typename T>
 int solve_steps(const void *hv, int magic, int kind, T *d_rhs, int64_t batch, double alpha_x, int nsteps,
-                void *stream, double *d_stat = nullptr)
+                void *stream, double *d_stat = nullptr, const double *ex = nullptr)
 {
     Handle *h = check(hv, magic);
     if (!h || !d_rhs || batch < 1 || nsteps < 0) return set_err(BTPS_E_ARG);
@@ -832,7 +847,7 @@ int solve_steps(const void *hv, int magic, int kind, T *d_rhs, int64_t batch, do
     for (int s = 0, l = 0; s < nsteps; ++l) {
         const int k = (nsteps - s < kmax) ? (nsteps - s) : kmax;
         const int rc = launch_one<T>(h, kind, d_rhs, batch, alpha_x, rev ? (l & 1) : 0, k, (cudaStream_t)stream,
-                                     d_stat ? d_stat + s : nullptr);
+                                     d_stat ? d_stat + s : nullptr, ex);
         if (rc != BTPS_OK) return rc;
         s += k;
     }
@@ -1183,6 +1198,13 @@ int ch_step_batched(penta_handle_t h, double *d_c, int64_t batch, double alpha, 
     return solve_steps<double>(h, MAGIC_PENTA, KIND_CH, d_c, batch, alpha, nsteps, stream);
 }
 
+int tri_cn_step_batched(tri_handle_t h, double *d_u, int64_t batch, double xa, double xb, double xc, int nsteps,
+                        void *stream)
+{
+    const double ex[3] = {xa, xb, xc};
+    return solve_steps<double>(h, MAGIC_TRI, KIND_TRICN, d_u, batch, 0.0, nsteps, stream, nullptr, ex);
+}
+
 int ch_step_batched_stat(penta_handle_t h, double *d_c, int64_t batch, double alpha, int nsteps, double *d_lbar,
                          void *stream)
 {
@@ -1227,10 +1249,11 @@ const char *btps_error_string(int code)
 
 int btps_plan_info(int kind, const void *handle, int elem_bytes, int *out)
 {
-    Handle *h = check(handle, kind == 0 ? MAGIC_TRI : MAGIC_PENTA);
-    if (!h || !out || (elem_bytes != 8 && elem_bytes != 4) || kind < 0 || kind > 2) return set_err(BTPS_E_ARG);
+    if (kind < 0 || kind > 3) return set_err(BTPS_E_ARG);
+    Handle *h = check(handle, (kind == 0 || kind == 3) ? MAGIC_TRI : MAGIC_PENTA);
+    if (!h || !out || (elem_bytes != 8 && elem_bytes != 4)) return set_err(BTPS_E_ARG);
     const DtypePlan &pl = h->plan[elem_bytes == 8 ? 0 : 1];
-    const int ks = (kind == 2) ? 1 : 0;
+    const int ks = (kind >= 2) ? 1 : 0;
     const Shape &sh = pl.shape[ks];
     const KernelSlot &sl = pl.k[ks][0][0].ent.func ? pl.k[ks][0][0] : pl.k[ks][0][1];
     out[0] = pl.two_pass ? 0 : pl.rows;

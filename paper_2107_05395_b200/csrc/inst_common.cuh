@@ -80,5 +80,7 @@ SweepEntry find_sweep_pentap_f64(int vec, int rows, int single, int tma, int ws,
 SweepEntry find_sweep_pentap_f32(int vec, int rows, int single, int tma, int ws, int fuse);
 SweepEntry find_sweep_chp_f64(int vec, int rows, int single, int tma, int ws, int fuse);
 SweepEntry find_sweep_chp_f32(int vec, int rows, int single, int tma, int ws, int fuse);
+SweepEntry find_sweep_tricn_f64(int vec, int rows, int single, int tma, int ws, int fuse);
+SweepEntry find_sweep_tricnp_f64(int vec, int rows, int single, int tma, int ws, int fuse);
 
 }  // namespace btps

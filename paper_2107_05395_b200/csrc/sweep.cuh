@@ -37,7 +37,10 @@
 namespace btps {
 
 // TRIP / PENTAP / CHP: the periodic (cyclic) forms of TRI / PENTA / CH
-enum Kind { KIND_TRI = 0, KIND_PENTA = 1, KIND_CH = 2, KIND_TRIP = 3, KIND_PENTAP = 4, KIND_CHP = 5 };
+// TRICN / TRICNP: Crank-Nicolson step (explicit three-point half + tri solve), truncated / periodic
+enum Kind {
+    KIND_TRI = 0, KIND_PENTA = 1, KIND_CH = 2, KIND_TRIP = 3, KIND_PENTAP = 4, KIND_CHP = 5, KIND_TRICN = 6, KIND_TRICNP = 7
+};
 
 constexpr int SCAN_STEPS = 5;   // Kogge-Stone steps held in the tables (scan width <= 32)
 constexpr int SCAN_LANES = 32;
@@ -51,6 +54,7 @@ struct SweepArgs {
     double per_vN;         // periodic tri: last entry of v, eq. 13a (-a_1/b_1)
     double per_invden;     // periodic tri: 1 / (1 + v.z), eq. 15
     int last_part, last_k; // periodic tri: partition and local row of row n-1
+    double ex[3];          // Crank-Nicolson step: explicit stencil xa, xb, xc (eq. 9)
     double per_H[16];      // periodic penta: (I + V^T Z)^{-1}, row-major (Woodbury)
     double per_w6[6];      // periodic penta: wrap-around entries e_0, a_0, e_1, f_{n-2}, c_{n-1}, f_{n-1}
     int wrow_part[4], wrow_k[4];  // periodic penta: partition / local row of rows 0, 1, n-2, n-1
@@ -144,9 +148,10 @@ __device__ __forceinline__ T ch_w(T c) { return fma_t<T>(c * c, c, -c); }
 // from the row arrays).
 template <int KIND>
 struct RecLayout {
-    static constexpr bool TRI = (KIND == KIND_TRI || KIND == KIND_TRIP);
+    static constexpr bool TRI = (KIND == KIND_TRI || KIND == KIND_TRIP || KIND == KIND_TRICN || KIND == KIND_TRICNP);
+    static constexpr bool PERT = (KIND == KIND_TRIP || KIND == KIND_TRICNP);  // Sherman-Morrison finish
     static constexpr bool WOOD = (KIND == KIND_PENTAP || KIND == KIND_CHP);  // rank-4 Woodbury correction
-    static constexpr int ELEMS = (KIND == KIND_TRI) ? 5 : (KIND == KIND_TRIP ? 6 : (WOOD ? 13 : 9));  // values per row
+    static constexpr int ELEMS = TRI ? (PERT ? 6 : 5) : (WOOD ? 13 : 9);  // values per row
     static constexpr int NC = TRI ? 1 : 2;                     // carries per direction
 };
 
@@ -235,7 +240,10 @@ sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
 {
     constexpr bool TRI = RecLayout<KIND>::TRI;
     constexpr bool ISCH = (KIND == KIND_CH || KIND == KIND_CHP);  // explicit Cahn-Hilliard half fused in
-    constexpr bool WRAP = (KIND == KIND_CHP);                     // ... with periodic differences
+    constexpr bool ISCN = (KIND == KIND_TRICN || KIND == KIND_TRICNP);  // explicit three-point half (eq. 9) fused in
+    constexpr bool HALO1 = ISCH || ISCN;                          // needs the rows r0-1 and r0+MR
+    constexpr bool WRAP = (KIND == KIND_CHP || KIND == KIND_TRICNP);  // ... with periodic differences
+    constexpr bool PERT = RecLayout<KIND>::PERT;
     constexpr bool WOOD = RecLayout<KIND>::WOOD;
     constexpr int NC = RecLayout<KIND>::NC;
     using Pair = Tup<T, 2>;
@@ -327,7 +335,7 @@ sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
             asm volatile("" : "+l"(rp));  // recompute the MR row addresses per tile: hoisted out of the loop they spill
 #pragma unroll
             for (int k = 0; k < MR; ++k) ld_sys<T, V>(v[k], rp + k * W);
-            if constexpr (ISCH) {
+            if constexpr (HALO1) {
 #pragma unroll
                 for (int e = 0; e < V; ++e) cm[e] = cp[e] = T(0);
                 if constexpr (!SINGLE) {
@@ -354,7 +362,7 @@ sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
                 }
                 pl += batch;
             }
-            if constexpr (ISCH) {
+            if constexpr (HALO1) {
                 // halo rows come from the neighbouring partitions' rows in global memory (still
                 // c^n: nobody stores before the barriers below).
 #pragma unroll
@@ -369,7 +377,7 @@ sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
         // ---- ksteps time steps on the tile while it is on chip (RHS = previous solution) ----
         const int nks = FUSE ? a.ksteps : 1;
         for (int ks = 0; ks < nks; ++ks) {
-        if constexpr (ISCH && !SINGLE) {
+        if constexpr (HALO1 && !SINGLE) {
             if (ks > 0) {
                 // halo rows of c^{n+ks}: the neighbouring partitions' first / last rows, published to
                 // exchange values 2NC (first row) and 2NC+1 (last row) at the end of the previous step
@@ -390,6 +398,24 @@ sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
             T gp[V];
 #pragma unroll
             for (int e = 0; e < V; ++e) gp[e] = T(0);
+            if constexpr (ISCN) {
+                // explicit half of Crank-Nicolson (eq. 9): f_k = xa c_{k-1} + xb c_k + xc c_{k+1}, in registers
+                const T xa = (T)a.ex[0], xb = (T)a.ex[1], xc = (T)a.ex[2];
+                T cprev[V];
+#pragma unroll
+                for (int e = 0; e < V; ++e) cprev[e] = cm[e];
+#pragma unroll
+                for (int k = 0; k < MR; ++k) {
+                    const bool row_ok = (k < nrow_part);
+#pragma unroll
+                    for (int e = 0; e < V; ++e) {
+                        const T cn = (k + 1 < MR) ? v[(k + 1 < MR) ? k + 1 : k][e] : cp[e];
+                        const T f = fma_t<T>(xa, cprev[e], fma_t<T>(xc, cn, xb * v[k][e]));
+                        cprev[e] = v[k][e];
+                        v[k][e] = row_ok ? f : T(0);  // padding rows stay identity rows with zero RHS
+                    }
+                }
+            }
 #pragma unroll
             for (int k = 0; k < MR; ++k) {
                 const Pair cf = RA[k];
@@ -706,7 +732,7 @@ sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
             }
 #undef XI
         }
-        if constexpr (KIND == KIND_TRIP) {
+        if constexpr (PERT) {
             // ---- eq. 15: x = y - (v.y)/(1 + v.z) z,  v.y = y_1 + v_N y_N ------------------------------
             T y0[V], yN[V];
 #pragma unroll
@@ -719,7 +745,7 @@ sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
                 }
             if constexpr (!SINGLE) {
                 // y_1 lives in partition 0, y_N in partition last_part: two more exchange planes
-                T *const pz = xb + (size_t)2 * NC * a.P * W + sl * V;
+                T *const pz = xb + (size_t)(2 * NC + (HALO1 ? 2 : 0)) * a.P * W + sl * V;
                 if (part == 0) {
 #pragma unroll
                     for (int e = 0; e < V; ++e) pz[e] = y0[e];
@@ -837,7 +863,7 @@ sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
                 if ((threadIdx.x & 31) == 0 && lsum != 0.0) atomicAdd(a.stat + ks, lsum * a.stat_scale);
             }
         }
-        if constexpr (ISCH && !SINGLE) {
+        if constexpr (HALO1 && !SINGLE) {
             if (ks + 1 < nks) {  // publish this partition's first / last rows: the neighbours' halo of the next step
                 const int hv = a.P * W, hx = part & (W - 1);
 #pragma unroll
@@ -870,7 +896,8 @@ sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
 //   tri   : co[0..n) inv, co[n..2n) nl, co[2n..3n) nch
 //   penta : inv, nle, nlb, ngam, ndel
 // -----------------------------------------------------------------------------------------------
-struct PerPenta {  // scalars of the cyclic pentadiagonal (Woodbury) correction
+struct PerPenta {  // scalars of the cyclic pentadiagonal (Woodbury) correction and of the CN explicit half
+    double ex[3];  // Crank-Nicolson: explicit stencil xa, xb, xc
     double H[16];  // (I + V^T Z)^{-1}, row-major
     double w6[6];  // wrap-around entries e_0, a_0, e_1, f_{n-2}, c_{n-1}, f_{n-1}
 };
@@ -882,19 +909,35 @@ __global__ void __launch_bounds__(128) two_pass_kernel(const T *__restrict__ co,
     const long long j = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (j >= batch) return;
     T *p = rhs + j;
-    if constexpr (KIND == KIND_TRI || KIND == KIND_TRIP) {
+    if constexpr (RecLayout<KIND>::TRI) {
         const T *inv = co, *nl = co + n, *nch = co + 2 * (size_t)n;
         T g = T(0);
-        for (int i = 0; i < n; ++i) {
-            g = fma_t<T>(__ldg(nl + i), g, __ldg(inv + i) * p[(long long)i * batch]);
-            p[(long long)i * batch] = g;
+        if constexpr (KIND == KIND_TRICN || KIND == KIND_TRICNP) {
+            // Crank-Nicolson step: explicit three-point half (eq. 9) formed on the fly (row i+1 is still c^n)
+            constexpr bool WRAPS = (KIND == KIND_TRICNP);
+            const T xa = (T)pp.ex[0], xb = (T)pp.ex[1], xc = (T)pp.ex[2];
+            const T c_first = p[0];
+            T cprev = WRAPS ? p[(long long)(n - 1) * batch] : T(0), cc = c_first;
+            for (int i = 0; i < n; ++i) {
+                const T cn = (i + 1 < n) ? p[(long long)(i + 1) * batch] : (WRAPS ? c_first : T(0));
+                const T f = fma_t<T>(xa, cprev, fma_t<T>(xc, cn, xb * cc));
+                g = fma_t<T>(__ldg(nl + i), g, __ldg(inv + i) * f);
+                p[(long long)i * batch] = g;
+                cprev = cc;
+                cc = cn;
+            }
+        } else {
+            for (int i = 0; i < n; ++i) {
+                g = fma_t<T>(__ldg(nl + i), g, __ldg(inv + i) * p[(long long)i * batch]);
+                p[(long long)i * batch] = g;
+            }
         }
         T x = g;
         for (int i = n - 2; i >= 0; --i) {
             x = fma_t<T>(__ldg(nch + i), x, p[(long long)i * batch]);
             p[(long long)i * batch] = x;
         }
-        if constexpr (KIND == KIND_TRIP) {
+        if constexpr (RecLayout<KIND>::PERT) {
             // eq. 15: alpha_x carries v_N, alpha_y 1/(1 + v.z); z follows nch in co
             const T *z = co + 3 * (size_t)n;
             const T nfac = -(fma_t<T>((T)alpha_x, g, x) * (T)alpha_y);  // x = y_1, g = y_N here

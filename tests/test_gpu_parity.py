@@ -706,3 +706,35 @@ def test_coarsening_statistic(lib, periodic, n, batch, tune):
     got_l = lbar.cpu().numpy()
     assert np.max(np.abs(got_l - ref_l) / ref_l) <= TOL_STEPS, (got_l, ref_l)
     assert np.all(got_l > 1.0)
+
+
+# ---- fused Crank-Nicolson diffusion step (eq. 9-11) -----------------------------------
+
+@pytest.mark.parametrize("periodic", [True, False])
+@pytest.mark.parametrize("n,batch", [(64, 4096 + 64), (256, 2048), (200, 1001), (512, 1024), (1024, 512), (20, 333), (1500, 256)])
+def test_tri_cn_step(lib, periodic, n, batch):
+    """The paper's diffusion benchmark scheme: explicit three-point half fused with the (periodic) solve;
+    11 steps against the oracle, sum conservation and the von Neumann factor in the periodic case."""
+    s, steps = 0.7, 11
+    lhs = ([-s] * n, [1 + 2 * s] * n, [-s] * n)
+    u0 = inputs.uniform_rhs(n, batch, seed=41)
+    u0[:, 0] = np.cos(2 * np.pi * 2 * np.arange(n) / n)
+    h = (lib.tri_factor_periodic if periodic else lib.tri_factor)(*lhs)
+    fo = (oracle.tri_periodic_factor if periodic else oracle.tri_factor)(*lhs)
+    ref = u0.copy()
+    oracle.tri_cn_step_interleaved(fo, ref, s, 1 - 2 * s, s, nsteps=steps)
+    outs = []
+    for fuse in (-1, 1):
+        try:
+            lib.btps_tune("fuse_steps", fuse)
+            d = dev(u0)
+            lib.tri_cn_step_batched(h, d, s, 1 - 2 * s, s, steps)
+        finally:
+            lib.btps_tune("fuse_steps", -1)
+        outs.append(d.cpu().numpy())
+    assert np.array_equal(outs[0], outs[1])
+    assert rel_err(outs[0], ref) <= TOL_STEPS, (n, batch, h.cn_plan())
+    if periodic:
+        assert np.max(np.abs(outs[0].sum(axis=0) - u0.sum(axis=0))) <= 1e-11
+        q = 4 * s * np.sin(np.pi * 2 / n) ** 2
+        assert np.max(np.abs(outs[0][:, 0] - u0[:, 0] * ((1 - q) / (1 + q)) ** steps)) <= 1e-12
