@@ -738,3 +738,30 @@ def test_tri_cn_step(lib, periodic, n, batch):
         assert np.max(np.abs(outs[0].sum(axis=0) - u0.sum(axis=0))) <= 1e-11
         q = 4 * s * np.sin(np.pi * 2 / n) ** 2
         assert np.max(np.abs(outs[0][:, 0] - u0[:, 0] * ((1 - q) / (1 + q)) ** steps)) <= 1e-12
+
+
+# ---- run-to-run determinism (a shared-memory race or a missing barrier would show up as a bitwise difference) --
+
+@pytest.mark.parametrize("n,batch", [(512, 8192), (1024, 4096), (64, 32768), (300, 5000)])
+def test_repeated_launches_are_bitwise_identical(lib, n, batch):
+    s = 0.5
+    sg, al = inputs.ch_params(256)
+    st = ([sg] * n, [-4 * sg] * n, [1 + 6 * sg] * n, [-4 * sg] * n, [sg] * n)
+    tl = ([-s] * n, [1 + 2 * s] * n, [-s] * n)
+    u = torch.from_numpy(inputs.uniform_rhs(n, batch, seed=77)).cuda()
+    cases = []
+    for h in (lib.tri_factor(*tl), lib.tri_factor_periodic(*tl)):
+        cases += [lambda x, h=h: lib.tri_solve_batched(h, x), lambda x, h=h: lib.tri_solve_steps(h, x, 9),
+                  lambda x, h=h: lib.tri_cn_step_batched(h, x, s, 1 - 2 * s, s, 9)]
+    for h in (lib.penta_factor(*st), lib.penta_factor_periodic(*st)):
+        cases += [lambda x, h=h: lib.penta_solve_batched(h, x), lambda x, h=h: lib.penta_solve_steps(h, x, 9),
+                  lambda x, h=h: lib.ch_step_batched(h, x, al, 9)]
+    for i, fn in enumerate(cases):
+        first = None
+        for rep in range(12):
+            x = (0.1 * u).clone()
+            fn(x)
+            if first is None:
+                first = x
+            else:
+                assert torch.equal(x, first), (i, rep, n, batch)
