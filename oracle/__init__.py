@@ -92,6 +92,11 @@ def _load():
                                                     ctypes.c_int, ctypes.c_double, ctypes.c_double, ctypes.c_double, _dp,
                                                     _ll, _ll, _ll, _ll, ctypes.c_int, ctypes.c_int]
         lib.orc_tri_cn_step_interleaved.restype = ctypes.c_int
+        lib.orc_penta_explicit.argtypes = [ctypes.c_int, _dp, _dp, ctypes.c_int, _dp]
+        lib.orc_penta_explicit.restype = None
+        lib.orc_penta_cn_step_interleaved.argtypes = [ctypes.c_int] + [_dp] * 8 + [ctypes.c_int, _dp, _dp, _ll, _ll, _ll,
+                                                                                   _ll, ctypes.c_int, ctypes.c_int]
+        lib.orc_penta_cn_step_interleaved.restype = ctypes.c_int
         _lib = lib
     return _lib
 
@@ -358,3 +363,29 @@ def tri_cn_step_interleaved(fac, u: np.ndarray, xa: float, xb: float, xc: float,
     return _load().orc_tri_cn_step_interleaved(fac.n, _p(fac.a), _p(fac.bh), _p(fac.ch), _p(z),
                                                fac.vN if per else 0.0, fac.den if per else 1.0, int(per), xa, xb, xc,
                                                _p(u), M, jlo, jhi, js, nsteps, nthreads)
+
+
+# ---- Crank-Nicolson hyperdiffusion step (eq. 17-19) -----------------------------------
+
+def penta_explicit(c, x5, periodic: bool) -> np.ndarray:
+    c, x5 = _f64(c), _f64(x5)
+    assert x5.size == 5
+    f = np.zeros_like(c)
+    _load().orc_penta_explicit(c.size, _p(c), _p(x5), int(periodic), _p(f))
+    return f
+
+
+def penta_cn_step_interleaved(fac, u: np.ndarray, x5, nsteps: int = 1, subset=None, nthreads: int = 0) -> int:
+    """``fac``: PentaFactor (truncated) or PentaPeriodicFactor (periodic).  In place on ``u`` (n, M)."""
+    assert u.ndim == 2 and u.shape[0] == fac.n
+    x5 = _f64(x5)
+    assert x5.size == 5
+    M = u.shape[1]
+    jlo, jhi, js = _subset(M, subset)
+    per = isinstance(fac, PentaPeriodicFactor)
+    Z = fac.Z if per else np.zeros(4)
+    H = fac.H if per else np.zeros(16)
+    w6 = fac.w6 if per else np.zeros(6)
+    return _load().orc_penta_cn_step_interleaved(fac.n, _p(fac.eps), _p(fac.beta), _p(fac.alpha), _p(fac.gamma),
+                                                 _p(fac.delta), _p(Z), _p(H), _p(w6), int(per), _p(x5), _p(u), M,
+                                                 jlo, jhi, js, nsteps, nthreads)

@@ -514,3 +514,53 @@ ORC_API int orc_tri_cn_step_interleaved(int n, const double *a, const double *bh
     }
     return used;
 }
+
+/* ------------------------------------------------------------------------------------
+ * Crank-Nicolson hyperdiffusion step, PAPER.md:284-296 (eq. 17-19): explicit five-point half
+ *     f_i = x0 C_{i-2} + x1 C_{i-1} + x2 C_i + x3 C_{i+1} + x4 C_{i+2}
+ * (eq. 18: x = (-s, 4s, 1 - 6s, 4s, -s), s = sigma_x) followed by the pentadiagonal solve with
+ * (s, -4s, 1 + 6s, -4s, s).  periodic != 0: indices mod n and the cyclic solve (Z, H, w6 as returned by
+ * orc_penta_periodic_factor); periodic == 0: ghost values zero and the plain solve [C-18].
+ * ---------------------------------------------------------------------------------- */
+ORC_API void orc_penta_explicit(int n, const double *c, const double *x5, int periodic, double *f)
+{
+    for (int i = 0; i < n; ++i) {
+        double acc = 0.0;
+        for (int o = -2; o <= 2; ++o) {
+            int j = i + o;
+            double v;
+            if (j >= 0 && j < n) v = c[j];
+            else v = periodic ? c[(j + n) % n] : 0.0;
+            acc += x5[o + 2] * v;
+        }
+        f[i] = acc;
+    }
+}
+
+ORC_API int orc_penta_cn_step_interleaved(int n, const double *eps, const double *beta, const double *alpha,
+                                          const double *gamma, const double *delta, const double *Z,
+                                          const double *H, const double *w6, int periodic, const double *x5,
+                                          double *buf, long long M, long long jlo, long long jhi,
+                                          long long jstride, int nsteps, int nthreads)
+{
+    int used = set_threads(nthreads);
+#pragma omp parallel
+    {
+        double *col = (double *)malloc((size_t)n * sizeof(double));
+        double *f = (double *)malloc((size_t)n * sizeof(double));
+#pragma omp for schedule(static)
+        for (long long j = jlo; j < jhi; j += jstride) {
+            for (int i = 0; i < n; ++i) col[i] = buf[(size_t)i * M + j];
+            for (int s = 0; s < nsteps; ++s) {
+                orc_penta_explicit(n, col, x5, periodic, f);
+                if (periodic) orc_penta_periodic_solve(n, eps, beta, alpha, gamma, delta, Z, H, w6, f);
+                else orc_penta_solve(n, eps, beta, alpha, gamma, delta, f);
+                memcpy(col, f, (size_t)n * sizeof(double));
+            }
+            for (int i = 0; i < n; ++i) buf[(size_t)i * M + j] = col[i];
+        }
+        free(col);
+        free(f);
+    }
+    return used;
+}

@@ -100,3 +100,51 @@ def test_periodic_ch_conserves_mass_and_matches_dense_model():
 def test_bad_inputs():
     with pytest.raises(oracle.FactorError):
         oracle.penta_periodic_factor(*([[1.0] * 4] * 5))  # n < 5
+
+
+# ---- Crank-Nicolson hyperdiffusion step (eq. 17-19) -----------------------------------
+
+def test_cn_hyperdiffusion_modal_amplification_and_mass():
+    """Periodic CN hyperdiffusion: cos(2 pi k j / N) is multiplied per step by (1 - q)/(1 + q),
+    q = 16 s sin^4(pi k / N) (symbol of the five-point stencil of eq. 18); the grid sum is conserved."""
+    n, s, steps = 64, 0.3, 20
+    j = np.arange(n)
+    ks = [0, 1, 2, 5, 31]
+    u = np.stack([np.cos(2 * np.pi * k * j / n) for k in ks], axis=1).copy()
+    u0 = u.copy()
+    f = oracle.penta_periodic_factor([s] * n, [-4 * s] * n, [1 + 6 * s] * n, [-4 * s] * n, [s] * n)
+    x5 = [-s, 4 * s, 1 - 6 * s, 4 * s, -s]
+    oracle.penta_cn_step_interleaved(f, u, x5, nsteps=steps)
+    for m, k in enumerate(ks):
+        q = 16 * s * np.sin(np.pi * k / n) ** 4
+        assert np.max(np.abs(u[:, m] - u0[:, m] * ((1 - q) / (1 + q)) ** steps)) <= 1e-13
+    rng = np.random.default_rng(6)
+    w = rng.uniform(-1, 1, (n, 3))
+    w0 = w.copy()
+    oracle.penta_cn_step_interleaved(f, w, x5, nsteps=steps)
+    assert np.max(np.abs(w.sum(axis=0) - w0.sum(axis=0))) <= 1e-13
+
+
+@pytest.mark.parametrize("periodic", [False, True])
+def test_cn_hyperdiffusion_dense_restatement(periodic):
+    n, s = 12, 0.4
+    I = np.eye(n)
+    L = -2 * I + np.diag(np.ones(n - 1), 1) + np.diag(np.ones(n - 1), -1)
+    if periodic:
+        L[0, -1] = L[-1, 0] = 1.0
+        D4 = L @ L
+    else:
+        D4 = np.zeros((n, n))   # truncated [1,-4,6,-4,1] (ghost values zero), not L @ L (DESIGN.md C-25)
+        for i in range(n):
+            for o, v in ((-2, 1.0), (-1, -4.0), (0, 6.0), (1, -4.0), (2, 1.0)):
+                if 0 <= i + o < n:
+                    D4[i, i + o] = v
+    rng = np.random.default_rng(7)
+    u = rng.uniform(-1, 1, (n, 4))
+    ref = np.linalg.solve(I + s * D4, (I - s * D4) @ u)
+    st = ([s] * n, [-4 * s] * n, [1 + 6 * s] * n, [-4 * s] * n, [s] * n)
+    f = (oracle.penta_periodic_factor if periodic else oracle.penta_factor)(*st)
+    x5 = [-s, 4 * s, 1 - 6 * s, 4 * s, -s]
+    assert np.max(np.abs(oracle.penta_explicit(u[:, 0], x5, periodic) - ((I - s * D4) @ u)[:, 0])) <= 1e-15
+    oracle.penta_cn_step_interleaved(f, u, x5)
+    assert np.max(np.abs(u - ref)) <= 1e-13
