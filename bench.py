@@ -258,6 +258,30 @@ def paper_table1(torch, b, inputs, sigma=0.5, steps=1000):
             "note": "paper's numbers: Tesla V100, whole step incl. a separate stencil pass; context only", "rows": rows}
 
 
+# Table 2: periodic Crank-Nicolson hyperdiffusion; the paper's caption says seconds, the
+# magnitudes suggest milliseconds and the step count is not stated: recorded verbatim, context only.
+PAPER_TABLE2_V100 = {(6, 64): 369.902, (6, 256): 461.727, (6, 1024): 658.475, (12, 64): 460.857, (12, 256): 429.127,
+                     (12, 1024): 1344.377, (16, 64): 1786.018, (16, 256): 6535.750, (16, 1024): 25893.904}
+
+
+def paper_table2(torch, b, inputs, sigma=0.5, steps=1000):
+    rows = []
+    x5 = [-sigma, 4 * sigma, 1 - 6 * sigma, 4 * sigma, -sigma]
+    for (lb, n), paper_v in sorted(PAPER_TABLE2_V100.items()):
+        batch = 1 << lb
+        h = b.penta_factor_periodic([sigma] * n, [-4 * sigma] * n, [1 + 6 * sigma] * n, [-4 * sigma] * n, [sigma] * n)
+        u = torch.empty(n, batch, dtype=torch.float64, device="cuda")
+        inputs.fill_uniform_device(u, n, seed=8)
+        fn = lambda t: b.penta_cn_step_batched(h, t, x5, steps)
+        fn(u)
+        ms = time_launches(torch, fn, [u], 1)
+        rows.append({"batch": batch, "n": n, "seconds_1000_steps": round(ms * 1e-3, 6),
+                     "paper_v100_value_units_unresolved": paper_v, "plan": h.cn_plan(8)})
+        del u
+    return {"workload": "periodic Crank-Nicolson hyperdiffusion, 1000 steps (penta_cn_step_batched, fused 8 steps per launch)",
+            "note": "paper's numbers: Tesla V100, units (s or ms) and step count not stated; context only", "rows": rows}
+
+
 def extra_table(torch, b, inputs, peak):
     """Throughput at the other BASELINE.json configs: single launches, cold (rotating over
     buffers whose total exceeds 4x L2 when one buffer would fit in L2)."""
@@ -481,6 +505,7 @@ def run_ours(args):
         torch.cuda.empty_cache()
         line["configs"] = extra_table(torch, b, inputs, peak)
         line["paper_table1"] = paper_table1(torch, b, inputs)
+        line["paper_table2"] = paper_table2(torch, b, inputs)
     if rank == 0:
         print(json.dumps(line), flush=True)
     if world > 1:

@@ -139,6 +139,17 @@ BTPS_API int tri_cn_step_batched(tri_handle_t h, double *d_u, int64_t batch, dou
                         int nsteps, void *stream);
 
 /* ------------------------------------------------------------------------------------------
+ * Fused Crank-Nicolson hyperdiffusion step.  PAPER.md:284-296 (eq. 17-19): per step
+ *   f_i = x5[0]*u[i-2] + x5[1]*u[i-1] + x5[2]*u[i] + x5[3]*u[i+1] + x5[4]*u[i+2]
+ * (eq. 18: x5 = (-s, 4s, 1-6s, 4s, -s), s = sigma_x; x5: HOST, 5 doubles) is built in registers and the
+ * pentadiagonal system of `h` (s, -4s, 1+6s, -4s, s) solved in the same kernel; nsteps steps, in place,
+ * fp64.  Periodic stencil and solve with a penta_factor_periodic handle (the paper's Table 2 benchmark),
+ * ghost values zero with a penta_factor handle.
+ * ---------------------------------------------------------------------------------------- */
+BTPS_API int penta_cn_step_batched(penta_handle_t h, double *d_u, int64_t batch, const double *x5, int nsteps,
+                          void *stream);
+
+/* ------------------------------------------------------------------------------------------
  * (a5) Fused semi-implicit Cahn-Hilliard step.  PAPER.md:365-392 (eq. 24, 25a, 26a-c):
  *   (I + sigma*D4) c^{n+1} = c^n + alpha * D2( (c^n)^3 - c^n ),   alpha = dt/dx^2,
  * truncated (non-periodic) stencils, ghost values zero (BASELINE.json config 5; DESIGN.md
@@ -188,7 +199,7 @@ BTPS_API const char *btps_error_string(int code);
  *   out[7] coefficient table bytes resident on the device for this plan,
  *   out[8] 1 if aligned batches are prefetched by TMA, out[9] 1 if carries use the warp scan.
  * kind: 0 = tri handle, 1 = penta handle (solve kernels), 2 = penta handle (fused CH step kernels),
- * 3 = tri handle (fused Crank-Nicolson step kernels). */
+ * 3 = tri handle (fused Crank-Nicolson step kernels), 4 = penta handle (fused Crank-Nicolson step kernels). */
 BTPS_API int btps_plan_info(int kind, const void *handle, int elem_bytes, int *out);
 
 /* Override the plan chosen at factor time (call BEFORE tri_factor / penta_factor; process

@@ -13,7 +13,7 @@ _LIB_PATH = os.path.join(_HERE, "libbtps.so")
 EXPORTS = [
     "tri_factor", "tri_factor_periodic", "tri_destroy", "penta_factor", "penta_factor_periodic", "penta_destroy",
     "tri_solve_batched", "tri_solve_batched_f32", "penta_solve_batched", "penta_solve_batched_f32",
-    "tri_solve_steps", "penta_solve_steps", "ch_step_batched", "ch_step_batched_stat", "tri_cn_step_batched",
+    "tri_solve_steps", "penta_solve_steps", "ch_step_batched", "ch_step_batched_stat", "tri_cn_step_batched", "penta_cn_step_batched",
     "tri_solve_batched_host", "penta_solve_batched_host", "ch_step_batched_host",
     "btps_last_error", "btps_error_string", "btps_plan_info", "btps_tune", "btps_launch_count",
 ]
@@ -63,6 +63,8 @@ def _load() -> ctypes.CDLL:
     lib.ch_step_batched.restype = ci
     lib.tri_cn_step_batched.argtypes = [vp, vp, i64, ctypes.c_double, ctypes.c_double, ctypes.c_double, ci, vp]
     lib.tri_cn_step_batched.restype = ci
+    lib.penta_cn_step_batched.argtypes = [vp, vp, i64, dp, ci, vp]
+    lib.penta_cn_step_batched.restype = ci
     lib.ch_step_batched_stat.argtypes = [vp, vp, i64, ctypes.c_double, ci, vp, vp]
     lib.ch_step_batched_stat.restype = ci
     for name in ("tri_solve_batched_host", "penta_solve_batched_host"):
@@ -145,6 +147,10 @@ class PentaHandle(_Handle):
     def ch_plan(self, elem_bytes: int = 8) -> dict:
         """Plan of the fused Cahn-Hilliard step kernels of this handle (btps_plan_info kind 2)."""
         return btps_plan_info(self, elem_bytes, kind=2)
+
+    def cn_plan(self, elem_bytes: int = 8) -> dict:
+        """Plan of the fused Crank-Nicolson hyperdiffusion step kernels (btps_plan_info kind 4)."""
+        return btps_plan_info(self, elem_bytes, kind=4)
 
 
 def tri_factor(a, b, c) -> TriHandle:
@@ -252,6 +258,14 @@ def ch_step_batched(h: PentaHandle, c, alpha: float, nsteps: int = 1, stream=Non
 def tri_cn_step_batched(h: TriHandle, u, xa: float, xb: float, xc: float, nsteps: int = 1, stream=None):
     p, batch = _dev_args(h, u, 8)
     _check(_lib.tri_cn_step_batched(h.ptr, p, batch, float(xa), float(xb), float(xc), int(nsteps), _stream(stream)))
+
+
+def penta_cn_step_batched(h: PentaHandle, u, x5, nsteps: int = 1, stream=None):
+    p, batch = _dev_args(h, u, 8)
+    x5 = _host64(x5)
+    if x5.size != 5:
+        raise ValueError("x5 must hold the five explicit stencil coefficients")
+    _check(_lib.penta_cn_step_batched(h.ptr, p, batch, _dptr(x5), int(nsteps), _stream(stream)))
 
 
 def ch_step_batched_stat(h: PentaHandle, c, alpha: float, nsteps: int, lbar, stream=None):

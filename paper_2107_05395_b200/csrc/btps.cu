@@ -82,7 +82,7 @@ struct Shape {
 struct DtypePlan {
     int elem = 8;
     int rows = 0, P = 0;
-    Shape shape[2];     // [0] solve (tri / penta), [1] fused CH step (penta handles)
+    Shape shape[3];     // [0] solve, [1] fused CH step (penta) / CN diffusion step (tri), [2] CN hyperdiffusion step (penta)
     int ws = 0;         // carries by the warp-shuffle scan
     int scan_log2 = 0;  // log2 of the scan width
     int tq = 32;        // partitions per scan-table row
@@ -93,7 +93,7 @@ struct DtypePlan {
     size_t soa_bytes = 0;
     // [kind slot][vector mode: 0 = plan.vec, 1 = scalar tail-safe][0 = TMA prefetch, 1 = direct loads]
     // kind slot 0 = solve, 1 = CH (penta handles only)
-    KernelSlot k[2][2][2];
+    KernelSlot k[3][2][2];
 };
 
 constexpr int MAGIC_TRI = 0x74726931;    // "tri1"
@@ -158,9 +158,10 @@ void choose_plan(int n, int elem, int handle_kind, DtypePlan &pl)
     int rows = g_tune.rows > 0 ? g_tune.rows : (n <= 8 ? 8 : (n <= 16 ? 16 : 32));
     if (rows != 8 && rows != 16 && rows != 32) rows = 32;
     int P = (n + rows - 1) / rows;
-    const int nshape = 2;  // [0] solves, [1] fused explicit-half steps (CH for penta handles, Crank-Nicolson for tri)
+    const int nshape = 3;  // [0] solves, [1] CH (penta) / CN diffusion (tri) steps, [2] CN hyperdiffusion steps (penta)
     for (int k = 0; k < nshape; ++k)
-        choose_shape(k == 0 ? handle_kind : (handle_kind == KIND_TRI ? KIND_TRICN : KIND_CH), elem, rows, P, pl.shape[k]);
+        choose_shape(k == 0 ? handle_kind : (handle_kind == KIND_TRI ? KIND_TRICN : (k == 1 ? KIND_CH : KIND_PENTACN)), elem,
+                     rows, P, pl.shape[k]);
     // the warp scan wants whole warps per group and at most 32 partitions: pad P with identity
     // partitions where that makes every family's group a whole number of warps
     int ws = (P > 1 && P <= 32 && g_tune.warp_scan != 0) ? 1 : 0;
@@ -508,11 +509,12 @@ void layout_slot(const DtypePlan &pl, const Shape &sh, int kind, KernelSlot &sl,
     const bool tri = (kind == KIND_TRI || kind == KIND_TRIP || kind == KIND_TRICN || kind == KIND_TRICNP);
     const int NC = tri ? 1 : 2;
     // kinds with an explicit half need one halo row on each side between fused steps
-    const bool is_ch = (kind == KIND_CH || kind == KIND_CHP || kind == KIND_TRICN || kind == KIND_TRICNP);
-    const bool wood = (kind == KIND_PENTAP || kind == KIND_CHP), pert = (kind == KIND_TRIP || kind == KIND_TRICNP);
+    const bool cn5 = (kind == KIND_PENTACN || kind == KIND_PENTACNP);  // two halo rows on each side
+    const bool is_ch = (kind == KIND_CH || kind == KIND_CHP || kind == KIND_TRICN || kind == KIND_TRICNP || cn5);
+    const bool wood = (kind == KIND_PENTAP || kind == KIND_CHP || kind == KIND_PENTACNP), pert = (kind == KIND_TRIP || kind == KIND_TRICNP);
     const size_t W = (size_t)sh.lanes * sl.vec;
     // CH: + the halo rows exchanged between fused steps; periodic tri: + y_1 and y_N of eq. 15
-    sl.xvals = 2 * NC + ((is_ch && halo) ? 2 : 0) + (pert ? 2 : 0);
+    sl.xvals = 2 * NC + ((is_ch && halo) ? (cn5 ? 4 : 2) : 0) + (pert ? 2 : 0);
     sl.xper = (int)(sl.xvals * pl.P * W);
     sl.xstride = sl.xper + (wood ? (int)(4 * W) : 0);  // cyclic penta: y at rows 0, 1, n-2, n-1
     const size_t xch = (pl.P > 1) ? (size_t)sh.tpc * sl.xstride * pl.elem : 0;
@@ -547,6 +549,8 @@ SweepEntry find_sweep(int kind, int elem_bytes, int vec, int rows, int single, i
         if (kind == KIND_CHP) return find_sweep_chp_f64(vec, rows, single, tma, ws, fuse);
         if (kind == KIND_TRICN) return find_sweep_tricn_f64(vec, rows, single, tma, ws, fuse);
         if (kind == KIND_TRICNP) return find_sweep_tricnp_f64(vec, rows, single, tma, ws, fuse);
+        if (kind == KIND_PENTACN) return find_sweep_pentacn_f64(vec, rows, single, tma, ws, fuse);
+        if (kind == KIND_PENTACNP) return find_sweep_pentacnp_f64(vec, rows, single, tma, ws, fuse);
         if (kind == KIND_PENTA) return find_sweep_penta_f64(vec, rows, single, tma, ws, fuse);
         return find_sweep_ch_f64(vec, rows, single, tma, ws, fuse);
     }
@@ -554,7 +558,8 @@ SweepEntry find_sweep(int kind, int elem_bytes, int vec, int rows, int single, i
     if (kind == KIND_TRIP) return find_sweep_trip_f32(vec, rows, single, tma, ws, fuse);
     if (kind == KIND_PENTAP) return find_sweep_pentap_f32(vec, rows, single, tma, ws, fuse);
     if (kind == KIND_CHP) return find_sweep_chp_f32(vec, rows, single, tma, ws, fuse);
-    if (kind == KIND_TRICN || kind == KIND_TRICNP) return SweepEntry{nullptr, nullptr, 0};  // fp64 only
+    if (kind == KIND_TRICN || kind == KIND_TRICNP || kind == KIND_PENTACN || kind == KIND_PENTACNP)
+        return SweepEntry{nullptr, nullptr, 0};  // the Crank-Nicolson steps are fp64 only
     if (kind == KIND_PENTA) return find_sweep_penta_f32(vec, rows, single, tma, ws, fuse);
     return find_sweep_ch_f32(vec, rows, single, tma, ws, fuse);
 }
@@ -562,7 +567,7 @@ SweepEntry find_sweep(int kind, int elem_bytes, int vec, int rows, int single, i
 void fit_plan(DtypePlan &pl, int handle_kind)
 {
     if (pl.two_pass) return;
-    for (int k = 0; k < 2; ++k) {
+    for (int k = 0; k < 3; ++k) {
         KernelSlot probe;
         probe.vec = 1;
         probe.tma = 0;
@@ -577,15 +582,19 @@ void fill_slots(Handle *h)
         DtypePlan &pl = h->plan[t];
         if (pl.two_pass) continue;
         const int single = (pl.P == 1) ? 1 : 0;
-        for (int ks = 0; ks < 2; ++ks) {
+        for (int ks = 0; ks < 3; ++ks) {
             int kind;
             if (h->kind == KIND_TRI) {
+                if (ks == 2) continue;
                 kind = (ks == 0) ? (h->periodic ? KIND_TRIP : KIND_TRI) : (h->periodic ? KIND_TRICNP : KIND_TRICN);
                 if (ks == 1 && pl.elem != 8) continue;  // the Crank-Nicolson step is fp64 only
                 // periodic explicit halves need whole partitions and at least two of them (halo wrap)
                 if (kind == KIND_TRICNP && (pl.P < 2 || pl.P * pl.rows != h->n)) continue;
             } else {
-                kind = (ks == 0) ? (h->periodic ? KIND_PENTAP : KIND_PENTA) : (h->periodic ? KIND_CHP : KIND_CH);
+                kind = (ks == 0) ? (h->periodic ? KIND_PENTAP : KIND_PENTA)
+                                 : (ks == 1 ? (h->periodic ? KIND_CHP : KIND_CH) : (h->periodic ? KIND_PENTACNP : KIND_PENTACN));
+                if (ks == 2 && pl.elem != 8) continue;
+                if (kind == KIND_PENTACNP && (pl.P < 2 || pl.P * pl.rows != h->n)) continue;
                 // the periodic CH kernels need whole partitions and at least two of them (halo wrap);
                 // other sizes run the two-pass form
                 if (kind == KIND_CHP && (pl.P < 2 || pl.P * pl.rows != h->n)) continue;
@@ -601,7 +610,8 @@ void fill_slots(Handle *h)
                     if (sl.tma && !tma_possible(pl, sh, sl.vec)) continue;
                     layout_slot(pl, sh, kind, sl);
                     bool can_fuse = true;
-                    if (sl.smem > SMEM_LIMIT && (kind == KIND_CH || kind == KIND_CHP || kind == KIND_TRICN || kind == KIND_TRICNP)) {
+                    if (sl.smem > SMEM_LIMIT && (kind == KIND_CH || kind == KIND_CHP || kind == KIND_TRICN || kind == KIND_TRICNP || kind == KIND_PENTACN ||
+                                                kind == KIND_PENTACNP)) {
                         // tight fit (N = 1024 fp64): drop the halo exchange rows, one step per launch
                         layout_slot(pl, sh, kind, sl, false);
                         can_fuse = false;
@@ -697,7 +707,7 @@ int launch_one(Handle *h, int kind, T *d_rhs, long long batch, double alpha_x, i
         const long long grid = (batch + block - 1) / block;
         const T *co = (const T *)pl.d_soa;
         PerPenta ppx = h->pp;
-        for (int i = 0; i < 3; ++i) ppx.ex[i] = ex ? ex[i] : 0.0;
+        for (int i = 0; i < 5; ++i) ppx.ex[i] = ex ? ex[i] : 0.0;
         for (int l = 0; l < ksteps; ++l) {
             if (kind == KIND_TRI && h->periodic)
                 two_pass_kernel<T, KIND_TRIP><<<(unsigned)grid, block, 0, st>>>(co, d_rhs, batch, h->n, h->per_vN, h->per_invden, h->pp);
@@ -711,6 +721,10 @@ int launch_one(Handle *h, int kind, T *d_rhs, long long batch, double alpha_x, i
                 two_pass_kernel<T, KIND_PENTAP><<<(unsigned)grid, block, 0, st>>>(co, d_rhs, batch, h->n, 0.0, 0.0, h->pp);
             else if (kind == KIND_PENTA)
                 two_pass_kernel<T, KIND_PENTA><<<(unsigned)grid, block, 0, st>>>(co, d_rhs, batch, h->n, 0.0, 0.0, h->pp);
+            else if (kind == KIND_PENTACN && h->periodic)
+                two_pass_kernel<T, KIND_PENTACNP><<<(unsigned)grid, block, 0, st>>>(co, d_rhs, batch, h->n, 0.0, 0.0, ppx);
+            else if (kind == KIND_PENTACN)
+                two_pass_kernel<T, KIND_PENTACN><<<(unsigned)grid, block, 0, st>>>(co, d_rhs, batch, h->n, 0.0, 0.0, ppx);
             else if (h->periodic)
                 two_pass_kernel<T, KIND_CHP><<<(unsigned)grid, block, 0, st>>>(co, d_rhs, batch, h->n, alpha_x, 0.0, h->pp);
             else
@@ -726,7 +740,7 @@ int launch_one(Handle *h, int kind, T *d_rhs, long long batch, double alpha_x, i
         return BTPS_OK;
     };
     if (pl.two_pass) return two_pass();
-    const int ks = (kind == KIND_CH || kind == KIND_TRICN) ? 1 : 0;
+    const int ks = (kind == KIND_CH || kind == KIND_TRICN) ? 1 : (kind == KIND_PENTACN ? 2 : 0);
     const Shape &sh = pl.shape[ks];
     // the vectorised kernels need whole vectors: batch % vec == 0 and an aligned base pointer;
     // TMA needs a 16-byte aligned base and row pitch
@@ -757,7 +771,7 @@ int launch_one(Handle *h, int kind, T *d_rhs, long long batch, double alpha_x, i
     a.per_invden = h->per_invden;
     a.last_part = (h->n - 1) / pl.rows;
     a.last_k = (h->n - 1) % pl.rows;
-    for (int i = 0; i < 3; ++i) a.ex[i] = ex ? ex[i] : 0.0;
+    for (int i = 0; i < 5; ++i) a.ex[i] = ex ? ex[i] : 0.0;
     for (int i = 0; i < 16; ++i) a.per_H[i] = h->pp.H[i];
     for (int i = 0; i < 6; ++i) a.per_w6[i] = h->pp.w6[i];
     {
@@ -1201,8 +1215,15 @@ int ch_step_batched(penta_handle_t h, double *d_c, int64_t batch, double alpha, 
 int tri_cn_step_batched(tri_handle_t h, double *d_u, int64_t batch, double xa, double xb, double xc, int nsteps,
                         void *stream)
 {
-    const double ex[3] = {xa, xb, xc};
+    const double ex[5] = {xa, xb, xc, 0.0, 0.0};
     return solve_steps<double>(h, MAGIC_TRI, KIND_TRICN, d_u, batch, 0.0, nsteps, stream, nullptr, ex);
+}
+
+int penta_cn_step_batched(penta_handle_t h, double *d_u, int64_t batch, const double *x5, int nsteps, void *stream)
+{
+    if (!x5) return set_err(BTPS_E_ARG);
+    const double ex[5] = {x5[0], x5[1], x5[2], x5[3], x5[4]};
+    return solve_steps<double>(h, MAGIC_PENTA, KIND_PENTACN, d_u, batch, 0.0, nsteps, stream, nullptr, ex);
 }
 
 int ch_step_batched_stat(penta_handle_t h, double *d_c, int64_t batch, double alpha, int nsteps, double *d_lbar,
@@ -1249,11 +1270,11 @@ const char *btps_error_string(int code)
 
 int btps_plan_info(int kind, const void *handle, int elem_bytes, int *out)
 {
-    if (kind < 0 || kind > 3) return set_err(BTPS_E_ARG);
+    if (kind < 0 || kind > 4) return set_err(BTPS_E_ARG);
     Handle *h = check(handle, (kind == 0 || kind == 3) ? MAGIC_TRI : MAGIC_PENTA);
     if (!h || !out || (elem_bytes != 8 && elem_bytes != 4)) return set_err(BTPS_E_ARG);
     const DtypePlan &pl = h->plan[elem_bytes == 8 ? 0 : 1];
-    const int ks = (kind >= 2) ? 1 : 0;
+    const int ks = (kind == 4) ? 2 : ((kind >= 2) ? 1 : 0);
     const Shape &sh = pl.shape[ks];
     const KernelSlot &sl = pl.k[ks][0][0].ent.func ? pl.k[ks][0][0] : pl.k[ks][0][1];
     out[0] = pl.two_pass ? 0 : pl.rows;

@@ -82,5 +82,7 @@ SweepEntry find_sweep_chp_f64(int vec, int rows, int single, int tma, int ws, in
 SweepEntry find_sweep_chp_f32(int vec, int rows, int single, int tma, int ws, int fuse);
 SweepEntry find_sweep_tricn_f64(int vec, int rows, int single, int tma, int ws, int fuse);
 SweepEntry find_sweep_tricnp_f64(int vec, int rows, int single, int tma, int ws, int fuse);
+SweepEntry find_sweep_pentacn_f64(int vec, int rows, int single, int tma, int ws, int fuse);
+SweepEntry find_sweep_pentacnp_f64(int vec, int rows, int single, int tma, int ws, int fuse);
 
 }  // namespace btps

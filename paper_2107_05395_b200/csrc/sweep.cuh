@@ -39,7 +39,8 @@ namespace btps {
 // TRIP / PENTAP / CHP: the periodic (cyclic) forms of TRI / PENTA / CH
 // TRICN / TRICNP: Crank-Nicolson step (explicit three-point half + tri solve), truncated / periodic
 enum Kind {
-    KIND_TRI = 0, KIND_PENTA = 1, KIND_CH = 2, KIND_TRIP = 3, KIND_PENTAP = 4, KIND_CHP = 5, KIND_TRICN = 6, KIND_TRICNP = 7
+    KIND_TRI = 0, KIND_PENTA = 1, KIND_CH = 2, KIND_TRIP = 3, KIND_PENTAP = 4, KIND_CHP = 5, KIND_TRICN = 6, KIND_TRICNP = 7,
+    KIND_PENTACN = 8, KIND_PENTACNP = 9  // Crank-Nicolson hyperdiffusion step (explicit five-point half + penta solve)
 };
 
 constexpr int SCAN_STEPS = 5;   // Kogge-Stone steps held in the tables (scan width <= 32)
@@ -54,7 +55,7 @@ struct SweepArgs {
     double per_vN;         // periodic tri: last entry of v, eq. 13a (-a_1/b_1)
     double per_invden;     // periodic tri: 1 / (1 + v.z), eq. 15
     int last_part, last_k; // periodic tri: partition and local row of row n-1
-    double ex[3];          // Crank-Nicolson step: explicit stencil xa, xb, xc (eq. 9)
+    double ex[5];          // Crank-Nicolson steps: explicit stencil, 3 (eq. 9) or 5 values (eq. 18)
     double per_H[16];      // periodic penta: (I + V^T Z)^{-1}, row-major (Woodbury)
     double per_w6[6];      // periodic penta: wrap-around entries e_0, a_0, e_1, f_{n-2}, c_{n-1}, f_{n-1}
     int wrow_part[4], wrow_k[4];  // periodic penta: partition / local row of rows 0, 1, n-2, n-1
@@ -150,7 +151,7 @@ template <int KIND>
 struct RecLayout {
     static constexpr bool TRI = (KIND == KIND_TRI || KIND == KIND_TRIP || KIND == KIND_TRICN || KIND == KIND_TRICNP);
     static constexpr bool PERT = (KIND == KIND_TRIP || KIND == KIND_TRICNP);  // Sherman-Morrison finish
-    static constexpr bool WOOD = (KIND == KIND_PENTAP || KIND == KIND_CHP);  // rank-4 Woodbury correction
+    static constexpr bool WOOD = (KIND == KIND_PENTAP || KIND == KIND_CHP || KIND == KIND_PENTACNP);  // rank-4 Woodbury correction
     static constexpr int ELEMS = TRI ? (PERT ? 6 : 5) : (WOOD ? 13 : 9);  // values per row
     static constexpr int NC = TRI ? 1 : 2;                     // carries per direction
 };
@@ -241,8 +242,11 @@ sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
     constexpr bool TRI = RecLayout<KIND>::TRI;
     constexpr bool ISCH = (KIND == KIND_CH || KIND == KIND_CHP);  // explicit Cahn-Hilliard half fused in
     constexpr bool ISCN = (KIND == KIND_TRICN || KIND == KIND_TRICNP);  // explicit three-point half (eq. 9) fused in
-    constexpr bool HALO1 = ISCH || ISCN;                          // needs the rows r0-1 and r0+MR
-    constexpr bool WRAP = (KIND == KIND_CHP || KIND == KIND_TRICNP);  // ... with periodic differences
+    constexpr bool ISCN5 = (KIND == KIND_PENTACN || KIND == KIND_PENTACNP);  // explicit five-point half (eq. 18)
+    constexpr bool HALO2 = ISCN5;                                 // needs two rows on each side
+    constexpr bool HALO1 = ISCH || ISCN || HALO2;                 // needs the rows r0-1 and r0+MR
+    constexpr int NHALO = HALO2 ? 4 : (HALO1 ? 2 : 0);            // exchange values for the fused steps' halos
+    constexpr bool WRAP = (KIND == KIND_CHP || KIND == KIND_TRICNP || KIND == KIND_PENTACNP);  // periodic differences
     constexpr bool PERT = RecLayout<KIND>::PERT;
     constexpr bool WOOD = RecLayout<KIND>::WOOD;
     constexpr int NC = RecLayout<KIND>::NC;
@@ -326,7 +330,8 @@ sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
         T *const p0 = rhs0 + (long long)tile * W;
 
         T v[MR][V];
-        [[maybe_unused]] T cm[V], cp[V];  // CH halo rows r0-1 and r0+MR (c^n)
+        [[maybe_unused]] T cm[V], cp[V];    // halo rows r0-1 and r0+MR (c^n)
+        [[maybe_unused]] T cm2[V], cp2[V];  // five-point stencil: rows r0-2 and r0+MR+1
         if constexpr (TMA) {
             // ---- take the prefetched tile out of the ring, then have it refilled ---------------
             mbar_wait(mbar, phase);
@@ -338,12 +343,22 @@ sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
             if constexpr (HALO1) {
 #pragma unroll
                 for (int e = 0; e < V; ++e) cm[e] = cp[e] = T(0);
+                if constexpr (HALO2) {
+#pragma unroll
+                    for (int e = 0; e < V; ++e) cm2[e] = cp2[e] = T(0);
+                }
                 if constexpr (!SINGLE) {
                     // periodic form (n a multiple of MR): row -1 is row n-1, row n is row 0
                     if (part > 0) ld_sys<T, V>(cm, rp - W);
                     else if (WRAP) ld_sys<T, V>(cm, ring + ((a.n - 1) * W + sl * V));
                     if (part + 1 < a.P) ld_sys<T, V>(cp, rp + MR * W);
                     else if (WRAP) ld_sys<T, V>(cp, ring + sl * V);
+                    if constexpr (HALO2) {
+                        if (part > 0) ld_sys<T, V>(cm2, rp - 2 * W);
+                        else if (WRAP) ld_sys<T, V>(cm2, ring + ((a.n - 2) * W + sl * V));
+                        if (part + 1 < a.P) ld_sys<T, V>(cp2, rp + (MR + 1) * W);
+                        else if (WRAP) ld_sys<T, V>(cp2, ring + (W + sl * V));
+                    }
                 }
             }
             group_sync(a.tpc, sub, tpt);  // every thread has drained the ring
@@ -371,6 +386,14 @@ sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
                 else if (WRAP && act) ld_sys<T, V>(cm, p0 + (long long)(a.n - 1) * batch);   // r0 == 0: row n-1
                 if (act && (r0 + MR < a.n)) ld_sys<T, V>(cp, p0 + (long long)MR * batch);
                 else if (WRAP && act) ld_sys<T, V>(cp, p0 - (long long)r0 * batch);          // row 0
+                if constexpr (HALO2) {
+#pragma unroll
+                    for (int e = 0; e < V; ++e) cm2[e] = cp2[e] = T(0);
+                    if (act && r0 > 1) ld_sys<T, V>(cm2, p0 - 2 * batch);
+                    else if (WRAP && act) ld_sys<T, V>(cm2, p0 + (long long)(a.n - 2) * batch);      // r0 == 0: row n-2
+                    if (act && (r0 + MR + 1 < a.n)) ld_sys<T, V>(cp2, p0 + (long long)(MR + 1) * batch);
+                    else if (WRAP && act) ld_sys<T, V>(cp2, p0 - (long long)(r0 - 1) * batch);       // row 1
+                }
             }
         }
 
@@ -389,6 +412,10 @@ sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
                     const int pp = (part + 1 < a.P) ? part + 1 : (WRAP ? 0 : -1);
                     cm[e] = (pm >= 0) ? xb[(2 * NC + 1) * hv + pm * W + ((sl * V + e) ^ (pm & hm))] : T(0);
                     cp[e] = (pp >= 0) ? xb[2 * NC * hv + pp * W + ((sl * V + e) ^ (pp & hm))] : T(0);
+                    if constexpr (HALO2) {  // values 2NC+2 / 2NC+3: second row / last-but-one row
+                        cm2[e] = (pm >= 0) ? xb[(2 * NC + 3) * hv + pm * W + ((sl * V + e) ^ (pm & hm))] : T(0);
+                        cp2[e] = (pp >= 0) ? xb[(2 * NC + 2) * hv + pp * W + ((sl * V + e) ^ (pp & hm))] : T(0);
+                    }
                 }
             }
         }
@@ -441,6 +468,30 @@ sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
             T g1[V], g2[V];  // g_{k-1}, g_{k-2}
 #pragma unroll
             for (int e = 0; e < V; ++e) g1[e] = g2[e] = T(0);
+            if constexpr (ISCN5) {
+                // explicit half of the Crank-Nicolson hyperdiffusion step (eq. 18), in registers:
+                // f_k = x0 c_{k-2} + x1 c_{k-1} + x2 c_k + x3 c_{k+1} + x4 c_{k+2}
+                const T x0 = (T)a.ex[0], x1 = (T)a.ex[1], x2 = (T)a.ex[2], x3 = (T)a.ex[3], x4 = (T)a.ex[4];
+                T c1[V], c2[V];
+#pragma unroll
+                for (int e = 0; e < V; ++e) { c1[e] = cm[e]; c2[e] = cm2[e]; }
+#pragma unroll
+                for (int k = 0; k < MR; ++k) {
+                    const bool row_ok = (k < nrow_part);
+#pragma unroll
+                    for (int e = 0; e < V; ++e) {
+                        const T n1 = (k + 1 < MR) ? v[(k + 1 < MR) ? k + 1 : k][e] : cp[e];
+                        const T n2 = (k + 2 < MR) ? v[(k + 2 < MR) ? k + 2 : k][e] : ((k + 2 == MR) ? cp[e] : cp2[e]);
+                        T f = fma_t<T>(x1, c1[e], x0 * c2[e]);
+                        f = fma_t<T>(x2, v[k][e], f);
+                        f = fma_t<T>(x3, n1, f);
+                        f = fma_t<T>(x4, n2, f);
+                        c2[e] = c1[e];
+                        c1[e] = v[k][e];
+                        v[k][e] = row_ok ? f : T(0);  // padding rows stay identity rows with zero RHS
+                    }
+                }
+            }
             if constexpr (ISCH) {
                 // explicit half: f_k = c_k + alpha_x (w_{k-1} - 2 w_k + w_{k+1}); cm / cp are the
                 // halo rows r0-1 and r0+MR fetched above (zero outside the system).
@@ -745,7 +796,7 @@ sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
                 }
             if constexpr (!SINGLE) {
                 // y_1 lives in partition 0, y_N in partition last_part: two more exchange planes
-                T *const pz = xb + (size_t)(2 * NC + (HALO1 ? 2 : 0)) * a.P * W + sl * V;
+                T *const pz = xb + (size_t)(2 * NC + NHALO) * a.P * W + sl * V;
                 if (part == 0) {
 #pragma unroll
                     for (int e = 0; e < V; ++e) pz[e] = y0[e];
@@ -870,6 +921,10 @@ sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
                 for (int e = 0; e < V; ++e) {
                     xb[2 * NC * hv + part * W + ((sl * V + e) ^ hx)] = v[0][e];
                     xb[(2 * NC + 1) * hv + part * W + ((sl * V + e) ^ hx)] = v[MR - 1][e];
+                    if constexpr (HALO2) {
+                        xb[(2 * NC + 2) * hv + part * W + ((sl * V + e) ^ hx)] = v[1][e];
+                        xb[(2 * NC + 3) * hv + part * W + ((sl * V + e) ^ hx)] = v[MR - 2][e];
+                    }
                 }
             }
         }
@@ -897,7 +952,7 @@ sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
 //   penta : inv, nle, nlb, ngam, ndel
 // -----------------------------------------------------------------------------------------------
 struct PerPenta {  // scalars of the cyclic pentadiagonal (Woodbury) correction and of the CN explicit half
-    double ex[3];  // Crank-Nicolson: explicit stencil xa, xb, xc
+    double ex[5];  // Crank-Nicolson: explicit stencil, 3 (eq. 9) or 5 values (eq. 18)
     double H[16];  // (I + V^T Z)^{-1}, row-major
     double w6[6];  // wrap-around entries e_0, a_0, e_1, f_{n-2}, c_{n-1}, f_{n-1}
 };
@@ -964,6 +1019,26 @@ __global__ void __launch_bounds__(128) two_pass_kernel(const T *__restrict__ co,
                 g2 = g1; g1 = g;
                 wm = wc; wc = wn; cc = cn;
             }
+        } else if constexpr (KIND == KIND_PENTACN || KIND == KIND_PENTACNP) {
+            // Crank-Nicolson hyperdiffusion: explicit five-point half (eq. 18) on the fly (rows i+1, i+2 still c^n)
+            constexpr bool WRAPS = (KIND == KIND_PENTACNP);
+            const T x0 = (T)pp.ex[0], x1 = (T)pp.ex[1], x2 = (T)pp.ex[2], x3 = (T)pp.ex[3], x4 = (T)pp.ex[4];
+            const T c_0 = p[0], c_1 = (n > 1) ? p[batch] : T(0);
+            T c2 = WRAPS ? p[(long long)(n - 2) * batch] : T(0), c1 = WRAPS ? p[(long long)(n - 1) * batch] : T(0);
+            T cc = c_0, cn1 = c_1;
+            for (int i = 0; i < n; ++i) {
+                const int i2 = i + 2;
+                const T cn2 = (i2 < n) ? p[(long long)i2 * batch] : (WRAPS ? (i2 == n ? c_0 : c_1) : T(0));
+                T f = fma_t<T>(x1, c1, x0 * c2);
+                f = fma_t<T>(x2, cc, f);
+                f = fma_t<T>(x3, cn1, f);
+                f = fma_t<T>(x4, cn2, f);
+                const T t = fma_t<T>(__ldg(nle + i), g2, __ldg(inv + i) * f);
+                const T g = fma_t<T>(__ldg(nlb + i), g1, t);
+                p[(long long)i * batch] = g;
+                g2 = g1; g1 = g;
+                c2 = c1; c1 = cc; cc = cn1; cn1 = cn2;
+            }
         } else {
             for (int i = 0; i < n; ++i) {
                 const T t = fma_t<T>(__ldg(nle + i), g2, __ldg(inv + i) * p[(long long)i * batch]);
@@ -979,7 +1054,7 @@ __global__ void __launch_bounds__(128) two_pass_kernel(const T *__restrict__ co,
             p[(long long)i * batch] = x;
             x2 = x1; x1 = x;
         }
-        if constexpr (KIND == KIND_PENTAP || KIND == KIND_CHP) {
+        if constexpr (RecLayout<KIND>::WOOD) {
             // cyclic matrix: x = y - Z H (V^T y) (Woodbury, C-31); Z's four columns follow ndel in co
             const T y0 = p[0], y1 = p[batch], yn2 = p[(long long)(n - 2) * batch], yn1 = p[(long long)(n - 1) * batch];
             const T t0 = fma_t<T>((T)pp.w6[1], yn1, (T)pp.w6[0] * yn2), t1 = (T)pp.w6[2] * yn1, t2 = (T)pp.w6[3] * y0;

@@ -765,3 +765,34 @@ def test_repeated_launches_are_bitwise_identical(lib, n, batch):
                 first = x
             else:
                 assert torch.equal(x, first), (i, rep, n, batch)
+
+
+# ---- fused Crank-Nicolson hyperdiffusion step (eq. 17-19) -----------------------------
+
+@pytest.mark.parametrize("periodic", [True, False])
+@pytest.mark.parametrize("n,batch", [(64, 4096 + 64), (256, 2048), (200, 1001), (512, 1024), (1024, 512), (20, 333), (1500, 256)])
+def test_penta_cn_step(lib, periodic, n, batch):
+    s, steps = 0.3, 11
+    st = ([s] * n, [-4 * s] * n, [1 + 6 * s] * n, [-4 * s] * n, [s] * n)
+    x5 = [-s, 4 * s, 1 - 6 * s, 4 * s, -s]
+    u0 = inputs.uniform_rhs(n, batch, seed=43)
+    u0[:, 0] = np.cos(2 * np.pi * 2 * np.arange(n) / n)
+    h = (lib.penta_factor_periodic if periodic else lib.penta_factor)(*st)
+    fo = (oracle.penta_periodic_factor if periodic else oracle.penta_factor)(*st)
+    ref = u0.copy()
+    oracle.penta_cn_step_interleaved(fo, ref, x5, nsteps=steps)
+    outs = []
+    for fuse in (-1, 1):
+        try:
+            lib.btps_tune("fuse_steps", fuse)
+            d = dev(u0)
+            lib.penta_cn_step_batched(h, d, x5, steps)
+        finally:
+            lib.btps_tune("fuse_steps", -1)
+        outs.append(d.cpu().numpy())
+    assert np.array_equal(outs[0], outs[1])
+    assert rel_err(outs[0], ref) <= TOL_STEPS, (n, batch, h.cn_plan())
+    if periodic:
+        assert np.max(np.abs(outs[0].sum(axis=0) - u0.sum(axis=0))) <= 1e-11
+        q = 16 * s * np.sin(np.pi * 2 / n) ** 4
+        assert np.max(np.abs(outs[0][:, 0] - u0[:, 0] * ((1 - q) / (1 + q)) ** steps)) <= 1e-12
