@@ -37,12 +37,16 @@ static SweepEntry pick_variant(int single, int tma, int ws, int fuse)
 template <typename T, int V, int KIND>
 static SweepEntry pick_rows(int rows, int single, int tma, int ws, int fuse)
 {
-    switch (rows) {
-        case 8: return pick_variant<T, V, 8, KIND>(single, tma, ws, fuse);
-        case 16: return pick_variant<T, V, 16, KIND>(single, tma, ws, fuse);
-        case 32: return pick_variant<T, V, 32, KIND>(single, tma, ws, fuse);
-        default: break;
+    // the base kinds exist for 8, 16 and 32 rows per thread (small n, tuning); the periodic and
+    // Crank-Nicolson kinds only for 32 (other plans run their two-pass form)
+    if constexpr (KIND == KIND_TRI || KIND == KIND_PENTA || KIND == KIND_CH) {
+        switch (rows) {
+            case 8: return pick_variant<T, V, 8, KIND>(single, tma, ws, fuse);
+            case 16: return pick_variant<T, V, 16, KIND>(single, tma, ws, fuse);
+            default: break;
+        }
     }
+    if (rows == 32) return pick_variant<T, V, 32, KIND>(single, tma, ws, fuse);
     SweepEntry none = {nullptr, nullptr, 0};
     return none;
 }
