@@ -53,7 +53,7 @@ std::atomic<long long> g_launches{0};
 // ------------------------------------------------------------------------------------------------
 struct Tune {
     int rows = -1, lanes = -1, vec = -1, tpc = -1, force_two_pass = -1, reverse = -1, prefetch = -1, pdl = -1,
-        warp_scan = -1, grid = -1, fuse = -1;
+        warp_scan = -1, grid = -1, fuse = -1, cluster = -1;
 };
 Tune g_tune;
 
@@ -69,7 +69,7 @@ struct KernelSlot {
     int xvals = 2;     // exchange values per (partition, system)
     int xstride = 0, xper = 0;  // exchange elements per group; offset of the periodic-penta values in it
     size_t smem = 0;
-    unsigned offX = 0, offM = 0, offR = 0;
+    unsigned offX = 0, offM = 0, offR = 0, offTl = 0;
     unsigned box_rows = 0, nboxes = 0;
     int max_grid = 0;  // occupancy * SM count, resolved at first launch
 };
@@ -94,6 +94,9 @@ struct DtypePlan {
     // [kind slot][vector mode: 0 = plan.vec, 1 = scalar tail-safe][0 = TMA prefetch, 1 = direct loads]
     // kind slot 0 = solve, 1 = CH (penta handles only)
     KernelSlot k[3][2][2];
+    // plain solves of long systems (16 < P <= 32): the tile's rows split over a cluster of two CTAs
+    Shape cshape;
+    KernelSlot ck;
 };
 
 constexpr int MAGIC_TRI = 0x74726931;    // "tri1"
@@ -564,6 +567,55 @@ SweepEntry find_sweep(int kind, int elem_bytes, int vec, int rows, int single, i
     return find_sweep_ch_f32(vec, rows, single, tma, ws, fuse);
 }
 
+SweepEntry find_sweep_cl(int kind, int elem_bytes, int fuse)
+{
+    if (kind == KIND_TRI) return elem_bytes == 8 ? find_sweep_cl_tri_f64(fuse) : find_sweep_cl_tri_f32(fuse);
+    if (kind == KIND_PENTA) return elem_bytes == 8 ? find_sweep_cl_penta_f64(fuse) : find_sweep_cl_penta_f32(fuse);
+    return SweepEntry{nullptr, nullptr, 0};
+}
+
+// Cluster-split plan (sweep.cuh, CL): for 16 < P <= 32 partitions one CTA could only keep 8 lanes x 16 B = 128-byte
+// row segments; two CTAs (two SMs) that each keep half of the partitions own a tile of 16 lanes = 256-byte segments,
+// which is what HBM wants.  Shared memory per CTA: its partitions' coefficient blocks, the scan
+// tables, the exchange area of ALL partitions (the pair scans half of the columns each) and the ring of its rows.
+void fill_cluster_slot(Handle *h, DtypePlan &pl)
+{
+    pl.ck = KernelSlot();
+    if (pl.two_pass || h->periodic || !pl.ws || g_tune.cluster == 0 || g_tune.prefetch == 0) return;
+    if (pl.rows != 32 || pl.P <= 16 || pl.P > 32 || (pl.P & 1)) return;
+    const int kind = h->kind;  // KIND_TRI / KIND_PENTA
+    const int NC = (kind == KIND_TRI) ? 1 : 2;
+    const int elems = (kind == KIND_TRI) ? RecLayout<KIND_TRI>::ELEMS : RecLayout<KIND_PENTA>::ELEMS;
+    Shape &sh = pl.cshape;
+    sh.lanes = 16;
+    sh.lanes_log2 = 4;
+    sh.vec = 16 / pl.elem;
+    sh.tpc = 1;
+    const int PL = pl.P / 2;
+    sh.threads = PL * sh.lanes;
+    KernelSlot &sl = pl.ck;
+    sl.vec = sh.vec;
+    sl.tma = 1;
+    const size_t W = (size_t)sh.lanes * sl.vec;
+    sl.xvals = 2 * NC;
+    sl.xper = (int)(sl.xvals * pl.P * W);
+    sl.xstride = sl.xper;
+    const size_t rows_bytes = (size_t)PL * elems * pl.rows * pl.elem;
+    sl.offTl = (unsigned)align16(rows_bytes);
+    sl.offX = (unsigned)align16(sl.offTl + (pl.blob_bytes - pl.offT));
+    sl.offM = (unsigned)align16(sl.offX + (size_t)sl.xstride * pl.elem);
+    sl.offR = (unsigned)align_up(sl.offM + 17 * 8, 128);
+    int g = 256 / pl.rows < PL ? 256 / pl.rows : PL;
+    while (PL % g != 0) --g;
+    sl.box_rows = (unsigned)(g * pl.rows);
+    sl.nboxes = (unsigned)(PL / g);
+    sl.smem = sl.offR + (size_t)PL * pl.rows * W * pl.elem;
+    if (sl.smem > SMEM_LIMIT) return;
+    sl.ent = find_sweep_cl(kind, pl.elem, 0);
+    sl.fused = find_sweep_cl(kind, pl.elem, 1);
+    if (sl.ent.func && sl.ent.max_threads < sh.threads) sl.ent = SweepEntry{nullptr, nullptr, 0};
+}
+
 void fit_plan(DtypePlan &pl, int handle_kind)
 {
     if (pl.two_pass) return;
@@ -580,6 +632,7 @@ void fill_slots(Handle *h)
 {
     for (int t = 0; t < 2; ++t) {
         DtypePlan &pl = h->plan[t];
+        fill_cluster_slot(h, pl);
         if (pl.two_pass) continue;
         const int single = (pl.P == 1) ? 1 : 0;
         for (int ks = 0; ks < 3; ++ks) {
@@ -627,7 +680,7 @@ void fill_slots(Handle *h)
     }
 }
 
-int resolve_slot(Handle *h, const Shape &sh, KernelSlot &sl)
+int resolve_slot(Handle *h, const Shape &sh, KernelSlot &sl, bool cluster = false)
 {
     std::lock_guard<std::mutex> lk(h->mu);
     if (sl.max_grid > 0) return BTPS_OK;
@@ -639,6 +692,28 @@ int resolve_slot(Handle *h, const Shape &sh, KernelSlot &sl)
     int occ = 0, sms = 0, dev = 0;
     CU_TRY(cudaGetDevice(&dev));
     CU_TRY(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    if (cluster) {
+        // co-resident clusters of two CTAs (each CTA fills an SM)
+        cudaLaunchConfig_t cfg = {};
+        cfg.gridDim = dim3((unsigned)(2 * sms));
+        cfg.blockDim = dim3((unsigned)sh.threads);
+        cfg.dynamicSmemBytes = sl.smem;
+        cudaLaunchAttribute at[1];
+        at[0].id = cudaLaunchAttributeClusterDimension;
+        at[0].val.clusterDim.x = 2;
+        at[0].val.clusterDim.y = 1;
+        at[0].val.clusterDim.z = 1;
+        cfg.attrs = at;
+        cfg.numAttrs = 1;
+        int ncl = 0;
+        CU_TRY(cudaOccupancyMaxActiveClusters(&ncl, sl.ent.func, &cfg));
+        if (ncl < 1) {
+            snprintf(tl_cuda_msg, sizeof(tl_cuda_msg), "cluster kernel does not fit: %d threads, %zu B smem", sh.threads, sl.smem);
+            return set_err(BTPS_E_CUDA);
+        }
+        sl.max_grid = 2 * ncl;
+        return BTPS_OK;
+    }
     CU_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, sl.ent.func, sh.threads, sl.smem));
     if (occ < 1) {
         snprintf(tl_cuda_msg, sizeof(tl_cuda_msg), "kernel does not fit: %d threads, %zu B smem", sh.threads,
@@ -741,7 +816,15 @@ int launch_one(Handle *h, int kind, T *d_rhs, long long batch, double alpha_x, i
     };
     if (pl.two_pass) return two_pass();
     const int ks = (kind == KIND_CH || kind == KIND_TRICN) ? 1 : (kind == KIND_PENTACN ? 2 : 0);
-    const Shape &sh = pl.shape[ks];
+    const bool tma_ok = (((uintptr_t)d_rhs % 16) == 0) && ((((size_t)batch * sizeof(T)) % 16) == 0) &&
+                        (batch < (1ll << 31));
+    // long systems: the cluster-split kernels when the batch is TMA-aligned and a multiple of the vector width
+    // (measured on B200: the pair's two cluster barriers per tile cost ~1.3 us, so by default it is used only
+    //  where the wider row segments win -- tridiagonal fp64 with >= 2^18 systems; btps_tune("cluster", 1) forces it
+    //  for every eligible plan, 0 switches it off)
+    const bool cl_wanted = (g_tune.cluster > 0) || (kind == KIND_TRI && sizeof(T) == 8 && batch >= (1ll << 18));
+    const bool use_cl = (ks == 0) && cl_wanted && pl.ck.ent.func && tma_ok && (batch % pl.cshape.vec == 0);
+    const Shape &sh = use_cl ? pl.cshape : pl.shape[ks];
     // the vectorised kernels need whole vectors: batch % vec == 0 and an aligned base pointer;
     // TMA needs a 16-byte aligned base and row pitch
     int s = 0;
@@ -749,15 +832,13 @@ int launch_one(Handle *h, int kind, T *d_rhs, long long batch, double alpha_x, i
         const bool ok = (batch % sh.vec == 0) && (((uintptr_t)d_rhs % (sizeof(T) * sh.vec)) == 0);
         if (!ok) s = 1;
     }
-    const bool tma_ok = (((uintptr_t)d_rhs % 16) == 0) && ((((size_t)batch * sizeof(T)) % 16) == 0) &&
-                        (batch < (1ll << 31));
     int d = (tma_ok && pl.k[ks][s][0].ent.func) ? 0 : 1;
     if (!pl.k[ks][s][d].ent.func && s == 0) s = 1;  // e.g. the wide variant has no direct-load twin that fits
     if (!pl.k[ks][s][d].ent.func) d = 1;
-    KernelSlot &sl = pl.k[ks][s][d];
+    KernelSlot &sl = use_cl ? pl.ck : pl.k[ks][s][d];
     if (!sl.ent.func) return two_pass();
     if (sl.max_grid == 0) {
-        const int rc = resolve_slot(h, sh, sl);
+        const int rc = resolve_slot(h, sh, sl, use_cl);
         if (rc != BTPS_OK) return rc;
     }
     SweepArgs a;
@@ -795,6 +876,7 @@ int launch_one(Handle *h, int kind, T *d_rhs, long long batch, double alpha_x, i
     a.xvals = sl.xvals;
     a.blob_bytes = pl.blob_bytes;
     a.offT = pl.offT;
+    a.offTl = use_cl ? sl.offTl : pl.offT;
     a.offX = sl.offX;
     a.offM = sl.offM;
     a.offR = sl.offR;
@@ -807,8 +889,10 @@ int launch_one(Handle *h, int kind, T *d_rhs, long long batch, double alpha_x, i
         if (rc != BTPS_OK) return rc;
     }
     long long grid = (a.num_tiles + sh.tpc - 1) / sh.tpc;
+    if (use_cl) grid = 2 * a.num_tiles;  // one cluster of two CTAs per tile in flight
     if (grid > sl.max_grid) grid = sl.max_grid;
-    if (g_tune.grid > 0 && grid > g_tune.grid) grid = g_tune.grid;
+    if (g_tune.grid > 0 && grid > g_tune.grid) grid = use_cl ? (g_tune.grid & ~1) : g_tune.grid;
+    if (use_cl && grid < 2) grid = 2;
     // several steps per launch need the fused instantiation; without one (direct-load variants)
     // the steps are launched one by one
     // (the statistic of eq. 30 is computed inside the fused kernels; elsewhere by a pass of its own)
@@ -1304,6 +1388,7 @@ int btps_tune(const char *key, int value)
     else if (!strcmp(key, "warp_scan")) g_tune.warp_scan = value;
     else if (!strcmp(key, "grid")) g_tune.grid = value;
     else if (!strcmp(key, "fuse_steps")) g_tune.fuse = value;
+    else if (!strcmp(key, "cluster")) g_tune.cluster = value;
     else return set_err(BTPS_E_ARG);
     return set_err(BTPS_OK);
 }

@@ -5,12 +5,12 @@
 
 namespace btps {
 
-template <typename T, int V, int MR, bool SINGLE, int KIND, bool TMA, bool WS, bool FUSE = false>
+template <typename T, int V, int MR, bool SINGLE, int KIND, bool TMA, bool WS, bool FUSE = false, bool CL = false>
 static SweepEntry make_entry()
 {
     SweepEntry e;
-    e.launch = &launch_sweep<T, V, MR, SINGLE, KIND, TMA, WS, FUSE>;
-    e.func = reinterpret_cast<const void *>(&sweep_kernel<T, V, MR, SINGLE, KIND, TMA, WS, FUSE>);
+    e.launch = &launch_sweep<T, V, MR, SINGLE, KIND, TMA, WS, FUSE, CL>;
+    e.func = reinterpret_cast<const void *>(&sweep_kernel<T, V, MR, SINGLE, KIND, TMA, WS, FUSE, CL>);
     e.max_threads = CtaShape<T, V, MR>::MAX_THREADS;
     return e;
 }
@@ -69,6 +69,19 @@ static SweepEntry pick_f32(int vec, int rows, int single, int tma, int ws, int f
     SweepEntry none = {nullptr, nullptr, 0};
     return none;
 }
+
+// cluster-split variants (rows of a tile over two CTAs): plain solves, 32 rows per thread, 16 bytes per thread
+template <typename T, int V, int KIND>
+static SweepEntry pick_cl(int fuse)
+{
+    return fuse ? make_entry<T, V, 32, false, KIND, true, true, true, true>()
+                : make_entry<T, V, 32, false, KIND, true, true, false, true>();
+}
+SweepEntry find_sweep_cl(int kind, int elem_bytes, int fuse);
+SweepEntry find_sweep_cl_tri_f64(int fuse);
+SweepEntry find_sweep_cl_tri_f32(int fuse);
+SweepEntry find_sweep_cl_penta_f64(int fuse);
+SweepEntry find_sweep_cl_penta_f32(int fuse);
 
 // kind in {TRI, PENTA, CH}; elem_bytes 8: vec in {1, 2}; 4: vec in {1, 2, 4}; rows in {8, 16, 32}
 SweepEntry find_sweep(int kind, int elem_bytes, int vec, int rows, int single, int tma, int ws, int fuse);

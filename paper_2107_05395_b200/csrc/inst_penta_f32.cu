@@ -6,4 +6,5 @@ SweepEntry find_sweep_penta_f32(int vec, int rows, int single, int tma, int ws, 
 {
     return pick_f32<KIND_PENTA>(vec, rows, single, tma, ws, fuse);
 }
+SweepEntry find_sweep_cl_penta_f32(int fuse) { return pick_cl<float, 4, KIND_PENTA>(fuse); }
 }  // namespace btps

@@ -6,4 +6,5 @@ SweepEntry find_sweep_penta_f64(int vec, int rows, int single, int tma, int ws, 
 {
     return pick_f64<KIND_PENTA>(vec, rows, single, tma, ws, fuse);
 }
+SweepEntry find_sweep_cl_penta_f64(int fuse) { return pick_cl<double, 2, KIND_PENTA>(fuse); }
 }  // namespace btps

@@ -6,4 +6,5 @@ SweepEntry find_sweep_tri_f32(int vec, int rows, int single, int tma, int ws, in
 {
     return pick_f32<KIND_TRI>(vec, rows, single, tma, ws, fuse);
 }
+SweepEntry find_sweep_cl_tri_f32(int fuse) { return pick_cl<float, 4, KIND_TRI>(fuse); }
 }  // namespace btps

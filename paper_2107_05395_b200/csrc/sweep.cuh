@@ -76,6 +76,7 @@ struct SweepArgs {
     int xvals;             // values per (partition, system) in the exchange area: 2*NC (+2 halo rows, CH)
     unsigned blob_bytes;   // multiple of 16
     unsigned offT;         // byte offset of the scan tables inside the blob (row records start at 0)
+    unsigned offTl;        // byte offset of the scan tables in shared memory (= offT unless the rows are split, CL)
     unsigned offX;         // byte offset of the exchange area in shared memory
     unsigned offM;         // byte offset of the per-group mbarriers (TMA kernels)
     unsigned offR;         // byte offset of the prefetch ring (TMA kernels), 128-B aligned
@@ -191,6 +192,33 @@ __device__ __forceinline__ void tma_load_2d(unsigned dst, const CUtensorMap *tm,
         ::"r"(dst), "l"(tm), "r"(c0), "r"(c1), "r"(bar) : "memory");
 }
 
+// ---- thread-block cluster primitives (CL kernels) ---------------------------------------------------
+__device__ __forceinline__ unsigned cluster_ctarank()
+{
+    unsigned r;
+    asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r));
+    return r;
+}
+__device__ __forceinline__ void cluster_sync()
+{
+    asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
+// shared-memory address of the same variable in CTA `rank` of the cluster
+__device__ __forceinline__ unsigned cluster_map(unsigned local_addr, unsigned rank)
+{
+    unsigned r;
+    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(local_addr), "r"(rank));
+    return r;
+}
+__device__ __forceinline__ void st_cluster(unsigned addr, double v)
+{
+    asm volatile("st.shared::cluster.f64 [%0], %1;" ::"r"(addr), "d"(v) : "memory");
+}
+__device__ __forceinline__ void st_cluster(unsigned addr, float v)
+{
+    asm volatile("st.shared::cluster.f32 [%0], %1;" ::"r"(addr), "f"(v) : "memory");
+}
+
 // Barrier over the threads of one tile group.  A CTA hosts `tpc` groups that walk their tiles
 // independently of one another (so one group's arithmetic overlaps another group's waits); a
 // group of one warp synchronises with __syncwarp, one group per CTA with the CTA barrier, and
@@ -232,10 +260,13 @@ __device__ __forceinline__ void scan_steps(int n, F &&f)
 //   TMA    next tile prefetched by TMA into the shared-memory ring (else direct global loads)
 //   WS     carries by the warp-shuffle scan (needs P <= 32 and whole-warp groups); else each
 //          thread walks the partitions before / after it serially (any P)
+//   CL     the tile's rows are split over a cluster of two CTAs (two SMs): CTA r keeps partitions
+//          [r*P/2, (r+1)*P/2) -- twice the systems per tile for long systems (wider row segments in HBM);
+//          carries cross the CTAs through distributed shared memory, cluster barriers order them
 //   FUSE   a.ksteps time steps per tile (separate instantiation: the step loop costs registers, so
 //          single-step launches run the FUSE = false kernel)
 // -----------------------------------------------------------------------------------------------
-template <typename T, int V, int MR, bool SINGLE, int KIND, bool TMA, bool WS, bool FUSE>
+template <typename T, int V, int MR, bool SINGLE, int KIND, bool TMA, bool WS, bool FUSE, bool CL = false>
 __global__ void __launch_bounds__(CtaShape<T, V, MR>::MAX_THREADS, 1)
 sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
 {
@@ -253,11 +284,15 @@ sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
     using Pair = Tup<T, 2>;
     extern __shared__ __align__(128) unsigned char smem[];
 
+    static_assert(!CL || (!SINGLE && TMA && WS && (KIND == KIND_TRI || KIND == KIND_PENTA)), "cluster split: plain solves only");
     const int W = a.lanes * V;
-    const int tpt = a.P * a.lanes;  // threads per tile group (SINGLE: P == 1)
+    [[maybe_unused]] const unsigned crank = CL ? cluster_ctarank() : 0u;  // which half of the rows this CTA keeps
+    const int PL = CL ? (a.P >> 1) : a.P;                                 // partitions kept by this CTA
+    const int tpt = PL * a.lanes;  // threads per tile group (SINGLE: P == 1)
     const int sub = SINGLE ? (threadIdx.x >> a.lanes_log2) : (threadIdx.x / tpt);
     const int lt = SINGLE ? (threadIdx.x & (a.lanes - 1)) : (threadIdx.x - sub * tpt);
-    const int part = SINGLE ? 0 : (lt >> a.lanes_log2);
+    const int plidx = SINGLE ? 0 : (lt >> a.lanes_log2);                  // partition index inside this CTA
+    const int part = plidx + (int)crank * PL;                             // partition index inside the system
     const int sl = lt & (a.lanes - 1);
     const int r0 = part * MR;
     const long long batch = a.batch;
@@ -271,10 +306,21 @@ sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
         if (lt == 0) mbar_init(mbar, 1);
     }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-    __syncthreads();
+    if constexpr (CL) cluster_sync();  // the peer CTA is resident (its shared memory may be written) from here on
+    else __syncthreads();
     if (threadIdx.x == 0) {
-        mbar_expect_tx(bbar, a.blob_bytes);
-        bulk_load(smem_u32(smem), a.blob, a.blob_bytes, bbar);
+        if constexpr (CL) {
+            // this CTA's partitions' coefficient blocks, then the scan tables behind them
+            const unsigned rows_bytes = (unsigned)(PL * RecLayout<KIND>::ELEMS * MR) * (unsigned)sizeof(T);
+            const unsigned tab_bytes = a.blob_bytes - a.offT;
+            mbar_expect_tx(bbar, rows_bytes + tab_bytes);
+            bulk_load(smem_u32(smem), reinterpret_cast<const unsigned char *>(a.blob) + (size_t)crank * rows_bytes,
+                      rows_bytes, bbar);
+            bulk_load(smem_u32(smem + a.offTl), reinterpret_cast<const unsigned char *>(a.blob) + a.offT, tab_bytes, bbar);
+        } else {
+            mbar_expect_tx(bbar, a.blob_bytes);
+            bulk_load(smem_u32(smem), a.blob, a.blob_bytes, bbar);
+        }
     }
     // Programmatic dependent launch (time-step loops): everything above overlaps the tail of the
     // previous launch on the stream; the batch itself is only touched after the wait.  Both
@@ -288,21 +334,23 @@ sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
 
     // coefficient arrays of this partition's rows (RecLayout): one base address, the arrays at
     // compile-time offsets from it
-    const T *const cb = reinterpret_cast<const T *>(smem) + (size_t)part * (RecLayout<KIND>::ELEMS * MR);
+    const T *const cb = reinterpret_cast<const T *>(smem) + (size_t)plidx * (RecLayout<KIND>::ELEMS * MR);
     const Pair *const RA = reinterpret_cast<const Pair *>(cb);                             // {inv, nl | nle}
     const T *const RB1 = cb + 2 * MR;                                                      // nch | nlb
     [[maybe_unused]] const Pair *const RBW = reinterpret_cast<const Pair *>(cb + 3 * MR);  // {chi, psi} | {ngam, ndel}
     [[maybe_unused]] const Pair *const RC0 = reinterpret_cast<const Pair *>(cb + 5 * MR);  // penta {chi1, chi2}
     [[maybe_unused]] const Pair *const RC1 = reinterpret_cast<const Pair *>(cb + 7 * MR);  // penta {psi1, psi2}
-    [[maybe_unused]] const T *const TAB = reinterpret_cast<const T *>(smem + a.offT);
+    [[maybe_unused]] const T *const TAB = reinterpret_cast<const T *>(smem + a.offTl);
     // exchange area of this group: [2*NC values][P][W], columns XOR-swizzled with the partition index
     [[maybe_unused]] T *const xb = reinterpret_cast<T *>(smem + a.offX) + (size_t)sub * a.xstride;
     // prefetch ring of this group: [P*MR rows][W]
-    [[maybe_unused]] const unsigned ring_bytes = (unsigned)(a.P * MR * W) * (unsigned)sizeof(T);
+    [[maybe_unused]] const unsigned ring_bytes = (unsigned)(PL * MR * W) * (unsigned)sizeof(T);
+    [[maybe_unused]] const int rbase = (int)crank * PL * MR;  // first row kept by this CTA
+    [[maybe_unused]] const unsigned xb_peer = CL ? cluster_map(smem_u32(smem + a.offX), crank ^ 1u) : 0u;
     [[maybe_unused]] T *const ring = reinterpret_cast<T *>(smem + a.offR + (size_t)sub * ring_bytes);
 
     const int ntiles = (int)a.num_tiles;
-    const int stride_tiles = gridDim.x * a.tpc;
+    const int stride_tiles = CL ? (int)(gridDim.x >> 1) : (int)(gridDim.x * a.tpc);
     T *const rhs0 = reinterpret_cast<T *>(a.rhs) + (long long)r0 * batch + (long long)sl * V;
 
     // one thread of the group asks the TMA unit for tile `t` (walking order); columns beyond the
@@ -313,10 +361,10 @@ sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
         const unsigned dst = smem_u32(ring);
         const unsigned box_bytes = a.box_rows * (unsigned)W * (unsigned)sizeof(T);
         for (unsigned b = 0; b < a.nboxes; ++b)
-            tma_load_2d(dst + b * box_bytes, &tmap, tile * W, (int)(b * a.box_rows), mbar);
+            tma_load_2d(dst + b * box_bytes, &tmap, tile * W, (int)(b * a.box_rows) + rbase, mbar);
     };
 
-    int t = blockIdx.x * a.tpc + sub;
+    int t = CL ? (int)(blockIdx.x >> 1) : (int)(blockIdx.x * a.tpc + sub);
     [[maybe_unused]] unsigned phase = 0;
     if constexpr (TMA) {
         if (lt == 0 && t < ntiles) tma_issue(t);
@@ -336,7 +384,7 @@ sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
             // ---- take the prefetched tile out of the ring, then have it refilled ---------------
             mbar_wait(mbar, phase);
             phase ^= 1u;
-            const T *rp = ring + (r0 * W + sl * V);
+            const T *rp = ring + ((r0 - rbase) * W + sl * V);
             asm volatile("" : "+l"(rp));  // recompute the MR row addresses per tile: hoisted out of the loop they spill
 #pragma unroll
             for (int k = 0; k < MR; ++k) ld_sys<T, V>(v[k], rp + k * W);
@@ -581,8 +629,23 @@ sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
                         xc[2 * vstr + XI(e)] = v[0][e];
                         xc[3 * vstr + XI(e)] = v[1][e];
                     }
+                    if constexpr (CL) {
+                        // the peer CTA scans half of the systems: it needs these values too
+                        const unsigned pa = xb_peer + (unsigned)((part * W + XI(e)) * (int)sizeof(T));
+                        const unsigned vb = (unsigned)(vstr * (int)sizeof(T));
+                        if constexpr (TRI) {
+                            st_cluster(pa, v[MR - 1][e]);
+                            st_cluster(pa + vb, v[0][e]);
+                        } else {
+                            st_cluster(pa, v[MR - 1][e]);
+                            st_cluster(pa + vb, glast2[e]);
+                            st_cluster(pa + 2 * vb, v[0][e]);
+                            st_cluster(pa + 3 * vb, v[1][e]);
+                        }
+                    }
                 }
-                group_sync(a.tpc, sub, tpt);
+                if constexpr (CL) cluster_sync();
+                else group_sync(a.tpc, sub, tpt);
                 {
                     // lane q of a `width`-lane segment holds partition q
                     const int lane = lt & 31;
@@ -605,9 +668,13 @@ sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
                         return (st < 4 || q < 16) ? val : T(0);
                     };
                     // job = the V systems of one owner thread column sg: V independent chains per lane
-                    for (int s0 = (lt >> 5) * spw; s0 < a.lanes; s0 += (tpt >> 5) * spw) {
+                    // (CL: each CTA of the pair scans half of the columns; a carry is written to the CTA that
+                    //  keeps its partition)
+                    const int job0 = CL ? (int)crank * (a.lanes >> 1) : 0;
+                    const int job1 = CL ? job0 + (a.lanes >> 1) : a.lanes;
+                    for (int s0 = job0 + (lt >> 5) * spw; s0 < job1; s0 += (tpt >> 5) * spw) {
                         const int sg = s0 + (lane >> a.scan_log2);
-                        const bool ok = (q < P) && (sg < a.lanes);
+                        const bool ok = (q < P) && (sg < job1);
                         T *xs = xb + (size_t)q * W;
                         if constexpr (FUSE) asm volatile("" : "+l"(xs));  // (as for rp: hoisted out of the step loop it spills)
                         const int qsw = q & wm;
@@ -682,13 +749,21 @@ sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
                                 const T x = __shfl_down_sync(0xffffffffu, bb[c][e], 1, wd);
                                 const int ix = (sg * V + e) ^ qsw;
                                 if (ok) {
-                                    xs[c * vstr + ix] = fb[c][e];
-                                    xs[(NC + c) * vstr + ix] = (q + 1 < P) ? x : T(0);
+                                    const T xv = (q + 1 < P) ? x : T(0);
+                                    if (!CL || (q >= PL) == (crank != 0u)) {
+                                        xs[c * vstr + ix] = fb[c][e];
+                                        xs[(NC + c) * vstr + ix] = xv;
+                                    } else {
+                                        const unsigned pa = xb_peer + (unsigned)((q * W + c * vstr + ix) * (int)sizeof(T));
+                                        st_cluster(pa, fb[c][e]);
+                                        st_cluster(pa + (unsigned)(NC * vstr * (int)sizeof(T)), xv);
+                                    }
                                 }
                             }
                     }
                 }
-                group_sync(a.tpc, sub, tpt);
+                if constexpr (CL) cluster_sync();
+                else group_sync(a.tpc, sub, tpt);
 #pragma unroll
                 for (int e = 0; e < V; ++e) {
 #pragma unroll
@@ -941,6 +1016,7 @@ sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
             }
         }
     }
+    if constexpr (CL) cluster_sync();  // no CTA of the pair leaves while the other may still write into it
 }
 // -----------------------------------------------------------------------------------------------
 // Two-pass kernel in the paper's own form (Alg. 2 / Alg. 4: one thread per system, g written to
@@ -1105,7 +1181,7 @@ struct SweepEntry {
     int max_threads;   // threads per CTA the kernel was compiled for
 };
 
-template <typename T, int V, int MR, bool SINGLE, int KIND, bool TMA, bool WS, bool FUSE>
+template <typename T, int V, int MR, bool SINGLE, int KIND, bool TMA, bool WS, bool FUSE, bool CL = false>
 cudaError_t launch_sweep(const SweepArgs &a, const CUtensorMap &tm, int grid, int block, size_t smem,
                          cudaStream_t st, int pdl)
 {
@@ -1114,12 +1190,23 @@ cudaError_t launch_sweep(const SweepArgs &a, const CUtensorMap &tm, int grid, in
     cfg.blockDim = dim3((unsigned)block);
     cfg.dynamicSmemBytes = smem;
     cfg.stream = st;
-    cudaLaunchAttribute attr[1];
-    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cudaLaunchAttribute attr[2];
+    int na = 0;
+    if (CL) {  // pairs of CTAs (two SMs) share a tile: grid is a multiple of 2
+        attr[na].id = cudaLaunchAttributeClusterDimension;
+        attr[na].val.clusterDim.x = 2;
+        attr[na].val.clusterDim.y = 1;
+        attr[na].val.clusterDim.z = 1;
+        ++na;
+    }
+    if (pdl) {
+        attr[na].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        attr[na].val.programmaticStreamSerializationAllowed = 1;
+        ++na;
+    }
     cfg.attrs = attr;
-    cfg.numAttrs = pdl ? 1 : 0;
-    return cudaLaunchKernelEx(&cfg, sweep_kernel<T, V, MR, SINGLE, KIND, TMA, WS, FUSE>, a, tm);
+    cfg.numAttrs = na;
+    return cudaLaunchKernelEx(&cfg, sweep_kernel<T, V, MR, SINGLE, KIND, TMA, WS, FUSE, CL>, a, tm);
 }
 
 }  // namespace btps

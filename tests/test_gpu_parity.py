@@ -796,3 +796,41 @@ def test_penta_cn_step(lib, periodic, n, batch):
         assert np.max(np.abs(outs[0].sum(axis=0) - u0.sum(axis=0))) <= 1e-11
         q = 16 * s * np.sin(np.pi * 2 / n) ** 4
         assert np.max(np.abs(outs[0][:, 0] - u0[:, 0] * ((1 - q) / (1 + q)) ** steps)) <= 1e-12
+
+
+# ---- cluster-split kernels (rows of a tile over two CTAs, carries through distributed shared memory) ----
+
+@pytest.mark.parametrize("n", [1024, 1000, 600, 544])
+@pytest.mark.parametrize("batch", [4096 + 32, 64, 2048 * 9])
+def test_cluster_split_equals_single_cta(lib, n, batch):
+    """17..32 partitions: plain solves run on clusters of two CTAs; same arithmetic, so bitwise equal to the
+    single-CTA kernels (btps_tune cluster = 1 forces the pair, 0 forbids it), for single solves and fused steps, and within tolerance of the oracle."""
+    lt, lp = rand_tri(n, n), rand_penta(n, n + 1)
+    rhs = inputs.uniform_rhs(n, batch, seed=51)
+    outs = {}
+    for cl in (1, 0):
+        try:
+            lib.btps_tune("cluster", cl)
+            ht, hp = lib.tri_factor(*lt), lib.penta_factor(*lp)
+            a, b_, c, d = dev(rhs), dev(rhs), dev(rhs), dev(rhs)
+            lib.tri_solve_batched(ht, a)
+            lib.penta_solve_batched(hp, b_)
+            lib.tri_solve_steps(ht, c, 11)
+            lib.penta_solve_steps(hp, d, 11)
+            f32 = dev(rhs.astype(np.float32))
+            lib.penta_solve_batched_f32(hp, f32)
+            outs[cl] = [x.cpu().numpy() for x in (a, b_, c, d, f32)]
+        finally:
+            lib.btps_tune("cluster", -1)
+    for x, y in zip(outs[1], outs[0]):
+        assert np.array_equal(x, y)
+    ref = rhs.copy()
+    oracle.tri_solve_interleaved(oracle.tri_factor(*lt), ref)
+    assert rel_err(outs[1][0], ref) <= TOL_SINGLE
+    ref = rhs.copy()
+    oracle.penta_solve_interleaved(oracle.penta_factor(*lp), ref)
+    assert rel_err(outs[1][1], ref) <= TOL_SINGLE
+    assert rel_err(outs[1][4].astype(np.float64), ref) <= TOL_F32
+    ref = rhs.copy()
+    oracle.penta_solve_interleaved(oracle.penta_factor(*lp), ref, nsteps=11)
+    assert rel_err(outs[1][3], ref) <= TOL_STEPS
