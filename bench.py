@@ -38,8 +38,8 @@ UNIT = "systems/s"
 L2_BYTES = 126 * 1024 * 1024
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full`
-# capture (profiles/r01c_ncu_full_summary.md), keyed by kernel.
-NCU_TRAFFIC_BYTES = {"tri": 268508160 + 209617408, "penta": 268541440 + 210829056, "ch": 268547840 + 209697536}
+# capture (profiles/r01d_ncu_full_summary.md), keyed by kernel.
+NCU_TRAFFIC_BYTES = {"tri": 268508416 + 210129664, "penta": 268596736 + 211245568, "ch": 268558336 + 211021056}
 
 
 def parse_args():
