@@ -834,3 +834,39 @@ def test_cluster_split_equals_single_cta(lib, n, batch):
     ref = rhs.copy()
     oracle.penta_solve_interleaved(oracle.penta_factor(*lp), ref, nsteps=11)
     assert rel_err(outs[1][3], ref) <= TOL_STEPS
+
+
+# ---- CUDA graph capture of a time-step loop ------------------------------------------------------------
+
+def test_time_loop_in_a_cuda_graph(lib):
+    """The calls only enqueue kernels on the caller's stream (no allocation, no host sync), so a whole
+    time-stepping loop can be captured once and replayed (launch-bound small problems)."""
+    n, batch, steps = 64, 1024, 24
+    sg, al = inputs.ch_params(256)
+    st = ([sg] * n, [-4 * sg] * n, [1 + 6 * sg] * n, [-4 * sg] * n, [sg] * n)
+    ht = lib.tri_factor(*inputs.tri_lhs(n, 0.5))
+    hp = lib.penta_factor_periodic(*st)
+    u0 = torch.from_numpy(inputs.uniform_rhs(n, batch, seed=61)).cuda()
+    c0 = 0.1 * u0
+    # eager reference (also warms up: first launches resolve occupancy outside the capture)
+    ue, ce = u0.clone(), c0.clone()
+    lib.tri_solve_steps(ht, ue, steps)
+    lib.ch_step_batched(hp, ce, al, steps)
+    ug, cg = u0.clone(), c0.clone()
+    g = torch.cuda.CUDAGraph()
+    s = torch.cuda.Stream()
+    s.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(s):
+        with torch.cuda.graph(g, stream=s):
+            lib.tri_solve_steps(ht, ug, steps, stream=s.cuda_stream)
+            lib.ch_step_batched(hp, cg, al, steps, stream=s.cuda_stream)
+    torch.cuda.current_stream().wait_stream(s)
+    ug.copy_(u0)
+    cg.copy_(c0)
+    g.replay()
+    torch.cuda.synchronize()
+    assert torch.equal(ug, ue) and torch.equal(cg, ce)
+    g.replay()   # second replay advances the state by another `steps`
+    torch.cuda.synchronize()
+    lib.tri_solve_steps(ht, ue, steps)
+    assert torch.equal(ug, ue)
