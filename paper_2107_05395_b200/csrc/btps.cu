@@ -63,7 +63,7 @@ Tune g_tune;
 struct KernelSlot {
     SweepEntry ent = {nullptr, nullptr, 0};
     SweepEntry fused = {nullptr, nullptr, 0};  // multi-step form of the same variant (TMA variants)
-    int fused_ready = 0;
+    int prefer_fused = 0;  // the fused instantiation spills less than the single-step one: use it for one step too
     int vec = 1;
     int tma = 0;       // 1: the TMA-prefetch variant (needs the ring in shared memory)
     int xvals = 2;     // exchange values per (partition, system)
@@ -689,6 +689,14 @@ int resolve_slot(Handle *h, const Shape &sh, KernelSlot &sl, bool cluster = fals
         CU_TRY(cudaFuncSetAttribute(sl.ent.func, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sl.smem));
     if (sl.fused.func && sl.smem > 48 * 1024)
         CU_TRY(cudaFuncSetAttribute(sl.fused.func, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sl.smem));
+    if (sl.fused.func) {
+        // both instantiations do the same arithmetic for one step; ptxas sometimes spills tile rows in one and not
+        // in the other (255-register variants), so take the one with the smaller local-memory frame
+        cudaFuncAttributes fa, fb;
+        CU_TRY(cudaFuncGetAttributes(&fa, sl.ent.func));
+        CU_TRY(cudaFuncGetAttributes(&fb, sl.fused.func));
+        sl.prefer_fused = (fb.localSizeBytes < fa.localSizeBytes) ? 1 : 0;
+    }
     int occ = 0, sms = 0, dev = 0;
     CU_TRY(cudaGetDevice(&dev));
     CU_TRY(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
@@ -896,7 +904,7 @@ int launch_one(Handle *h, int kind, T *d_rhs, long long batch, double alpha_x, i
     // several steps per launch need the fused instantiation; without one (direct-load variants)
     // the steps are launched one by one
     // (the statistic of eq. 30 is computed inside the fused kernels; elsewhere by a pass of its own)
-    const bool fused = (ksteps > 1 || stat) && sl.fused.func;
+    const bool fused = (ksteps > 1 || stat || sl.prefer_fused) && sl.fused.func;
     const int nlaunch = fused ? 1 : ksteps;
     a.ksteps = fused ? ksteps : 1;
     a.stat = fused ? stat : nullptr;
