@@ -208,7 +208,8 @@ BTPS_API int btps_plan_info(int kind, const void *handle, int elem_bytes, int *o
  * (0: never use the TMA prefetch variant), "warp_scan" (0: serial carry walk), "pdl" (0: no
  * programmatic dependent launch attribute), "fuse_steps" (time steps advanced per launch while a tile
  * is on chip in *_solve_steps / ch_step_batched: default 8, 1 = one launch per step), "grid" (cap on
- * the number of CTAs), "cluster" (1: run every eligible plain solve of 17..32 partitions on clusters of two CTAs
+ * the number of CTAs), "cyclic_in_scan" (0: periodic pentadiagonal handles apply the cyclic correction row by row
+ * instead of folding it into the carry scan), "cluster" (1: run every eligible plain solve of 17..32 partitions on clusters of two CTAs
  * that split the rows of a tile, 0: never; default: tridiagonal fp64 batches of >= 2^18 systems), "reverse"
  * (0/1: alternate the tile order on successive steps of *_solve_steps / ch_step_batched so a
  * step starts on the data the previous one left in L2).  value < 0 restores the default. */

@@ -20,7 +20,8 @@ LIB = os.path.join(HERE, "libbtps.so")
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC,-fvisibility=hidden"]
 UNITS = ["btps.cu"] + [f"inst_{k}_{t}.cu" for k in ("tri", "penta", "ch", "trip", "pentap", "chp") for t in ("f64", "f32")] + \
-        ["inst_tricn_f64.cu", "inst_tricnp_f64.cu", "inst_pentacn_f64.cu", "inst_pentacnp_f64.cu"]
+        ["inst_tricn_f64.cu", "inst_tricnp_f64.cu", "inst_pentacn_f64.cu", "inst_pentacnp_f64.cu",
+         "inst_pentapf_f64.cu", "inst_pentapf_f32.cu", "inst_chpf_f64.cu", "inst_pentacnpf_f64.cu"]
 HEADERS = ["sweep.cuh", "inst_common.cuh", os.path.join(ROOT, "include", "btps.h")]
 
 

@@ -53,7 +53,7 @@ std::atomic<long long> g_launches{0};
 // ------------------------------------------------------------------------------------------------
 struct Tune {
     int rows = -1, lanes = -1, vec = -1, tpc = -1, force_two_pass = -1, reverse = -1, prefetch = -1, pdl = -1,
-        warp_scan = -1, grid = -1, fuse = -1, cluster = -1;
+        warp_scan = -1, grid = -1, fuse = -1, cluster = -1, cyclic_scan = -1;
 };
 Tune g_tune;
 
@@ -84,6 +84,7 @@ struct DtypePlan {
     int rows = 0, P = 0;
     Shape shape[3];     // [0] solve, [1] fused CH step (penta) / CN diffusion step (tri), [2] CN hyperdiffusion step (penta)
     int ws = 0;         // carries by the warp-shuffle scan
+    int wfast = 0;      // periodic penta handle: the cyclic correction is folded into the scan (KIND_*F kernels)
     int scan_log2 = 0;  // log2 of the scan width
     int tq = 32;        // partitions per scan-table row
     bool two_pass = false;
@@ -108,6 +109,7 @@ struct Handle {
     bool periodic = false;                    // tri: cyclic matrix solved by Sherman-Morrison (KIND_TRIP kernels)
     double per_vN = 0.0, per_invden = 0.0;    // eq. 13a / 15 scalars of the periodic solve
     PerPenta pp = {};                         // periodic penta: Woodbury scalars (H, wrap-around entries)
+    double per_ngl = 0.0;                     // periodic penta: -gamma at row n-2
     int n;
     int device;
     DtypePlan plan[2];  // 0: fp64, 1: fp32
@@ -338,7 +340,8 @@ void put_scan_tables(std::vector<unsigned char> &blob, const DtypePlan &pl, int 
 
 size_t scan_table_bytes(const DtypePlan &pl, int nc, size_t elem)
 {
-    const int slots = pl.ws ? 2 * SCAN_STEPS : 2;  // ws: 8 step slots + merged step 4 + chi
+    int slots = pl.ws ? 2 * SCAN_STEPS : 2;  // ws: 8 step slots + merged step 4 + chi
+    if (pl.wfast) slots += 4;                // GZ (slots 10-11) and XZ (12-13): carries of A' z = e_r
     return (size_t)slots * nc * nc * pl.tq * elem;
 }
 
@@ -398,8 +401,10 @@ void build_blob_penta(int n, DtypePlan &pl, const std::vector<double> &inv, cons
                       const std::vector<double> *Z = nullptr)
 {
     const int MR = pl.rows, P = pl.P, Np = P * MR;
-    // coefficient values per row: the periodic form carries the rows of Z = A'^{-1} U (n x 4, row-major)
-    const int RT = Z ? RecLayout<KIND_PENTAP>::ELEMS : RecLayout<KIND_PENTA>::ELEMS;
+    // coefficient values per row: the periodic form carries the rows of Z = A'^{-1} U (n x 4, row-major), or, with the
+    // cyclic correction folded into the scan, the local solves of the unit vectors in the two end partitions
+    const int RT = Z ? (pl.wfast ? RecLayout<KIND_PENTAPF>::ELEMS : RecLayout<KIND_PENTAP>::ELEMS)
+                     : RecLayout<KIND_PENTA>::ELEMS;
     auto at = [&](const std::vector<double> &v, int i, double pad) { return i < n ? v[i] : pad; };
     pl.offT = (unsigned)align16((size_t)Np * RT * sizeof(T));
     pl.blob_bytes = (unsigned)align16(pl.offT + scan_table_bytes(pl, 2, sizeof(T)));
@@ -452,7 +457,7 @@ void build_blob_penta(int n, DtypePlan &pl, const std::vector<double> &inv, cons
             putv(5, i, 1, chi[1][k]);
             putv(7, i, 0, psi[0][k]);
             putv(7, i, 1, psi[1][k]);
-            if (Z)
+            if (Z && !pl.wfast)
                 for (int m = 0; m < 4; ++m) putv(m < 2 ? 9 : 11, i, m & 1, i < n ? (*Z)[(size_t)i * 4 + m] : 0.0);
         }
         // carries: (g at the last row, g at the last-but-one row) forward; (x at the first row, x at
@@ -471,6 +476,39 @@ void build_blob_penta(int n, DtypePlan &pl, const std::vector<double> &inv, cons
         Chi0[p].m[3] = chi[1][1];
     }
     put_scan_tables<T>(blob, pl, 2, Phi, Psi, Chi0);
+    if (Z && pl.wfast) {
+        // Column m of Z solves A' z = e_r, r = (0, 1, n-2, n-1)[m].  In the partitioned form it is "local solve + chi GZ +
+        // psi XZ": GZ_p = (g at the last two rows of partition p-1), XZ_p = (z at the first two rows of partition p+1), and
+        // the local (zero-carry) solve is nonzero only in the partition that holds row r (n = P*MR: partition 0 or P-1).
+        const int tq = pl.tq;
+        const int urow[4] = {0, 1, n - 2, n - 1};
+        std::vector<double> g(n), loc(MR);
+        for (int m = 0; m < 4; ++m) {
+            for (int i = 0; i < n; ++i) {  // forward sweep of e_r with the sweep multipliers
+                const double r = (i == urow[m]) ? 1.0 : 0.0;
+                g[i] = inv[i] * r + (i >= 2 ? nle[i] * g[i - 2] : 0.0) + (i >= 1 ? nlb[i] * g[i - 1] : 0.0);
+            }
+            for (int p = 0; p < P; ++p) {
+                const double gz[2] = {p > 0 ? g[p * MR - 1] : 0.0, p > 0 ? g[p * MR - 2] : 0.0};
+                const double xz[2] = {p + 1 < P ? (*Z)[(size_t)((p + 1) * MR) * 4 + m] : 0.0,
+                                      p + 1 < P ? (*Z)[(size_t)((p + 1) * MR + 1) * 4 + m] : 0.0};
+                for (int c = 0; c < 2; ++c) {
+                    put<T>(blob, pl.offT + ((size_t)(40 + c * 4 + m) * tq + p) * sizeof(T), gz[c]);
+                    put<T>(blob, pl.offT + ((size_t)(48 + c * 4 + m) * tq + p) * sizeof(T), xz[c]);
+                }
+            }
+            // local solve in the end partition that holds row r
+            const int p = (m < 2) ? 0 : P - 1, r0 = p * MR;
+            for (int k = 0; k < MR; ++k) {
+                const int i = r0 + k;
+                const double r = (i == urow[m]) ? 1.0 : 0.0;
+                loc[k] = inv[i] * r + (k >= 2 ? nle[i] * loc[k - 2] : 0.0) + (k >= 1 ? nlb[i] * loc[k - 1] : 0.0);
+            }
+            for (int k = MR - 2; k >= 0; --k)
+                loc[k] = loc[k] + ngam[r0 + k] * loc[k + 1] + (k + 2 < MR ? ndel[r0 + k] * loc[k + 2] : 0.0);
+            for (int k = 0; k < MR; ++k) putv(9, r0 + k, m & 1, loc[k]);
+        }
+    }
 }
 
 template <typename T>
@@ -512,12 +550,13 @@ void layout_slot(const DtypePlan &pl, const Shape &sh, int kind, KernelSlot &sl,
     const bool tri = (kind == KIND_TRI || kind == KIND_TRIP || kind == KIND_TRICN || kind == KIND_TRICNP);
     const int NC = tri ? 1 : 2;
     // kinds with an explicit half need one halo row on each side between fused steps
-    const bool cn5 = (kind == KIND_PENTACN || kind == KIND_PENTACNP);  // two halo rows on each side
-    const bool is_ch = (kind == KIND_CH || kind == KIND_CHP || kind == KIND_TRICN || kind == KIND_TRICNP || cn5);
+    const bool cn5 = (kind == KIND_PENTACN || kind == KIND_PENTACNP || kind == KIND_PENTACNPF);  // two halo rows on each side
+    const bool is_ch = (kind == KIND_CH || kind == KIND_CHP || kind == KIND_CHPF || kind == KIND_TRICN || kind == KIND_TRICNP || cn5);
     const bool wood = (kind == KIND_PENTAP || kind == KIND_CHP || kind == KIND_PENTACNP), pert = (kind == KIND_TRIP || kind == KIND_TRICNP);
+    const bool woodf = (kind == KIND_PENTAPF || kind == KIND_CHPF || kind == KIND_PENTACNPF);  // + 2 values: nw for the end partitions
     const size_t W = (size_t)sh.lanes * sl.vec;
     // CH: + the halo rows exchanged between fused steps; periodic tri: + y_1 and y_N of eq. 15
-    sl.xvals = 2 * NC + ((is_ch && halo) ? (cn5 ? 4 : 2) : 0) + (pert ? 2 : 0);
+    sl.xvals = 2 * NC + ((is_ch && halo) ? (cn5 ? 4 : 2) : 0) + (pert ? 2 : 0) + (woodf ? 2 : 0);
     sl.xper = (int)(sl.xvals * pl.P * W);
     sl.xstride = sl.xper + (wood ? (int)(4 * W) : 0);  // cyclic penta: y at rows 0, 1, n-2, n-1
     const size_t xch = (pl.P > 1) ? (size_t)sh.tpc * sl.xstride * pl.elem : 0;
@@ -554,12 +593,17 @@ SweepEntry find_sweep(int kind, int elem_bytes, int vec, int rows, int single, i
         if (kind == KIND_TRICNP) return find_sweep_tricnp_f64(vec, rows, single, tma, ws, fuse);
         if (kind == KIND_PENTACN) return find_sweep_pentacn_f64(vec, rows, single, tma, ws, fuse);
         if (kind == KIND_PENTACNP) return find_sweep_pentacnp_f64(vec, rows, single, tma, ws, fuse);
+        if (kind == KIND_PENTAPF) return find_sweep_pentapf_f64(vec, rows, single, tma, ws, fuse);
+        if (kind == KIND_CHPF) return find_sweep_chpf_f64(vec, rows, single, tma, ws, fuse);
+        if (kind == KIND_PENTACNPF) return find_sweep_pentacnpf_f64(vec, rows, single, tma, ws, fuse);
         if (kind == KIND_PENTA) return find_sweep_penta_f64(vec, rows, single, tma, ws, fuse);
         return find_sweep_ch_f64(vec, rows, single, tma, ws, fuse);
     }
     if (kind == KIND_TRI) return find_sweep_tri_f32(vec, rows, single, tma, ws, fuse);
     if (kind == KIND_TRIP) return find_sweep_trip_f32(vec, rows, single, tma, ws, fuse);
     if (kind == KIND_PENTAP) return find_sweep_pentap_f32(vec, rows, single, tma, ws, fuse);
+    if (kind == KIND_PENTAPF) return find_sweep_pentapf_f32(vec, rows, single, tma, ws, fuse);
+    if (kind == KIND_CHPF || kind == KIND_PENTACNPF) return SweepEntry{nullptr, nullptr, 0};
     if (kind == KIND_CHP) return find_sweep_chp_f32(vec, rows, single, tma, ws, fuse);
     if (kind == KIND_TRICN || kind == KIND_TRICNP || kind == KIND_PENTACN || kind == KIND_PENTACNP)
         return SweepEntry{nullptr, nullptr, 0};  // the Crank-Nicolson steps are fp64 only
@@ -648,6 +692,7 @@ void fill_slots(Handle *h)
                                  : (ks == 1 ? (h->periodic ? KIND_CHP : KIND_CH) : (h->periodic ? KIND_PENTACNP : KIND_PENTACN));
                 if (ks == 2 && pl.elem != 8) continue;
                 if (kind == KIND_PENTACNP && (pl.P < 2 || pl.P * pl.rows != h->n)) continue;
+                if (pl.wfast) kind = (ks == 0) ? KIND_PENTAPF : (ks == 1 ? KIND_CHPF : KIND_PENTACNPF);
                 // the periodic CH kernels need whole partitions and at least two of them (halo wrap);
                 // other sizes run the two-pass form
                 if (kind == KIND_CHP && (pl.P < 2 || pl.P * pl.rows != h->n)) continue;
@@ -664,7 +709,7 @@ void fill_slots(Handle *h)
                     layout_slot(pl, sh, kind, sl);
                     bool can_fuse = true;
                     if (sl.smem > SMEM_LIMIT && (kind == KIND_CH || kind == KIND_CHP || kind == KIND_TRICN || kind == KIND_TRICNP || kind == KIND_PENTACN ||
-                                                kind == KIND_PENTACNP)) {
+                                                kind == KIND_PENTACNP) && !pl.wfast) {
                         // tight fit (N = 1024 fp64): drop the halo exchange rows, one step per launch
                         layout_slot(pl, sh, kind, sl, false);
                         can_fuse = false;
@@ -870,6 +915,7 @@ int launch_one(Handle *h, int kind, T *d_rhs, long long batch, double alpha_x, i
             a.wrow_k[i] = wr[i] % pl.rows;
         }
     }
+    a.per_ngl = h->per_ngl;
     a.xstride = sl.xstride;
     a.xper = sl.xper;
     a.n = h->n;
@@ -1147,6 +1193,7 @@ static penta_handle_t make_penta_handle(int n, const std::vector<double> &inv, c
     h->kind = KIND_PENTA;
     h->periodic = (Z != nullptr);
     if (pp) h->pp = *pp;
+    h->per_ngl = (Z && n >= 2) ? ngam[n - 2] : 0.0;
     h->n = n;
     h->device = 0;
     std::vector<double> zc[4];
@@ -1161,6 +1208,8 @@ static penta_handle_t make_penta_handle(int n, const std::vector<double> &inv, c
     for (int t = 0; t < 2; ++t) {
         DtypePlan &pl = h->plan[t];
         choose_plan(n, t == 0 ? 8 : 4, h->kind, pl);
+        // periodic: fold the cyclic correction into the carry scan when the partitions are whole (n = P*32, P >= 2)
+        pl.wfast = (Z && pl.ws && pl.rows == 32 && pl.P >= 2 && pl.P * pl.rows == n && g_tune.cyclic_scan != 0) ? 1 : 0;
         std::vector<unsigned char> blob, soa;
         if (t == 0) {
             build_blob_penta<double>(n, pl, inv, nle, nlb, ngam, ndel, blob, Z);
@@ -1397,6 +1446,7 @@ int btps_tune(const char *key, int value)
     else if (!strcmp(key, "grid")) g_tune.grid = value;
     else if (!strcmp(key, "fuse_steps")) g_tune.fuse = value;
     else if (!strcmp(key, "cluster")) g_tune.cluster = value;
+    else if (!strcmp(key, "cyclic_in_scan")) g_tune.cyclic_scan = value;
     else return set_err(BTPS_E_ARG);
     return set_err(BTPS_OK);
 }

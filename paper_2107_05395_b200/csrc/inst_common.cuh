@@ -15,11 +15,27 @@ static SweepEntry make_entry()
     return e;
 }
 
+template <typename T, int V, int MR, int KIND>
+static SweepEntry pick_variant_general(int single, int tma, int ws, int fuse);
+
 // variants: single partition (no carries) with / without TMA; partitioned with the warp scan
 // (with / without TMA) or with the serial carry walk (direct loads only); the fused multi-step
 // form exists for the TMA variants
 template <typename T, int V, int MR, int KIND>
 static SweepEntry pick_variant(int single, int tma, int ws, int fuse)
+{
+    if constexpr (RecLayout<KIND>::WOODF) {
+        // cyclic correction folded into the warp scan: partitioned, warp-scan variants only
+        if (single || !ws) return SweepEntry{nullptr, nullptr, 0};
+        if (fuse) return tma ? make_entry<T, V, MR, false, KIND, true, true, true>() : SweepEntry{nullptr, nullptr, 0};
+        return tma ? make_entry<T, V, MR, false, KIND, true, true>() : make_entry<T, V, MR, false, KIND, false, true>();
+    } else {
+        return pick_variant_general<T, V, MR, KIND>(single, tma, ws, fuse);
+    }
+}
+
+template <typename T, int V, int MR, int KIND>
+static SweepEntry pick_variant_general(int single, int tma, int ws, int fuse)
 {
     if (fuse) {
         if (!tma) return SweepEntry{nullptr, nullptr, 0};
@@ -101,5 +117,9 @@ SweepEntry find_sweep_tricn_f64(int vec, int rows, int single, int tma, int ws, 
 SweepEntry find_sweep_tricnp_f64(int vec, int rows, int single, int tma, int ws, int fuse);
 SweepEntry find_sweep_pentacn_f64(int vec, int rows, int single, int tma, int ws, int fuse);
 SweepEntry find_sweep_pentacnp_f64(int vec, int rows, int single, int tma, int ws, int fuse);
+SweepEntry find_sweep_pentapf_f64(int vec, int rows, int single, int tma, int ws, int fuse);
+SweepEntry find_sweep_pentapf_f32(int vec, int rows, int single, int tma, int ws, int fuse);
+SweepEntry find_sweep_chpf_f64(int vec, int rows, int single, int tma, int ws, int fuse);
+SweepEntry find_sweep_pentacnpf_f64(int vec, int rows, int single, int tma, int ws, int fuse);
 
 }  // namespace btps

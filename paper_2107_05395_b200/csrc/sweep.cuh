@@ -40,7 +40,9 @@ namespace btps {
 // TRICN / TRICNP: Crank-Nicolson step (explicit three-point half + tri solve), truncated / periodic
 enum Kind {
     KIND_TRI = 0, KIND_PENTA = 1, KIND_CH = 2, KIND_TRIP = 3, KIND_PENTAP = 4, KIND_CHP = 5, KIND_TRICN = 6, KIND_TRICNP = 7,
-    KIND_PENTACN = 8, KIND_PENTACNP = 9  // Crank-Nicolson hyperdiffusion step (explicit five-point half + penta solve)
+    KIND_PENTACN = 8, KIND_PENTACNP = 9,  // Crank-Nicolson hyperdiffusion step (explicit five-point half + penta solve)
+    // PENTAP / CHP / PENTACNP with the cyclic correction folded into the carry scan (whole partitions, P >= 2)
+    KIND_PENTAPF = 10, KIND_CHPF = 11, KIND_PENTACNPF = 12
 };
 
 constexpr int SCAN_STEPS = 5;   // Kogge-Stone steps held in the tables (scan width <= 32)
@@ -61,6 +63,7 @@ struct SweepArgs {
     int wrow_part[4], wrow_k[4];  // periodic penta: partition / local row of rows 0, 1, n-2, n-1
     int xstride;           // elements of exchange area per group
     int xper;              // element offset (inside a group's area) of the 4 x W periodic-penta values
+    double per_ngl;        // periodic penta, correction in the scan: -gamma at row n-2
     double *stat;          // CH, fused kernels: device array, stat[ks] += stat_scale * sum over this launch's runs of
                            // 1 / (1 - <C^2>) after step ks (eq. 30); nullptr: no statistic
     double stat_scale;     // 1 / batch
@@ -135,6 +138,9 @@ __device__ __forceinline__ T ch_w(T c) { return fma_t<T>(c * c, c, -c); }
 //           sweeps to the incoming forward / backward carry
 //   periodic tri (6 MR): as tri, plus 5: z = A'^{-1} u of the Sherman-Morrison splitting
 //   periodic penta (13 MR): as penta, plus 9: {z0, z1}  11: {z2, z3}, the rows of Z = A'^{-1} U (Woodbury)
+//   periodic penta, correction in the scan (11 MR): as penta, plus 9: {zl0, zl1}, the local (zero-carry) solves of the
+//           unit vectors at rows 0, 1 (first partition) / n-2, n-1 (last partition), zero elsewhere; scan table slots
+//           10-11: GZ_q, 12-13: XZ_q (2 x 4 each): the carries of A' z = e_r for r = 0, 1, n-2, n-1
 //   penta (9 MR): 0: {inv, nle}  2: nlb    3: {ngam, ndel}   5: {chi1, chi2}   7: {psi1, psi2}
 //           inv = 1/alpha_i, nle = -eps_i/alpha_i, nlb = -beta_i/alpha_i, ngam = -gamma_i, ndel = -delta_i
 // followed at offT by the carry-scan tables, indexed [slot][m][q] with q = partition (tq entries),
@@ -153,7 +159,9 @@ struct RecLayout {
     static constexpr bool TRI = (KIND == KIND_TRI || KIND == KIND_TRIP || KIND == KIND_TRICN || KIND == KIND_TRICNP);
     static constexpr bool PERT = (KIND == KIND_TRIP || KIND == KIND_TRICNP);  // Sherman-Morrison finish
     static constexpr bool WOOD = (KIND == KIND_PENTAP || KIND == KIND_CHP || KIND == KIND_PENTACNP);  // rank-4 Woodbury correction
-    static constexpr int ELEMS = TRI ? (PERT ? 6 : 5) : (WOOD ? 13 : 9);  // values per row
+    // the same correction folded into the carries
+    static constexpr bool WOODF = (KIND == KIND_PENTAPF || KIND == KIND_CHPF || KIND == KIND_PENTACNPF);
+    static constexpr int ELEMS = TRI ? (PERT ? 6 : 5) : (WOOD ? 13 : (WOODF ? 11 : 9));  // values per row
     static constexpr int NC = TRI ? 1 : 2;                     // carries per direction
 };
 
@@ -271,13 +279,15 @@ __global__ void __launch_bounds__(CtaShape<T, V, MR>::MAX_THREADS, 1)
 sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
 {
     constexpr bool TRI = RecLayout<KIND>::TRI;
-    constexpr bool ISCH = (KIND == KIND_CH || KIND == KIND_CHP);  // explicit Cahn-Hilliard half fused in
+    constexpr bool ISCH = (KIND == KIND_CH || KIND == KIND_CHP || KIND == KIND_CHPF);  // explicit Cahn-Hilliard half fused in
     constexpr bool ISCN = (KIND == KIND_TRICN || KIND == KIND_TRICNP);  // explicit three-point half (eq. 9) fused in
-    constexpr bool ISCN5 = (KIND == KIND_PENTACN || KIND == KIND_PENTACNP);  // explicit five-point half (eq. 18)
+    constexpr bool ISCN5 = (KIND == KIND_PENTACN || KIND == KIND_PENTACNP || KIND == KIND_PENTACNPF);  // explicit five-point half (eq. 18)
     constexpr bool HALO2 = ISCN5;                                 // needs two rows on each side
     constexpr bool HALO1 = ISCH || ISCN || HALO2;                 // needs the rows r0-1 and r0+MR
     constexpr int NHALO = HALO2 ? 4 : (HALO1 ? 2 : 0);            // exchange values for the fused steps' halos
-    constexpr bool WRAP = (KIND == KIND_CHP || KIND == KIND_TRICNP || KIND == KIND_PENTACNP);  // periodic differences
+    constexpr bool WRAP = (KIND == KIND_CHP || KIND == KIND_TRICNP || KIND == KIND_PENTACNP || KIND == KIND_CHPF ||
+                           KIND == KIND_PENTACNPF);  // periodic differences
+    constexpr bool WOODF = RecLayout<KIND>::WOODF;
     constexpr bool PERT = RecLayout<KIND>::PERT;
     constexpr bool WOOD = RecLayout<KIND>::WOOD;
     constexpr int NC = RecLayout<KIND>::NC;
@@ -704,6 +714,16 @@ sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
                                 }
                             }
                         });
+                        [[maybe_unused]] T yn1[V], yn2[V];  // cyclic penta: y at rows n-1, n-2 (true g at the last rows)
+                        if constexpr (WOODF) {
+#pragma unroll
+                            for (int e = 0; e < V; ++e) {
+                                const T i0 = __shfl_sync(0xffffffffu, fb[0][e], P - 1, wd);
+                                const T i1 = __shfl_sync(0xffffffffu, fb[1][e], P - 1, wd);
+                                yn1[e] = i0;                                  // x_{n-1} = g_{n-1}
+                                yn2[e] = fma_t<T>((T)a.per_ngl, i0, i1);      // x_{n-2} = g_{n-2} - gamma_{n-2} x_{n-1}
+                            }
+                        }
                         {
                             // carry INTO partition q = inclusive result of partition q-1; then the local
                             // back-substitution's first rows given that carry: u = x^_first + chi G
@@ -742,14 +762,46 @@ sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
                                 }
                             }
                         });
+                        // Cyclic correction in the scan: x = y - Z w with w = H V^T y.  Column m of Z = A'^{-1} e_r is
+                        // itself "local solve + chi GZ^m + psi XZ^m", so -Z w only shifts the carries,
+                        // G_q += GZ_q nw, X_q += XZ_q nw (nw = -w), plus the local solves in the two end partitions.
+                        [[maybe_unused]] T nw[4][V];
+                        if constexpr (WOODF) {
+#pragma unroll
+                            for (int e = 0; e < V; ++e) {
+                                const T y0 = __shfl_sync(0xffffffffu, bb[0][e], 0, wd);  // true x at rows 0, 1
+                                const T y1 = __shfl_sync(0xffffffffu, bb[1][e], 0, wd);
+                                const T t0 = fma_t<T>((T)a.per_w6[1], yn1[e], (T)a.per_w6[0] * yn2[e]);
+                                const T t1 = (T)a.per_w6[2] * yn1[e];
+                                const T t2 = (T)a.per_w6[3] * y0;
+                                const T t3 = fma_t<T>((T)a.per_w6[5], y1, (T)a.per_w6[4] * y0);
+#pragma unroll
+                                for (int m = 0; m < 4; ++m)
+                                    nw[m][e] = -fma_t<T>((T)a.per_H[m * 4 + 3], t3, fma_t<T>((T)a.per_H[m * 4 + 2], t2,
+                                                          fma_t<T>((T)a.per_H[m * 4 + 1], t1, (T)a.per_H[m * 4] * t0)));
+                            }
+                        }
 #pragma unroll
                         for (int c = 0; c < NC; ++c)
 #pragma unroll
                             for (int e = 0; e < V; ++e) {
-                                const T x = __shfl_down_sync(0xffffffffu, bb[c][e], 1, wd);
+                                T x = __shfl_down_sync(0xffffffffu, bb[c][e], 1, wd);
                                 const int ix = (sg * V + e) ^ qsw;
+                                x = (q + 1 < P) ? x : T(0);
+                                if constexpr (WOODF) {
+                                    const T *const gz = tb + (40 + c * 4) * mstr;  // slots 10-11: GZ_q, row c
+                                    const T *const xz = tb + (48 + c * 4) * mstr;  // slots 12-13: XZ_q, row c
+#pragma unroll
+                                    for (int m = 0; m < 4; ++m) {
+                                        fb[c][e] = fma_t<T>(gz[m * mstr], nw[m][e], fb[c][e]);
+                                        x = fma_t<T>(xz[m * mstr], nw[m][e], x);
+                                    }
+                                    // the end partitions also need nw itself: (nw0, nw1) for partition 0, (nw2, nw3) for P-1
+                                    if (ok && (q == 0 || q == P - 1))
+                                        xs[(2 * NC + NHALO + c) * vstr + ix] = nw[(q == 0 ? 0 : 2) + c][e];
+                                }
                                 if (ok) {
-                                    const T xv = (q + 1 < P) ? x : T(0);
+                                    const T xv = x;
                                     if (!CL || (q >= PL) == (crank != 0u)) {
                                         xs[c * vstr + ix] = fb[c][e];
                                         xs[(NC + c) * vstr + ix] = xv;
@@ -853,6 +905,23 @@ sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
                         x = fma_t<T>(G[1][e], cc.v[1], x);
                         x = fma_t<T>(X[0][e], cs.v[0], x);
                         v[k][e] = fma_t<T>(X[1][e], cs.v[1], x);
+                    }
+                }
+            }
+            if constexpr (WOODF) {
+                if (part == 0 || part == P - 1) {  // local solves of the unit vectors at the system's ends
+                    T wl0[V], wl1[V];
+#pragma unroll
+                    for (int e = 0; e < V; ++e) {
+                        wl0[e] = xc[(2 * NC + NHALO) * vstr + XI(e)];
+                        wl1[e] = xc[(2 * NC + NHALO + 1) * vstr + XI(e)];
+                    }
+                    const Pair *const RZL = reinterpret_cast<const Pair *>(cb + 9 * MR);
+#pragma unroll
+                    for (int k = 0; k < MR; ++k) {
+                        const Pair zl = RZL[k];
+#pragma unroll
+                        for (int e = 0; e < V; ++e) v[k][e] = fma_t<T>(wl1[e], zl.v[1], fma_t<T>(wl0[e], zl.v[0], v[k][e]));
                     }
                 }
             }

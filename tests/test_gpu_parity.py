@@ -870,3 +870,37 @@ def test_time_loop_in_a_cuda_graph(lib):
     torch.cuda.synchronize()
     lib.tri_solve_steps(ht, ue, steps)
     assert torch.equal(ug, ue)
+
+
+# ---- cyclic correction folded into the carry scan vs applied row by row ---------------------------------
+
+@pytest.mark.parametrize("n", [64, 256, 512, 1024])
+def test_cyclic_correction_in_scan_matches_rowwise(lib, n):
+    """Periodic penta handles with whole partitions fold x = y - Z H V^T y into the carries (KIND_*F kernels);
+    btps_tune('cyclic_in_scan', 0) applies it row by row.  Both must match the oracle; general (non-Toeplitz) LHS."""
+    batch = 2048 + 32
+    lhs = rand_cyclic_penta(n, n + 3)
+    sg, al = inputs.ch_params(256)
+    st = ([sg] * n, [-4 * sg] * n, [1 + 6 * sg] * n, [-4 * sg] * n, [sg] * n)
+    x5 = [-0.3, 1.2, 1 - 1.8, 1.2, -0.3]
+    rhs = inputs.uniform_rhs(n, batch, seed=71)
+    fo, fs = oracle.penta_periodic_factor(*lhs), oracle.penta_periodic_factor(*st)
+    r1 = rhs.copy(); oracle.penta_periodic_solve_interleaved(fo, r1)
+    r2 = 0.1 * rhs; oracle.ch_periodic_step_interleaved(fs, r2, al, nsteps=9)
+    r3 = rhs.copy(); oracle.penta_cn_step_interleaved(fs, r3, x5, nsteps=9)
+    for mode in (-1, 0):
+        try:
+            lib.btps_tune("cyclic_in_scan", mode)
+            h, hs = lib.penta_factor_periodic(*lhs), lib.penta_factor_periodic(*st)
+        finally:
+            lib.btps_tune("cyclic_in_scan", -1)
+        d1, d2, d3, d4 = dev(rhs), dev(0.1 * rhs), dev(rhs), dev(rhs.astype(np.float32))
+        lib.penta_solve_batched(h, d1)
+        lib.ch_step_batched(hs, d2, al, 9)
+        lib.penta_cn_step_batched(hs, d3, x5, 9)
+        lib.penta_solve_batched_f32(h, d4)
+        assert rel_err(d1.cpu().numpy(), r1) <= TOL_SINGLE, (mode, n)
+        assert rel_err(d2.cpu().numpy(), r2) <= TOL_STEPS, (mode, n)
+        assert rel_err(d3.cpu().numpy(), r3) <= TOL_STEPS, (mode, n)
+        assert rel_err(d4.cpu().numpy().astype(np.float64), r1) <= TOL_F32, (mode, n)
+        assert np.max(np.abs(d2.cpu().numpy().sum(axis=0) - (0.1 * rhs).sum(axis=0))) <= 1e-13
