@@ -942,7 +942,7 @@ int launch_one(Handle *h, int kind, T *d_rhs, long long batch, double alpha_x, i
         const int rc = make_tmap<T>(&tm, d_rhs, batch, h->n, (int)W, sl.box_rows);
         if (rc != BTPS_OK) return rc;
     }
-    long long grid = (a.num_tiles + sh.tpc - 1) / sh.tpc;
+    long long grid = a.num_tiles;  // one tile per CTA first (tile order is group-major), capped at the resident CTAs
     if (use_cl) grid = 2 * a.num_tiles;  // one cluster of two CTAs per tile in flight
     if (grid > sl.max_grid) grid = sl.max_grid;
     if (g_tune.grid > 0 && grid > g_tune.grid) grid = use_cl ? (g_tune.grid & ~1) : g_tune.grid;

@@ -374,7 +374,9 @@ sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
             tma_load_2d(dst + b * box_bytes, &tmap, tile * W, (int)(b * a.box_rows) + rbase, mbar);
     };
 
-    int t = CL ? (int)(blockIdx.x >> 1) : (int)(blockIdx.x * a.tpc + sub);
+    // group-major tile order: consecutive tiles go to different CTAs, so a small batch spreads over all SMs
+    // before any CTA runs a second group
+    int t = CL ? (int)(blockIdx.x >> 1) : (int)(blockIdx.x + sub * gridDim.x);
     [[maybe_unused]] unsigned phase = 0;
     if constexpr (TMA) {
         if (lt == 0 && t < ntiles) tma_issue(t);
