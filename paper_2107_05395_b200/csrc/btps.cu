@@ -341,14 +341,15 @@ void put_scan_tables(std::vector<unsigned char> &blob, const DtypePlan &pl, int 
 size_t scan_table_bytes(const DtypePlan &pl, int nc, size_t elem)
 {
     int slots = pl.ws ? 2 * SCAN_STEPS : 2;  // ws: 8 step slots + merged step 4 + chi
-    if (pl.wfast) slots += 4;                // GZ (slots 10-11) and XZ (12-13): carries of A' z = e_r
+    if (pl.wfast) slots += (nc == 2) ? 4 : 2;  // GZ / XZ: carries of A' z = e_r (penta: slots 10-13) or A' z = u (tri: 10, 11)
     return (size_t)slots * nc * nc * pl.tq * elem;
 }
 
 template <typename T>
 void build_blob_tri(int n, DtypePlan &pl, const std::vector<double> &inv, const std::vector<double> &nl,
                     const std::vector<double> &nch, std::vector<unsigned char> &blob,
-                    const std::vector<double> *z = nullptr)
+                    const std::vector<double> *z = nullptr, const std::vector<double> *zfwd = nullptr, double u0 = 0.0,
+                    double uN = 0.0)
 {
     const int MR = pl.rows, P = pl.P, Np = P * MR;
     // coefficient values per row: the periodic form carries z = A'^{-1} u as a sixth array
@@ -385,13 +386,36 @@ void build_blob_tri(int n, DtypePlan &pl, const std::vector<double> &inv, const 
             putv(2, i, 0, at(nch, i, 0.0));
             putv(3, i, 0, chi[k]);
             putv(3, i, 1, psi[k]);
-            if (z) put<T>(blob, ((size_t)(i / MR) * RT * MR + (size_t)5 * MR + (i % MR)) * sizeof(T), at(*z, i, 0.0));
+            if (z && !pl.wfast) put<T>(blob, ((size_t)(i / MR) * RT * MR + (size_t)5 * MR + (i % MR)) * sizeof(T), at(*z, i, 0.0));
         }
         Phi[p].m[0] = phi[MR - 1];
         Psi[p].m[0] = psi[0];
         Chi0[p].m[0] = chi[0];
     }
     put_scan_tables<T>(blob, pl, 1, Phi, Psi, Chi0);
+    if (z && pl.wfast) {
+        // z = A'^{-1} u in the partitioned form is "local solve + chi GZ + psi XZ": GZ_p = forward-sweep value of u at the last
+        // row of partition p-1, XZ_p = z at the first row of partition p+1; the local (zero-carry) solve of u is nonzero only
+        // in partition 0 (u_0 = -b_0 at row 0) and partition P-1 (u_{n-1} = c_{n-1} at row n-1); n = P*MR here.
+        const int tq = pl.tq;
+        for (int p = 0; p < P; ++p) {
+            put<T>(blob, pl.offT + ((size_t)10 * tq + p) * sizeof(T), p > 0 ? (*zfwd)[p * MR - 1] : 0.0);
+            put<T>(blob, pl.offT + ((size_t)11 * tq + p) * sizeof(T), p + 1 < P ? (*z)[(p + 1) * MR] : 0.0);
+        }
+        std::vector<double> loc(MR);
+        for (int e = 0; e < 2; ++e) {
+            const int p = e == 0 ? 0 : P - 1, r0 = p * MR;
+            double g = 0.0;
+            for (int k = 0; k < MR; ++k) {
+                const double r = (e == 0 && k == 0) ? u0 : ((e == 1 && k == MR - 1) ? uN : 0.0);
+                g = nl[r0 + k] * (k > 0 ? g : 0.0) + inv[r0 + k] * r;
+                loc[k] = g;
+            }
+            for (int k = MR - 2; k >= 0; --k) loc[k] = loc[k] + nch[r0 + k] * loc[k + 1];
+            for (int k = 0; k < MR; ++k)
+                put<T>(blob, ((size_t)p * RT * MR + (size_t)5 * MR + k) * sizeof(T), loc[k]);
+        }
+    }
 }
 
 template <typename T>
@@ -547,16 +571,19 @@ size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 // shared-memory layout of one kernel variant: [blob][exchange][mbarriers][ring]
 void layout_slot(const DtypePlan &pl, const Shape &sh, int kind, KernelSlot &sl, bool halo = true)
 {
-    const bool tri = (kind == KIND_TRI || kind == KIND_TRIP || kind == KIND_TRICN || kind == KIND_TRICNP);
+    const bool tri = (kind == KIND_TRI || kind == KIND_TRIP || kind == KIND_TRICN || kind == KIND_TRICNP || kind == KIND_TRIPF ||
+                      kind == KIND_TRICNPF);
+    const bool pertf = (kind == KIND_TRIPF || kind == KIND_TRICNPF);  // + 1 value: nfac for the end partitions
     const int NC = tri ? 1 : 2;
     // kinds with an explicit half need one halo row on each side between fused steps
     const bool cn5 = (kind == KIND_PENTACN || kind == KIND_PENTACNP || kind == KIND_PENTACNPF);  // two halo rows on each side
-    const bool is_ch = (kind == KIND_CH || kind == KIND_CHP || kind == KIND_CHPF || kind == KIND_TRICN || kind == KIND_TRICNP || cn5);
+    const bool is_ch = (kind == KIND_CH || kind == KIND_CHP || kind == KIND_CHPF || kind == KIND_TRICN || kind == KIND_TRICNP ||
+                        kind == KIND_TRICNPF || cn5);
     const bool wood = (kind == KIND_PENTAP || kind == KIND_CHP || kind == KIND_PENTACNP), pert = (kind == KIND_TRIP || kind == KIND_TRICNP);
     const bool woodf = (kind == KIND_PENTAPF || kind == KIND_CHPF || kind == KIND_PENTACNPF);  // + 2 values: nw for the end partitions
     const size_t W = (size_t)sh.lanes * sl.vec;
     // CH: + the halo rows exchanged between fused steps; periodic tri: + y_1 and y_N of eq. 15
-    sl.xvals = 2 * NC + ((is_ch && halo) ? (cn5 ? 4 : 2) : 0) + (pert ? 2 : 0) + (woodf ? 2 : 0);
+    sl.xvals = 2 * NC + ((is_ch && halo) ? (cn5 ? 4 : 2) : 0) + (pert ? 2 : 0) + (woodf ? 2 : 0) + (pertf ? 1 : 0);
     sl.xper = (int)(sl.xvals * pl.P * W);
     sl.xstride = sl.xper + (wood ? (int)(4 * W) : 0);  // cyclic penta: y at rows 0, 1, n-2, n-1
     const size_t xch = (pl.P > 1) ? (size_t)sh.tpc * sl.xstride * pl.elem : 0;
@@ -596,6 +623,8 @@ SweepEntry find_sweep(int kind, int elem_bytes, int vec, int rows, int single, i
         if (kind == KIND_PENTAPF) return find_sweep_pentapf_f64(vec, rows, single, tma, ws, fuse);
         if (kind == KIND_CHPF) return find_sweep_chpf_f64(vec, rows, single, tma, ws, fuse);
         if (kind == KIND_PENTACNPF) return find_sweep_pentacnpf_f64(vec, rows, single, tma, ws, fuse);
+        if (kind == KIND_TRIPF) return find_sweep_tripf_f64(vec, rows, single, tma, ws, fuse);
+        if (kind == KIND_TRICNPF) return find_sweep_tricnpf_f64(vec, rows, single, tma, ws, fuse);
         if (kind == KIND_PENTA) return find_sweep_penta_f64(vec, rows, single, tma, ws, fuse);
         return find_sweep_ch_f64(vec, rows, single, tma, ws, fuse);
     }
@@ -603,7 +632,8 @@ SweepEntry find_sweep(int kind, int elem_bytes, int vec, int rows, int single, i
     if (kind == KIND_TRIP) return find_sweep_trip_f32(vec, rows, single, tma, ws, fuse);
     if (kind == KIND_PENTAP) return find_sweep_pentap_f32(vec, rows, single, tma, ws, fuse);
     if (kind == KIND_PENTAPF) return find_sweep_pentapf_f32(vec, rows, single, tma, ws, fuse);
-    if (kind == KIND_CHPF || kind == KIND_PENTACNPF) return SweepEntry{nullptr, nullptr, 0};
+    if (kind == KIND_TRIPF) return find_sweep_tripf_f32(vec, rows, single, tma, ws, fuse);
+    if (kind == KIND_CHPF || kind == KIND_PENTACNPF || kind == KIND_TRICNPF) return SweepEntry{nullptr, nullptr, 0};
     if (kind == KIND_CHP) return find_sweep_chp_f32(vec, rows, single, tma, ws, fuse);
     if (kind == KIND_TRICN || kind == KIND_TRICNP || kind == KIND_PENTACN || kind == KIND_PENTACNP)
         return SweepEntry{nullptr, nullptr, 0};  // the Crank-Nicolson steps are fp64 only
@@ -687,6 +717,7 @@ void fill_slots(Handle *h)
                 if (ks == 1 && pl.elem != 8) continue;  // the Crank-Nicolson step is fp64 only
                 // periodic explicit halves need whole partitions and at least two of them (halo wrap)
                 if (kind == KIND_TRICNP && (pl.P < 2 || pl.P * pl.rows != h->n)) continue;
+                if (pl.wfast) kind = (ks == 0) ? KIND_TRIPF : KIND_TRICNPF;
             } else {
                 kind = (ks == 0) ? (h->periodic ? KIND_PENTAP : KIND_PENTA)
                                  : (ks == 1 ? (h->periodic ? KIND_CHP : KIND_CH) : (h->periodic ? KIND_PENTACNP : KIND_PENTACN));
@@ -1085,7 +1116,8 @@ extern "C" {
 // shared by tri_factor and tri_factor_periodic: tables + upload for a factored (possibly modified) matrix
 static tri_handle_t make_tri_handle(int n, const std::vector<double> &inv, const std::vector<double> &nl,
                                     const std::vector<double> &nch, const std::vector<double> *z, double vN,
-                                    double invden)
+                                    double invden, const std::vector<double> *zfwd = nullptr, double u0 = 0.0,
+                                    double uN = 0.0)
 {
     Handle *h = new Handle();
     h->magic = MAGIC_TRI;
@@ -1098,14 +1130,16 @@ static tri_handle_t make_tri_handle(int n, const std::vector<double> &inv, const
     for (int t = 0; t < 2; ++t) {
         DtypePlan &pl = h->plan[t];
         choose_plan(n, t == 0 ? 8 : 4, h->kind, pl);
+        // periodic: fold the Sherman-Morrison finish into the carry scan when the partitions are whole (n = P*32, P >= 2)
+        pl.wfast = (z && zfwd && pl.ws && pl.rows == 32 && pl.P >= 2 && pl.P * pl.rows == n && g_tune.cyclic_scan != 0) ? 1 : 0;
         std::vector<unsigned char> blob, soa;
         std::vector<const std::vector<double> *> arrs = {&inv, &nl, &nch};
         if (z) arrs.push_back(z);
         if (t == 0) {
-            build_blob_tri<double>(n, pl, inv, nl, nch, blob, z);
+            build_blob_tri<double>(n, pl, inv, nl, nch, blob, z, zfwd, u0, uN);
             build_soa<double>(arrs, n, soa);
         } else {
-            build_blob_tri<float>(n, pl, inv, nl, nch, blob, z);
+            build_blob_tri<float>(n, pl, inv, nl, nch, blob, z, zfwd, u0, uN);
             build_soa<float>(arrs, n, soa);
         }
         pl.soa_bytes = soa.size();
@@ -1162,9 +1196,11 @@ tri_handle_t tri_factor_periodic(int n, const double *a, const double *b, const 
     z[0] = -b[0];
     z[n - 1] = c[n - 1];
     double g = 0.0;
+    std::vector<double> zfwd(n);
     for (int i = 0; i < n; ++i) {  // forward sweep of A' z = u with the sweep multipliers
         g = nl[i] * g + inv[i] * z[i];
         z[i] = g;
+        zfwd[i] = g;
     }
     for (int i = n - 2; i >= 0; --i) z[i] = z[i] + nch[i] * z[i + 1];
     const double vN = -a[0] / b[0];
@@ -1173,7 +1209,7 @@ tri_handle_t tri_factor_periodic(int n, const double *a, const double *b, const 
         set_err(BTPS_E_PIVOT, n);
         return nullptr;
     }
-    return make_tri_handle(n, inv, nl, nch, &z, vN, 1.0 / den);
+    return make_tri_handle(n, inv, nl, nch, &z, vN, 1.0 / den, &zfwd, -b[0], c[n - 1]);
 }
 
 void tri_destroy(tri_handle_t hv)

@@ -24,7 +24,7 @@ static SweepEntry pick_variant_general(int single, int tma, int ws, int fuse);
 template <typename T, int V, int MR, int KIND>
 static SweepEntry pick_variant(int single, int tma, int ws, int fuse)
 {
-    if constexpr (RecLayout<KIND>::WOODF) {
+    if constexpr (RecLayout<KIND>::WOODF || RecLayout<KIND>::PERTF) {
         // cyclic correction folded into the warp scan: partitioned, warp-scan variants only
         if (single || !ws) return SweepEntry{nullptr, nullptr, 0};
         if (fuse) return tma ? make_entry<T, V, MR, false, KIND, true, true, true>() : SweepEntry{nullptr, nullptr, 0};
@@ -121,5 +121,8 @@ SweepEntry find_sweep_pentapf_f64(int vec, int rows, int single, int tma, int ws
 SweepEntry find_sweep_pentapf_f32(int vec, int rows, int single, int tma, int ws, int fuse);
 SweepEntry find_sweep_chpf_f64(int vec, int rows, int single, int tma, int ws, int fuse);
 SweepEntry find_sweep_pentacnpf_f64(int vec, int rows, int single, int tma, int ws, int fuse);
+SweepEntry find_sweep_tripf_f64(int vec, int rows, int single, int tma, int ws, int fuse);
+SweepEntry find_sweep_tripf_f32(int vec, int rows, int single, int tma, int ws, int fuse);
+SweepEntry find_sweep_tricnpf_f64(int vec, int rows, int single, int tma, int ws, int fuse);
 
 }  // namespace btps

@@ -42,7 +42,8 @@ enum Kind {
     KIND_TRI = 0, KIND_PENTA = 1, KIND_CH = 2, KIND_TRIP = 3, KIND_PENTAP = 4, KIND_CHP = 5, KIND_TRICN = 6, KIND_TRICNP = 7,
     KIND_PENTACN = 8, KIND_PENTACNP = 9,  // Crank-Nicolson hyperdiffusion step (explicit five-point half + penta solve)
     // PENTAP / CHP / PENTACNP with the cyclic correction folded into the carry scan (whole partitions, P >= 2)
-    KIND_PENTAPF = 10, KIND_CHPF = 11, KIND_PENTACNPF = 12
+    KIND_PENTAPF = 10, KIND_CHPF = 11, KIND_PENTACNPF = 12,
+    KIND_TRIPF = 13, KIND_TRICNPF = 14  // TRIP / TRICNP with the Sherman-Morrison finish folded into the carry scan
 };
 
 constexpr int SCAN_STEPS = 5;   // Kogge-Stone steps held in the tables (scan width <= 32)
@@ -136,6 +137,8 @@ __device__ __forceinline__ T ch_w(T c) { return fma_t<T>(c * c, c, -c); }
 //   tri   (5 MR): 0: {inv, nl}   2: nch    3: {chi, psi}
 //           inv = 1/b^_i, nl = -a_i/b^_i, nch = -c^_i; chi/psi = response of the finished local
 //           sweeps to the incoming forward / backward carry
+//   periodic tri, finish in the scan (6 MR): as tri, plus 5: zl, the local (zero-carry) solve of u in the first and
+//           last partition (zero elsewhere); scan table slots 10: GZ_q, 11: XZ_q, the carries of A' z = u
 //   periodic tri (6 MR): as tri, plus 5: z = A'^{-1} u of the Sherman-Morrison splitting
 //   periodic penta (13 MR): as penta, plus 9: {z0, z1}  11: {z2, z3}, the rows of Z = A'^{-1} U (Woodbury)
 //   periodic penta, correction in the scan (11 MR): as penta, plus 9: {zl0, zl1}, the local (zero-carry) solves of the
@@ -156,12 +159,13 @@ __device__ __forceinline__ T ch_w(T c) { return fma_t<T>(c * c, c, -c); }
 // from the row arrays).
 template <int KIND>
 struct RecLayout {
-    static constexpr bool TRI = (KIND == KIND_TRI || KIND == KIND_TRIP || KIND == KIND_TRICN || KIND == KIND_TRICNP);
+    static constexpr bool PERTF = (KIND == KIND_TRIPF || KIND == KIND_TRICNPF);  // Sherman-Morrison finish in the scan
+    static constexpr bool TRI = (KIND == KIND_TRI || KIND == KIND_TRIP || KIND == KIND_TRICN || KIND == KIND_TRICNP || PERTF);
     static constexpr bool PERT = (KIND == KIND_TRIP || KIND == KIND_TRICNP);  // Sherman-Morrison finish
     static constexpr bool WOOD = (KIND == KIND_PENTAP || KIND == KIND_CHP || KIND == KIND_PENTACNP);  // rank-4 Woodbury correction
     // the same correction folded into the carries
     static constexpr bool WOODF = (KIND == KIND_PENTAPF || KIND == KIND_CHPF || KIND == KIND_PENTACNPF);
-    static constexpr int ELEMS = TRI ? (PERT ? 6 : 5) : (WOOD ? 13 : (WOODF ? 11 : 9));  // values per row
+    static constexpr int ELEMS = TRI ? ((PERT || PERTF) ? 6 : 5) : (WOOD ? 13 : (WOODF ? 11 : 9));  // values per row
     static constexpr int NC = TRI ? 1 : 2;                     // carries per direction
 };
 
@@ -280,13 +284,14 @@ sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
 {
     constexpr bool TRI = RecLayout<KIND>::TRI;
     constexpr bool ISCH = (KIND == KIND_CH || KIND == KIND_CHP || KIND == KIND_CHPF);  // explicit Cahn-Hilliard half fused in
-    constexpr bool ISCN = (KIND == KIND_TRICN || KIND == KIND_TRICNP);  // explicit three-point half (eq. 9) fused in
+    constexpr bool ISCN = (KIND == KIND_TRICN || KIND == KIND_TRICNP || KIND == KIND_TRICNPF);  // explicit three-point half (eq. 9) fused in
     constexpr bool ISCN5 = (KIND == KIND_PENTACN || KIND == KIND_PENTACNP || KIND == KIND_PENTACNPF);  // explicit five-point half (eq. 18)
     constexpr bool HALO2 = ISCN5;                                 // needs two rows on each side
     constexpr bool HALO1 = ISCH || ISCN || HALO2;                 // needs the rows r0-1 and r0+MR
     constexpr int NHALO = HALO2 ? 4 : (HALO1 ? 2 : 0);            // exchange values for the fused steps' halos
     constexpr bool WRAP = (KIND == KIND_CHP || KIND == KIND_TRICNP || KIND == KIND_PENTACNP || KIND == KIND_CHPF ||
-                           KIND == KIND_PENTACNPF);  // periodic differences
+                           KIND == KIND_PENTACNPF || KIND == KIND_TRICNPF);  // periodic differences
+    constexpr bool PERTF = RecLayout<KIND>::PERTF;
     constexpr bool WOODF = RecLayout<KIND>::WOODF;
     constexpr bool PERT = RecLayout<KIND>::PERT;
     constexpr bool WOOD = RecLayout<KIND>::WOOD;
@@ -716,7 +721,11 @@ sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
                                 }
                             }
                         });
-                        [[maybe_unused]] T yn1[V], yn2[V];  // cyclic penta: y at rows n-1, n-2 (true g at the last rows)
+                        [[maybe_unused]] T yn1[V], yn2[V];  // cyclic forms: y at rows n-1, n-2 (true g at the last rows)
+                        if constexpr (PERTF) {
+#pragma unroll
+                            for (int e = 0; e < V; ++e) yn1[e] = __shfl_sync(0xffffffffu, fb[0][e], P - 1, wd);  // y_N = g_N
+                        }
                         if constexpr (WOODF) {
 #pragma unroll
                             for (int e = 0; e < V; ++e) {
@@ -768,6 +777,15 @@ sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
                         // itself "local solve + chi GZ^m + psi XZ^m", so -Z w only shifts the carries,
                         // G_q += GZ_q nw, X_q += XZ_q nw (nw = -w), plus the local solves in the two end partitions.
                         [[maybe_unused]] T nw[4][V];
+                        if constexpr (PERTF) {
+                            // Sherman-Morrison in the scan: x = y + nfac z, nfac = -(y_1 + v_N y_N)/(1 + v.z), and z is
+                            // itself "local solve + chi GZ + psi XZ": G_q += GZ_q nfac, X_q += XZ_q nfac
+#pragma unroll
+                            for (int e = 0; e < V; ++e) {
+                                const T y0 = __shfl_sync(0xffffffffu, bb[0][e], 0, wd);
+                                nw[0][e] = -(fma_t<T>((T)a.per_vN, yn1[e], y0) * (T)a.per_invden);
+                            }
+                        }
                         if constexpr (WOODF) {
 #pragma unroll
                             for (int e = 0; e < V; ++e) {
@@ -790,6 +808,11 @@ sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
                                 T x = __shfl_down_sync(0xffffffffu, bb[c][e], 1, wd);
                                 const int ix = (sg * V + e) ^ qsw;
                                 x = (q + 1 < P) ? x : T(0);
+                                if constexpr (PERTF) {
+                                    fb[c][e] = fma_t<T>(tb[10 * sstr], nw[0][e], fb[c][e]);
+                                    x = fma_t<T>(tb[11 * sstr], nw[0][e], x);
+                                    if (ok && (q == 0 || q == P - 1)) xs[(2 * NC + NHALO) * vstr + ix] = nw[0][e];
+                                }
                                 if constexpr (WOODF) {
                                     const T *const gz = tb + (40 + c * 4) * mstr;  // slots 10-11: GZ_q, row c
                                     const T *const xz = tb + (48 + c * 4) * mstr;  // slots 12-13: XZ_q, row c
@@ -907,6 +930,20 @@ sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
                         x = fma_t<T>(G[1][e], cc.v[1], x);
                         x = fma_t<T>(X[0][e], cs.v[0], x);
                         v[k][e] = fma_t<T>(X[1][e], cs.v[1], x);
+                    }
+                }
+            }
+            if constexpr (PERTF) {
+                if (part == 0 || part == P - 1) {  // local solve of u in the end partitions
+                    const T *const RZ = cb + 5 * MR;
+                    T nf[V];
+#pragma unroll
+                    for (int e = 0; e < V; ++e) nf[e] = xc[(2 * NC + NHALO) * vstr + XI(e)];
+#pragma unroll
+                    for (int k = 0; k < MR; ++k) {
+                        const T zk = RZ[k];
+#pragma unroll
+                        for (int e = 0; e < V; ++e) v[k][e] = fma_t<T>(nf[e], zk, v[k][e]);
                     }
                 }
             }

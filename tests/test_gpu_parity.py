@@ -904,3 +904,33 @@ def test_cyclic_correction_in_scan_matches_rowwise(lib, n):
         assert rel_err(d3.cpu().numpy(), r3) <= TOL_STEPS, (mode, n)
         assert rel_err(d4.cpu().numpy().astype(np.float64), r1) <= TOL_F32, (mode, n)
         assert np.max(np.abs(d2.cpu().numpy().sum(axis=0) - (0.1 * rhs).sum(axis=0))) <= 1e-13
+
+
+@pytest.mark.parametrize("n", [64, 256, 512, 1024])
+def test_sherman_morrison_in_scan_matches_rowwise(lib, n):
+    """Periodic tri handles with whole partitions fold x = y - (v.y)/(1+v.z) z into the carries (KIND_TRIPF / TRICNPF)."""
+    batch = 2048 + 32
+    lhs = rand_cyclic(n, n + 5)
+    s = 0.7
+    tl = ([-s] * n, [1 + 2 * s] * n, [-s] * n)
+    rhs = inputs.uniform_rhs(n, batch, seed=73)
+    fo, fs = oracle.tri_periodic_factor(*lhs), oracle.tri_periodic_factor(*tl)
+    r1 = rhs.copy(); oracle.tri_periodic_solve_interleaved(fo, r1)
+    r2 = rhs.copy(); oracle.tri_cn_step_interleaved(fs, r2, s, 1 - 2 * s, s, nsteps=9)
+    r3 = rhs.copy(); oracle.tri_periodic_solve_interleaved(fo, r3, nsteps=9)
+    for mode in (-1, 0):
+        try:
+            lib.btps_tune("cyclic_in_scan", mode)
+            h, hs = lib.tri_factor_periodic(*lhs), lib.tri_factor_periodic(*tl)
+        finally:
+            lib.btps_tune("cyclic_in_scan", -1)
+        d1, d2, d3, d4 = dev(rhs), dev(rhs), dev(rhs), dev(rhs.astype(np.float32))
+        lib.tri_solve_batched(h, d1)
+        lib.tri_cn_step_batched(hs, d2, s, 1 - 2 * s, s, 9)
+        lib.tri_solve_steps(h, d3, 9)
+        lib.tri_solve_batched_f32(h, d4)
+        assert rel_err(d1.cpu().numpy(), r1) <= TOL_SINGLE, (mode, n)
+        assert rel_err(d2.cpu().numpy(), r2) <= TOL_STEPS, (mode, n)
+        assert rel_err(d3.cpu().numpy(), r3) <= TOL_STEPS, (mode, n)
+        assert rel_err(d4.cpu().numpy().astype(np.float64), r1) <= TOL_F32, (mode, n)
+        assert np.max(np.abs(d2.cpu().numpy().sum(axis=0) - rhs.sum(axis=0))) <= 1e-11
