@@ -19,6 +19,9 @@
  *    no host synchronisation, no allocation, no host<->device copy.
  *  - Handles are immutable after creation, own their device-side coefficient tables, may be
  *    used from several streams at once, and must be destroyed by the matching *_destroy.
+ *    A handle belongs to the CUDA device that was current when it was factored (one process
+ *    per GPU sets its device first); using it while another device is current fails with
+ *    BTPS_E_DEVICE.
  *  - Status codes: 0 = success, negative = BTPS_E_* below.  The failing call also records the
  *    code (and, for factor failures, the 1-based row of the bad pivot) per host thread; read
  *    it with btps_last_error().
@@ -46,6 +49,7 @@ extern "C" {
 #define BTPS_E_PIVOT (-2)   /* zero / non-finite pivot in the factorisation (row reported)        */
 #define BTPS_E_CUDA (-3)    /* a CUDA runtime call failed (cudaGetLastError text via btps_error_string) */
 #define BTPS_E_ALIGN (-4)   /* device pointer not aligned to sizeof(element)                      */
+#define BTPS_E_DEVICE (-5)  /* handle used while another CUDA device is current than at its creation */
 
 typedef struct btps_tri_s *tri_handle_t;
 typedef struct btps_penta_s *penta_handle_t;

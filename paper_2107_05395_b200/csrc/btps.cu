@@ -859,6 +859,9 @@ int launch_one(Handle *h, int kind, T *d_rhs, long long batch, double alpha_x, i
                cudaStream_t st, double *stat = nullptr, const double *ex = nullptr)
 {
     DtypePlan &pl = h->plan[sizeof(T) == 8 ? 0 : 1];
+    // a handle's tables live on the device that was current when it was factored
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev != h->device) return set_err(BTPS_E_DEVICE);
     // the paper's own 2R+2W form (Alg. 2 / 4), ksteps launches: plans too large for the on-chip tables,
     // and periodic CH shapes the partitioned kernels do not cover (n not a multiple of the rows per thread)
     auto two_pass = [&]() -> int {
@@ -1126,7 +1129,7 @@ static tri_handle_t make_tri_handle(int n, const std::vector<double> &inv, const
     h->per_vN = vN;
     h->per_invden = invden;
     h->n = n;
-    h->device = 0;
+    if (cudaGetDevice(&h->device) != cudaSuccess) h->device = -1;
     for (int t = 0; t < 2; ++t) {
         DtypePlan &pl = h->plan[t];
         choose_plan(n, t == 0 ? 8 : 4, h->kind, pl);
@@ -1231,7 +1234,7 @@ static penta_handle_t make_penta_handle(int n, const std::vector<double> &inv, c
     if (pp) h->pp = *pp;
     h->per_ngl = (Z && n >= 2) ? ngam[n - 2] : 0.0;
     h->n = n;
-    h->device = 0;
+    if (cudaGetDevice(&h->device) != cudaSuccess) h->device = -1;
     std::vector<double> zc[4];
     std::vector<const std::vector<double> *> arrs = {&inv, &nle, &nlb, &ngam, &ndel};
     if (Z) {
@@ -1441,6 +1444,7 @@ const char *btps_error_string(int code)
         case BTPS_E_PIVOT: return "zero or non-finite pivot (no pivoting; see btps_last_error row)";
         case BTPS_E_CUDA: return tl_cuda_msg[0] ? tl_cuda_msg : "CUDA runtime failure";
         case BTPS_E_ALIGN: return "device pointer not aligned to the element size";
+        case BTPS_E_DEVICE: return "handle used on a device other than the one it was factored on";
         default: return "unknown";
     }
 }
