@@ -53,7 +53,7 @@ std::atomic<long long> g_launches{0};
 // ------------------------------------------------------------------------------------------------
 struct Tune {
     int rows = -1, lanes = -1, vec = -1, tpc = -1, force_two_pass = -1, reverse = -1, prefetch = -1, pdl = -1,
-        warp_scan = -1, grid = -1, fuse = -1, cluster = -1, cyclic_scan = -1;
+        warp_scan = -1, grid = -1, fuse = -1, cluster = -1, cyclic_scan = -1, one_step_fused = -1;
 };
 Tune g_tune;
 
@@ -984,7 +984,8 @@ int launch_one(Handle *h, int kind, T *d_rhs, long long batch, double alpha_x, i
     // several steps per launch need the fused instantiation; without one (direct-load variants)
     // the steps are launched one by one
     // (the statistic of eq. 30 is computed inside the fused kernels; elsewhere by a pass of its own)
-    const bool fused = (ksteps > 1 || stat || sl.prefer_fused) && sl.fused.func;
+    const bool want_fused1 = g_tune.one_step_fused >= 0 ? g_tune.one_step_fused > 0 : sl.prefer_fused != 0;
+    const bool fused = (ksteps > 1 || stat || want_fused1) && sl.fused.func;
     const int nlaunch = fused ? 1 : ksteps;
     a.ksteps = fused ? ksteps : 1;
     a.stat = fused ? stat : nullptr;
@@ -1487,6 +1488,7 @@ int btps_tune(const char *key, int value)
     else if (!strcmp(key, "fuse_steps")) g_tune.fuse = value;
     else if (!strcmp(key, "cluster")) g_tune.cluster = value;
     else if (!strcmp(key, "cyclic_in_scan")) g_tune.cyclic_scan = value;
+    else if (!strcmp(key, "one_step_fused")) g_tune.one_step_fused = value;
     else return set_err(BTPS_E_ARG);
     return set_err(BTPS_OK);
 }

@@ -934,3 +934,32 @@ def test_sherman_morrison_in_scan_matches_rowwise(lib, n):
         assert rel_err(d3.cpu().numpy(), r3) <= TOL_STEPS, (mode, n)
         assert rel_err(d4.cpu().numpy().astype(np.float64), r1) <= TOL_F32, (mode, n)
         assert np.max(np.abs(d2.cpu().numpy().sum(axis=0) - rhs.sum(axis=0))) <= 1e-11
+
+
+# ---- one-step calls through either instantiation of a kernel ---------------------------------------------
+
+@pytest.mark.parametrize("n", [64, 512])
+def test_one_step_through_fused_instantiation_is_bitwise_equal(lib, n):
+    """btps_tune('one_step_fused', 0/1) picks the single-step or the multi-step instantiation for a one-step call
+    (default: the one with the smaller local-memory frame); the arithmetic is the same, so the results are too."""
+    batch = 4096 + 64
+    rhs = inputs.uniform_rhs(n, batch, seed=81)
+    _, al = inputs.ch_params(n)
+    ht, hp, hc = lib.tri_factor(*rand_tri(n, n + 1)), lib.penta_factor(*rand_penta(n, n + 2)), lib.penta_factor(*inputs.ch_lhs(n))
+    hpp, htp = lib.penta_factor_periodic(*rand_cyclic_penta(n, n + 3)), lib.tri_factor_periodic(*rand_cyclic(n, n + 5))
+    got = {}
+    for mode in (0, 1):
+        try:
+            lib.btps_tune("one_step_fused", mode)
+            d = [dev(rhs), dev(rhs), dev(0.1 * rhs), dev(rhs), dev(rhs)]
+            lib.tri_solve_batched(ht, d[0])
+            lib.penta_solve_batched(hp, d[1])
+            lib.ch_step_batched(hc, d[2], al, 1)
+            lib.penta_solve_batched(hpp, d[3])
+            lib.tri_solve_batched(htp, d[4])
+            torch.cuda.synchronize()
+        finally:
+            lib.btps_tune("one_step_fused", -1)
+        got[mode] = d
+    for a, c in zip(got[0], got[1]):
+        assert torch.equal(a, c)
