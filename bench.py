@@ -165,6 +165,13 @@ def oracle_step_fn(n, sample, seed):
     return step, state
 
 
+def workload_config(n, batch):
+    """The workload both arms name in `config` (the reference arm times a bounded sample of it)."""
+    return {"workload": f"BASELINE.json configs[1] shape (N={n}, batch={batch} per GPU, fp64, interleaved): "
+                        "per step one tri sweep + one penta sweep + one fused CH step",
+            "n": n, "batch_per_gpu": batch}
+
+
 def run_reference(args):
     """--impl reference: the oracle as it stands, on this box's host cores (rank 0 only)."""
     if int(os.environ.get("RANK", "0")) != 0:
@@ -186,8 +193,8 @@ def run_reference(args):
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
         "data": "synthetic (seeded; DESIGN.md input recipe)",
-        "config": {"workload": "BASELINE.json configs[1] shape: N=512, fp64, interleaved; bounded sample",
-                   "n": n, "sample_systems": sample},
+        "config": {**workload_config(n, args.batch), "parallelism": "host cores (rank 0 only)",
+                   "sample_systems_per_step": sample},
         "cpu_baseline": {"value": value, "unit": UNIT, "cores": state["cores"], "kind": "oracle", "sample": desc},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
@@ -488,9 +495,7 @@ def run_ours(args):
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
         "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64", "data": "synthetic (seeded; DESIGN.md input recipe)",
-        "config": {"workload": "BASELINE.json configs[1] shape (N=512, batch=65536 per GPU, fp64, interleaved): "
-                               "per step one tri sweep + one penta sweep + one fused CH step",
-                   "n": n, "batch_per_gpu": batch, "l2": "inputs larger than L2 (3 x 256 MiB buffers per step)",
+        "config": {**workload_config(n, batch), "l2": "inputs larger than L2 (3 x 256 MiB buffers per step)",
                    "parallelism": f"dp{world} (independent shards, no collective)"},
         "unknowns_per_s": value * n, "hbm_gbs_step": round(3 * alg_bytes / ms_per_step / 1e6, 1),
         "frac_of_peak_step": round(3 * alg_bytes / ms_per_step / 1e6 / peak, 4),
