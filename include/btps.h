@@ -217,9 +217,11 @@ BTPS_API int btps_plan_info(int kind, const void *handle, int elem_bytes, int *o
  * that split the rows of a tile, 0: never; default: tridiagonal fp64 batches of >= 2^18 systems), "reverse"
  * (0/1: alternate the tile order on successive steps of *_solve_steps / ch_step_batched so a
  * step starts on the data the previous one left in L2), "one_step_fused" (1: one-step calls run the multi-step
- * instantiation of their kernel, 0: the single-step one; default: whichever keeps the smaller local-memory frame).
- * value < 0 restores the default.  "pdl", "fuse_steps", "grid", "cluster", "reverse" and "one_step_fused" are read
- * at launch time, the others when a handle is built. */
+ * instantiation of their kernel, 0: the single-step one; default: whichever keeps the smaller local-memory frame),
+ * "host_chunk_kib" (size in KiB of the column chunks the *_host calls pipeline through the device; default 32768:
+ * measured best on B200 / PCIe Gen5, 43.5 GB/s in each direction at once).
+ * value < 0 restores the default.  "pdl", "fuse_steps", "grid", "cluster", "reverse", "one_step_fused" and
+ * "host_chunk_kib" are read at launch time, the others when a handle is built. */
 BTPS_API int btps_tune(const char *key, int value);
 
 /* Number of kernel launches issued by this library in this process (bench.py's gpu_launches). */

@@ -53,7 +53,7 @@ std::atomic<long long> g_launches{0};
 // ------------------------------------------------------------------------------------------------
 struct Tune {
     int rows = -1, lanes = -1, vec = -1, tpc = -1, force_two_pass = -1, reverse = -1, prefetch = -1, pdl = -1,
-        warp_scan = -1, grid = -1, fuse = -1, cluster = -1, cyclic_scan = -1, one_step_fused = -1;
+        warp_scan = -1, grid = -1, fuse = -1, cluster = -1, cyclic_scan = -1, one_step_fused = -1, host_chunk_kib = -1;
 };
 Tune g_tune;
 
@@ -1080,7 +1080,8 @@ int solve_host(const void *hv, int magic, int kind, T *h_rhs, int64_t batch, dou
     std::lock_guard<std::mutex> lk(g_pipe.mu);
     const int n = h->n;
     // chunk width: about 32 MiB per chunk, a multiple of 256 systems, at least 4 chunks when possible
-    long long wc = (long long)((32ull << 20) / ((size_t)n * sizeof(T)));
+    const size_t target = g_tune.host_chunk_kib > 0 ? ((size_t)g_tune.host_chunk_kib << 10) : (32ull << 20);
+    long long wc = (long long)(target / ((size_t)n * sizeof(T)));
     wc = (wc / 256) * 256;
     if (wc < 256) wc = 256;
     if (wc > batch) wc = batch;
@@ -1489,6 +1490,7 @@ int btps_tune(const char *key, int value)
     else if (!strcmp(key, "cluster")) g_tune.cluster = value;
     else if (!strcmp(key, "cyclic_in_scan")) g_tune.cyclic_scan = value;
     else if (!strcmp(key, "one_step_fused")) g_tune.one_step_fused = value;
+    else if (!strcmp(key, "host_chunk_kib")) g_tune.host_chunk_kib = value;
     else return set_err(BTPS_E_ARG);
     return set_err(BTPS_OK);
 }
