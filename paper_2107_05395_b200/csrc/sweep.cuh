@@ -1141,6 +1141,37 @@ struct PerPenta {  // scalars of the cyclic pentadiagonal (Woodbury) correction 
     double w6[6];  // wrap-around entries e_0, a_0, e_1, f_{n-2}, c_{n-1}, f_{n-1}
 };
 
+// Rows streamed through a thread in a fixed order, a block of 8 rows at a time (16 in fp32 when a row needs at most two coefficients): the loads of the NEXT block are
+// issued first (fetch(k) must not depend on a store body() makes for an earlier k), then the coefficients of this
+// block (coef(k): read-only path), then body(k, value, coefficients) runs the recurrence and stores.  The compiler
+// cannot move a load of rhs above an earlier store to rhs by itself, so without this every row waits for its own
+// load; the arithmetic and its order are unchanged.
+template <typename T, int NCF>
+struct RowCoef {
+    T c[NCF];
+};
+template <typename T, int NCF, typename Fetch, typename Coef, typename Body>
+__device__ __forceinline__ void pipelined_rows(int count, Fetch fetch, Coef coef, Body body)
+{
+    constexpr int TP_U = (sizeof(T) == 4 && NCF < 3) ? 16 : 8;  // (measured: 16 loses with three coefficients per row)
+    T cur[TP_U], nxt[TP_U];
+#pragma unroll
+    for (int u = 0; u < TP_U; ++u) cur[u] = (u < count) ? fetch(u) : T(0);
+    for (int k0 = 0; k0 < count; k0 += TP_U) {
+#pragma unroll
+        for (int u = 0; u < TP_U; ++u) nxt[u] = (k0 + TP_U + u < count) ? fetch(k0 + TP_U + u) : T(0);
+        RowCoef<T, NCF> cf[TP_U];
+#pragma unroll
+        for (int u = 0; u < TP_U; ++u)
+            if (k0 + u < count) cf[u] = coef(k0 + u);
+#pragma unroll
+        for (int u = 0; u < TP_U; ++u)
+            if (k0 + u < count) body(k0 + u, cur[u], cf[u]);
+#pragma unroll
+        for (int u = 0; u < TP_U; ++u) cur[u] = nxt[u];
+    }
+}
+
 template <typename T, int KIND>
 __global__ void __launch_bounds__(128) two_pass_kernel(const T *__restrict__ co, T *rhs, long long batch,
                                                        int n, double alpha_x, double alpha_y, const PerPenta pp)
@@ -1148,6 +1179,7 @@ __global__ void __launch_bounds__(128) two_pass_kernel(const T *__restrict__ co,
     const long long j = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (j >= batch) return;
     T *p = rhs + j;
+    auto row = [&](int r) -> T { return p[(long long)r * batch]; };
     if constexpr (RecLayout<KIND>::TRI) {
         const T *inv = co, *nl = co + n, *nch = co + 2 * (size_t)n;
         T g = T(0);
@@ -1157,30 +1189,35 @@ __global__ void __launch_bounds__(128) two_pass_kernel(const T *__restrict__ co,
             const T xa = (T)pp.ex[0], xb = (T)pp.ex[1], xc = (T)pp.ex[2];
             const T c_first = p[0];
             T cprev = WRAPS ? p[(long long)(n - 1) * batch] : T(0), cc = c_first;
-            for (int i = 0; i < n; ++i) {
-                const T cn = (i + 1 < n) ? p[(long long)(i + 1) * batch] : (WRAPS ? c_first : T(0));
-                const T f = fma_t<T>(xa, cprev, fma_t<T>(xc, cn, xb * cc));
-                g = fma_t<T>(__ldg(nl + i), g, __ldg(inv + i) * f);
-                p[(long long)i * batch] = g;
-                cprev = cc;
-                cc = cn;
-            }
+            pipelined_rows<T, 2>(n, [&](int k) -> T { return (k + 1 < n) ? row(k + 1) : (WRAPS ? c_first : T(0)); },
+                              [&](int i) { return RowCoef<T, 2>{{__ldg(nl + i), __ldg(inv + i)}}; },
+                              [&](int i, T cn, const RowCoef<T, 2> &cf) {
+                                  const T f = fma_t<T>(xa, cprev, fma_t<T>(xc, cn, xb * cc));
+                                  g = fma_t<T>(cf.c[0], g, cf.c[1] * f);
+                                  p[(long long)i * batch] = g;
+                                  cprev = cc;
+                                  cc = cn;
+                              });
         } else {
-            for (int i = 0; i < n; ++i) {
-                g = fma_t<T>(__ldg(nl + i), g, __ldg(inv + i) * p[(long long)i * batch]);
-                p[(long long)i * batch] = g;
-            }
+            pipelined_rows<T, 2>(n, row, [&](int i) { return RowCoef<T, 2>{{__ldg(nl + i), __ldg(inv + i)}}; },
+                                 [&](int i, T d, const RowCoef<T, 2> &cf) {
+                                     g = fma_t<T>(cf.c[0], g, cf.c[1] * d);
+                                     p[(long long)i * batch] = g;
+                                 });
         }
         T x = g;
-        for (int i = n - 2; i >= 0; --i) {
-            x = fma_t<T>(__ldg(nch + i), x, p[(long long)i * batch]);
-            p[(long long)i * batch] = x;
-        }
+        pipelined_rows<T, 1>(n - 1, [&](int k) -> T { return row(n - 2 - k); },
+                             [&](int k) { return RowCoef<T, 1>{{__ldg(nch + (n - 2 - k))}}; },
+                             [&](int k, T d, const RowCoef<T, 1> &cf) {
+                                 x = fma_t<T>(cf.c[0], x, d);
+                                 p[(long long)(n - 2 - k) * batch] = x;
+                             });
         if constexpr (RecLayout<KIND>::PERT) {
             // eq. 15: alpha_x carries v_N, alpha_y 1/(1 + v.z); z follows nch in co
             const T *z = co + 3 * (size_t)n;
             const T nfac = -(fma_t<T>((T)alpha_x, g, x) * (T)alpha_y);  // x = y_1, g = y_N here
-            for (int i = 0; i < n; ++i) p[(long long)i * batch] = fma_t<T>(nfac, __ldg(z + i), p[(long long)i * batch]);
+            pipelined_rows<T, 1>(n, row, [&](int i) { return RowCoef<T, 1>{{__ldg(z + i)}}; },
+                                 [&](int i, T y, const RowCoef<T, 1> &cf) { p[(long long)i * batch] = fma_t<T>(nfac, cf.c[0], y); });
         }
     } else {
         const T *inv = co, *nle = co + n, *nlb = co + 2 * (size_t)n, *ngam = co + 3 * (size_t)n,
@@ -1191,18 +1228,19 @@ __global__ void __launch_bounds__(128) two_pass_kernel(const T *__restrict__ co,
             const T ax = (T)alpha_x;
             const T c_first = p[0];
             T wm = WRAPS ? ch_w<T>(p[(long long)(n - 1) * batch]) : T(0), cc = c_first, wc = ch_w<T>(cc);
-            for (int i = 0; i < n; ++i) {
-                const T cn = (i + 1 < n) ? p[(long long)(i + 1) * batch] : (WRAPS ? c_first : T(0));
-                const T wn = ch_w<T>(cn);
-                T s = wm + wn;
-                s = fma_t<T>(T(-2), wc, s);
-                const T f = fma_t<T>(ax, s, cc);
-                const T t = fma_t<T>(__ldg(nle + i), g2, __ldg(inv + i) * f);
-                const T g = fma_t<T>(__ldg(nlb + i), g1, t);
-                p[(long long)i * batch] = g;
-                g2 = g1; g1 = g;
-                wm = wc; wc = wn; cc = cn;
-            }
+            pipelined_rows<T, 3>(n, [&](int k) -> T { return (k + 1 < n) ? row(k + 1) : (WRAPS ? c_first : T(0)); },
+                              [&](int i) { return RowCoef<T, 3>{{__ldg(nle + i), __ldg(inv + i), __ldg(nlb + i)}}; },
+                              [&](int i, T cn, const RowCoef<T, 3> &cf) {
+                                  const T wn = ch_w<T>(cn);
+                                  T s = wm + wn;
+                                  s = fma_t<T>(T(-2), wc, s);
+                                  const T f = fma_t<T>(ax, s, cc);
+                                  const T t = fma_t<T>(cf.c[0], g2, cf.c[1] * f);
+                                  const T g = fma_t<T>(cf.c[2], g1, t);
+                                  p[(long long)i * batch] = g;
+                                  g2 = g1; g1 = g;
+                                  wm = wc; wc = wn; cc = cn;
+                              });
         } else if constexpr (KIND == KIND_PENTACN || KIND == KIND_PENTACNP) {
             // Crank-Nicolson hyperdiffusion: explicit five-point half (eq. 18) on the fly (rows i+1, i+2 still c^n)
             constexpr bool WRAPS = (KIND == KIND_PENTACNP);
@@ -1210,34 +1248,40 @@ __global__ void __launch_bounds__(128) two_pass_kernel(const T *__restrict__ co,
             const T c_0 = p[0], c_1 = (n > 1) ? p[batch] : T(0);
             T c2 = WRAPS ? p[(long long)(n - 2) * batch] : T(0), c1 = WRAPS ? p[(long long)(n - 1) * batch] : T(0);
             T cc = c_0, cn1 = c_1;
-            for (int i = 0; i < n; ++i) {
-                const int i2 = i + 2;
-                const T cn2 = (i2 < n) ? p[(long long)i2 * batch] : (WRAPS ? (i2 == n ? c_0 : c_1) : T(0));
-                T f = fma_t<T>(x1, c1, x0 * c2);
-                f = fma_t<T>(x2, cc, f);
-                f = fma_t<T>(x3, cn1, f);
-                f = fma_t<T>(x4, cn2, f);
-                const T t = fma_t<T>(__ldg(nle + i), g2, __ldg(inv + i) * f);
-                const T g = fma_t<T>(__ldg(nlb + i), g1, t);
-                p[(long long)i * batch] = g;
-                g2 = g1; g1 = g;
-                c2 = c1; c1 = cc; cc = cn1; cn1 = cn2;
-            }
+            pipelined_rows<T, 3>(n, [&](int k) -> T {
+                                  const int i2 = k + 2;
+                                  return (i2 < n) ? row(i2) : (WRAPS ? (i2 == n ? c_0 : c_1) : T(0));
+                              },
+                              [&](int i) { return RowCoef<T, 3>{{__ldg(nle + i), __ldg(inv + i), __ldg(nlb + i)}}; },
+                              [&](int i, T cn2, const RowCoef<T, 3> &cf) {
+                                  T f = fma_t<T>(x1, c1, x0 * c2);
+                                  f = fma_t<T>(x2, cc, f);
+                                  f = fma_t<T>(x3, cn1, f);
+                                  f = fma_t<T>(x4, cn2, f);
+                                  const T t = fma_t<T>(cf.c[0], g2, cf.c[1] * f);
+                                  const T g = fma_t<T>(cf.c[2], g1, t);
+                                  p[(long long)i * batch] = g;
+                                  g2 = g1; g1 = g;
+                                  c2 = c1; c1 = cc; cc = cn1; cn1 = cn2;
+                              });
         } else {
-            for (int i = 0; i < n; ++i) {
-                const T t = fma_t<T>(__ldg(nle + i), g2, __ldg(inv + i) * p[(long long)i * batch]);
-                const T g = fma_t<T>(__ldg(nlb + i), g1, t);
-                p[(long long)i * batch] = g;
-                g2 = g1; g1 = g;
-            }
+            pipelined_rows<T, 3>(n, row, [&](int i) { return RowCoef<T, 3>{{__ldg(nle + i), __ldg(inv + i), __ldg(nlb + i)}}; },
+                                 [&](int i, T d, const RowCoef<T, 3> &cf) {
+                                     const T t = fma_t<T>(cf.c[0], g2, cf.c[1] * d);
+                                     const T g = fma_t<T>(cf.c[2], g1, t);
+                                     p[(long long)i * batch] = g;
+                                     g2 = g1; g1 = g;
+                                 });
         }
         T x1 = g1, x2 = T(0);
-        for (int i = n - 2; i >= 0; --i) {
-            const T t = fma_t<T>(__ldg(ndel + i), x2, p[(long long)i * batch]);
-            const T x = fma_t<T>(__ldg(ngam + i), x1, t);
-            p[(long long)i * batch] = x;
-            x2 = x1; x1 = x;
-        }
+        pipelined_rows<T, 2>(n - 1, [&](int k) -> T { return row(n - 2 - k); },
+                             [&](int k) { return RowCoef<T, 2>{{__ldg(ndel + (n - 2 - k)), __ldg(ngam + (n - 2 - k))}}; },
+                             [&](int k, T d, const RowCoef<T, 2> &cf) {
+                                 const T t = fma_t<T>(cf.c[0], x2, d);
+                                 const T x = fma_t<T>(cf.c[1], x1, t);
+                                 p[(long long)(n - 2 - k) * batch] = x;
+                                 x2 = x1; x1 = x;
+                             });
         if constexpr (RecLayout<KIND>::WOOD) {
             // cyclic matrix: x = y - Z H (V^T y) (Woodbury, C-31); Z's four columns follow ndel in co
             const T y0 = p[0], y1 = p[batch], yn2 = p[(long long)(n - 2) * batch], yn1 = p[(long long)(n - 1) * batch];
@@ -1248,12 +1292,13 @@ __global__ void __launch_bounds__(128) two_pass_kernel(const T *__restrict__ co,
                 nw[m] = -fma_t<T>((T)pp.H[m * 4 + 3], t3, fma_t<T>((T)pp.H[m * 4 + 2], t2,
                                   fma_t<T>((T)pp.H[m * 4 + 1], t1, (T)pp.H[m * 4] * t0)));
             const T *z0 = co + 5 * (size_t)n, *z1 = co + 6 * (size_t)n, *z2 = co + 7 * (size_t)n, *z3 = co + 8 * (size_t)n;
-            for (int i = 0; i < n; ++i) {
-                T x = fma_t<T>(nw[0], __ldg(z0 + i), p[(long long)i * batch]);
-                x = fma_t<T>(nw[1], __ldg(z1 + i), x);
-                x = fma_t<T>(nw[2], __ldg(z2 + i), x);
-                p[(long long)i * batch] = fma_t<T>(nw[3], __ldg(z3 + i), x);
-            }
+            pipelined_rows<T, 4>(n, row, [&](int i) { return RowCoef<T, 4>{{__ldg(z0 + i), __ldg(z1 + i), __ldg(z2 + i), __ldg(z3 + i)}}; },
+                                 [&](int i, T y, const RowCoef<T, 4> &cf) {
+                                     T x = fma_t<T>(nw[0], cf.c[0], y);
+                                     x = fma_t<T>(nw[1], cf.c[1], x);
+                                     x = fma_t<T>(nw[2], cf.c[2], x);
+                                     p[(long long)i * batch] = fma_t<T>(nw[3], cf.c[3], x);
+                                 });
         }
     }
 }

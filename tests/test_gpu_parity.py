@@ -963,3 +963,33 @@ def test_one_step_through_fused_instantiation_is_bitwise_equal(lib, n):
         got[mode] = d
     for a, c in zip(got[0], got[1]):
         assert torch.equal(a, c)
+
+
+@pytest.mark.parametrize("n", [5, 9, 17, 37, 131])
+def test_two_pass_kernel_ragged_row_blocks(lib, n):
+    """The two-pass form streams rows in blocks of 8 (16 in fp32): sizes around the block edges, general LHS,
+    plain and periodic, fp64 and fp32, a batch that is not a multiple of the thread block."""
+    batch = 300
+    lt, lp, ltp, lpp = rand_tri(n, n), rand_penta(n, n + 1), rand_cyclic(n, n + 2), rand_cyclic_penta(n, n + 3)
+    try:
+        lib.btps_tune("force_two_pass", 1)
+        ht, hp = lib.tri_factor(*lt), lib.penta_factor(*lp)
+        htp, hpp = lib.tri_factor_periodic(*ltp), lib.penta_factor_periodic(*lpp)
+    finally:
+        lib.btps_tune("force_two_pass", -1)
+    assert ht.plan()["rows_per_thread"] == 0 and hpp.plan()["rows_per_thread"] == 0
+    rhs = inputs.uniform_rhs(n, batch, seed=90 + n)
+    cases = ((ht, oracle.tri_factor(*lt), lib.tri_solve_batched, lib.tri_solve_batched_f32, oracle.tri_solve_interleaved),
+             (hp, oracle.penta_factor(*lp), lib.penta_solve_batched, lib.penta_solve_batched_f32, oracle.penta_solve_interleaved),
+             (htp, oracle.tri_periodic_factor(*ltp), lib.tri_solve_batched, lib.tri_solve_batched_f32,
+              oracle.tri_periodic_solve_interleaved),
+             (hpp, oracle.penta_periodic_factor(*lpp), lib.penta_solve_batched, lib.penta_solve_batched_f32,
+              oracle.penta_periodic_solve_interleaved))
+    for h, fac, solve, solve32, osolve in cases:
+        r32 = rhs.astype(np.float32)
+        ref = rhs.copy(); osolve(fac, ref)
+        ref32 = r32.astype(np.float64); osolve(fac, ref32)
+        d, d32 = dev(rhs), dev(r32)
+        solve(h, d); solve32(h, d32)
+        assert rel_err(d.cpu().numpy(), ref) <= TOL_SINGLE, n
+        assert rel_err(d32.cpu().numpy().astype(np.float64), ref32) <= TOL_F32, n
