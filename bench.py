@@ -261,7 +261,7 @@ def paper_table1(torch, b, inputs, sigma=0.5, steps=1000):
         rows.append({"batch": batch, "n": n, "seconds_1000_steps": round(ms * 1e-3, 6),
                      "paper_v100_seconds": paper_s, "plan": h.cn_plan(8)})
         del u
-    return {"workload": "periodic Crank-Nicolson diffusion, 1000 steps (tri_cn_step_batched, fused 8 steps per launch)",
+    return {"workload": "periodic Crank-Nicolson diffusion, 1000 steps (tri_cn_step_batched, up to 64 steps per launch)",
             "note": "paper's numbers: Tesla V100, whole step incl. a separate stencil pass; context only", "rows": rows}
 
 
@@ -285,7 +285,7 @@ def paper_table2(torch, b, inputs, sigma=0.5, steps=1000):
         rows.append({"batch": batch, "n": n, "seconds_1000_steps": round(ms * 1e-3, 6),
                      "paper_v100_value_units_unresolved": paper_v, "plan": h.cn_plan(8)})
         del u
-    return {"workload": "periodic Crank-Nicolson hyperdiffusion, 1000 steps (penta_cn_step_batched, fused 8 steps per launch)",
+    return {"workload": "periodic Crank-Nicolson hyperdiffusion, 1000 steps (penta_cn_step_batched, up to 64 steps per launch)",
             "note": "paper's numbers: Tesla V100, units (s or ms) and step count not stated; context only", "rows": rows}
 
 
@@ -322,15 +322,15 @@ def extra_table(torch, b, inputs, peak):
         gbs = 2.0 * size / ms / 1e6
         extra = {}
         if steps_per_call > 1:
-            # time loops advance up to 8 steps per launch while a tile is on chip (btps_tune "fuse_steps"):
-            # HBM then moves 2*N*M*sizeof(T) per 8 steps, so the per-step figure below is an EFFECTIVE rate
+            # time loops advance up to 64 steps per launch while a tile is on chip (btps_tune "fuse_steps"):
+            # HBM then moves 2*N*M*sizeof(T) per launch, so the per-step figure below is an EFFECTIVE rate
             # (it may exceed the HBM peak); the same loop with one launch per step is timed beside it.
             b.btps_tune("fuse_steps", 1)
             try:
                 ms1 = time_launches(torch, fn, bufs, launches) / steps_per_call
             finally:
                 b.btps_tune("fuse_steps", -1)
-            extra = {"fused_steps_per_launch": 8, "ms_per_solve_one_step_per_launch": round(ms1, 5),
+            extra = {"fused_steps_per_launch": min(64, steps_per_call), "ms_per_solve_one_step_per_launch": round(ms1, 5),
                      "hbm_gbs_one_step_per_launch": round(2.0 * size / ms1 / 1e6, 1),
                      "frac_one_step_per_launch": round(2.0 * size / ms1 / 1e6 / peak, 4),
                      "note": "hbm_gbs / frac_of_measured_peak are effective (per-step algorithmic bytes / time)"}

@@ -211,7 +211,7 @@ BTPS_API int btps_plan_info(int kind, const void *handle, int elem_bytes, int *o
  * "vec" (systems per thread: 1, 2, 4), "tiles_per_cta", "force_two_pass" (0/1), "prefetch"
  * (0: never use the TMA prefetch variant), "warp_scan" (0: serial carry walk), "pdl" (0: no
  * programmatic dependent launch attribute), "fuse_steps" (time steps advanced per launch while a tile
- * is on chip in *_solve_steps / ch_step_batched: default 8, 1 = one launch per step), "grid" (cap on
+ * is on chip in *_solve_steps / ch_step_batched: default and maximum 64, 1 = one launch per step), "grid" (cap on
  * the number of CTAs), "cyclic_in_scan" (0: periodic pentadiagonal handles apply the cyclic correction row by row
  * instead of folding it into the carry scan), "cluster" (1: run every eligible plain solve of 17..32 partitions on clusters of two CTAs
  * that split the rows of a tile, 0: never; default: tridiagonal fp64 batches of >= 2^18 systems), "reverse"

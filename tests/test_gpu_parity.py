@@ -501,15 +501,15 @@ def test_full_size_sampled(lib, kind, n, lb, f32):
 
 @pytest.mark.parametrize("n,batch", [(300, 2048 + 32), (20, 640), (512, 1024), (1000, 512)])
 def test_fused_steps_equal_single_step_launches(lib, n, batch):
-    """tri/penta_solve_steps and ch_step_batched advance up to 8 steps per launch; the arithmetic per
+    """tri/penta_solve_steps and ch_step_batched advance up to 64 steps per launch; the arithmetic per
     step is the same as one launch per step, so the results must be bitwise equal -- and both must
     match the oracle's step-by-step loop."""
-    steps = 11  # one launch of 8 + one of 3
+    steps = 11  # one launch by default, 8 + 3 with fuse_steps = 8
     lt, lp, lc = inputs.tri_lhs(n, 0.5), inputs.penta_lhs(n, 0.5), inputs.penta_lhs(n, 0.7)
     rhs = inputs.uniform_rhs(n, batch, seed=31)
     c0 = 0.5 * rhs
     outs = {}
-    for fuse in (1, -1, 3):
+    for fuse in (1, -1, 3, 8):
         try:
             lib.btps_tune("fuse_steps", fuse)
             ht, hp, hc = lib.tri_factor(*lt), lib.penta_factor(*lp), lib.penta_factor(*lc)
@@ -521,12 +521,12 @@ def test_fused_steps_equal_single_step_launches(lib, n, batch):
             outs[fuse] = (dt_.cpu().numpy(), dp_.cpu().numpy(), dc_.cpu().numpy(), lib.btps_launch_count() - n0)
         finally:
             lib.btps_tune("fuse_steps", -1)
-    # 11 steps: 11 launches unfused, 2 (8 + 3) by default, 4 with fuse_steps = 3; a variant without a
-    # fused form (CH at n = 1000: no room for the halo exchange rows) falls back to one launch per step
-    assert outs[1][3] == 3 * steps and 3 * 2 <= outs[-1][3] <= outs[3][3] < 3 * steps
+    # 11 steps: 11 launches unfused, 1 by default, 2 (8 + 3) with fuse_steps = 8, 4 with fuse_steps = 3; a variant
+    # without a fused form (CH at n = 1000: no room for the halo exchange rows) falls back to one launch per step
+    assert outs[1][3] == 3 * steps and 3 <= outs[-1][3] <= outs[8][3] <= outs[3][3] < 3 * steps
     if n <= 512:
-        assert outs[-1][3] == 3 * 2 and outs[3][3] == 3 * 4
-    for k in (-1, 3):
+        assert outs[-1][3] == 3 and outs[8][3] == 3 * 2 and outs[3][3] == 3 * 4
+    for k in (-1, 3, 8):
         for a, b_ in zip(outs[1][:3], outs[k][:3]):
             assert np.array_equal(a, b_)
     ref = rhs.copy()
