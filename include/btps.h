@@ -220,8 +220,10 @@ BTPS_API int btps_plan_info(int kind, const void *handle, int elem_bytes, int *o
  * instantiation of their kernel, 0: the single-step one; default: whichever keeps the smaller local-memory frame),
  * "host_chunk_kib" (size in KiB of the column chunks the *_host calls pipeline through the device; default 32768:
  * measured best on B200 / PCIe Gen5, 43.5 GB/s in each direction at once).
- * value < 0 restores the default.  "pdl", "fuse_steps", "grid", "cluster", "reverse", "one_step_fused" and
- * "host_chunk_kib" are read at launch time, the others when a handle is built. */
+ * "hold_stores" (1: a tile's stores wait until the next tile's prefetch has landed, 0: never; default: the kinds
+ * and tile sizes where that was measured to win -- tridiagonal kinds and the plain fp64 pentadiagonal solve on full tiles).
+ * value < 0 restores the default.  "pdl", "fuse_steps", "grid", "cluster", "reverse", "one_step_fused",
+ * "host_chunk_kib" and "hold_stores" are read at launch time, the others when a handle is built. */
 BTPS_API int btps_tune(const char *key, int value);
 
 /* Number of kernel launches issued by this library in this process (bench.py's gpu_launches). */

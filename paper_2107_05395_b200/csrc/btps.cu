@@ -53,7 +53,7 @@ std::atomic<long long> g_launches{0};
 // ------------------------------------------------------------------------------------------------
 struct Tune {
     int rows = -1, lanes = -1, vec = -1, tpc = -1, force_two_pass = -1, reverse = -1, prefetch = -1, pdl = -1,
-        warp_scan = -1, grid = -1, fuse = -1, cluster = -1, cyclic_scan = -1, one_step_fused = -1, host_chunk_kib = -1;
+        warp_scan = -1, grid = -1, fuse = -1, cluster = -1, cyclic_scan = -1, one_step_fused = -1, host_chunk_kib = -1, hold_stores = -1;
 };
 Tune g_tune;
 
@@ -960,6 +960,18 @@ int launch_one(Handle *h, int kind, T *d_rhs, long long batch, double alpha_x, i
     a.lanes_log2 = sh.lanes_log2;
     a.tpc = sh.tpc;
     a.reverse = reverse;
+    {
+        // stores held until the next tile has landed (sweep.cuh, store phase).  Measured on B200, fp64 unless noted:
+        // tridiagonal kinds (plain, periodic, Crank-Nicolson; also fp32) with one full-size tile per CTA gain 4-12 %
+        // (N = 480 / 512 / 992 / 1024), 96 KB tiles (N = 768) lose 4-9 %; the plain pentadiagonal solve gains 4-6 % on
+        // 16-lane tiles (N <= 512) and loses up to 8 % on 8-lane ones; Cahn-Hilliard, periodic penta, fp32 penta lose.
+        const bool tri_family = (kind == KIND_TRI || kind == KIND_TRICN);
+        const size_t tile_bytes = (size_t)pl.P * pl.rows * sh.lanes * sl.vec * sizeof(T);
+        // (and at least 8 tiles per CTA: with 3-4 it loses ~10 %)
+        const bool full_tile = (sh.tpc == 1) && !use_cl && tile_bytes >= (112u << 10) && a.num_tiles >= 8ll * sl.max_grid;
+        const bool penta_ok = (kind == KIND_PENTA) && sizeof(T) == 8 && !h->periodic && sh.lanes == 16;
+        a.hold_stores = g_tune.hold_stores >= 0 ? (g_tune.hold_stores > 0) : ((full_tile && (tri_family || penta_ok)) ? 1 : 0);
+    }
     a.scan_log2 = pl.scan_log2;
     a.tq = pl.tq;
     a.ksteps = ksteps;
@@ -1495,6 +1507,7 @@ int btps_tune(const char *key, int value)
     else if (!strcmp(key, "cyclic_in_scan")) g_tune.cyclic_scan = value;
     else if (!strcmp(key, "one_step_fused")) g_tune.one_step_fused = value;
     else if (!strcmp(key, "host_chunk_kib")) g_tune.host_chunk_kib = value;
+    else if (!strcmp(key, "hold_stores")) g_tune.hold_stores = value;
     else return set_err(BTPS_E_ARG);
     return set_err(BTPS_OK);
 }

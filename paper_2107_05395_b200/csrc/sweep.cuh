@@ -74,6 +74,7 @@ struct SweepArgs {
     int lanes_log2;
     int tpc;               // tile groups per CTA (each walks its own tiles)
     int reverse;           // 1: walk the tiles from the last to the first
+    int hold_stores;       // 1: a tile's stores wait until the next tile's TMA load has landed
     int scan_log2;         // warp scan: log2 of the scan width (smallest power of two >= P)
     int tq;                // partitions per scan-table row (max(32, P))
     int ksteps;            // time steps advanced per tile while it is on chip (>= 1)
@@ -1114,6 +1115,13 @@ sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
         }  // ksteps
 
         // ---- store ---------------------------------------------------------------------------
+        if constexpr (TMA) {
+            // Kinds with little arithmetic reach the stores while the next tile's load is still streaming in, and the
+            // two then slow each other down (measured: tri fp64 N=512, 2^20 systems 0.85 -> 0.93 of the peak with the
+            // stores held back; the pentadiagonal kinds arrive later by themselves and lose 0-4 %): wait for the
+            // ring's barrier first (the same wait the next iteration starts with; it does not consume the phase).
+            if (a.hold_stores && t + stride_tiles < ntiles) mbar_wait(mbar, phase);
+        }
         {
             T *ps = p0;
             asm volatile("" : "+l"(ps));  // keep the store addresses from being shared with the loads

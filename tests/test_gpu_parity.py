@@ -993,3 +993,33 @@ def test_two_pass_kernel_ragged_row_blocks(lib, n):
         solve(h, d); solve32(h, d32)
         assert rel_err(d.cpu().numpy(), ref) <= TOL_SINGLE, n
         assert rel_err(d32.cpu().numpy().astype(np.float64), ref32) <= TOL_F32, n
+
+
+def test_held_stores_are_bitwise_equal(lib):
+    """btps_tune('hold_stores', 1) makes a tile's stores wait for the next tile's prefetch (a scheduling change only):
+    same results as with 0, on a batch of many tiles per CTA, for every kernel family."""
+    n, batch = 512, 32 * 148 * 3 + 64
+    rhs = inputs.uniform_rhs(n, batch, seed=97)
+    _, al = inputs.ch_params(n)
+    ht, hp, hc = lib.tri_factor(*rand_tri(n, 3)), lib.penta_factor(*rand_penta(n, 4)), lib.penta_factor(*inputs.ch_lhs(n))
+    htp = lib.tri_factor_periodic(*rand_cyclic(n, 5))
+    got = {}
+    for mode in (0, 1):
+        try:
+            lib.btps_tune("hold_stores", mode)
+            d = [dev(rhs), dev(rhs), dev(0.1 * rhs), dev(rhs), dev(rhs.astype(np.float32)), dev(rhs)]
+            lib.tri_solve_batched(ht, d[0])
+            lib.penta_solve_batched(hp, d[1])
+            lib.ch_step_batched(hc, d[2], al, 3)
+            lib.tri_solve_batched(htp, d[3])
+            lib.tri_solve_batched_f32(ht, d[4])
+            lib.tri_cn_step_batched(ht, d[5], 0.3, 0.4, 0.3, 2)
+            torch.cuda.synchronize()
+        finally:
+            lib.btps_tune("hold_stores", -1)
+        got[mode] = d
+    for a, c in zip(got[0], got[1]):
+        assert torch.equal(a, c)
+    ref = rhs.copy()
+    oracle.tri_solve_interleaved(oracle.tri_factor(*rand_tri(n, 3)), ref)
+    assert rel_err(got[1][0].cpu().numpy(), ref) <= TOL_SINGLE
