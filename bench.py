@@ -38,8 +38,8 @@ UNIT = "systems/s"
 L2_BYTES = 126 * 1024 * 1024
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full`
-# capture (profiles/r01e_ncu_full_summary.md), keyed by kernel.
-NCU_TRAFFIC_BYTES = {"tri": 268509440 + 210128896, "penta": 268541184 + 210305024, "ch": 268547840 + 209750016}
+# capture (profiles/r01f_ncu_full_summary.md), keyed by kernel.
+NCU_TRAFFIC_BYTES = {"tri": 268507904 + 209516800, "penta": 268542720 + 209016320, "ch": 268549632 + 209529088}
 
 
 def parse_args():
