@@ -907,11 +907,12 @@ int launch_one(Handle *h, int kind, T *d_rhs, long long batch, double alpha_x, i
                         (batch < (1ll << 31));
     // long systems: the cluster-split kernels when the batch is TMA-aligned and a multiple of the vector width
     // (measured on B200: the pair's two cluster barriers per tile cost ~1.3 us, so by default it is used only
-    //  where the wider row segments win -- tridiagonal fp64, 32 partitions (993 <= N <= 1024), >= 2^19 systems: 0.71 / 0.68
-    //  against 0.69 / 0.65 of the peak at 2^19 / 2^20; with 24 partitions (N = 768) it loses 0.56 against 0.75;
+    //  where the wider row segments win -- tridiagonal fp64, 32 partitions (N = 992 / 1024), >= 2^22 systems: 0.70
+    //  against 0.69 of the peak; at 2^19 / 2^20 the single CTA with held stores (hold_stores below) now wins, 0.77 / 0.75
+    //  against 0.72 / 0.71 for the pair; with 24 partitions (N = 768) the pair loses 0.56 against 0.75;
     //  btps_tune("cluster", 1) forces it for every eligible plan, 0 switches it off)
     const bool cl_wanted = (g_tune.cluster > 0) ||
-                           (g_tune.cluster < 0 && kind == KIND_TRI && sizeof(T) == 8 && pl.P == 32 && batch >= (1ll << 19));
+                           (g_tune.cluster < 0 && kind == KIND_TRI && sizeof(T) == 8 && pl.P == 32 && batch >= (1ll << 22));
     const bool use_cl = (ks == 0) && cl_wanted && pl.ck.ent.func && tma_ok && (batch % pl.cshape.vec == 0);
     const Shape &sh = use_cl ? pl.cshape : pl.shape[ks];
     // the vectorised kernels need whole vectors: batch % vec == 0 and an aligned base pointer;
