@@ -27,6 +27,8 @@ def main():
     ap.add_argument("--log2-batch", type=int, nargs="+", default=[19])
     ap.add_argument("--batch", type=int, nargs="+", default=[], help="batch sizes that are not powers of two")
     ap.add_argument("--key", action="append", nargs="+", default=[], metavar=("NAME", "VALUE"))
+    ap.add_argument("--plan-key", action="append", nargs=2, default=[], metavar=("NAME", "VALUE"),
+                    help="tune key read when a handle is built (rows, lanes, vec, tiles_per_cta, ...): set once, before the factor call")
     ap.add_argument("--reps", type=int, default=8)
     ap.add_argument("--peak-gbs", type=float, default=6549.8)
     args = ap.parse_args()
@@ -36,6 +38,8 @@ def main():
     import paper_2107_05395_b200.binding as b
 
     n, r = args.n, 0.5
+    for k, v in args.plan_key:
+        b.btps_tune(k, int(v))
     dt = torch.float64 if args.dtype == "f64" else torch.float32
     if args.kind == "tri":
         h = b.tri_factor(np.full(n, -r), np.full(n, 1 + 2 * r), np.full(n, -r))
@@ -43,6 +47,7 @@ def main():
     else:
         h = b.penta_factor(np.full(n, r), np.full(n, -4 * r), np.full(n, 1 + 6 * r), np.full(n, -4 * r), np.full(n, r))
         solve = b.penta_solve_batched if args.dtype == "f64" else b.penta_solve_batched_f32
+    print("plan:", h.plan(8 if args.dtype == "f64" else 4), flush=True)
     keys = [k[0] for k in args.key]
     values = [[int(v) for v in k[1:]] for k in args.key]
     for m in [1 << lm for lm in args.log2_batch] + list(args.batch):
