@@ -55,8 +55,11 @@ def main():
     l = lbar.cpu().numpy()
     t = dt * np.arange(1, steps + 1)
     sel = t >= args.fit_from
-    r = float(np.corrcoef(np.log(t[sel]), l[sel])[0, 1])
-    slope, icpt = np.polyfit(np.log(t[sel]), l[sel], 1)
+    if int(sel.sum()) >= 3:
+        r = float(np.corrcoef(np.log(t[sel]), l[sel])[0, 1])
+        slope, icpt = np.polyfit(np.log(t[sel]), l[sel], 1)
+    else:  # a run shorter than the regression window: no fit
+        r = slope = icpt = float("nan")
     print(f"N={n} runs={args.runs} steps={steps} dt={dt:.6g} sigma={sigma:.6g} alpha={alpha:.6g}")
     print(f"wall {wall:.2f} s  ({wall / steps * 1e3:.4f} ms/step, {args.runs * steps / wall:.3e} run-steps/s)")
     print(f"max |mass drift| over the runs: {drift:.3e}   max |C|: {float(c.abs().max()):.4f}")
