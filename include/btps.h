@@ -229,6 +229,17 @@ BTPS_API int btps_tune(const char *key, int value);
 /* Number of kernel launches issued by this library in this process (bench.py's gpu_launches). */
 BTPS_API int64_t btps_launch_count(void);
 
+/* Which kernel a call would launch, without launching it: writes into buf (len bytes, NUL-terminated) the template
+ * arguments of sweep_kernel<...> exactly as profilers print them ("double, 2, 32, 0, 1, 1, 1, 0, 0" = element type,
+ * systems per thread, rows per thread, single partition, kind, TMA prefetch, warp scan, fused steps, cluster split),
+ * or "two_pass_kernel" for the 2R + 2W form.  kind as in btps_plan_info; batch and nsteps as in the call asked about
+ * (the choice depends on the batch's alignment and size and on nsteps > 1); an allocation-aligned base pointer is
+ * assumed.  bench.py uses it to check that a committed ncu capture (profiles/) is of the kernels it has just timed. */
+BTPS_API int btps_kernel_tag(int kind, const void *handle, int elem_bytes, int64_t batch, int nsteps, char *buf, int len);
+
+/* Identifier of this build of the library: a hash of the kernel sources, set by the build script. */
+BTPS_API const char *btps_build_id(void);
+
 #ifdef __cplusplus
 }
 #endif

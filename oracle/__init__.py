@@ -24,15 +24,24 @@ _LIB = os.path.join(_HERE, "liboracle.so")
 _lib = None
 
 
+def sanitized() -> bool:
+    """ORACLE_SANITIZE=1: build and load the oracle with AddressSanitizer + UndefinedBehaviorSanitizer (tests run the
+    pin suite once that way, in a child process that preloads libasan; see tests/test_oracle_sanitized.py)."""
+    return os.environ.get("ORACLE_SANITIZE", "") not in ("", "0")
+
+
 def build(force: bool = False) -> str:
     """Compile oracle.c with gcc (-O2, FMA contraction off, OpenMP over systems)."""
-    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
-        tmp = _LIB + f".tmp{os.getpid()}"
-        cmd = ["gcc", "-std=c99", "-O2", "-ffp-contract=off", "-fopenmp", "-fPIC", "-shared",
-               "-fvisibility=hidden", "-Wall", "-Wextra", "-o", tmp, _SRC, "-lm"]
+    lib = os.path.join(_HERE, "liboracle_san.so") if sanitized() else _LIB
+    if force or not os.path.exists(lib) or os.path.getmtime(lib) < os.path.getmtime(_SRC):
+        tmp = lib + f".tmp{os.getpid()}"
+        opt = ["-O1", "-g", "-fsanitize=address,undefined", "-fno-sanitize-recover=all", "-fno-omit-frame-pointer"] \
+            if sanitized() else ["-O2"]
+        cmd = ["gcc", "-std=c99"] + opt + ["-ffp-contract=off", "-fopenmp", "-fPIC", "-shared",
+                                           "-fvisibility=hidden", "-Wall", "-Wextra", "-o", tmp, _SRC, "-lm"]
         subprocess.run(cmd, check=True)
-        os.replace(tmp, _LIB)
-    return _LIB
+        os.replace(tmp, lib)
+    return lib
 
 
 _dp = ctypes.POINTER(ctypes.c_double)

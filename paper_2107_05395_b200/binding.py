@@ -15,7 +15,8 @@ EXPORTS = [
     "tri_solve_batched", "tri_solve_batched_f32", "penta_solve_batched", "penta_solve_batched_f32",
     "tri_solve_steps", "penta_solve_steps", "ch_step_batched", "ch_step_batched_stat", "tri_cn_step_batched", "penta_cn_step_batched",
     "tri_solve_batched_host", "penta_solve_batched_host", "ch_step_batched_host",
-    "btps_last_error", "btps_error_string", "btps_plan_info", "btps_tune", "btps_launch_count",
+    "btps_last_error", "btps_error_string", "btps_plan_info", "btps_tune", "btps_launch_count", "btps_kernel_tag",
+    "btps_build_id",
 ]
 
 
@@ -83,6 +84,10 @@ def _load() -> ctypes.CDLL:
     lib.btps_tune.restype = ci
     lib.btps_launch_count.argtypes = []
     lib.btps_launch_count.restype = i64
+    lib.btps_kernel_tag.argtypes = [ci, vp, ci, i64, ci, ctypes.c_char_p, ci]
+    lib.btps_kernel_tag.restype = ci
+    lib.btps_build_id.argtypes = []
+    lib.btps_build_id.restype = ctypes.c_char_p
     return lib
 
 
@@ -328,3 +333,14 @@ def btps_tune(key: str, value: int):
 
 def btps_launch_count() -> int:
     return int(_lib.btps_launch_count())
+
+
+def btps_kernel_tag(h: _Handle, elem_bytes: int, batch: int, nsteps: int = 1, kind: int = None) -> str:
+    """btps.h btps_kernel_tag: template arguments of the kernel such a call would launch (nothing is launched)."""
+    buf = ctypes.create_string_buffer(96)
+    _check(_lib.btps_kernel_tag(h.kind if kind is None else kind, h.ptr, elem_bytes, int(batch), int(nsteps), buf, 96))
+    return buf.value.decode()
+
+
+def btps_build_id() -> str:
+    return _lib.btps_build_id().decode()

@@ -44,6 +44,16 @@ def _run(cmd):
     return r.stdout + r.stderr
 
 
+def build_id() -> str:
+    """Hash of the kernel sources (csrc/*.cu, *.cuh, include/btps.h): what btps_build_id() returns."""
+    import hashlib
+    h = hashlib.sha1()
+    for name in sorted(UNITS) + HEADERS:
+        with open(name if os.path.isabs(name) else os.path.join(CSRC, name), "rb") as f:
+            h.update(f.read())
+    return h.hexdigest()[:12]
+
+
 def build(force: bool = False, verbose: bool = False) -> str:
     """Compile csrc/*.cu -> libbtps.so.  Returns the library path."""
     os.makedirs(OBJ, exist_ok=True)
@@ -51,10 +61,12 @@ def build(force: bool = False, verbose: bool = False) -> str:
     if not force and os.path.exists(LIB) and os.path.getmtime(LIB) >= src_time:
         return LIB
     nvcc = _nvcc()
+    bid = build_id()
 
     def compile_one(unit):
         obj = os.path.join(OBJ, unit.replace(".cu", ".o"))
         cmd = [nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + \
+              ([f'-DBTPS_BUILD_ID="{bid}"'] if unit == "btps.cu" else []) + \
               ["-c", os.path.join(CSRC, unit), "-o", obj]
         out = _run(cmd)
         if verbose:

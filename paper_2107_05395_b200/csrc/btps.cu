@@ -13,6 +13,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <map>
 #include <mutex>
 #include <vector>
 
@@ -761,10 +762,12 @@ int resolve_slot(Handle *h, const Shape &sh, KernelSlot &sl, bool cluster = fals
     std::lock_guard<std::mutex> lk(h->mu);
     if (sl.max_grid > 0) return BTPS_OK;
     if (!sl.ent.func) return set_err(BTPS_E_ARG);
-    if (sl.smem > 48 * 1024)
-        CU_TRY(cudaFuncSetAttribute(sl.ent.func, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sl.smem));
-    if (sl.fused.func && sl.smem > 48 * 1024)
-        CU_TRY(cudaFuncSetAttribute(sl.fused.func, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sl.smem));
+    // The attribute belongs to the kernel FUNCTION, which handles of different n share (sweep_kernel is not a
+    // template of P or n): every setter therefore asks for the same value, the per-CTA maximum of sm_100a, so
+    // that no handle ever lowers what another live handle needs (two handles of different n used in turn).
+    CU_TRY(cudaFuncSetAttribute(sl.ent.func, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_LIMIT));
+    if (sl.fused.func)
+        CU_TRY(cudaFuncSetAttribute(sl.fused.func, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_LIMIT));
     if (sl.fused.func) {
         // both instantiations do the same arithmetic for one step; ptxas sometimes spills tile rows in one and not
         // in the other (255-register variants), so take the one with the smaller local-memory frame
@@ -856,7 +859,7 @@ int make_tmap(CUtensorMap *tm, T *d_rhs, long long batch, int n, int W, unsigned
 // one sweep launch (kind = KIND_TRI / KIND_PENTA / KIND_CH) on a device buffer
 template <typename T>
 int launch_one(Handle *h, int kind, T *d_rhs, long long batch, double alpha_x, int reverse, int ksteps,
-               cudaStream_t st, double *stat = nullptr, const double *ex = nullptr)
+               cudaStream_t st, double *stat = nullptr, const double *ex = nullptr, const char **tag_out = nullptr)
 {
     DtypePlan &pl = h->plan[sizeof(T) == 8 ? 0 : 1];
     // a handle's tables live on the device that was current when it was factored
@@ -865,6 +868,10 @@ int launch_one(Handle *h, int kind, T *d_rhs, long long batch, double alpha_x, i
     // the paper's own 2R+2W form (Alg. 2 / 4), ksteps launches: plans too large for the on-chip tables,
     // and periodic CH shapes the partitioned kernels do not cover (n not a multiple of the rows per thread)
     auto two_pass = [&]() -> int {
+        if (tag_out) {  // btps_kernel_tag: name the kernel, launch nothing
+            *tag_out = "two_pass_kernel";
+            return BTPS_OK;
+        }
         const int block = 128;
         const long long grid = (batch + block - 1) / block;
         const T *co = (const T *)pl.d_soa;
@@ -927,7 +934,8 @@ int launch_one(Handle *h, int kind, T *d_rhs, long long batch, double alpha_x, i
     if (!pl.k[ks][s][d].ent.func) d = 1;
     KernelSlot &sl = use_cl ? pl.ck : pl.k[ks][s][d];
     if (!sl.ent.func) return two_pass();
-    if (sl.max_grid == 0) {
+    {
+        // takes the handle's lock: max_grid / prefer_fused are written by the first launch of this slot
         const int rc = resolve_slot(h, sh, sl, use_cl);
         if (rc != BTPS_OK) return rc;
     }
@@ -985,6 +993,11 @@ int launch_one(Handle *h, int kind, T *d_rhs, long long batch, double alpha_x, i
     a.offR = sl.offR;
     a.box_rows = sl.box_rows;
     a.nboxes = sl.nboxes;
+    if (tag_out) {  // btps_kernel_tag: name the kernel this call would launch, launch nothing
+        const bool f1 = g_tune.one_step_fused >= 0 ? g_tune.one_step_fused > 0 : sl.prefer_fused != 0;
+        *tag_out = (((ksteps > 1 || stat || f1) && sl.fused.func) ? sl.fused : sl.ent).tag;
+        return BTPS_OK;
+    }
     CUtensorMap tm;
     memset(&tm, 0, sizeof(tm));
     if (sl.tma) {
@@ -1062,31 +1075,61 @@ int solve_steps(const void *hv, int magic, int kind, T *d_rhs, int64_t batch, do
 // host-buffer path: column chunks, 3 streams, strided 2-D copies in and out
 // ------------------------------------------------------------------------------------------------
 struct HostPipe {
-    std::mutex mu;
+    std::mutex mu;  // one host-buffer call at a time per device
     static constexpr int NBUF = 3;
     cudaStream_t st[NBUF] = {nullptr, nullptr, nullptr};
     void *buf[NBUF] = {nullptr, nullptr, nullptr};
     size_t cap = 0;
     bool ready = false;
 };
-HostPipe g_pipe;
 
-int pipe_prepare(size_t bytes)
+// one pipe (3 streams + 3 staging buffers) per CUDA device, created on first use with that device current
+std::mutex g_pipes_mu;
+std::map<int, HostPipe *> g_pipes;
+
+HostPipe *pipe_for(int device)
 {
-    if (!g_pipe.ready) {
-        for (int i = 0; i < HostPipe::NBUF; ++i) CU_TRY(cudaStreamCreateWithFlags(&g_pipe.st[i], cudaStreamNonBlocking));
-        g_pipe.ready = true;
+    std::lock_guard<std::mutex> lk(g_pipes_mu);
+    HostPipe *&p = g_pipes[device];
+    if (!p) p = new HostPipe();
+    return p;
+}
+
+int pipe_prepare(HostPipe &pp, size_t bytes)
+{
+    if (!pp.ready) {
+        for (int i = 0; i < HostPipe::NBUF; ++i) CU_TRY(cudaStreamCreateWithFlags(&pp.st[i], cudaStreamNonBlocking));
+        pp.ready = true;
     }
-    if (bytes > g_pipe.cap) {
+    if (bytes > pp.cap) {
         for (int i = 0; i < HostPipe::NBUF; ++i) {
-            if (g_pipe.buf[i]) CU_TRY(cudaFree(g_pipe.buf[i]));
-            g_pipe.buf[i] = nullptr;
+            if (pp.buf[i]) CU_TRY(cudaFree(pp.buf[i]));
+            pp.buf[i] = nullptr;
         }
-        g_pipe.cap = 0;
-        for (int i = 0; i < HostPipe::NBUF; ++i) CU_TRY(cudaMalloc(&g_pipe.buf[i], bytes));
-        g_pipe.cap = bytes;
+        pp.cap = 0;
+        for (int i = 0; i < HostPipe::NBUF; ++i) CU_TRY(cudaMalloc(&pp.buf[i], bytes));
+        pp.cap = bytes;
     }
     return BTPS_OK;
+}
+
+// strided host <-> device copy of a column chunk: [n rows] x [w systems], host pitch = batch elements.
+// cudaMemcpy2DAsync takes pitches up to cudaDevAttrMaxPitch (2^31 - 1 bytes); wider batches go row by row.
+template <typename T>
+cudaError_t copy_chunk(T *dev, T *host, long long w, long long batch, int n, bool to_device, cudaStream_t st)
+{
+    const size_t hp = (size_t)batch * sizeof(T), dp = (size_t)w * sizeof(T);
+    if (hp <= (size_t)0x7fffffff) {
+        return to_device ? cudaMemcpy2DAsync(dev, dp, host, hp, dp, (size_t)n, cudaMemcpyHostToDevice, st)
+                         : cudaMemcpy2DAsync(host, hp, dev, dp, dp, (size_t)n, cudaMemcpyDeviceToHost, st);
+    }
+    for (int i = 0; i < n; ++i) {
+        const cudaError_t e = to_device
+            ? cudaMemcpyAsync(dev + (size_t)i * w, host + (size_t)i * batch, dp, cudaMemcpyHostToDevice, st)
+            : cudaMemcpyAsync(host + (size_t)i * batch, dev + (size_t)i * w, dp, cudaMemcpyDeviceToHost, st);
+        if (e != cudaSuccess) return e;
+    }
+    return cudaSuccess;
 }
 
 template <typename T>
@@ -1094,37 +1137,51 @@ int solve_host(const void *hv, int magic, int kind, T *h_rhs, int64_t batch, dou
 {
     Handle *h = check(hv, magic);
     if (!h || !h_rhs || batch < 1 || nsteps < 0) return set_err(BTPS_E_ARG);
-    std::lock_guard<std::mutex> lk(g_pipe.mu);
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev != h->device) return set_err(BTPS_E_DEVICE);
+    HostPipe &pp = *pipe_for(dev);
+    std::lock_guard<std::mutex> lk(pp.mu);
     const int n = h->n;
-    // chunk width: about 32 MiB per chunk, a multiple of 256 systems, at least 4 chunks when possible
+    // chunk width: about 32 MiB per chunk, a multiple of 256 systems; batches that would give fewer than 4 chunks are
+    // cut into 4 (down to 256 systems per chunk) so that copies in, kernels and copies out of different chunks overlap
     const size_t target = g_tune.host_chunk_kib > 0 ? ((size_t)g_tune.host_chunk_kib << 10) : (32ull << 20);
     long long wc = (long long)(target / ((size_t)n * sizeof(T)));
-    wc = (wc / 256) * 256;
+    if (g_tune.host_chunk_kib <= 0 && wc * 4 > batch) wc = (batch + 3) / 4;
+    wc = ((wc + 255) / 256) * 256;
     if (wc < 256) wc = 256;
     if (wc > batch) wc = batch;
     const size_t chunk_bytes = (size_t)n * wc * sizeof(T);
-    int rc = pipe_prepare(chunk_bytes);
+    int rc = pipe_prepare(pp, chunk_bytes);
     if (rc != BTPS_OK) return rc;
     const bool rev = g_tune.reverse > 0;
+    // any failure inside the loop: stop issuing, then wait for what is already in flight -- asynchronous copies
+    // must not still be writing into the caller's buffer after this call has returned
+    cudaError_t cerr = cudaSuccess;
+    const char *what = "";
     int ci = 0;
-    for (long long j0 = 0; j0 < batch; j0 += wc, ++ci) {
+    for (long long j0 = 0; j0 < batch && rc == BTPS_OK && cerr == cudaSuccess; j0 += wc, ++ci) {
         const long long w = (batch - j0 < wc) ? (batch - j0) : wc;
         const int b = ci % HostPipe::NBUF;
-        cudaStream_t st = g_pipe.st[b];
-        T *d = (T *)g_pipe.buf[b];
-        CU_TRY(cudaMemcpy2DAsync(d, (size_t)w * sizeof(T), h_rhs + j0, (size_t)batch * sizeof(T),
-                                 (size_t)w * sizeof(T), (size_t)n, cudaMemcpyHostToDevice, st));
+        cudaStream_t st = pp.st[b];
+        T *d = (T *)pp.buf[b];
+        cerr = copy_chunk<T>(d, h_rhs + j0, w, batch, n, true, st);
+        if (cerr != cudaSuccess) { what = "host-to-device chunk copy"; break; }
         const int kmax = fuse_limit(h->plan[sizeof(T) == 8 ? 0 : 1]);
-        for (int s = 0, l = 0; s < nsteps; ++l) {
+        for (int s = 0, l = 0; s < nsteps && rc == BTPS_OK; ++l) {
             const int k = (nsteps - s < kmax) ? (nsteps - s) : kmax;
             rc = launch_one<T>(h, kind, d, w, alpha_x, rev ? (l & 1) : 0, k, st);
-            if (rc != BTPS_OK) return rc;
             s += k;
         }
-        CU_TRY(cudaMemcpy2DAsync(h_rhs + j0, (size_t)batch * sizeof(T), d, (size_t)w * sizeof(T),
-                                 (size_t)w * sizeof(T), (size_t)n, cudaMemcpyDeviceToHost, st));
+        if (rc != BTPS_OK) break;
+        cerr = copy_chunk<T>(d, h_rhs + j0, w, batch, n, false, st);
+        if (cerr != cudaSuccess) { what = "device-to-host chunk copy"; break; }
     }
-    for (int i = 0; i < HostPipe::NBUF; ++i) CU_TRY(cudaStreamSynchronize(g_pipe.st[i]));
+    for (int i = 0; i < HostPipe::NBUF; ++i) {
+        const cudaError_t e = cudaStreamSynchronize(pp.st[i]);
+        if (e != cudaSuccess && cerr == cudaSuccess) { cerr = e; what = "cudaStreamSynchronize"; }
+    }
+    if (rc != BTPS_OK) return rc;
+    if (cerr != cudaSuccess) return cuda_fail(cerr, what);
     return set_err(BTPS_OK);
 }
 
@@ -1514,5 +1571,29 @@ int btps_tune(const char *key, int value)
 }
 
 int64_t btps_launch_count(void) { return (int64_t)g_launches.load(std::memory_order_relaxed); }
+
+#ifndef BTPS_BUILD_ID
+#define BTPS_BUILD_ID "unknown"
+#endif
+const char *btps_build_id(void) { return BTPS_BUILD_ID; }
+
+int btps_kernel_tag(int kind, const void *handle, int elem_bytes, int64_t batch, int nsteps, char *buf, int len)
+{
+    if (kind < 0 || kind > 4 || !buf || len < 1 || batch < 1 || nsteps < 1 || (elem_bytes != 8 && elem_bytes != 4))
+        return set_err(BTPS_E_ARG);
+    Handle *h = check(handle, (kind == 0 || kind == 3) ? MAGIC_TRI : MAGIC_PENTA);
+    if (!h) return set_err(BTPS_E_ARG);
+    static const int kinds[5] = {KIND_TRI, KIND_PENTA, KIND_CH, KIND_TRICN, KIND_PENTACN};
+    if (elem_bytes == 4 && kind >= 2) return set_err(BTPS_E_ARG);  // the fused steps are fp64 only
+    const char *tag = nullptr;
+    // a base pointer aligned like a fresh allocation: the choice depends on the alignment of pointer and pitch only
+    void *fake = (void *)(uintptr_t)4096;
+    const double ex[5] = {0, 1, 0, 0, 0};
+    const int rc = elem_bytes == 8 ? launch_one<double>(h, kinds[kind], (double *)fake, batch, 0.0, 0, nsteps, nullptr, nullptr, ex, &tag)
+                                   : launch_one<float>(h, kinds[kind], (float *)fake, batch, 0.0, 0, nsteps, nullptr, nullptr, ex, &tag);
+    if (rc != BTPS_OK) return rc;
+    snprintf(buf, (size_t)len, "%s", tag ? tag : "");
+    return set_err(BTPS_OK);
+}
 
 }  // extern "C"

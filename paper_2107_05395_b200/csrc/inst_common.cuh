@@ -2,6 +2,7 @@
 // kind and element type so that nvcc compiles them in parallel).
 #pragma once
 #include "sweep.cuh"
+#include <cstdio>
 
 namespace btps {
 
@@ -12,6 +13,11 @@ static SweepEntry make_entry()
     e.launch = &launch_sweep<T, V, MR, SINGLE, KIND, TMA, WS, FUSE, CL>;
     e.func = reinterpret_cast<const void *>(&sweep_kernel<T, V, MR, SINGLE, KIND, TMA, WS, FUSE, CL>);
     e.max_threads = CtaShape<T, V, MR>::MAX_THREADS;
+    static char tag[64];
+    static const int once = snprintf(tag, sizeof(tag), "%s, %d, %d, %d, %d, %d, %d, %d, %d", sizeof(T) == 8 ? "double" : "float", V,
+                                     MR, (int)SINGLE, KIND, (int)TMA, (int)WS, (int)FUSE, (int)CL);
+    (void)once;
+    e.tag = tag;
     return e;
 }
 

@@ -1340,6 +1340,7 @@ struct SweepEntry {
     sweep_launch_fn launch;
     const void *func;  // for cudaFuncSetAttribute / occupancy queries
     int max_threads;   // threads per CTA the kernel was compiled for
+    const char *tag;   // the template arguments as profilers print them: "double, 2, 32, 0, 0, 1, 1, 0, 0"
 };
 
 template <typename T, int V, int MR, bool SINGLE, int KIND, bool TMA, bool WS, bool FUSE, bool CL = false>
