@@ -317,6 +317,10 @@ def time_in_graph(torch, fn_of_buf, bufs, launches, repeats=3):
     return ts[len(ts) // 2]
 
 
+KIND_INDEX = {"tri": 0, "tri_periodic": 0, "tri_f32s": 0, "penta": 1, "penta_periodic": 1, "penta_f32s": 1, "ch": 2,
+              "ch_periodic": 2}
+
+
 def make_cell(torch, b, inputs, kind, n, batch, elem, steps_per_call=1):
     """(handle, fn(buf, stream=None), buffers) of one cell; buffers rotate when one would stay in L2."""
     dt = torch.float64 if elem == 8 else torch.float32
@@ -327,7 +331,13 @@ def make_cell(torch, b, inputs, kind, n, batch, elem, steps_per_call=1):
         t = torch.empty(n, batch, dtype=dt, device="cuda")
         inputs.fill_uniform_device(t, n, seed=100 + k, scale=0.1 if kind.startswith("ch") else 1.0)
         bufs.append(t)
-    if kind in ("tri", "tri_periodic"):
+    if kind == "tri_f32s":
+        h = b.tri_factor(*inputs.tri_lhs(n, 0.5))
+        fn = lambda t, s=None: b.tri_solve_batched_f32s(h, t, s)
+    elif kind == "penta_f32s":
+        h = b.penta_factor(*inputs.penta_lhs(n, 0.5))
+        fn = lambda t, s=None: b.penta_solve_batched_f32s(h, t, s)
+    elif kind in ("tri", "tri_periodic"):
         h = b.tri_factor(*inputs.tri_lhs(n, 0.5)) if kind == "tri" else b.tri_factor_periodic(*inputs.tri_lhs(n, 0.5))
         one = b.tri_solve_batched if elem == 8 else b.tri_solve_batched_f32
         fn = (lambda t, s=None: one(h, t, s)) if steps_per_call == 1 else \
@@ -372,12 +382,12 @@ def extra_table(torch, b, inputs, peak):
             extra.update({"fused_steps_per_launch": min(64, steps_per_call), "ms_per_solve_one_step_per_launch": round(ms1, 5),
                           "frac_one_step_per_launch": round(2.0 * size / ms1 / 1e6 / peak, 4),
                           "note": "frac is effective (per-step algorithmic bytes / time)"})
-        kidx = {"tri": 0, "tri_periodic": 0, "penta": 1, "penta_periodic": 1, "ch": 2, "ch_periodic": 2}[kind]
+        kidx = KIND_INDEX[kind]
         out.append({"config": name, "kind": kind, "n": n, "batch": batch, "dtype": "f64" if elem == 8 else "f32",
                     **extra, "ms_per_solve": round(ms, 5), "systems_per_s": batch / ms * 1e3,
                     "hbm_gbs": round(gbs, 1), "frac": round(gbs / peak, 4),
                     "cold": "rotating %d buffers" % len(bufs) if len(bufs) > 1 else "buffer > 2x L2",
-                    "kernel": b.btps_kernel_tag(h, elem, batch, steps_per_call, kind=kidx)})
+                    "kernel": b.btps_kernel_tag(h, 12 if kind.endswith("f32s") else elem, batch, steps_per_call, kind=kidx)})
         del bufs
         torch.cuda.empty_cache()
 
@@ -392,6 +402,10 @@ def extra_table(torch, b, inputs, peak):
         entry("f1 periodic (single step)", "ch_periodic", n, 65536, 8)
     entry("f1 periodic CH, 2^20 runs (1000 steps per call)", "ch_periodic", 256, 1 << 20, 8, steps_per_call=1000,
           launches=1)
+    # fp32 in HBM, fp64 arithmetic (algorithmic bytes = 2 * N * M * 4)
+    for kind in ("tri_f32s", "penta_f32s"):
+        for n, lb in ((512, 16), (64, 20), (256, 20), (1024, 19)):
+            entry("f4 fp32 storage, fp64 sweeps", kind, n, 1 << lb, 4)
     # systems longer than 1024 rows
     for kind in ("tri", "penta"):
         for n in (2048, 4096):
@@ -458,9 +472,10 @@ def run_cells(args):
         fn(bufs[0])
         ms = time_launches(torch, fn, bufs, max(4, min(20, len(bufs))), repeats=5)
         gbs = 2.0 * n * batch * elem / ms / 1e6
-        kidx = {"tri": 0, "tri_periodic": 0, "penta": 1, "penta_periodic": 1, "ch": 2, "ch_periodic": 2}[kind]
+        kidx = KIND_INDEX[kind]
         print(json.dumps({"cell": cell, "tune": args.tune, "ms": round(ms, 5), "hbm_gbs": round(gbs, 1),
-                          "frac": round(gbs / peak, 4), "kernel": b.btps_kernel_tag(h, elem, batch, 1, kind=kidx),
+                          "frac": round(gbs / peak, 4),
+                          "kernel": b.btps_kernel_tag(h, 12 if kind.endswith("f32s") else elem, batch, 1, kind=kidx),
                           "plan": h.ch_plan(elem) if kind.startswith("ch") else h.plan(elem)}), flush=True)
         del bufs
         torch.cuda.empty_cache()

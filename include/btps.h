@@ -122,6 +122,18 @@ BTPS_API int penta_solve_batched(penta_handle_t h, double *d_rhs, int64_t batch,
 BTPS_API int penta_solve_batched_f32(penta_handle_t h, float *d_rhs, int64_t batch, void *stream);
 
 /* ------------------------------------------------------------------------------------------
+ * The same solves with the batch STORED in fp32 and every sweep COMPUTED in fp64 (storage type /=
+ * compute type).  d_rhs: DEVICE, n*batch floats, interleaved, solved in place: each element is read once as a float,
+ * widened to double, carried through the forward elimination, back-substitution and carry correction in fp64 registers
+ * with the handle's fp64 tables (eq. 3-6 / Sec. 4.1 as above), and rounded to float once when it is stored.  HBM moves
+ * half the bytes of the fp64 calls; the result is the fp64 solution of the (exactly representable) float right-hand
+ * side, rounded to nearest float -- about 6e-8 relative to each entry, against ~1e-6 for the all-fp32 *_f32 calls.
+ * Non-periodic handles with n <= 1024 (the register-resident plans); other handles fail with BTPS_E_ARG.
+ * ---------------------------------------------------------------------------------------- */
+BTPS_API int tri_solve_batched_f32s(tri_handle_t h, float *d_rhs, int64_t batch, void *stream);
+BTPS_API int penta_solve_batched_f32s(penta_handle_t h, float *d_rhs, int64_t batch, void *stream);
+
+/* ------------------------------------------------------------------------------------------
  * (a6) Time-step driver: nsteps successive solves with RHS = previous solution (the paper
  * times "just the time-stepping sections"; implicit diffusion / hyperdiffusion
  * loops PAPER.md:120-136, 288-296, in BASELINE.json's backward-Euler form, C-22).
@@ -230,9 +242,10 @@ BTPS_API int btps_tune(const char *key, int value);
 BTPS_API int64_t btps_launch_count(void);
 
 /* Which kernel a call would launch, without launching it: writes into buf (len bytes, NUL-terminated) the template
- * arguments of sweep_kernel<...> exactly as profilers print them ("double, 2, 32, 0, 1, 1, 1, 0, 0" = element type,
- * systems per thread, rows per thread, single partition, kind, TMA prefetch, warp scan, fused steps, cluster split),
- * or "two_pass_kernel" for the 2R + 2W form.  kind as in btps_plan_info; batch and nsteps as in the call asked about
+ * arguments of sweep_kernel<...> exactly as profilers print them ("double, 2, 32, 0, 1, 1, 1, 0, 0, double" = arithmetic
+ * type, systems per thread, rows per thread, single partition, kind, TMA prefetch, warp scan, fused steps, cluster
+ * split, storage type), or "two_pass_kernel" for the 2R + 2W form.  kind as in btps_plan_info; elem_bytes 8, 4, or 12
+ * for the *_f32s calls (4-byte storage, 8-byte arithmetic); batch and nsteps as in the call asked about
  * (the choice depends on the batch's alignment and size and on nsteps > 1); an allocation-aligned base pointer is
  * assumed.  bench.py uses it to check that a committed ncu capture (profiles/) is of the kernels it has just timed. */
 BTPS_API int btps_kernel_tag(int kind, const void *handle, int elem_bytes, int64_t batch, int nsteps, char *buf, int len);

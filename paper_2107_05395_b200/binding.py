@@ -13,6 +13,7 @@ _LIB_PATH = os.path.join(_HERE, "libbtps.so")
 EXPORTS = [
     "tri_factor", "tri_factor_periodic", "tri_destroy", "penta_factor", "penta_factor_periodic", "penta_destroy",
     "tri_solve_batched", "tri_solve_batched_f32", "penta_solve_batched", "penta_solve_batched_f32",
+    "tri_solve_batched_f32s", "penta_solve_batched_f32s",
     "tri_solve_steps", "penta_solve_steps", "ch_step_batched", "ch_step_batched_stat", "tri_cn_step_batched", "penta_cn_step_batched",
     "tri_solve_batched_host", "penta_solve_batched_host", "ch_step_batched_host",
     "btps_last_error", "btps_error_string", "btps_plan_info", "btps_tune", "btps_launch_count", "btps_kernel_tag",
@@ -52,7 +53,7 @@ def _load() -> ctypes.CDLL:
     lib.penta_destroy.argtypes = [vp]
     lib.penta_destroy.restype = None
     for name in ("tri_solve_batched", "tri_solve_batched_f32", "penta_solve_batched",
-                 "penta_solve_batched_f32"):
+                 "penta_solve_batched_f32", "tri_solve_batched_f32s", "penta_solve_batched_f32s"):
         fn = getattr(lib, name)
         fn.argtypes = [vp, vp, i64, vp]
         fn.restype = ci
@@ -207,20 +208,39 @@ def penta_factor_periodic(e, a, d, c, f) -> PentaHandle:
     return PentaHandle(ptr, n)
 
 
+_torch = None
+_raw_stream = None
+
+
+def _torch_mod():
+    """torch, imported on first use (callers hold device memory in torch tensors; nothing here computes with it)."""
+    global _torch, _raw_stream
+    if _torch is None:
+        import torch
+        _torch = torch
+        # the current stream's raw handle without building a torch.cuda.Stream object (the object costs ~3 us per call)
+        _raw_stream = getattr(torch._C, "_cuda_getCurrentRawStream", None)
+    return _torch
+
+
 def _dev_args(h: _Handle, t, elem_bytes: int):
     """t: a CUDA torch tensor holding n*batch elements (any shape, contiguous) -> (ptr, batch)."""
+    torch = _torch or _torch_mod()
+    if t.dtype is not (torch.float64 if elem_bytes == 8 else torch.float32):
+        raise ValueError(f"expected a floating tensor with {elem_bytes}-byte elements")
     if not t.is_cuda or not t.is_contiguous():
         raise ValueError("expected a contiguous CUDA tensor")
-    if t.element_size() != elem_bytes or not t.dtype.is_floating_point:
-        raise ValueError(f"expected a floating tensor with {elem_bytes}-byte elements")
-    if t.numel() % h.n:
+    size = t.numel()
+    if size % h.n:
         raise ValueError("tensor size is not a multiple of n")
-    return t.data_ptr(), t.numel() // h.n
+    return t.data_ptr(), size // h.n
 
 
 def _stream(stream):
     if stream is None:
-        import torch
+        torch = _torch or _torch_mod()
+        if _raw_stream is not None:
+            return _raw_stream(torch.cuda.current_device())
         return torch.cuda.current_stream().cuda_stream
     return int(stream)
 
@@ -243,6 +263,17 @@ def penta_solve_batched(h: PentaHandle, rhs, stream=None):
 def penta_solve_batched_f32(h: PentaHandle, rhs, stream=None):
     p, batch = _dev_args(h, rhs, 4)
     _check(_lib.penta_solve_batched_f32(h.ptr, p, batch, _stream(stream)))
+
+
+def tri_solve_batched_f32s(h: TriHandle, rhs, stream=None):
+    """btps.h tri_solve_batched_f32s: float32 tensor in HBM, fp64 arithmetic."""
+    p, batch = _dev_args(h, rhs, 4)
+    _check(_lib.tri_solve_batched_f32s(h.ptr, p, batch, _stream(stream)))
+
+
+def penta_solve_batched_f32s(h: PentaHandle, rhs, stream=None):
+    p, batch = _dev_args(h, rhs, 4)
+    _check(_lib.penta_solve_batched_f32s(h.ptr, p, batch, _stream(stream)))
 
 
 def tri_solve_steps(h: TriHandle, rhs, nsteps: int, stream=None):

@@ -22,7 +22,7 @@ NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", 
 UNITS = ["btps.cu"] + [f"inst_{k}_{t}.cu" for k in ("tri", "penta", "ch", "trip", "pentap", "chp") for t in ("f64", "f32")] + \
         ["inst_tricn_f64.cu", "inst_tricnp_f64.cu", "inst_pentacn_f64.cu", "inst_pentacnp_f64.cu",
          "inst_pentapf_f64.cu", "inst_pentapf_f32.cu", "inst_chpf_f64.cu", "inst_pentacnpf_f64.cu",
-         "inst_tripf_f64.cu", "inst_tripf_f32.cu", "inst_tricnpf_f64.cu"]
+         "inst_tripf_f64.cu", "inst_tripf_f32.cu", "inst_tricnpf_f64.cu", "inst_f32s.cu"]
 HEADERS = ["sweep.cuh", "inst_common.cuh", os.path.join(ROOT, "include", "btps.h")]
 
 

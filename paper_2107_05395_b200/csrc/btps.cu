@@ -15,6 +15,7 @@
 #include <cstring>
 #include <map>
 #include <mutex>
+#include <type_traits>
 #include <vector>
 
 using namespace btps;
@@ -70,7 +71,7 @@ struct KernelSlot {
     int xvals = 2;     // exchange values per (partition, system)
     int xstride = 0, xper = 0;  // exchange elements per group; offset of the periodic-penta values in it
     size_t smem = 0;
-    unsigned offX = 0, offM = 0, offR = 0, offTl = 0;
+    unsigned offX = 0, offM = 0, offR = 0, offTl = 0, offIn = 0;
     unsigned box_rows = 0, nboxes = 0;
     int max_grid = 0;  // occupancy * SM count, resolved at first launch
 };
@@ -96,7 +97,14 @@ struct DtypePlan {
     // [kind slot][vector mode: 0 = plan.vec, 1 = scalar tail-safe][0 = TMA prefetch, 1 = direct loads]
     // kind slot 0 = solve, 1 = CH (penta handles only)
     KernelSlot k[3][2][2];
-    // plain solves of long systems (16 < P <= 32): the tile's rows split over a cluster of two CTAs
+    // fp64 plan only: the plain solve on fp32 storage (the *_f32s calls): [vector mode][0 = TMA prefetch, 1 = direct loads]
+    KernelSlot ks32[2][2];
+    // plain solves of long systems (P > 16): the tile's rows split over a thread-block cluster of csz CTAs (two, four
+    // or eight SMs), each keeping PLc partitions; carries cross the CTAs as a chain through distributed shared memory
+    int csz = 0, PLc = 0, scan_log2_cl = 0;
+    unsigned offTc = 0;         // byte offset in the blob of the csz per-CTA scan-table blocks
+    unsigned tab_bytes_cl = 0;  // bytes of one such block
+    unsigned blob_total = 0;    // blob bytes on the device (blob_bytes = what the single-CTA kernels stage)
     Shape cshape;
     KernelSlot ck;
 };
@@ -183,6 +191,22 @@ void choose_plan(int n, int elem, int handle_kind, DtypePlan &pl)
         while (Pp <= 32 && !fits(Pp)) ++Pp;
         if (Pp <= 32) P = Pp;
         else ws = 0;
+    }
+    // cluster-chain plan (sweep.cuh, CL): csz = 2 / 4 / 8 CTAs with at most 16 partitions each (16 lanes x 16 bytes =
+    // 256-byte row segments); whole warps per CTA want an even number of partitions per CTA
+    pl.csz = pl.PLc = 0;
+    if (rows == 32 && P > 16 && g_tune.cluster != 0 && g_tune.prefetch != 0) {
+        const int k = P <= 32 ? 2 : (P + 15) / 16;  // as few CTAs as 16 partitions each allow; at most 8 (portable cluster size)
+        if (k <= 8) {
+            int PLc = (P + k - 1) / k;
+            PLc += (PLc & 1);
+            if (PLc <= 16 && (k * PLc == P || P > 32)) {
+                pl.csz = k;
+                pl.PLc = PLc;
+                pl.scan_log2_cl = ilog2(PLc);
+                if (P > 32) P = k * PLc;  // no warp-scan plan of one CTA exists: pad to whole CTAs (identity partitions)
+            }
+        }
     }
     pl.two_pass = (g_tune.force_two_pass > 0);
     for (int k = 0; k < nshape; ++k) {
@@ -297,19 +321,33 @@ Mat matmul(const Mat &x, const Mat &y, int nc)
     return r;
 }
 
+// scan-table slots of the partitions [q0, q0 + P) at byte offset `base` of the blob, tq entries per table row
 template <typename T>
-void put_scan_tables(std::vector<unsigned char> &blob, const DtypePlan &pl, int nc, const std::vector<Mat> &Phi,
-                     const std::vector<Mat> &Psi, const std::vector<Mat> &Chi0)
+void put_scan_slots(std::vector<unsigned char> &blob, size_t base, int q0, int P, int tq, int nc, bool ws, bool chain,
+                    const std::vector<Mat> &PhiAll, const std::vector<Mat> &PsiAll, const std::vector<Mat> &Chi0All)
 {
-    const int P = pl.P, tq = pl.tq, ne = nc * nc;
+    const int ne = nc * nc;
+    const std::vector<Mat> Phi(PhiAll.begin() + q0, PhiAll.begin() + q0 + P), Psi(PsiAll.begin() + q0, PsiAll.begin() + q0 + P),
+        Chi0(Chi0All.begin() + q0, Chi0All.begin() + q0 + P);
     auto put_slot = [&](int slot, const std::vector<Mat> &v) {
         for (int q = 0; q < P; ++q)
             for (int m = 0; m < ne; ++m)
-                put<T>(blob, pl.offT + (((size_t)slot * ne + m) * tq + q) * sizeof(T), v[q].m[m]);
+                put<T>(blob, base + (((size_t)slot * ne + m) * tq + q) * sizeof(T), v[q].m[m]);
     };
     put_slot(0, Phi);
     put_slot(1, Psi);
-    if (!pl.ws) return;
+    if (!ws) return;
+    if (chain) {
+        // cluster chain (sweep.cuh, CL): how a carry that enters this block of partitions from the neighbouring CTA reaches
+        // partition q -- slot 10: Phi_q Phi_{q-1} ... Phi_first (forward), slot 11: Psi_q Psi_{q+1} ... Psi_last (backward)
+        std::vector<Mat> Fi(P), Bi(P);
+        Fi[0] = Phi[0];
+        for (int q = 1; q < P; ++q) Fi[q] = matmul(Phi[q], Fi[q - 1], nc);
+        Bi[P - 1] = Psi[P - 1];
+        for (int q = P - 2; q >= 0; --q) Bi[q] = matmul(Psi[q], Bi[q + 1], nc);
+        put_slot(10, Fi);
+        put_slot(11, Bi);
+    }
     std::vector<Mat> A = Phi, B = Psi;
     const Mat zero;
     // step 0 multipliers: no partner below / above the ends
@@ -337,6 +375,51 @@ void put_scan_tables(std::vector<unsigned char> &blob, const DtypePlan &pl, int 
         }
     }
     put_slot(9, Chi0);
+}
+
+template <typename T>
+void put_scan_tables(std::vector<unsigned char> &blob, DtypePlan &pl, int nc, const std::vector<Mat> &Phi,
+                     const std::vector<Mat> &Psi, const std::vector<Mat> &Chi0)
+{
+    put_scan_slots<T>(blob, pl.offT, 0, pl.P, pl.tq, nc, pl.ws != 0, false, Phi, Psi, Chi0);
+    pl.blob_total = pl.blob_bytes;
+    if (pl.csz) {
+        // one table block per CTA of the cluster chain, behind everything the single-CTA kernels stage
+        pl.offTc = pl.blob_bytes;
+        pl.tab_bytes_cl = (unsigned)align16((size_t)13 * nc * nc * SCAN_LANES * sizeof(T));
+        pl.blob_total = pl.offTc + (unsigned)pl.csz * pl.tab_bytes_cl;
+        blob.resize(pl.blob_total, 0);
+        const int k = pl.csz, PL = pl.PLc, ne = nc * nc;
+        for (int r = 0; r < k; ++r)
+            put_scan_slots<T>(blob, pl.offTc + (size_t)r * pl.tab_bytes_cl, r * PL, PL, SCAN_LANES, nc, true, true, Phi, Psi, Chi0);
+        // slot 12 of CTA r's block: how the other CTAs' contributions reach it.  Entry s < r: C_{r,s} = PhiT_{r-1} ... PhiT_{s+1}
+        // (forward; PhiT_c = product of the Phi of CTA c's partitions, identity for s = r - 1); entry 8 + s, s > r:
+        // D_{r,s} = PsiT_{r+1} ... PsiT_{s-1} (backward, identity for s = r + 1).
+        std::vector<Mat> PhiT(k), PsiT(k);
+        for (int c = 0; c < k; ++c) {
+            Mat f = Phi[c * PL], b = Psi[c * PL + PL - 1];
+            for (int q = 1; q < PL; ++q) f = matmul(Phi[c * PL + q], f, nc);
+            for (int q = PL - 2; q >= 0; --q) b = matmul(Psi[c * PL + q], b, nc);
+            PhiT[c] = f;
+            PsiT[c] = b;
+        }
+        Mat ident;
+        ident.m[0] = 1.0;
+        if (nc == 2) ident.m[3] = 1.0;
+        for (int r = 0; r < k; ++r) {
+            const size_t base = pl.offTc + (size_t)r * pl.tab_bytes_cl + (size_t)12 * ne * SCAN_LANES * sizeof(T);
+            Mat c = ident;
+            for (int sb = r - 1; sb >= 0; --sb) {
+                if (sb < r - 1) c = matmul(c, PhiT[sb + 1], nc);
+                for (int m = 0; m < ne; ++m) put<T>(blob, base + ((size_t)m * SCAN_LANES + sb) * sizeof(T), c.m[m]);
+            }
+            Mat d = ident;
+            for (int sb = r + 1; sb < k; ++sb) {
+                if (sb > r + 1) d = matmul(d, PsiT[sb - 1], nc);
+                for (int m = 0; m < ne; ++m) put<T>(blob, base + ((size_t)m * SCAN_LANES + 8 + sb) * sizeof(T), d.m[m]);
+            }
+        }
+    }
 }
 
 size_t scan_table_bytes(const DtypePlan &pl, int nc, size_t elem)
@@ -570,8 +653,9 @@ constexpr size_t SMEM_LIMIT = 227 * 1024;
 size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
 // shared-memory layout of one kernel variant: [blob][exchange][mbarriers][ring]
-void layout_slot(const DtypePlan &pl, const Shape &sh, int kind, KernelSlot &sl, bool halo = true)
+void layout_slot(const DtypePlan &pl, const Shape &sh, int kind, KernelSlot &sl, bool halo = true, int selem = 0)
 {
+    if (selem == 0) selem = pl.elem;  // bytes per element of the batch in global memory / in the ring
     const bool tri = (kind == KIND_TRI || kind == KIND_TRIP || kind == KIND_TRICN || kind == KIND_TRICNP || kind == KIND_TRIPF ||
                       kind == KIND_TRICNPF);
     const bool pertf = (kind == KIND_TRIPF || kind == KIND_TRICNPF);  // + 1 value: nfac for the end partitions
@@ -597,13 +681,13 @@ void layout_slot(const DtypePlan &pl, const Shape &sh, int kind, KernelSlot &sl,
     while (pl.P % g != 0) --g;
     sl.box_rows = (unsigned)(g * pl.rows);
     sl.nboxes = (unsigned)(pl.P / g);
-    const size_t ring = (size_t)sh.tpc * Np * W * pl.elem;
+    const size_t ring = (size_t)sh.tpc * Np * W * selem;
     sl.smem = sl.tma ? sl.offR + ring : sl.offM + 17 * 8;
 }
 
-bool tma_possible(const DtypePlan &pl, const Shape &sh, int vec)
+bool tma_possible(const DtypePlan &pl, const Shape &sh, int vec, int selem = 0)
 {
-    const size_t wb = (size_t)sh.lanes * vec * pl.elem;  // bytes of one tile row
+    const size_t wb = (size_t)sh.lanes * vec * (selem ? selem : pl.elem);  // bytes of one tile row
     if (g_tune.prefetch == 0) return false;
     if (pl.P > 1 && !pl.ws) return false;       // the serial carry walk has no TMA variant
     if (wb % 16 != 0 || sh.lanes * vec > 256) return false;
@@ -649,15 +733,14 @@ SweepEntry find_sweep_cl(int kind, int elem_bytes, int fuse)
     return SweepEntry{nullptr, nullptr, 0};
 }
 
-// Cluster-split plan (sweep.cuh, CL): for 16 < P <= 32 partitions one CTA could only keep 8 lanes x 16 B = 128-byte
-// row segments; two CTAs (two SMs) that each keep half of the partitions own a tile of 16 lanes = 256-byte segments,
-// which is what HBM wants.  Shared memory per CTA: its partitions' coefficient blocks, the scan
-// tables, the exchange area of ALL partitions (the pair scans half of the columns each) and the ring of its rows.
+// Cluster-chain plan (sweep.cuh, CL): a tile's rows are split over csz CTAs of one thread-block cluster (csz SMs), each
+// keeping PLc <= 16 partitions on 16 lanes x 16 bytes = 256-byte row segments, which is what HBM and the TLB want
+// (DESIGN.md "Long systems").  Shared memory per CTA: its partitions' coefficient blocks, its own scan-table block, the
+// exchange area of its partitions, the two carry inboxes and the ring of its rows.
 void fill_cluster_slot(Handle *h, DtypePlan &pl)
 {
     pl.ck = KernelSlot();
-    if (pl.two_pass || h->periodic || !pl.ws || g_tune.cluster == 0 || g_tune.prefetch == 0) return;
-    if (pl.rows != 32 || pl.P <= 16 || pl.P > 32 || (pl.P & 1)) return;
+    if (!pl.csz || h->periodic || g_tune.cluster == 0 || g_tune.prefetch == 0 || pl.rows != 32) return;
     const int kind = h->kind;  // KIND_TRI / KIND_PENTA
     const int NC = (kind == KIND_TRI) ? 1 : 2;
     const int elems = (kind == KIND_TRI) ? RecLayout<KIND_TRI>::ELEMS : RecLayout<KIND_PENTA>::ELEMS;
@@ -666,20 +749,21 @@ void fill_cluster_slot(Handle *h, DtypePlan &pl)
     sh.lanes_log2 = 4;
     sh.vec = 16 / pl.elem;
     sh.tpc = 1;
-    const int PL = pl.P / 2;
+    const int PL = pl.PLc;
     sh.threads = PL * sh.lanes;
     KernelSlot &sl = pl.ck;
     sl.vec = sh.vec;
     sl.tma = 1;
     const size_t W = (size_t)sh.lanes * sl.vec;
     sl.xvals = 2 * NC;
-    sl.xper = (int)(sl.xvals * pl.P * W);
+    sl.xper = (int)(sl.xvals * PL * W);
     sl.xstride = sl.xper;
     const size_t rows_bytes = (size_t)PL * elems * pl.rows * pl.elem;
     sl.offTl = (unsigned)align16(rows_bytes);
-    sl.offX = (unsigned)align16(sl.offTl + (pl.blob_bytes - pl.offT));
-    sl.offM = (unsigned)align16(sl.offX + (size_t)sl.xstride * pl.elem);
-    sl.offR = (unsigned)align_up(sl.offM + 17 * 8, 128);
+    sl.offX = (unsigned)align16(sl.offTl + pl.tab_bytes_cl);
+    sl.offIn = (unsigned)align16(sl.offX + (size_t)sl.xstride * pl.elem);
+    sl.offM = (unsigned)align16(sl.offIn + (size_t)2 * 8 * NC * W * pl.elem);  // [forward | backward][8 senders][NC][W]
+    sl.offR = (unsigned)align_up(sl.offM + 49 * 8, 128);  // 17 barriers as everywhere + 2 x 16 inbox barriers
     int g = 256 / pl.rows < PL ? 256 / pl.rows : PL;
     while (PL % g != 0) --g;
     sl.box_rows = (unsigned)(g * pl.rows);
@@ -708,6 +792,22 @@ void fill_slots(Handle *h)
     for (int t = 0; t < 2; ++t) {
         DtypePlan &pl = h->plan[t];
         fill_cluster_slot(h, pl);
+        if (t == 0 && !h->periodic && !pl.two_pass && (pl.P == 1 || (pl.ws && pl.rows == 32))) {
+            // fp32 storage, fp64 arithmetic: the plain solve kernels of the fp64 plan with a ring of floats
+            const Shape &sh = pl.shape[0];
+            for (int s = 0; s < 2; ++s)
+                for (int d = 0; d < 2; ++d) {
+                    KernelSlot &sl = pl.ks32[s][d];
+                    sl = KernelSlot();
+                    sl.vec = (s == 0) ? sh.vec : 1;
+                    sl.tma = (d == 0) ? 1 : 0;
+                    if (sl.vec > 2 || (sl.tma && !tma_possible(pl, sh, sl.vec, 4))) continue;
+                    layout_slot(pl, sh, h->kind, sl, true, 4);
+                    if (sl.smem > SMEM_LIMIT) continue;
+                    sl.ent = find_sweep_f32s(h->kind, sl.vec, pl.rows, pl.P == 1 ? 1 : 0, sl.tma, pl.ws);
+                    if (sl.ent.func && sl.ent.max_threads < sh.threads) sl.ent = SweepEntry{nullptr, nullptr, 0};
+                }
+        }
         if (pl.two_pass) continue;
         const int single = (pl.P == 1) ? 1 : 0;
         for (int ks = 0; ks < 3; ++ks) {
@@ -757,7 +857,7 @@ void fill_slots(Handle *h)
     }
 }
 
-int resolve_slot(Handle *h, const Shape &sh, KernelSlot &sl, bool cluster = false)
+int resolve_slot(Handle *h, const Shape &sh, KernelSlot &sl, int cluster = 0)
 {
     std::lock_guard<std::mutex> lk(h->mu);
     if (sl.max_grid > 0) return BTPS_OK;
@@ -782,12 +882,12 @@ int resolve_slot(Handle *h, const Shape &sh, KernelSlot &sl, bool cluster = fals
     if (cluster) {
         // co-resident clusters of two CTAs (each CTA fills an SM)
         cudaLaunchConfig_t cfg = {};
-        cfg.gridDim = dim3((unsigned)(2 * sms));
+        cfg.gridDim = dim3((unsigned)(cluster * (sms / cluster)));
         cfg.blockDim = dim3((unsigned)sh.threads);
         cfg.dynamicSmemBytes = sl.smem;
         cudaLaunchAttribute at[1];
         at[0].id = cudaLaunchAttributeClusterDimension;
-        at[0].val.clusterDim.x = 2;
+        at[0].val.clusterDim.x = (unsigned)cluster;
         at[0].val.clusterDim.y = 1;
         at[0].val.clusterDim.z = 1;
         cfg.attrs = at;
@@ -798,7 +898,7 @@ int resolve_slot(Handle *h, const Shape &sh, KernelSlot &sl, bool cluster = fals
             snprintf(tl_cuda_msg, sizeof(tl_cuda_msg), "cluster kernel does not fit: %d threads, %zu B smem", sh.threads, sl.smem);
             return set_err(BTPS_E_CUDA);
         }
-        sl.max_grid = 2 * ncl;
+        sl.max_grid = cluster * ncl;
         return BTPS_OK;
     }
     CU_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, sl.ent.func, sh.threads, sl.smem));
@@ -856,11 +956,23 @@ int make_tmap(CUtensorMap *tm, T *d_rhs, long long batch, int n, int W, unsigned
     return BTPS_OK;
 }
 
-// one sweep launch (kind = KIND_TRI / KIND_PENTA / KIND_CH) on a device buffer
+// 17..32 partitions (512 < N <= 1024): one CTA keeps such a tile on 8 lanes = 128-byte row segments, the chain of two
+// CTAs on 256-byte ones.  Where the pair wins by default (measured on B200).
 template <typename T>
-int launch_one(Handle *h, int kind, T *d_rhs, long long batch, double alpha_x, int reverse, int ksteps,
+bool cl_pays(int kind, const DtypePlan &pl, long long batch)
+{
+    // measured on B200 (profiles/r02_long_systems.md): the pair's two carry exchanges per tile cost ~1.5 us, which only
+    // pays where the single CTA's 128-byte segments are at their worst -- tridiagonal, 32 partitions (N = 992 / 1024),
+    // batches of >= 2^22 systems: 0.72 / 0.71 (fp64 / fp32) against 0.69 / 0.69.  Pentadiagonal: the pair loses everywhere.
+    return kind == KIND_TRI && pl.P == 32 && pl.csz == 2 && batch >= (1ll << 22);
+}
+
+// one sweep launch (kind = KIND_TRI / KIND_PENTA / KIND_CH) on a device buffer
+template <typename T, typename S = T>
+int launch_one(Handle *h, int kind, S *d_rhs, long long batch, double alpha_x, int reverse, int ksteps,
                cudaStream_t st, double *stat = nullptr, const double *ex = nullptr, const char **tag_out = nullptr)
 {
+    constexpr bool MIXED = !std::is_same<T, S>::value;  // fp32 in HBM, fp64 arithmetic: plain solves of the fp64 plan
     DtypePlan &pl = h->plan[sizeof(T) == 8 ? 0 : 1];
     // a handle's tables live on the device that was current when it was factored
     int dev = -1;
@@ -872,6 +984,11 @@ int launch_one(Handle *h, int kind, T *d_rhs, long long batch, double alpha_x, i
             *tag_out = "two_pass_kernel";
             return BTPS_OK;
         }
+        if (MIXED) {  // the two-pass form writes g to global memory: in fp32 storage that would not be an fp64 solve
+            snprintf(tl_cuda_msg, sizeof(tl_cuda_msg), "fp32-storage solves need the on-chip plan (n <= 1024)");
+            return set_err(BTPS_E_ARG);
+        }
+        T *const dr = (T *)(void *)d_rhs;  // (same type unless MIXED, which has returned above)
         const int block = 128;
         const long long grid = (batch + block - 1) / block;
         const T *co = (const T *)pl.d_soa;
@@ -879,64 +996,65 @@ int launch_one(Handle *h, int kind, T *d_rhs, long long batch, double alpha_x, i
         for (int i = 0; i < 5; ++i) ppx.ex[i] = ex ? ex[i] : 0.0;
         for (int l = 0; l < ksteps; ++l) {
             if (kind == KIND_TRI && h->periodic)
-                two_pass_kernel<T, KIND_TRIP><<<(unsigned)grid, block, 0, st>>>(co, d_rhs, batch, h->n, h->per_vN, h->per_invden, h->pp);
+                two_pass_kernel<T, KIND_TRIP><<<(unsigned)grid, block, 0, st>>>(co, dr, batch, h->n, h->per_vN, h->per_invden, h->pp);
             else if (kind == KIND_TRI)
-                two_pass_kernel<T, KIND_TRI><<<(unsigned)grid, block, 0, st>>>(co, d_rhs, batch, h->n, 0.0, 0.0, h->pp);
+                two_pass_kernel<T, KIND_TRI><<<(unsigned)grid, block, 0, st>>>(co, dr, batch, h->n, 0.0, 0.0, h->pp);
             else if (kind == KIND_TRICN && h->periodic)
-                two_pass_kernel<T, KIND_TRICNP><<<(unsigned)grid, block, 0, st>>>(co, d_rhs, batch, h->n, h->per_vN, h->per_invden, ppx);
+                two_pass_kernel<T, KIND_TRICNP><<<(unsigned)grid, block, 0, st>>>(co, dr, batch, h->n, h->per_vN, h->per_invden, ppx);
             else if (kind == KIND_TRICN)
-                two_pass_kernel<T, KIND_TRICN><<<(unsigned)grid, block, 0, st>>>(co, d_rhs, batch, h->n, 0.0, 0.0, ppx);
+                two_pass_kernel<T, KIND_TRICN><<<(unsigned)grid, block, 0, st>>>(co, dr, batch, h->n, 0.0, 0.0, ppx);
             else if (kind == KIND_PENTA && h->periodic)
-                two_pass_kernel<T, KIND_PENTAP><<<(unsigned)grid, block, 0, st>>>(co, d_rhs, batch, h->n, 0.0, 0.0, h->pp);
+                two_pass_kernel<T, KIND_PENTAP><<<(unsigned)grid, block, 0, st>>>(co, dr, batch, h->n, 0.0, 0.0, h->pp);
             else if (kind == KIND_PENTA)
-                two_pass_kernel<T, KIND_PENTA><<<(unsigned)grid, block, 0, st>>>(co, d_rhs, batch, h->n, 0.0, 0.0, h->pp);
+                two_pass_kernel<T, KIND_PENTA><<<(unsigned)grid, block, 0, st>>>(co, dr, batch, h->n, 0.0, 0.0, h->pp);
             else if (kind == KIND_PENTACN && h->periodic)
-                two_pass_kernel<T, KIND_PENTACNP><<<(unsigned)grid, block, 0, st>>>(co, d_rhs, batch, h->n, 0.0, 0.0, ppx);
+                two_pass_kernel<T, KIND_PENTACNP><<<(unsigned)grid, block, 0, st>>>(co, dr, batch, h->n, 0.0, 0.0, ppx);
             else if (kind == KIND_PENTACN)
-                two_pass_kernel<T, KIND_PENTACN><<<(unsigned)grid, block, 0, st>>>(co, d_rhs, batch, h->n, 0.0, 0.0, ppx);
+                two_pass_kernel<T, KIND_PENTACN><<<(unsigned)grid, block, 0, st>>>(co, dr, batch, h->n, 0.0, 0.0, ppx);
             else if (h->periodic)
-                two_pass_kernel<T, KIND_CHP><<<(unsigned)grid, block, 0, st>>>(co, d_rhs, batch, h->n, alpha_x, 0.0, h->pp);
+                two_pass_kernel<T, KIND_CHP><<<(unsigned)grid, block, 0, st>>>(co, dr, batch, h->n, alpha_x, 0.0, h->pp);
             else
-                two_pass_kernel<T, KIND_CH><<<(unsigned)grid, block, 0, st>>>(co, d_rhs, batch, h->n, alpha_x, 0.0, h->pp);
+                two_pass_kernel<T, KIND_CH><<<(unsigned)grid, block, 0, st>>>(co, dr, batch, h->n, alpha_x, 0.0, h->pp);
             g_launches.fetch_add(1, std::memory_order_relaxed);
             CU_TRY(cudaGetLastError());
             if (stat) {
-                lbar_kernel<T><<<(unsigned)grid, block, 0, st>>>(d_rhs, batch, h->n, stat + l, 1.0 / (double)batch);
+                lbar_kernel<T><<<(unsigned)grid, block, 0, st>>>(dr, batch, h->n, stat + l, 1.0 / (double)batch);
                 g_launches.fetch_add(1, std::memory_order_relaxed);
                 CU_TRY(cudaGetLastError());
             }
         }
         return BTPS_OK;
     };
-    if (pl.two_pass) return two_pass();
     const int ks = (kind == KIND_CH || kind == KIND_TRICN) ? 1 : (kind == KIND_PENTACN ? 2 : 0);
-    const bool tma_ok = (((uintptr_t)d_rhs % 16) == 0) && ((((size_t)batch * sizeof(T)) % 16) == 0) &&
+    const bool tma_ok = (((uintptr_t)d_rhs % 16) == 0) && ((((size_t)batch * sizeof(S)) % 16) == 0) &&
                         (batch < (1ll << 31));
-    // long systems: the cluster-split kernels when the batch is TMA-aligned and a multiple of the vector width
-    // (measured on B200: the pair's two cluster barriers per tile cost ~1.3 us, so by default it is used only
-    //  where the wider row segments win -- tridiagonal fp64, 32 partitions (N = 992 / 1024), >= 2^22 systems: 0.70
-    //  against 0.69 of the peak; at 2^19 / 2^20 the single CTA with held stores (hold_stores below) now wins, 0.77 / 0.75
-    //  against 0.72 / 0.71 for the pair; with 24 partitions (N = 768) the pair loses 0.56 against 0.75;
-    //  btps_tune("cluster", 1) forces it for every eligible plan, 0 switches it off)
-    const bool cl_wanted = (g_tune.cluster > 0) ||
-                           (g_tune.cluster < 0 && kind == KIND_TRI && sizeof(T) == 8 && pl.P == 32 && batch >= (1ll << 22));
-    const bool use_cl = (ks == 0) && cl_wanted && pl.ck.ent.func && tma_ok && (batch % pl.cshape.vec == 0);
+    // long systems: the cluster-chain kernels when the batch is TMA-aligned and a multiple of the vector width.
+    // More than 32 partitions (N > 1024) have no other on-chip plan; for 17..32 partitions the default comes from
+    // measurements on B200; btps_tune("cluster", 1) forces the chain for every eligible plan,
+    // 0 switches it off.
+    const bool cl_default = (pl.P > 32) || cl_pays<T>(kind, pl, batch);
+    const bool cl_wanted = (g_tune.cluster > 0) || (g_tune.cluster < 0 && cl_default);
+    const bool use_cl = !MIXED && (ks == 0) && (kind == KIND_TRI || kind == KIND_PENTA) && cl_wanted && pl.ck.ent.func && tma_ok &&
+                        (batch % pl.cshape.vec == 0);
+    if (!use_cl && pl.two_pass) return two_pass();
     const Shape &sh = use_cl ? pl.cshape : pl.shape[ks];
     // the vectorised kernels need whole vectors: batch % vec == 0 and an aligned base pointer;
     // TMA needs a 16-byte aligned base and row pitch
     int s = 0;
     if (sh.vec > 1) {
-        const bool ok = (batch % sh.vec == 0) && (((uintptr_t)d_rhs % (sizeof(T) * sh.vec)) == 0);
+        const bool ok = (batch % sh.vec == 0) && (((uintptr_t)d_rhs % (sizeof(S) * sh.vec)) == 0);
         if (!ok) s = 1;
     }
-    int d = (tma_ok && pl.k[ks][s][0].ent.func) ? 0 : 1;
-    if (!pl.k[ks][s][d].ent.func && s == 0) s = 1;  // e.g. the wide variant has no direct-load twin that fits
-    if (!pl.k[ks][s][d].ent.func) d = 1;
-    KernelSlot &sl = use_cl ? pl.ck : pl.k[ks][s][d];
+    auto slot_at = [&](int sv, int dv) -> KernelSlot & { return MIXED ? pl.ks32[sv][dv] : pl.k[ks][sv][dv]; };
+    if (MIXED && (ks != 0 || h->periodic)) return set_err(BTPS_E_ARG);
+    int d = (tma_ok && slot_at(s, 0).ent.func) ? 0 : 1;
+    if (!slot_at(s, d).ent.func && s == 0) s = 1;  // e.g. the wide variant has no direct-load twin that fits
+    if (!slot_at(s, d).ent.func) d = 1;
+    KernelSlot &sl = use_cl ? pl.ck : slot_at(s, d);
     if (!sl.ent.func) return two_pass();
     {
         // takes the handle's lock: max_grid / prefer_fused are written by the first launch of this slot
-        const int rc = resolve_slot(h, sh, sl, use_cl);
+        const int rc = resolve_slot(h, sh, sl, use_cl ? pl.csz : 0);
         if (rc != BTPS_OK) return rc;
     }
     SweepArgs a;
@@ -964,7 +1082,7 @@ int launch_one(Handle *h, int kind, T *d_rhs, long long batch, double alpha_x, i
     a.xstride = sl.xstride;
     a.xper = sl.xper;
     a.n = h->n;
-    a.P = pl.P;
+    a.P = use_cl ? pl.csz * pl.PLc : pl.P;
     a.lanes = sh.lanes;
     a.lanes_log2 = sh.lanes_log2;
     a.tpc = sh.tpc;
@@ -975,18 +1093,22 @@ int launch_one(Handle *h, int kind, T *d_rhs, long long batch, double alpha_x, i
         // (N = 480 / 512 / 992 / 1024), 96 KB tiles (N = 768) lose 4-9 %; the plain pentadiagonal solve gains 4-6 % on
         // 16-lane tiles (N <= 512) and loses up to 8 % on 8-lane ones; Cahn-Hilliard, periodic penta, fp32 penta lose.
         const bool tri_family = (kind == KIND_TRI || kind == KIND_TRICN);
-        const size_t tile_bytes = (size_t)pl.P * pl.rows * sh.lanes * sl.vec * sizeof(T);
+        const size_t tile_bytes = (size_t)pl.P * pl.rows * sh.lanes * sl.vec * sizeof(S);
         // (and at least 8 tiles per CTA: with 3-4 it loses ~10 %)
         const bool full_tile = (sh.tpc == 1) && !use_cl && tile_bytes >= (112u << 10) && a.num_tiles >= 8ll * sl.max_grid;
         const bool penta_ok = (kind == KIND_PENTA) && sizeof(T) == 8 && !h->periodic && sh.lanes == 16;
         a.hold_stores = g_tune.hold_stores >= 0 ? (g_tune.hold_stores > 0) : ((full_tile && (tri_family || penta_ok)) ? 1 : 0);
     }
+    a.csz = use_cl ? pl.csz : 1;
+    a.scan_log2_cl = pl.scan_log2_cl;
+    a.tab_bytes_cl = pl.tab_bytes_cl;
+    a.offIn = sl.offIn;
     a.scan_log2 = pl.scan_log2;
-    a.tq = pl.tq;
+    a.tq = use_cl ? SCAN_LANES : pl.tq;  // (the per-CTA table blocks of the cluster kernels have 32 entries per row)
     a.ksteps = ksteps;
     a.xvals = sl.xvals;
     a.blob_bytes = pl.blob_bytes;
-    a.offT = pl.offT;
+    a.offT = use_cl ? pl.offTc : pl.offT;
     a.offTl = use_cl ? sl.offTl : pl.offT;
     a.offX = sl.offX;
     a.offM = sl.offM;
@@ -1001,14 +1123,14 @@ int launch_one(Handle *h, int kind, T *d_rhs, long long batch, double alpha_x, i
     CUtensorMap tm;
     memset(&tm, 0, sizeof(tm));
     if (sl.tma) {
-        const int rc = make_tmap<T>(&tm, d_rhs, batch, h->n, (int)W, sl.box_rows);
+        const int rc = make_tmap<S>(&tm, d_rhs, batch, h->n, (int)W, sl.box_rows);
         if (rc != BTPS_OK) return rc;
     }
     long long grid = a.num_tiles;  // one tile per CTA first (tile order is group-major), capped at the resident CTAs
-    if (use_cl) grid = 2 * a.num_tiles;  // one cluster of two CTAs per tile in flight
+    if (use_cl) grid = (long long)pl.csz * a.num_tiles;  // one cluster per tile in flight
     if (grid > sl.max_grid) grid = sl.max_grid;
-    if (g_tune.grid > 0 && grid > g_tune.grid) grid = use_cl ? (g_tune.grid & ~1) : g_tune.grid;
-    if (use_cl && grid < 2) grid = 2;
+    if (g_tune.grid > 0 && grid > g_tune.grid) grid = use_cl ? (g_tune.grid / pl.csz) * pl.csz : g_tune.grid;
+    if (use_cl && grid < pl.csz) grid = pl.csz;
     // several steps per launch need the fused instantiation; without one (direct-load variants)
     // the steps are launched one by one
     // (the statistic of eq. 30 is computed inside the fused kernels; elsewhere by a pass of its own)
@@ -1024,7 +1146,7 @@ int launch_one(Handle *h, int kind, T *d_rhs, long long batch, double alpha_x, i
         if (e != cudaSuccess) return cuda_fail(e, "sweep launch");
         if (stat && !fused) {
             const int block = 128;
-            lbar_kernel<T><<<(unsigned)((batch + block - 1) / block), block, 0, st>>>(d_rhs, batch, h->n, stat + l,
+            lbar_kernel<T><<<(unsigned)((batch + block - 1) / block), block, 0, st>>>((T *)(void *)d_rhs, batch, h->n, stat + l,
                                                                                       1.0 / (double)batch);
             g_launches.fetch_add(1, std::memory_order_relaxed);
             CU_TRY(cudaGetLastError());
@@ -1038,7 +1160,7 @@ int launch_one(Handle *h, int kind, T *d_rhs, long long batch, double alpha_x, i
 // and one write per `fuse` steps.  The two-pass kernel advances one step per launch.
 int fuse_limit(const DtypePlan &pl)
 {
-    if (pl.two_pass) return 1;
+    if (pl.two_pass && !pl.ck.fused.func) return 1;
     // measured on B200: 8 -> 64 steps per launch still gains 5-15 % (fewer tile round trips and launches); the gain
     // from 32 to 64 is ~2 %, so 64 is both the default and the cap
     const int k = g_tune.fuse > 0 ? g_tune.fuse : 64;
@@ -1052,19 +1174,19 @@ Handle *check(const void *hv, int magic)
     return h;
 }
 
-template <typename T>
-int solve_steps(const void *hv, int magic, int kind, T *d_rhs, int64_t batch, double alpha_x, int nsteps,
+template <typename T, typename S = T>
+int solve_steps(const void *hv, int magic, int kind, S *d_rhs, int64_t batch, double alpha_x, int nsteps,
                 void *stream, double *d_stat = nullptr, const double *ex = nullptr)
 {
     Handle *h = check(hv, magic);
     if (!h || !d_rhs || batch < 1 || nsteps < 0) return set_err(BTPS_E_ARG);
-    if ((uintptr_t)d_rhs % sizeof(T)) return set_err(BTPS_E_ALIGN);
+    if ((uintptr_t)d_rhs % sizeof(S)) return set_err(BTPS_E_ALIGN);
     const bool rev = g_tune.reverse > 0;
-    const int kmax = fuse_limit(h->plan[sizeof(T) == 8 ? 0 : 1]);
+    const int kmax = std::is_same<T, S>::value ? fuse_limit(h->plan[sizeof(T) == 8 ? 0 : 1]) : 1;
     for (int s = 0, l = 0; s < nsteps; ++l) {
         const int k = (nsteps - s < kmax) ? (nsteps - s) : kmax;
-        const int rc = launch_one<T>(h, kind, d_rhs, batch, alpha_x, rev ? (l & 1) : 0, k, (cudaStream_t)stream,
-                                     d_stat ? d_stat + s : nullptr, ex);
+        const int rc = launch_one<T, S>(h, kind, d_rhs, batch, alpha_x, rev ? (l & 1) : 0, k, (cudaStream_t)stream,
+                                        d_stat ? d_stat + s : nullptr, ex);
         if (rc != BTPS_OK) return rc;
         s += k;
     }
@@ -1455,6 +1577,14 @@ int penta_solve_batched_f32(penta_handle_t h, float *d_rhs, int64_t batch, void 
 {
     return solve_steps<float>(h, MAGIC_PENTA, KIND_PENTA, d_rhs, batch, 0.0, 1, stream);
 }
+int tri_solve_batched_f32s(tri_handle_t h, float *d_rhs, int64_t batch, void *stream)
+{
+    return solve_steps<double, float>(h, MAGIC_TRI, KIND_TRI, d_rhs, batch, 0.0, 1, stream);
+}
+int penta_solve_batched_f32s(penta_handle_t h, float *d_rhs, int64_t batch, void *stream)
+{
+    return solve_steps<double, float>(h, MAGIC_PENTA, KIND_PENTA, d_rhs, batch, 0.0, 1, stream);
+}
 int tri_solve_steps(tri_handle_t h, double *d_rhs, int64_t batch, int nsteps, void *stream)
 {
     return solve_steps<double>(h, MAGIC_TRI, KIND_TRI, d_rhs, batch, 0.0, nsteps, stream);
@@ -1579,8 +1709,9 @@ const char *btps_build_id(void) { return BTPS_BUILD_ID; }
 
 int btps_kernel_tag(int kind, const void *handle, int elem_bytes, int64_t batch, int nsteps, char *buf, int len)
 {
-    if (kind < 0 || kind > 4 || !buf || len < 1 || batch < 1 || nsteps < 1 || (elem_bytes != 8 && elem_bytes != 4))
+    if (kind < 0 || kind > 4 || !buf || len < 1 || batch < 1 || nsteps < 1 || (elem_bytes != 8 && elem_bytes != 4 && elem_bytes != 12))
         return set_err(BTPS_E_ARG);
+    if (elem_bytes == 12 && (kind > 1 || nsteps != 1)) return set_err(BTPS_E_ARG);  // *_f32s: plain single solves
     Handle *h = check(handle, (kind == 0 || kind == 3) ? MAGIC_TRI : MAGIC_PENTA);
     if (!h) return set_err(BTPS_E_ARG);
     static const int kinds[5] = {KIND_TRI, KIND_PENTA, KIND_CH, KIND_TRICN, KIND_PENTACN};
@@ -1590,7 +1721,8 @@ int btps_kernel_tag(int kind, const void *handle, int elem_bytes, int64_t batch,
     void *fake = (void *)(uintptr_t)4096;
     const double ex[5] = {0, 1, 0, 0, 0};
     const int rc = elem_bytes == 8 ? launch_one<double>(h, kinds[kind], (double *)fake, batch, 0.0, 0, nsteps, nullptr, nullptr, ex, &tag)
-                                   : launch_one<float>(h, kinds[kind], (float *)fake, batch, 0.0, 0, nsteps, nullptr, nullptr, ex, &tag);
+                 : elem_bytes == 4 ? launch_one<float>(h, kinds[kind], (float *)fake, batch, 0.0, 0, nsteps, nullptr, nullptr, ex, &tag)
+                                   : launch_one<double, float>(h, kinds[kind], (float *)fake, batch, 0.0, 0, 1, nullptr, nullptr, ex, &tag);
     if (rc != BTPS_OK) return rc;
     snprintf(buf, (size_t)len, "%s", tag ? tag : "");
     return set_err(BTPS_OK);

@@ -6,16 +6,16 @@
 
 namespace btps {
 
-template <typename T, int V, int MR, bool SINGLE, int KIND, bool TMA, bool WS, bool FUSE = false, bool CL = false>
+template <typename T, int V, int MR, bool SINGLE, int KIND, bool TMA, bool WS, bool FUSE = false, bool CL = false, typename S = T>
 static SweepEntry make_entry()
 {
     SweepEntry e;
-    e.launch = &launch_sweep<T, V, MR, SINGLE, KIND, TMA, WS, FUSE, CL>;
-    e.func = reinterpret_cast<const void *>(&sweep_kernel<T, V, MR, SINGLE, KIND, TMA, WS, FUSE, CL>);
+    e.launch = &launch_sweep<T, V, MR, SINGLE, KIND, TMA, WS, FUSE, CL, S>;
+    e.func = reinterpret_cast<const void *>(&sweep_kernel<T, V, MR, SINGLE, KIND, TMA, WS, FUSE, CL, S>);
     e.max_threads = CtaShape<T, V, MR>::MAX_THREADS;
-    static char tag[64];
-    static const int once = snprintf(tag, sizeof(tag), "%s, %d, %d, %d, %d, %d, %d, %d, %d", sizeof(T) == 8 ? "double" : "float", V,
-                                     MR, (int)SINGLE, KIND, (int)TMA, (int)WS, (int)FUSE, (int)CL);
+    static char tag[72];
+    static const int once = snprintf(tag, sizeof(tag), "%s, %d, %d, %d, %d, %d, %d, %d, %d, %s", sizeof(T) == 8 ? "double" : "float", V,
+                                     MR, (int)SINGLE, KIND, (int)TMA, (int)WS, (int)FUSE, (int)CL, sizeof(S) == 8 ? "double" : "float");
     (void)once;
     e.tag = tag;
     return e;
@@ -100,6 +100,7 @@ static SweepEntry pick_cl(int fuse)
                 : make_entry<T, V, 32, false, KIND, true, true, false, true>();
 }
 SweepEntry find_sweep_cl(int kind, int elem_bytes, int fuse);
+SweepEntry find_sweep_f32s(int kind, int vec, int rows, int single, int tma, int ws);
 SweepEntry find_sweep_cl_tri_f64(int fuse);
 SweepEntry find_sweep_cl_tri_f32(int fuse);
 SweepEntry find_sweep_cl_penta_f64(int fuse);

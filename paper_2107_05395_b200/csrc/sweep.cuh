@@ -87,6 +87,11 @@ struct SweepArgs {
     unsigned offR;         // byte offset of the prefetch ring (TMA kernels), 128-B aligned
     unsigned box_rows;     // rows per TMA box (<= 256)
     unsigned nboxes;       // boxes per tile = ceil(P*MR / box_rows)
+    // cluster-split kernels (CL): the rows of a tile over `csz` CTAs of one thread-block cluster
+    int csz;               // CTAs per cluster (2, 4 or 8); each keeps P / csz partitions
+    int scan_log2_cl;      // log2 of the scan width inside one CTA (smallest power of two >= P / csz)
+    unsigned tab_bytes_cl; // bytes of one CTA's scan-table block (csz blocks back to back at offT in the blob)
+    unsigned offIn;        // byte offset (shared memory) of the carry inboxes: [forward | backward][NC][W]
 };
 
 template <typename T, int N>
@@ -95,28 +100,30 @@ struct alignas((sizeof(T) * N) <= 16 ? (sizeof(T) * N) : 16) Tup {
 };
 
 // ---- access to V adjacent systems (global or shared) ------------------------------------------
-template <typename T, int V>
-__device__ __forceinline__ void ld_sys(T (&d)[V], const T *p)
+// S = storage type of the batch (global memory / prefetch ring), T = type of the registers and of all arithmetic:
+// the same, or S = float with T = double (fp32 in HBM, fp64 sweeps: the *_f32s calls)
+template <typename T, int V, typename S>
+__device__ __forceinline__ void ld_sys(T (&d)[V], const S *p)
 {
     if constexpr (V == 1) {
-        d[0] = *p;
+        d[0] = (T)*p;
     } else {
-        const Tup<T, V> t = *reinterpret_cast<const Tup<T, V> *>(p);
+        const Tup<S, V> t = *reinterpret_cast<const Tup<S, V> *>(p);
 #pragma unroll
-        for (int e = 0; e < V; ++e) d[e] = t.v[e];
+        for (int e = 0; e < V; ++e) d[e] = (T)t.v[e];
     }
 }
 
-template <typename T, int V>
-__device__ __forceinline__ void st_sys(T *p, const T (&s)[V])
+template <typename T, int V, typename S>
+__device__ __forceinline__ void st_sys(S *p, const T (&s)[V])
 {
     if constexpr (V == 1) {
-        *p = s[0];
+        *p = (S)s[0];
     } else {
-        Tup<T, V> t;
+        Tup<S, V> t;
 #pragma unroll
-        for (int e = 0; e < V; ++e) t.v[e] = s[e];
-        *reinterpret_cast<Tup<T, V> *>(p) = t;
+        for (int e = 0; e < V; ++e) t.v[e] = (S)s[e];
+        *reinterpret_cast<Tup<S, V> *>(p) = t;
     }
 }
 
@@ -223,6 +230,41 @@ __device__ __forceinline__ unsigned cluster_map(unsigned local_addr, unsigned ra
     asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(local_addr), "r"(rank));
     return r;
 }
+__device__ __forceinline__ unsigned cluster_nctarank()
+{
+    unsigned r;
+    asm volatile("mov.u32 %0, %%cluster_nctarank;" : "=r"(r));
+    return r;
+}
+// arrive (release at cluster scope) on an mbarrier in another CTA of the cluster: orders this thread's earlier
+// st.shared::cluster writes before the arrival
+__device__ __forceinline__ void mbar_arrive_remote(unsigned remote_bar)
+{
+    asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" ::"r"(remote_bar) : "memory");
+}
+// wait on a local mbarrier whose arrivals come from another CTA (acquire at cluster scope).  A neighbour that never
+// arrives would otherwise hang the device: after ~4 s without progress the kernel traps (the launch then fails with
+// an error instead of spinning forever).
+__device__ __forceinline__ void mbar_wait_cluster(unsigned bar, unsigned parity)
+{
+    unsigned done = 0;
+    unsigned long long t0 = 0;
+    for (unsigned spin = 0;; ++spin) {
+        asm volatile(
+            "{\n"
+            ".reg .pred p;\n"
+            "mbarrier.try_wait.parity.acquire.cluster.shared::cta.b64 p, [%1], %2;\n"
+            "selp.u32 %0, 1, 0, p;\n"
+            "}\n" : "=r"(done) : "r"(bar), "r"(parity) : "memory");
+        if (done) return;
+        if ((spin & 1023u) == 1023u) {
+            unsigned long long now;
+            asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(now));
+            if (t0 == 0) t0 = now;
+            else if (now - t0 > 4000000000ull) __trap();
+        }
+    }
+}
 __device__ __forceinline__ void st_cluster(unsigned addr, double v)
 {
     asm volatile("st.shared::cluster.f64 [%0], %1;" ::"r"(addr), "d"(v) : "memory");
@@ -279,7 +321,7 @@ __device__ __forceinline__ void scan_steps(int n, F &&f)
 //   FUSE   a.ksteps time steps per tile (separate instantiation: the step loop costs registers, so
 //          single-step launches run the FUSE = false kernel)
 // -----------------------------------------------------------------------------------------------
-template <typename T, int V, int MR, bool SINGLE, int KIND, bool TMA, bool WS, bool FUSE, bool CL = false>
+template <typename T, int V, int MR, bool SINGLE, int KIND, bool TMA, bool WS, bool FUSE, bool CL = false, typename S = T>
 __global__ void __launch_bounds__(CtaShape<T, V, MR>::MAX_THREADS, 1)
 sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
 {
@@ -302,8 +344,9 @@ sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
 
     static_assert(!CL || (!SINGLE && TMA && WS && (KIND == KIND_TRI || KIND == KIND_PENTA)), "cluster split: plain solves only");
     const int W = a.lanes * V;
-    [[maybe_unused]] const unsigned crank = CL ? cluster_ctarank() : 0u;  // which half of the rows this CTA keeps
-    const int PL = CL ? (a.P >> 1) : a.P;                                 // partitions kept by this CTA
+    [[maybe_unused]] const unsigned crank = CL ? cluster_ctarank() : 0u;  // which block of the rows this CTA keeps
+    [[maybe_unused]] const int csz = CL ? a.csz : 1;                      // CTAs that share a tile
+    const int PL = CL ? (a.P / a.csz) : a.P;                              // partitions kept by this CTA
     const int tpt = PL * a.lanes;  // threads per tile group (SINGLE: P == 1)
     const int sub = SINGLE ? (threadIdx.x >> a.lanes_log2) : (threadIdx.x / tpt);
     const int lt = SINGLE ? (threadIdx.x & (a.lanes - 1)) : (threadIdx.x - sub * tpt);
@@ -314,10 +357,24 @@ sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
     const long long batch = a.batch;
 
     // ---- stage the coefficient image once per CTA: one asynchronous bulk copy ---------------------
-    // mbarrier slots at offM: 0..15 = the groups' prefetch rings, 16 = the coefficient image
+    // mbarrier slots at offM: 0..15 = the groups' prefetch rings, 16 = the coefficient image,
+    // CL: 17 + job / 33 + job = forward / backward carry inbox of scan job `job` (a column of owner threads, 16 per
+    // CTA), filled by the neighbouring CTAs of the cluster.  One barrier per job: a warp that runs two jobs per tile
+    // step must not need its second job's carry from a neighbour that is still waiting for this warp's first job.
     [[maybe_unused]] const unsigned mbar = smem_u32(smem + a.offM) + 8u * sub;
     const unsigned bbar = smem_u32(smem + a.offM) + 8u * 16u;
-    if (threadIdx.x == 0) mbar_init(bbar, 1);
+    [[maybe_unused]] const unsigned fin_bar = smem_u32(smem + a.offM) + 8u * 17u;
+    [[maybe_unused]] const unsigned bin_bar = smem_u32(smem + a.offM) + 8u * 33u;
+    if (threadIdx.x == 0) {
+        mbar_init(bbar, 1);
+        if constexpr (CL) {  // per tile step one arrival from every CTA below (forward) / above (backward)
+            const unsigned nlo = crank > 0u ? crank : 1u, nhi = (int)crank + 1 < csz ? (unsigned)csz - 1u - crank : 1u;
+            for (int jb = 0; jb < a.lanes; ++jb) {
+                mbar_init(fin_bar + 8u * jb, nlo);
+                mbar_init(bin_bar + 8u * jb, nhi);
+            }
+        }
+    }
     if constexpr (TMA) {
         if (lt == 0) mbar_init(mbar, 1);
     }
@@ -326,13 +383,14 @@ sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
     else __syncthreads();
     if (threadIdx.x == 0) {
         if constexpr (CL) {
-            // this CTA's partitions' coefficient blocks, then the scan tables behind them
+            // this CTA's partitions' coefficient blocks, then its own scan-table block behind them
             const unsigned rows_bytes = (unsigned)(PL * RecLayout<KIND>::ELEMS * MR) * (unsigned)sizeof(T);
-            const unsigned tab_bytes = a.blob_bytes - a.offT;
-            mbar_expect_tx(bbar, rows_bytes + tab_bytes);
+            mbar_expect_tx(bbar, rows_bytes + a.tab_bytes_cl);
             bulk_load(smem_u32(smem), reinterpret_cast<const unsigned char *>(a.blob) + (size_t)crank * rows_bytes,
                       rows_bytes, bbar);
-            bulk_load(smem_u32(smem + a.offTl), reinterpret_cast<const unsigned char *>(a.blob) + a.offT, tab_bytes, bbar);
+            bulk_load(smem_u32(smem + a.offTl),
+                      reinterpret_cast<const unsigned char *>(a.blob) + a.offT + (size_t)crank * a.tab_bytes_cl,
+                      a.tab_bytes_cl, bbar);
         } else {
             mbar_expect_tx(bbar, a.blob_bytes);
             bulk_load(smem_u32(smem), a.blob, a.blob_bytes, bbar);
@@ -360,14 +418,18 @@ sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
     // exchange area of this group: [2*NC values][P][W], columns XOR-swizzled with the partition index
     [[maybe_unused]] T *const xb = reinterpret_cast<T *>(smem + a.offX) + (size_t)sub * a.xstride;
     // prefetch ring of this group: [P*MR rows][W]
-    [[maybe_unused]] const unsigned ring_bytes = (unsigned)(PL * MR * W) * (unsigned)sizeof(T);
+    [[maybe_unused]] const unsigned ring_bytes = (unsigned)(PL * MR * W) * (unsigned)sizeof(S);
     [[maybe_unused]] const int rbase = (int)crank * PL * MR;  // first row kept by this CTA
-    [[maybe_unused]] const unsigned xb_peer = CL ? cluster_map(smem_u32(smem + a.offX), crank ^ 1u) : 0u;
-    [[maybe_unused]] T *const ring = reinterpret_cast<T *>(smem + a.offR + (size_t)sub * ring_bytes);
+    // carry inboxes of this CTA (CL): [forward | backward][sending CTA: 8 slots][NC][W], written by the other CTAs of the
+    // cluster through distributed shared memory
+    [[maybe_unused]] T *const inbox = reinterpret_cast<T *>(smem + a.offIn);
+    [[maybe_unused]] const unsigned inbox_u32 = smem_u32(smem + a.offIn);
+    [[maybe_unused]] unsigned cphase = 0;  // parity of the inbox barriers: one phase per tile step
+    [[maybe_unused]] S *const ring = reinterpret_cast<S *>(smem + a.offR + (size_t)sub * ring_bytes);
 
     const int ntiles = (int)a.num_tiles;
-    const int stride_tiles = CL ? (int)(gridDim.x >> 1) : (int)(gridDim.x * a.tpc);
-    T *const rhs0 = reinterpret_cast<T *>(a.rhs) + (long long)r0 * batch + (long long)sl * V;
+    const int stride_tiles = CL ? (int)(gridDim.x / (unsigned)csz) : (int)(gridDim.x * a.tpc);
+    S *const rhs0 = reinterpret_cast<S *>(a.rhs) + (long long)r0 * batch + (long long)sl * V;
 
     // one thread of the group asks the TMA unit for tile `t` (walking order); columns beyond the
     // batch and rows beyond n are zero-filled by the unit
@@ -375,14 +437,14 @@ sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
         const int tile = a.reverse ? ntiles - 1 - t : t;
         mbar_expect_tx(mbar, ring_bytes);
         const unsigned dst = smem_u32(ring);
-        const unsigned box_bytes = a.box_rows * (unsigned)W * (unsigned)sizeof(T);
+        const unsigned box_bytes = a.box_rows * (unsigned)W * (unsigned)sizeof(S);
         for (unsigned b = 0; b < a.nboxes; ++b)
             tma_load_2d(dst + b * box_bytes, &tmap, tile * W, (int)(b * a.box_rows) + rbase, mbar);
     };
 
     // group-major tile order: consecutive tiles go to different CTAs, so a small batch spreads over all SMs
     // before any CTA runs a second group
-    int t = CL ? (int)(blockIdx.x >> 1) : (int)(blockIdx.x + sub * gridDim.x);
+    int t = CL ? (int)(blockIdx.x / (unsigned)csz) : (int)(blockIdx.x + sub * gridDim.x);
     [[maybe_unused]] unsigned phase = 0;
     if constexpr (TMA) {
         if (lt == 0 && t < ntiles) tma_issue(t);
@@ -393,7 +455,7 @@ sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
         const long long j = (long long)tile * W + (long long)sl * V;
         const bool act = (j < batch);  // V > 1 requires batch % V == 0
         const int nrow = act ? nrow_part : 0;  // rows stored by this thread
-        T *const p0 = rhs0 + (long long)tile * W;
+        S *const p0 = rhs0 + (long long)tile * W;
 
         T v[MR][V];
         [[maybe_unused]] T cm[V], cp[V];    // halo rows r0-1 and r0+MR (c^n)
@@ -402,7 +464,7 @@ sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
             // ---- take the prefetched tile out of the ring, then have it refilled ---------------
             mbar_wait(mbar, phase);
             phase ^= 1u;
-            const T *rp = ring + ((r0 - rbase) * W + sl * V);
+            const S *rp = ring + ((r0 - rbase) * W + sl * V);
             asm volatile("" : "+l"(rp));  // recompute the MR row addresses per tile: hoisted out of the loop they spill
 #pragma unroll
             for (int k = 0; k < MR; ++k) ld_sys<T, V>(v[k], rp + k * W);
@@ -432,7 +494,7 @@ sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
         } else {
             // ---- load: all MR rows issued back to back (independent of the recurrence) ---------
             // (one running row pointer: keeping MR separate 64-bit addresses alive would cost 2*MR registers)
-            const T *pl = p0;
+            const S *pl = p0;
 #pragma unroll
             for (int k = 0; k < MR; ++k) {
                 if (k < nrow) {
@@ -625,13 +687,15 @@ sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
         // last NC rows), NC..2NC-1: backward (x^ at its first NC rows); the scan overwrites them
         // with the incoming carries G (forward) and X (backward) of that partition.
         if constexpr (!SINGLE) {
-            const int P = a.P;
+            // partitions that exchange carries inside this CTA (CL: the CTA's own block of the system's partitions; the
+            // carries across the CTAs of the cluster travel through the inboxes, see the scan below)
+            const int P = CL ? PL : a.P;
             const int tq = a.tq;
             const int wm = W - 1;
             // this thread's columns of its partition: element e lives at xc[XI(e)]
-            T *xc = xb + (size_t)part * W;
+            T *xc = xb + (size_t)(CL ? plidx : part) * W;
             if constexpr (FUSE) asm volatile("" : "+l"(xc));
-            const int xsw = part & wm;
+            const int xsw = (CL ? plidx : part) & wm;
 #define XI(e) (((sl * V + (e)) ^ xsw))
             const int vstr = P * W;  // elements between successive values
             [[maybe_unused]] T G[NC][V], X[NC][V];
@@ -647,29 +711,15 @@ sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
                         xc[2 * vstr + XI(e)] = v[0][e];
                         xc[3 * vstr + XI(e)] = v[1][e];
                     }
-                    if constexpr (CL) {
-                        // the peer CTA scans half of the systems: it needs these values too
-                        const unsigned pa = xb_peer + (unsigned)((part * W + XI(e)) * (int)sizeof(T));
-                        const unsigned vb = (unsigned)(vstr * (int)sizeof(T));
-                        if constexpr (TRI) {
-                            st_cluster(pa, v[MR - 1][e]);
-                            st_cluster(pa + vb, v[0][e]);
-                        } else {
-                            st_cluster(pa, v[MR - 1][e]);
-                            st_cluster(pa + vb, glast2[e]);
-                            st_cluster(pa + 2 * vb, v[0][e]);
-                            st_cluster(pa + 3 * vb, v[1][e]);
-                        }
-                    }
                 }
-                if constexpr (CL) cluster_sync();
-                else group_sync(a.tpc, sub, tpt);
+                group_sync(a.tpc, sub, tpt);
                 {
                     // lane q of a `width`-lane segment holds partition q
+                    const int slog = CL ? a.scan_log2_cl : a.scan_log2;
                     const int lane = lt & 31;
-                    const int wd = 1 << a.scan_log2;
+                    const int wd = 1 << slog;
                     const int q = lane & (wd - 1);
-                    const int spw = 32 >> a.scan_log2;  // jobs per warp pass
+                    const int spw = 32 >> slog;  // jobs per warp pass
                     const T *tb = TAB + q;
                     if constexpr (FUSE) asm volatile("" : "+l"(tb));
                     const int mstr = tq;                // elements between matrix entries
@@ -686,12 +736,10 @@ sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
                         return (st < 4 || q < 16) ? val : T(0);
                     };
                     // job = the V systems of one owner thread column sg: V independent chains per lane
-                    // (CL: each CTA of the pair scans half of the columns; a carry is written to the CTA that
-                    //  keeps its partition)
-                    const int job0 = CL ? (int)crank * (a.lanes >> 1) : 0;
-                    const int job1 = CL ? job0 + (a.lanes >> 1) : a.lanes;
+                    const int job0 = 0;
+                    const int job1 = a.lanes;
                     for (int s0 = job0 + (lt >> 5) * spw; s0 < job1; s0 += (tpt >> 5) * spw) {
-                        const int sg = s0 + (lane >> a.scan_log2);
+                        const int sg = s0 + (lane >> slog);
                         const bool ok = (q < P) && (sg < job1);
                         T *xs = xb + (size_t)q * W;
                         if constexpr (FUSE) asm volatile("" : "+l"(xs));  // (as for rp: hoisted out of the step loop it spills)
@@ -705,7 +753,7 @@ sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
                                 fb[c][e] = ok ? xs[c * vstr + ix] : T(0);
                                 bb[c][e] = ok ? xs[(NC + c) * vstr + ix] : T(0);
                             }
-                        scan_steps<sizeof(T) == 4>(a.scan_log2, [&](int st) {
+                        scan_steps<sizeof(T) == 4>(slog, [&](int st) {
                             T m[NC * NC];
 #pragma unroll
                             for (int i = 0; i < NC * NC; ++i) m[i] = fwm(st, i);
@@ -722,6 +770,61 @@ sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
                                 }
                             }
                         });
+                        // CL: carries across the CTAs of the cluster, two exchanges whatever the cluster size.  fb is the inclusive
+                        // scan of this CTA's partitions with zero carry-in; its last value F (this CTA's contribution to every
+                        // carry above it) goes to the inboxes of ALL CTAs above.  The carry into this CTA's first partition is then
+                        // sum over the CTAs s below of C_s F_s with C_s = Phi-products over the CTAs between (table slot 12, LHS
+                        // only), and it reaches partition q through Phi_q ... Phi_first (slot 10).
+                        [[maybe_unused]] T fin[NC][V];
+                        if constexpr (CL) {
+                            if (ok && q == P - 1) {
+                                for (int r = (int)crank + 1; r < csz; ++r) {
+                                    const unsigned rin = cluster_map(inbox_u32, (unsigned)r);
+#pragma unroll
+                                    for (int c = 0; c < NC; ++c)
+#pragma unroll
+                                        for (int e = 0; e < V; ++e)
+                                            st_cluster(rin + (unsigned)((((int)crank * NC + c) * W + sg * V + e) * (int)sizeof(T)), fb[c][e]);
+                                    mbar_arrive_remote(cluster_map(fin_bar, (unsigned)r) + 8u * sg);
+                                }
+                            }
+#pragma unroll
+                            for (int c = 0; c < NC; ++c)
+#pragma unroll
+                                for (int e = 0; e < V; ++e) fin[c][e] = T(0);
+                            if (crank > 0u && sg < job1) {
+                                mbar_wait_cluster(fin_bar + 8u * sg, cphase);
+                                for (int sb = 0; sb < (int)crank; ++sb) {
+                                    T cm_[NC * NC];
+#pragma unroll
+                                    for (int i = 0; i < NC * NC; ++i) cm_[i] = TAB[12 * sstr + i * mstr + sb];
+#pragma unroll
+                                    for (int e = 0; e < V; ++e) {
+                                        T f[NC];
+#pragma unroll
+                                        for (int c = 0; c < NC; ++c) f[c] = ok ? inbox[(sb * NC + c) * W + sg * V + e] : T(0);
+                                        if constexpr (TRI) {
+                                            fin[0][e] = fma_t<T>(cm_[0], f[0], fin[0][e]);
+                                        } else {
+                                            fin[0][e] = fma_t<T>(cm_[1], f[1], fma_t<T>(cm_[0], f[0], fin[0][e]));
+                                            fin[1][e] = fma_t<T>(cm_[3], f[1], fma_t<T>(cm_[2], f[0], fin[1][e]));
+                                        }
+                                    }
+                                }
+                                T m[NC * NC];
+#pragma unroll
+                                for (int i = 0; i < NC * NC; ++i) m[i] = tb[10 * sstr + i * mstr];
+#pragma unroll
+                                for (int e = 0; e < V; ++e) {
+                                    if constexpr (TRI) {
+                                        fb[0][e] = fma_t<T>(m[0], fin[0][e], fb[0][e]);
+                                    } else {
+                                        fb[0][e] = fma_t<T>(m[1], fin[1][e], fma_t<T>(m[0], fin[0][e], fb[0][e]));
+                                        fb[1][e] = fma_t<T>(m[3], fin[1][e], fma_t<T>(m[2], fin[0][e], fb[1][e]));
+                                    }
+                                }
+                            }
+                        }
                         [[maybe_unused]] T yn1[V], yn2[V];  // cyclic forms: y at rows n-1, n-2 (true g at the last rows)
                         if constexpr (PERTF) {
 #pragma unroll
@@ -747,7 +850,8 @@ sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
 #pragma unroll
                                 for (int c = 0; c < NC; ++c) {
                                     const T g = __shfl_up_sync(0xffffffffu, fb[c][e], 1, wd);
-                                    fb[c][e] = (q == 0) ? T(0) : g;
+                                    if constexpr (CL) fb[c][e] = (q == 0) ? fin[c][e] : g;
+                                    else fb[c][e] = (q == 0) ? T(0) : g;
                                 }
                                 if constexpr (TRI) {
                                     bb[0][e] = fma_t<T>(ch[0], fb[0][e], bb[0][e]);
@@ -757,7 +861,7 @@ sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
                                 }
                             }
                         }
-                        scan_steps<sizeof(T) == 4>(a.scan_log2, [&](int st) {
+                        scan_steps<sizeof(T) == 4>(slog, [&](int st) {
                             T m[NC * NC];
 #pragma unroll
                             for (int i = 0; i < NC * NC; ++i) m[i] = bwm(st, i);
@@ -774,6 +878,59 @@ sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
                                 }
                             }
                         });
+                        // CL: the backward carries the same way, downwards (bb already holds the true forward carries through u):
+                        // this CTA's first inclusive value goes to ALL CTAs below; the carry into its last partition is the sum
+                        // over the CTAs r above of D_r B_r (slot 12, entries 8 + r) and reaches partition q through slot 11.
+                        [[maybe_unused]] T bin[NC][V];
+                        if constexpr (CL) {
+                            if (ok && q == 0) {
+                                for (int r = 0; r < (int)crank; ++r) {
+                                    const unsigned rin = cluster_map(inbox_u32, (unsigned)r);
+#pragma unroll
+                                    for (int c = 0; c < NC; ++c)
+#pragma unroll
+                                        for (int e = 0; e < V; ++e)
+                                            st_cluster(rin + (unsigned)((((8 + (int)crank) * NC + c) * W + sg * V + e) * (int)sizeof(T)), bb[c][e]);
+                                    mbar_arrive_remote(cluster_map(bin_bar, (unsigned)r) + 8u * sg);
+                                }
+                            }
+#pragma unroll
+                            for (int c = 0; c < NC; ++c)
+#pragma unroll
+                                for (int e = 0; e < V; ++e) bin[c][e] = T(0);
+                            if ((int)crank + 1 < csz && sg < job1) {
+                                mbar_wait_cluster(bin_bar + 8u * sg, cphase);
+                                for (int sb = (int)crank + 1; sb < csz; ++sb) {
+                                    T dm_[NC * NC];
+#pragma unroll
+                                    for (int i = 0; i < NC * NC; ++i) dm_[i] = TAB[12 * sstr + i * mstr + 8 + sb];
+#pragma unroll
+                                    for (int e = 0; e < V; ++e) {
+                                        T f[NC];
+#pragma unroll
+                                        for (int c = 0; c < NC; ++c) f[c] = ok ? inbox[((8 + sb) * NC + c) * W + sg * V + e] : T(0);
+                                        if constexpr (TRI) {
+                                            bin[0][e] = fma_t<T>(dm_[0], f[0], bin[0][e]);
+                                        } else {
+                                            bin[0][e] = fma_t<T>(dm_[1], f[1], fma_t<T>(dm_[0], f[0], bin[0][e]));
+                                            bin[1][e] = fma_t<T>(dm_[3], f[1], fma_t<T>(dm_[2], f[0], bin[1][e]));
+                                        }
+                                    }
+                                }
+                                T m[NC * NC];
+#pragma unroll
+                                for (int i = 0; i < NC * NC; ++i) m[i] = tb[11 * sstr + i * mstr];
+#pragma unroll
+                                for (int e = 0; e < V; ++e) {
+                                    if constexpr (TRI) {
+                                        bb[0][e] = fma_t<T>(m[0], bin[0][e], bb[0][e]);
+                                    } else {
+                                        bb[0][e] = fma_t<T>(m[1], bin[1][e], fma_t<T>(m[0], bin[0][e], bb[0][e]));
+                                        bb[1][e] = fma_t<T>(m[3], bin[1][e], fma_t<T>(m[2], bin[0][e], bb[1][e]));
+                                    }
+                                }
+                            }
+                        }
                         // Cyclic correction in the scan: x = y - Z w with w = H V^T y.  Column m of Z = A'^{-1} e_r is
                         // itself "local solve + chi GZ^m + psi XZ^m", so -Z w only shifts the carries,
                         // G_q += GZ_q nw, X_q += XZ_q nw (nw = -w), plus the local solves in the two end partitions.
@@ -808,7 +965,8 @@ sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
                             for (int e = 0; e < V; ++e) {
                                 T x = __shfl_down_sync(0xffffffffu, bb[c][e], 1, wd);
                                 const int ix = (sg * V + e) ^ qsw;
-                                x = (q + 1 < P) ? x : T(0);
+                                if constexpr (CL) x = (q + 1 < P) ? x : bin[c][e];
+                                else x = (q + 1 < P) ? x : T(0);
                                 if constexpr (PERTF) {
                                     fb[c][e] = fma_t<T>(tb[10 * sstr], nw[0][e], fb[c][e]);
                                     x = fma_t<T>(tb[11 * sstr], nw[0][e], x);
@@ -823,25 +981,19 @@ sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
                                         x = fma_t<T>(xz[m * mstr], nw[m][e], x);
                                     }
                                     // the end partitions also need nw itself: (nw0, nw1) for partition 0, (nw2, nw3) for P-1
+                                    // (selected, not indexed: a run-time index would put nw into local memory)
                                     if (ok && (q == 0 || q == P - 1))
-                                        xs[(2 * NC + NHALO + c) * vstr + ix] = nw[(q == 0 ? 0 : 2) + c][e];
+                                        xs[(2 * NC + NHALO + c) * vstr + ix] = (q == 0) ? nw[c][e] : nw[2 + c][e];
                                 }
                                 if (ok) {
-                                    const T xv = x;
-                                    if (!CL || (q >= PL) == (crank != 0u)) {
-                                        xs[c * vstr + ix] = fb[c][e];
-                                        xs[(NC + c) * vstr + ix] = xv;
-                                    } else {
-                                        const unsigned pa = xb_peer + (unsigned)((q * W + c * vstr + ix) * (int)sizeof(T));
-                                        st_cluster(pa, fb[c][e]);
-                                        st_cluster(pa + (unsigned)(NC * vstr * (int)sizeof(T)), xv);
-                                    }
+                                    xs[c * vstr + ix] = fb[c][e];
+                                    xs[(NC + c) * vstr + ix] = x;
                                 }
                             }
                     }
                 }
-                if constexpr (CL) cluster_sync();
-                else group_sync(a.tpc, sub, tpt);
+                if constexpr (CL) cphase ^= 1u;  // both inbox barriers have completed one phase (or are unused at the chain's ends)
+                group_sync(a.tpc, sub, tpt);
 #pragma unroll
                 for (int e = 0; e < V; ++e) {
 #pragma unroll
@@ -1123,7 +1275,7 @@ sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
             if (a.hold_stores && t + stride_tiles < ntiles) mbar_wait(mbar, phase);
         }
         {
-            T *ps = p0;
+            S *ps = p0;
             asm volatile("" : "+l"(ps));  // keep the store addresses from being shared with the loads
 #pragma unroll
             for (int k = 0; k < MR; ++k) {
@@ -1343,7 +1495,7 @@ struct SweepEntry {
     const char *tag;   // the template arguments as profilers print them: "double, 2, 32, 0, 0, 1, 1, 0, 0"
 };
 
-template <typename T, int V, int MR, bool SINGLE, int KIND, bool TMA, bool WS, bool FUSE, bool CL = false>
+template <typename T, int V, int MR, bool SINGLE, int KIND, bool TMA, bool WS, bool FUSE, bool CL = false, typename S = T>
 cudaError_t launch_sweep(const SweepArgs &a, const CUtensorMap &tm, int grid, int block, size_t smem,
                          cudaStream_t st, int pdl)
 {
@@ -1354,9 +1506,9 @@ cudaError_t launch_sweep(const SweepArgs &a, const CUtensorMap &tm, int grid, in
     cfg.stream = st;
     cudaLaunchAttribute attr[2];
     int na = 0;
-    if (CL) {  // pairs of CTAs (two SMs) share a tile: grid is a multiple of 2
+    if (CL) {  // a.csz CTAs (SMs) share a tile: grid is a multiple of a.csz
         attr[na].id = cudaLaunchAttributeClusterDimension;
-        attr[na].val.clusterDim.x = 2;
+        attr[na].val.clusterDim.x = (unsigned)a.csz;
         attr[na].val.clusterDim.y = 1;
         attr[na].val.clusterDim.z = 1;
         ++na;
@@ -1368,7 +1520,7 @@ cudaError_t launch_sweep(const SweepArgs &a, const CUtensorMap &tm, int grid, in
     }
     cfg.attrs = attr;
     cfg.numAttrs = na;
-    return cudaLaunchKernelEx(&cfg, sweep_kernel<T, V, MR, SINGLE, KIND, TMA, WS, FUSE, CL>, a, tm);
+    return cudaLaunchKernelEx(&cfg, sweep_kernel<T, V, MR, SINGLE, KIND, TMA, WS, FUSE, CL, S>, a, tm);
 }
 
 }  // namespace btps

@@ -376,3 +376,72 @@ def test_penta_not_diagonally_dominant(lib, n):
     d = torch.from_numpy(r32).cuda()
     lib.penta_solve_batched_f32(h, d)
     assert rel_err(d.cpu().numpy().astype(np.float64), ref) <= max(TOL_F32, 16 * 1.2e-7 * cond)
+
+
+# ---- fp32 storage, fp64 arithmetic (SURVEY 8(f4)) ------------------------------------------------------------------------
+
+TOL_F32S = 1.0e-7   # rounding of the stored result to float: 2^-24 = 6e-8 relative per entry (+ fp64 arithmetic)
+
+
+@pytest.mark.parametrize("n", [1, 2, 5, 31, 32, 33, 64, 100, 256, 512, 777, 1000, 1024])
+def test_f32_storage_f64_arithmetic(lib, n):
+    """*_f32s: the batch lives in HBM as floats, the sweeps run in fp64.  Oracle = the fp64 oracle on the same
+    (float-representable) inputs, rounded to float as the store does; tolerance = the output rounding.  The all-fp32
+    path on the same inputs is checked to be the less accurate one (that is the point of the variant)."""
+    lt, lp = inputs.tri_lhs(n, 0.5), inputs.penta_lhs(n, 0.5)
+    ht, hp = lib.tri_factor(*lt), lib.penta_factor(*lp)
+    for batch in (1, 333, 2048 + 64):
+        r32 = inputs.uniform_rhs(n, batch, seed=70 + n).astype(np.float32)
+        for kind in ("tri", "penta"):
+            ref = r32.astype(np.float64)
+            if kind == "tri":
+                oracle.tri_solve_interleaved(oracle.tri_factor(*lt), ref)
+            else:
+                oracle.penta_solve_interleaved(oracle.penta_factor(*lp), ref)
+            ref32 = ref.astype(np.float32).astype(np.float64)
+            d = torch.from_numpy(r32).cuda()
+            (lib.tri_solve_batched_f32s(ht, d) if kind == "tri" else lib.penta_solve_batched_f32s(hp, d))
+            got = d.cpu().numpy().astype(np.float64)
+            # at most one float ulp from the correctly rounded fp64 solution, entry by entry
+            ulp = np.spacing(np.abs(ref32).astype(np.float32)).astype(np.float64)
+            assert np.all(np.abs(got - ref32) <= ulp + 1e-300), (n, batch, kind)
+            assert rel_err(got, ref) <= TOL_F32S, (n, batch, kind)
+            if n >= 64 and batch > 1000:
+                d2 = torch.from_numpy(r32).cuda()
+                (lib.tri_solve_batched_f32(ht, d2) if kind == "tri" else lib.penta_solve_batched_f32(hp, d2))
+                assert rel_err(got, ref) < rel_err(d2.cpu().numpy().astype(np.float64), ref), (n, kind)
+
+
+@pytest.mark.parametrize("kind,n,lb", [("tri", 512, 16), ("penta", 512, 16), ("tri", 1024, 19), ("penta", 64, 20)])
+def test_f32_storage_full_size_sampled(lib, kind, n, lb):
+    batch = 1 << lb
+    d = torch.empty(n, batch, dtype=torch.float32, device="cuda")
+    inputs.fill_uniform_device(d, n, seed=23)
+    ids = sample_ids(batch, 2048)
+    gi = torch.from_numpy(ids).cuda()
+    ref = inputs.uniform_rhs(n, len(ids), seed=23, systems=ids.astype(np.uint64)).astype(np.float32).astype(np.float64)
+    if kind == "tri":
+        lhs = inputs.tri_lhs(n, 0.5)
+        h = lib.tri_factor(*lhs)
+        lib.tri_solve_batched_f32s(h, d)
+        oracle.tri_solve_interleaved(oracle.tri_factor(*lhs), ref)
+    else:
+        lhs = inputs.penta_lhs(n, 0.5)
+        h = lib.penta_factor(*lhs)
+        lib.penta_solve_batched_f32s(h, d)
+        oracle.penta_solve_interleaved(oracle.penta_factor(*lhs), ref)
+    assert lib.btps_kernel_tag(h, 12, batch).endswith("float") and lib.btps_kernel_tag(h, 12, batch).startswith("double")
+    assert rel_err(d[:, gi].cpu().numpy().astype(np.float64), ref) <= TOL_F32S
+    assert bool(torch.isfinite(d).all())
+
+
+def test_f32_storage_rejects_what_it_does_not_cover(lib):
+    n = 2048
+    h = lib.tri_factor(*inputs.tri_lhs(n, 0.5))
+    d = torch.zeros(n, 64, dtype=torch.float32, device="cuda")
+    with pytest.raises(lib.BtpsError):
+        lib.tri_solve_batched_f32s(h, d)
+    hp = lib.tri_factor_periodic(*inputs.tri_lhs(64, 0.5))
+    d = torch.zeros(64, 64, dtype=torch.float32, device="cuda")
+    with pytest.raises(lib.BtpsError):
+        lib.tri_solve_batched_f32s(hp, d)

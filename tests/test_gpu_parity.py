@@ -440,7 +440,7 @@ def test_partition_padding_and_serial_walk(lib, n):
     if n <= 1024:
         assert plan["warp_scan"] == 1
     else:
-        assert plan["warp_scan"] == 0
+        assert plan["warp_scan"] == 0   # the single-CTA fallback plan (unaligned batches); aligned ones run the cluster chain
 
 
 def test_plan_reports_tma_and_ch_shape(lib):
@@ -798,13 +798,17 @@ def test_penta_cn_step(lib, periodic, n, batch):
         assert np.max(np.abs(outs[0][:, 0] - u0[:, 0] * ((1 - q) / (1 + q)) ** steps)) <= 1e-12
 
 
-# ---- cluster-split kernels (rows of a tile over two CTAs, carries through distributed shared memory) ----
+# ---- cluster-chain kernels (rows of a tile over 2 / 4 / 8 CTAs, carries through distributed shared memory) ----
 
-@pytest.mark.parametrize("n", [1024, 1000, 600, 544])
+@pytest.mark.parametrize("n", [1024, 1000, 600, 544, 1500, 2048, 2500, 4096, 3000])
 @pytest.mark.parametrize("batch", [4096 + 32, 64, 2048 * 9])
-def test_cluster_split_equals_single_cta(lib, n, batch):
-    """17..32 partitions: plain solves run on clusters of two CTAs; same arithmetic, so bitwise equal to the
-    single-CTA kernels (btps_tune cluster = 1 forces the pair, 0 forbids it), for single solves and fused steps, and within tolerance of the oracle."""
+def test_cluster_chain_against_oracle(lib, n, batch):
+    """More than 16 partitions: plain solves can run on a thread-block cluster whose CTAs each keep a block of the rows
+    (two CTAs up to N = 1024, four up to 2048, eight up to 4096); carries cross the CTAs as a chain through distributed
+    shared memory.  btps_tune cluster = 1 forces the chain for every eligible plan (0 forbids it).  Single solves, fused
+    steps and fp32 against the oracle, and against the library's other plan for the same system."""
+    if n * batch > 40_000_000:
+        batch = 2048 * 3
     lt, lp = rand_tri(n, n), rand_penta(n, n + 1)
     rhs = inputs.uniform_rhs(n, batch, seed=51)
     outs = {}
@@ -812,6 +816,9 @@ def test_cluster_split_equals_single_cta(lib, n, batch):
         try:
             lib.btps_tune("cluster", cl)
             ht, hp = lib.tri_factor(*lt), lib.penta_factor(*lp)
+            tags = (lib.btps_kernel_tag(ht, 8, batch), lib.btps_kernel_tag(hp, 8, batch), lib.btps_kernel_tag(hp, 4, batch))
+            # ninth template argument: cluster split ("two_pass_kernel" has none)
+            assert all(len(t.split(", ")) > 8 and t.split(", ")[8] == "1" for t in tags) == (cl == 1), tags
             a, b_, c, d = dev(rhs), dev(rhs), dev(rhs), dev(rhs)
             lib.tri_solve_batched(ht, a)
             lib.penta_solve_batched(hp, b_)
@@ -819,21 +826,62 @@ def test_cluster_split_equals_single_cta(lib, n, batch):
             lib.penta_solve_steps(hp, d, 11)
             f32 = dev(rhs.astype(np.float32))
             lib.penta_solve_batched_f32(hp, f32)
-            outs[cl] = [x.cpu().numpy() for x in (a, b_, c, d, f32)]
+            g32 = dev(rhs.astype(np.float32))
+            lib.tri_solve_batched_f32(ht, g32)
+            outs[cl] = [x.cpu().numpy() for x in (a, b_, c, d, f32, g32)]
         finally:
             lib.btps_tune("cluster", -1)
-    for x, y in zip(outs[1], outs[0]):
-        assert np.array_equal(x, y)
-    ref = rhs.copy()
-    oracle.tri_solve_interleaved(oracle.tri_factor(*lt), ref)
-    assert rel_err(outs[1][0], ref) <= TOL_SINGLE
-    ref = rhs.copy()
-    oracle.penta_solve_interleaved(oracle.penta_factor(*lp), ref)
-    assert rel_err(outs[1][1], ref) <= TOL_SINGLE
-    assert rel_err(outs[1][4].astype(np.float64), ref) <= TOL_F32
-    ref = rhs.copy()
-    oracle.penta_solve_interleaved(oracle.penta_factor(*lp), ref, nsteps=11)
-    assert rel_err(outs[1][3], ref) <= TOL_STEPS
+    r32 = rhs.astype(np.float32).astype(np.float64)
+    for cl in (1, 0):
+        ref = rhs.copy()
+        oracle.tri_solve_interleaved(oracle.tri_factor(*lt), ref)
+        assert rel_err(outs[cl][0], ref) <= TOL_SINGLE, cl
+        ref = rhs.copy()
+        oracle.penta_solve_interleaved(oracle.penta_factor(*lp), ref)
+        assert rel_err(outs[cl][1], ref) <= TOL_SINGLE, cl
+        ref = rhs.copy()
+        oracle.tri_solve_interleaved(oracle.tri_factor(*lt), ref, nsteps=11)
+        assert rel_err(outs[cl][2], ref) <= TOL_STEPS, cl
+        ref = rhs.copy()
+        oracle.penta_solve_interleaved(oracle.penta_factor(*lp), ref, nsteps=11)
+        assert rel_err(outs[cl][3], ref) <= TOL_STEPS, cl
+        ref = r32.copy()
+        oracle.penta_solve_interleaved(oracle.penta_factor(*lp), ref)
+        assert rel_err(outs[cl][4].astype(np.float64), ref) <= TOL_F32, cl
+        ref = r32.copy()
+        oracle.tri_solve_interleaved(oracle.tri_factor(*lt), ref)
+        assert rel_err(outs[cl][5].astype(np.float64), ref) <= TOL_F32, cl
+
+
+@pytest.mark.parametrize("n", [1024, 2048, 4096])
+def test_cluster_chain_repeats_bitwise_and_many_tiles(lib, n):
+    """The chain hands carries from CTA to CTA through mbarrier-signalled inboxes that are reused tile after tile and
+    step after step: many tiles per cluster (grid capped) with fused steps, run 6 times, must give the same bits and
+    match the oracle."""
+    batch = 32 * 37
+    lt, lp = inputs.tri_lhs(n, 0.5), inputs.penta_lhs(n, 0.5)
+    rhs = inputs.uniform_rhs(n, batch, seed=52)
+    rt, rp = rhs.copy(), rhs.copy()
+    oracle.tri_solve_interleaved(oracle.tri_factor(*lt), rt, nsteps=5)
+    oracle.penta_solve_interleaved(oracle.penta_factor(*lp), rp, nsteps=5)
+    try:
+        lib.btps_tune("cluster", 1)
+        lib.btps_tune("grid", 16)
+        ht, hp = lib.tri_factor(*lt), lib.penta_factor(*lp)
+        first = None
+        for rep in range(6):
+            a, b_ = dev(rhs), dev(rhs)
+            lib.tri_solve_steps(ht, a, 5)
+            lib.penta_solve_steps(hp, b_, 5)
+            got = (a.cpu().numpy(), b_.cpu().numpy())
+            if first is None:
+                first = got
+                assert rel_err(got[0], rt) <= TOL_STEPS and rel_err(got[1], rp) <= TOL_STEPS
+            else:
+                assert np.array_equal(first[0], got[0]) and np.array_equal(first[1], got[1])
+    finally:
+        lib.btps_tune("cluster", -1)
+        lib.btps_tune("grid", -1)
 
 
 # ---- CUDA graph capture of a time-step loop ------------------------------------------------------------
