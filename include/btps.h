@@ -28,6 +28,12 @@
  *  - No pivoting (the paper has none): a zero or non-finite pivot makes the
  *    factor call fail with BTPS_E_PIVOT.
  *  - There is no CPU fallback anywhere: every call that touches a batch needs a CUDA device.
+ *  - Numerical behaviour: the kernels evaluate the paper's LU solve (no pivoting) partition-wise -- 32 rows per
+ *    thread, carries across partitions by a scan whose multipliers are products of up to 32 elimination multipliers
+ *    l_i = a_i / b^_i.  For diagonally dominant A (every benchmark of the paper) |l_i| < 1.  For valid but
+ *    non-dominant A those products grow as the rounding error of Alg. 2's own recurrence does; results then agree
+ *    with the sequential algorithm to rounding times cond(A), not to the last bits (C-33).
+ *  - btps_tune is process-global and not synchronised: set it before the threads that factor and solve start.
  */
 #ifndef BTPS_H_
 #define BTPS_H_

@@ -294,7 +294,7 @@ int factor_penta_host(int n, const double *e, const double *a, const double *d, 
 
 // ------------------------------------------------------------------------------------------------
 // factor tables for the partitioned sweep; fp64 host arithmetic, rounded to
-// T when written into the blob.  Rows are padded to Np = P*rows with identity rows.
+// T when written into the blob.  Rows are padded to Np = P*rows with all-zero rows (inv = 0: a padding row solves to exactly 0).
 // ------------------------------------------------------------------------------------------------
 
 // Carry-scan tables (sweep.cuh, RecLayout): slot 0 / 1 = forward / backward carry matrices of each
@@ -465,7 +465,7 @@ void build_blob_tri(int n, DtypePlan &pl, const std::vector<double> &inv, const 
         }
         for (int k = 0; k < MR; ++k) {
             const int i = r0 + k;
-            putv(0, i, 0, at(inv, i, 1.0));
+            putv(0, i, 0, at(inv, i, 0.0));  // padding rows: g = 0 * f, whatever the explicit half put there
             putv(0, i, 1, at(nl, i, 0.0));
             putv(2, i, 0, at(nch, i, 0.0));
             putv(3, i, 0, chi[k]);
@@ -556,7 +556,7 @@ void build_blob_penta(int n, DtypePlan &pl, const std::vector<double> &inv, cons
         }
         for (int k = 0; k < MR; ++k) {
             const int i = r0 + k;
-            putv(0, i, 0, at(inv, i, 1.0));
+            putv(0, i, 0, at(inv, i, 0.0));  // padding rows: g = 0 * f, whatever the explicit half put there
             putv(0, i, 1, at(nle, i, 0.0));
             putv(2, i, 0, at(nlb, i, 0.0));
             putv(3, i, 0, at(ngam, i, 0.0));

@@ -69,7 +69,7 @@ struct SweepArgs {
                            // 1 / (1 - <C^2>) after step ks (eq. 30); nullptr: no statistic
     double stat_scale;     // 1 / batch
     int n;                 // true number of rows
-    int P;                 // partitions per system (rows padded to P*MR with identity rows)
+    int P;                 // partitions per system (rows padded to P*MR with all-zero table rows)
     int lanes;             // threads side by side on adjacent systems (power of two <= 32)
     int lanes_log2;
     int tpc;               // tile groups per CTA (each walks its own tiles)
@@ -138,7 +138,7 @@ __device__ __forceinline__ float fma_t<float>(float a, float b, float c) { retur
 template <typename T>
 __device__ __forceinline__ T ch_w(T c) { return fma_t<T>(c * c, c, -c); }
 
-// Coefficient image ("blob"), all in element type T, rows padded to Np = P*MR with identity rows.
+// Coefficient image ("blob"), all in element type T, rows padded to Np = P*MR with all-zero rows (a padding row solves to exactly 0).
 // One block per partition (MR rows), inside it a structure of arrays with one entry per row, pairs
 // {T,T} where one phase of a row needs two values (one LDS.128 in fp64), so that a thread addresses
 // everything as one base + compile-time offsets; element offsets of the arrays in units of MR:
@@ -179,6 +179,17 @@ struct RecLayout {
 
 // ---- TMA / mbarrier primitives (PTX) -------------------------------------------------------------
 __device__ __forceinline__ unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
+
+// A shared-memory pointer passed through an opaque 32-bit register: the compiler recomputes what it derives from it where
+// it is used (hoisted out of the tile / step loops those addresses spill) and still knows the result to be shared memory
+// (LDS / STS; through a 64-bit generic register it would emit generic LD / ST).
+template <typename P>
+__device__ __forceinline__ P *opaque_shared(P *p)
+{
+    unsigned a32 = smem_u32(p);
+    asm volatile("" : "+r"(a32));
+    return reinterpret_cast<P *>(__cvta_shared_to_generic((size_t)a32));
+}
 
 __device__ __forceinline__ void mbar_init(unsigned bar, unsigned count)
 {
@@ -464,8 +475,10 @@ sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
             // ---- take the prefetched tile out of the ring, then have it refilled ---------------
             mbar_wait(mbar, phase);
             phase ^= 1u;
-            const S *rp = ring + ((r0 - rbase) * W + sl * V);
-            asm volatile("" : "+l"(rp));  // recompute the MR row addresses per tile: hoisted out of the loop they spill
+            // (the address goes through an opaque 32-bit register so that the MR row addresses are recomputed per tile
+            //  -- hoisted out of the loop they spill -- and comes back as a pointer the compiler still knows to be shared
+            //  memory: LDS, not generic LD)
+            const S *rp = opaque_shared(ring + ((r0 - rbase) * W + sl * V));
 #pragma unroll
             for (int k = 0; k < MR; ++k) ld_sys<T, V>(v[k], rp + k * W);
             if constexpr (HALO1) {
@@ -561,13 +574,14 @@ sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
                 for (int e = 0; e < V; ++e) cprev[e] = cm[e];
 #pragma unroll
                 for (int k = 0; k < MR; ++k) {
-                    const bool row_ok = (k < nrow_part);
+                    // (padding rows need no masking: their table rows have inv = nl = 0, so whatever f holds there,
+                    //  g and x of a padding row come out as exact zeros)
 #pragma unroll
                     for (int e = 0; e < V; ++e) {
                         const T cn = (k + 1 < MR) ? v[(k + 1 < MR) ? k + 1 : k][e] : cp[e];
                         const T f = fma_t<T>(xa, cprev[e], fma_t<T>(xc, cn, xb * v[k][e]));
                         cprev[e] = v[k][e];
-                        v[k][e] = row_ok ? f : T(0);  // padding rows stay identity rows with zero RHS
+                        v[k][e] = f;
                     }
                 }
             }
@@ -605,7 +619,6 @@ sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
                 for (int e = 0; e < V; ++e) { c1[e] = cm[e]; c2[e] = cm2[e]; }
 #pragma unroll
                 for (int k = 0; k < MR; ++k) {
-                    const bool row_ok = (k < nrow_part);
 #pragma unroll
                     for (int e = 0; e < V; ++e) {
                         const T n1 = (k + 1 < MR) ? v[(k + 1 < MR) ? k + 1 : k][e] : cp[e];
@@ -616,7 +629,7 @@ sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
                         f = fma_t<T>(x4, n2, f);
                         c2[e] = c1[e];
                         c1[e] = v[k][e];
-                        v[k][e] = row_ok ? f : T(0);  // padding rows stay identity rows with zero RHS
+                        v[k][e] = f;  // (padding rows: inv = 0 in their table rows, see above)
                     }
                 }
             }
@@ -631,14 +644,12 @@ sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
                 for (int k = 0; k < MR; ++k) {
                     const Pair cf = RA[k];
                     const T nlb = RB1[k];
-                    const bool row_ok = (k < nrow_part);
 #pragma unroll
                     for (int e = 0; e < V; ++e) {
                         const T wn = ch_w<T>((k + 1 < MR) ? v[(k + 1 < MR) ? k + 1 : k][e] : cp[e]);
                         T s = wm[e] + wn;
                         s = fma_t<T>(T(-2), wc[e], s);
-                        T f = fma_t<T>(ax, s, v[k][e]);
-                        f = row_ok ? f : T(0);  // padding rows stay identity rows with zero RHS
+                        const T f = fma_t<T>(ax, s, v[k][e]);  // (padding rows: inv = 0 in their table rows, see above)
                         wm[e] = wc[e];
                         wc[e] = wn;
                         const T t2 = fma_t<T>(cf.v[1], g2[e], cf.v[0] * f);
@@ -694,7 +705,7 @@ sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
             const int wm = W - 1;
             // this thread's columns of its partition: element e lives at xc[XI(e)]
             T *xc = xb + (size_t)(CL ? plidx : part) * W;
-            if constexpr (FUSE) asm volatile("" : "+l"(xc));
+            if constexpr (FUSE) xc = opaque_shared(xc);
             const int xsw = (CL ? plidx : part) & wm;
 #define XI(e) (((sl * V + (e)) ^ xsw))
             const int vstr = P * W;  // elements between successive values
@@ -721,7 +732,7 @@ sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
                     const int q = lane & (wd - 1);
                     const int spw = 32 >> slog;  // jobs per warp pass
                     const T *tb = TAB + q;
-                    if constexpr (FUSE) asm volatile("" : "+l"(tb));
+                    if constexpr (FUSE) tb = opaque_shared(tb);
                     const int mstr = tq;                // elements between matrix entries
                     const int sstr = NC * NC * tq;      // elements between table slots
                     // multipliers of step st: slots 2st (forward) / 2st+1 (backward); step 4 shares
@@ -742,7 +753,7 @@ sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
                         const int sg = s0 + (lane >> slog);
                         const bool ok = (q < P) && (sg < job1);
                         T *xs = xb + (size_t)q * W;
-                        if constexpr (FUSE) asm volatile("" : "+l"(xs));  // (as for rp: hoisted out of the step loop it spills)
+                        if constexpr (FUSE) xs = opaque_shared(xs);  // (as for rp: hoisted out of the step loop it spills)
                         const int qsw = q & wm;
                         T fb[NC][V], bb[NC][V];  // forward / backward scan state (then the carries G / X)
 #pragma unroll
