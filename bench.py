@@ -68,6 +68,7 @@ def parse_args():
                     help="time one cell instead of the headline step, e.g. tri,1024,19,f64 (kinds: tri, penta, ch, "
                          "tri_periodic, penta_periodic, ch_periodic); may be repeated")
     ap.add_argument("--tune", action="append", default=[], metavar="KEY=VALUE", help="btps_tune setting applied first")
+    ap.add_argument("--rotate", type=int, default=0, help="--cell: rotate over this many buffers (default: as many as keep the cell cold)")
     return ap.parse_args()
 
 
@@ -321,11 +322,12 @@ KIND_INDEX = {"tri": 0, "tri_periodic": 0, "tri_f32s": 0, "penta": 1, "penta_per
               "ch_periodic": 2}
 
 
-def make_cell(torch, b, inputs, kind, n, batch, elem, steps_per_call=1):
+def make_cell(torch, b, inputs, kind, n, batch, elem, steps_per_call=1, rotate=0):
     """(handle, fn(buf, stream=None), buffers) of one cell; buffers rotate when one would stay in L2."""
     dt = torch.float64 if elem == 8 else torch.float32
     size = n * batch * elem
     nbuf = 1 if size > 2 * L2_BYTES else int(min(64, math.ceil(4 * L2_BYTES / size)))
+    nbuf = rotate if rotate > 0 else nbuf
     bufs = []
     for k in range(nbuf):
         t = torch.empty(n, batch, dtype=dt, device="cuda")
@@ -471,9 +473,9 @@ def run_cells(args):
     for cell in args.cell:
         kind, n, lb, dt = cell.split(",")
         n, batch, elem = int(n), 1 << int(lb), 8 if dt == "f64" else 4
-        h, fn, bufs = make_cell(torch, b, inputs, kind, n, batch, elem)
+        h, fn, bufs = make_cell(torch, b, inputs, kind, n, batch, elem, rotate=args.rotate)
         fn(bufs[0])
-        ms = time_launches(torch, fn, bufs, max(4, min(20, len(bufs))), repeats=5)
+        ms = time_launches(torch, fn, bufs, max(4, min(20, len(bufs))) if not args.rotate else 12, repeats=5)
         gbs = 2.0 * n * batch * elem / ms / 1e6
         kidx = KIND_INDEX[kind]
         print(json.dumps({"cell": cell, "tune": args.tune, "ms": round(ms, 5), "hbm_gbs": round(gbs, 1),

@@ -225,10 +225,12 @@ BTPS_API const char *btps_error_string(int code);
 BTPS_API int btps_plan_info(int kind, const void *handle, int elem_bytes, int *out);
 
 /* Override the plan chosen at factor time (call BEFORE tri_factor / penta_factor; process
- * global).  key is one of "rows" (rows per thread: 8, 16, 32), "lanes" (32, 16, 8, 4),
+ * global).  key is one of "rows" (rows per thread: 32; 8 and 16 only in a library built with BTPS_TUNING_VARIANTS=1,
+ * otherwise BTPS_E_ARG), "lanes" (32, 16, 8, 4),
  * "vec" (systems per thread: 1, 2, 4), "tiles_per_cta", "force_two_pass" (0/1), "prefetch"
- * (0: never use the TMA prefetch variant), "warp_scan" (0: serial carry walk), "pdl" (0: no
- * programmatic dependent launch attribute), "fuse_steps" (time steps advanced per launch while a tile
+ * (0: never use the TMA prefetch variant), "warp_scan" (0: serial carry walk), "pdl" (1 / 0: launch with / without the
+ * programmatic-dependent-launch attribute; default: with it for batches of at most 128 MiB, where hiding the launch
+ * latency gains 3-17 %; larger ones are indifferent or lose), "fuse_steps" (time steps advanced per launch while a tile
  * is on chip in *_solve_steps / ch_step_batched: default and maximum 64, 1 = one launch per step), "grid" (cap on
  * the number of CTAs), "cyclic_in_scan" (0: periodic pentadiagonal handles apply the cyclic correction row by row
  * instead of folding it into the carry scan), "cluster" (1: run every eligible plain solve of 17..32 partitions on clusters of two CTAs
@@ -240,6 +242,8 @@ BTPS_API int btps_plan_info(int kind, const void *handle, int elem_bytes, int *o
  * measured best on B200 / PCIe Gen5, 43.5 GB/s in each direction at once).
  * "hold_stores" (1: a tile's stores wait until the next tile's prefetch has landed, 0: never; default: the kinds
  * and tile sizes where that was measured to win -- tridiagonal kinds and the plain fp64 pentadiagonal solve on full tiles).
+ * "blk_pad" (bytes of padding behind every partition's coefficient block in shared memory, a multiple of 16: moves the
+ * coefficient reads of the partitions that share a warp onto different banks).
  * value < 0 restores the default.  "pdl", "fuse_steps", "grid", "cluster", "reverse", "one_step_fused",
  * "host_chunk_kib" and "hold_stores" are read at launch time, the others when a handle is built. */
 BTPS_API int btps_tune(const char *key, int value);

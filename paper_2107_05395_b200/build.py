@@ -19,6 +19,10 @@ LIB = os.path.join(HERE, "libbtps.so")
 
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC,-fvisibility=hidden"]
+# BTPS_TUNING_VARIANTS=1: also compile the partitioned kernels with 8 / 16 rows per thread (btps_tune("rows", 8 | 16)),
+# which only A/B measurements use; the default library leaves them out (a third of its size)
+if os.environ.get("BTPS_TUNING_VARIANTS", "") not in ("", "0"):
+    NVCC_FLAGS = NVCC_FLAGS + ["-DBTPS_TUNING_VARIANTS"]
 UNITS = ["btps.cu"] + [f"inst_{k}_{t}.cu" for k in ("tri", "penta", "ch", "trip", "pentap", "chp") for t in ("f64", "f32")] + \
         ["inst_tricn_f64.cu", "inst_tricnp_f64.cu", "inst_pentacn_f64.cu", "inst_pentacnp_f64.cu",
          "inst_pentapf_f64.cu", "inst_pentapf_f32.cu", "inst_chpf_f64.cu", "inst_pentacnpf_f64.cu",
@@ -51,6 +55,7 @@ def build_id() -> str:
     for name in sorted(UNITS) + HEADERS:
         with open(name if os.path.isabs(name) else os.path.join(CSRC, name), "rb") as f:
             h.update(f.read())
+    h.update(" ".join(NVCC_FLAGS).encode())
     return h.hexdigest()[:12]
 
 
@@ -58,10 +63,12 @@ def build(force: bool = False, verbose: bool = False) -> str:
     """Compile csrc/*.cu -> libbtps.so.  Returns the library path."""
     os.makedirs(OBJ, exist_ok=True)
     src_time = _newest(UNITS + HEADERS + [os.path.abspath(__file__)])
-    if not force and os.path.exists(LIB) and os.path.getmtime(LIB) >= src_time:
+    bid = build_id()
+    stamp = os.path.join(OBJ, "build_id.txt")
+    same_flags = os.path.exists(stamp) and open(stamp).read().strip() == bid
+    if not force and os.path.exists(LIB) and os.path.getmtime(LIB) >= src_time and same_flags:
         return LIB
     nvcc = _nvcc()
-    bid = build_id()
 
     def compile_one(unit):
         obj = os.path.join(OBJ, unit.replace(".cu", ".o"))
@@ -79,6 +86,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
     _run([nvcc, "-shared", "-o", tmp] + objs + ["-gencode", "arch=compute_100a,code=sm_100a",
                                                   "-Xcompiler", "-fPIC", "-cudart", "static"])
     os.replace(tmp, LIB)
+    with open(stamp, "w") as f:
+        f.write(bid + "\n")
     return LIB
 
 

@@ -55,7 +55,7 @@ std::atomic<long long> g_launches{0};
 // ------------------------------------------------------------------------------------------------
 struct Tune {
     int rows = -1, lanes = -1, vec = -1, tpc = -1, force_two_pass = -1, reverse = -1, prefetch = -1, pdl = -1,
-        warp_scan = -1, grid = -1, fuse = -1, cluster = -1, cyclic_scan = -1, one_step_fused = -1, host_chunk_kib = -1, hold_stores = -1;
+        warp_scan = -1, grid = -1, fuse = -1, cluster = -1, blk_pad = -1, cyclic_scan = -1, one_step_fused = -1, host_chunk_kib = -1, hold_stores = -1;
 };
 Tune g_tune;
 
@@ -105,6 +105,7 @@ struct DtypePlan {
     unsigned offTc = 0;         // byte offset in the blob of the csz per-CTA scan-table blocks
     unsigned tab_bytes_cl = 0;  // bytes of one such block
     unsigned blob_total = 0;    // blob bytes on the device (blob_bytes = what the single-CTA kernels stage)
+    int blk_pad = 0;            // bytes of padding behind every partition's coefficient block (blk_stride)
     Shape cshape;
     KernelSlot ck;
 };
@@ -124,6 +125,8 @@ struct Handle {
     DtypePlan plan[2];  // 0: fp64, 1: fp32
     std::mutex mu;      // guards lazy occupancy resolution
 };
+
+int blk_stride(const DtypePlan &pl, int RT) { return RT * pl.rows + pl.blk_pad / pl.elem; }
 
 int ilog2(int v)
 {
@@ -213,6 +216,7 @@ void choose_plan(int n, int elem, int handle_kind, DtypePlan &pl)
         finish_shape(elem, rows, P, pl.shape[k]);
         if (P * pl.shape[k].lanes > thread_cap(rows, pl.shape[k].vec, elem)) pl.two_pass = true;
     }
+    pl.blk_pad = g_tune.blk_pad >= 0 ? (g_tune.blk_pad / 16) * 16 : 0;
     pl.rows = rows;
     pl.P = P;
     pl.ws = ws;
@@ -220,6 +224,10 @@ void choose_plan(int n, int elem, int handle_kind, DtypePlan &pl)
     pl.tq = P > SCAN_LANES ? P : SCAN_LANES;
 }
 
+// Elements between the coefficient blocks of successive partitions: the block itself (RT arrays of `rows` entries) plus
+// padding.  The threads of one partition read the same coefficient (a broadcast); the 2 or 4 partitions that share a warp
+// read theirs one block apart, and an unpadded block (5 or 9 arrays x 32 rows x 8 bytes) is a multiple of 128 bytes, which
+// puts them all on the same banks.  pl.blk_pad bytes of padding (a multiple of 16) walk them onto different banks.
 template <typename T>
 void put(std::vector<unsigned char> &blob, size_t off, double v)
 {
@@ -439,13 +447,13 @@ void build_blob_tri(int n, DtypePlan &pl, const std::vector<double> &inv, const 
     // coefficient values per row: the periodic form carries z = A'^{-1} u as a sixth array
     const int RT = z ? RecLayout<KIND_TRIP>::ELEMS : RecLayout<KIND_TRI>::ELEMS;
     auto at = [&](const std::vector<double> &v, int i, double pad) { return i < n ? v[i] : pad; };
-    pl.offT = (unsigned)align16((size_t)Np * RT * sizeof(T));
+    pl.offT = (unsigned)align16((size_t)P * blk_stride(pl, RT) * sizeof(T));
     pl.blob_bytes = (unsigned)align16(pl.offT + scan_table_bytes(pl, 1, sizeof(T)));
     blob.assign(pl.blob_bytes, 0);
     std::vector<double> phi(MR), chi(MR), psi(MR);
     std::vector<Mat> Phi(P), Psi(P), Chi0(P);
     auto putv = [&](int arr, int i, int j, double v) {  // partition block, array at offset arr*MR, row i, value j
-        const size_t blk = (size_t)(i / MR) * RT * MR;
+        const size_t blk = (size_t)(i / MR) * blk_stride(pl, RT);
         put<T>(blob, (blk + (size_t)arr * MR + (size_t)(i % MR) * (arr == 2 ? 1 : 2) + j) * sizeof(T), v);
     };
     for (int p = 0; p < P; ++p) {
@@ -470,7 +478,7 @@ void build_blob_tri(int n, DtypePlan &pl, const std::vector<double> &inv, const 
             putv(2, i, 0, at(nch, i, 0.0));
             putv(3, i, 0, chi[k]);
             putv(3, i, 1, psi[k]);
-            if (z && !pl.wfast) put<T>(blob, ((size_t)(i / MR) * RT * MR + (size_t)5 * MR + (i % MR)) * sizeof(T), at(*z, i, 0.0));
+            if (z && !pl.wfast) put<T>(blob, ((size_t)(i / MR) * blk_stride(pl, RT) + (size_t)5 * MR + (i % MR)) * sizeof(T), at(*z, i, 0.0));
         }
         Phi[p].m[0] = phi[MR - 1];
         Psi[p].m[0] = psi[0];
@@ -497,7 +505,7 @@ void build_blob_tri(int n, DtypePlan &pl, const std::vector<double> &inv, const 
             }
             for (int k = MR - 2; k >= 0; --k) loc[k] = loc[k] + nch[r0 + k] * loc[k + 1];
             for (int k = 0; k < MR; ++k)
-                put<T>(blob, ((size_t)p * RT * MR + (size_t)5 * MR + k) * sizeof(T), loc[k]);
+                put<T>(blob, ((size_t)p * blk_stride(pl, RT) + (size_t)5 * MR + k) * sizeof(T), loc[k]);
         }
     }
 }
@@ -514,7 +522,7 @@ void build_blob_penta(int n, DtypePlan &pl, const std::vector<double> &inv, cons
     const int RT = Z ? (pl.wfast ? RecLayout<KIND_PENTAPF>::ELEMS : RecLayout<KIND_PENTAP>::ELEMS)
                      : RecLayout<KIND_PENTA>::ELEMS;
     auto at = [&](const std::vector<double> &v, int i, double pad) { return i < n ? v[i] : pad; };
-    pl.offT = (unsigned)align16((size_t)Np * RT * sizeof(T));
+    pl.offT = (unsigned)align16((size_t)P * blk_stride(pl, RT) * sizeof(T));
     pl.blob_bytes = (unsigned)align16(pl.offT + scan_table_bytes(pl, 2, sizeof(T)));
     blob.assign(pl.blob_bytes, 0);
     std::vector<double> phi[2], chi[2], psi[2];
@@ -525,7 +533,7 @@ void build_blob_penta(int n, DtypePlan &pl, const std::vector<double> &inv, cons
     }
     std::vector<Mat> Phi(P), Psi(P), Chi0(P);
     auto putv = [&](int arr, int i, int j, double v) {  // partition block, array at offset arr*MR, row i, value j
-        const size_t blk = (size_t)(i / MR) * RT * MR;
+        const size_t blk = (size_t)(i / MR) * blk_stride(pl, RT);
         put<T>(blob, (blk + (size_t)arr * MR + (size_t)(i % MR) * (arr == 2 ? 1 : 2) + j) * sizeof(T), v);
     };
     for (int p = 0; p < P; ++p) {
@@ -758,7 +766,7 @@ void fill_cluster_slot(Handle *h, DtypePlan &pl)
     sl.xvals = 2 * NC;
     sl.xper = (int)(sl.xvals * PL * W);
     sl.xstride = sl.xper;
-    const size_t rows_bytes = (size_t)PL * elems * pl.rows * pl.elem;
+    const size_t rows_bytes = (size_t)PL * blk_stride(pl, elems) * pl.elem;
     sl.offTl = (unsigned)align16(rows_bytes);
     sl.offX = (unsigned)align16(sl.offTl + pl.tab_bytes_cl);
     sl.offIn = (unsigned)align16(sl.offX + (size_t)sl.xstride * pl.elem);
@@ -1099,6 +1107,7 @@ int launch_one(Handle *h, int kind, S *d_rhs, long long batch, double alpha_x, i
         const bool penta_ok = (kind == KIND_PENTA) && sizeof(T) == 8 && !h->periodic && sh.lanes == 16;
         a.hold_stores = g_tune.hold_stores >= 0 ? (g_tune.hold_stores > 0) : ((full_tile && (tri_family || penta_ok)) ? 1 : 0);
     }
+    a.blk = blk_stride(pl, h->kind == KIND_TRI ? (h->periodic ? 6 : 5) : (h->periodic ? (pl.wfast ? 11 : 13) : 9));  // = RecLayout<KIND>::ELEMS of the kernel
     a.csz = use_cl ? pl.csz : 1;
     a.scan_log2_cl = pl.scan_log2_cl;
     a.tab_bytes_cl = pl.tab_bytes_cl;
@@ -1140,8 +1149,13 @@ int launch_one(Handle *h, int kind, S *d_rhs, long long batch, double alpha_x, i
     a.ksteps = fused ? ksteps : 1;
     a.stat = fused ? stat : nullptr;
     a.stat_scale = 1.0 / (double)batch;
+    // Programmatic dependent launch (the next launch's prologue -- barrier set-up, table staging -- overlaps this launch's
+    // tail).  Measured on B200 (profiles/r02a_headline_ab.md): launches of up to ~30 us gain 3-17 % from it (N = 64 ... 256 up
+    // to 2^16 systems), batches of 256 MiB are indifferent (+-1 %), N = 1024 from 2^16 systems loses 5-7 % and the
+    // three-kernel step of bench.py 4.5 %: on by default for batches of at most 128 MiB.
+    const int pdl = g_tune.pdl >= 0 ? (g_tune.pdl > 0) : ((size_t)h->n * (size_t)batch * sizeof(S) <= ((size_t)128 << 20));
     for (int l = 0; l < nlaunch; ++l) {
-        const cudaError_t e = (fused ? sl.fused : sl.ent).launch(a, tm, (int)grid, sh.threads, sl.smem, st, g_tune.pdl != 0);
+        const cudaError_t e = (fused ? sl.fused : sl.ent).launch(a, tm, (int)grid, sh.threads, sl.smem, st, pdl);
         g_launches.fetch_add(1, std::memory_order_relaxed);
         if (e != cudaSuccess) return cuda_fail(e, "sweep launch");
         if (stat && !fused) {
@@ -1680,7 +1694,13 @@ int btps_plan_info(int kind, const void *handle, int elem_bytes, int *out)
 int btps_tune(const char *key, int value)
 {
     if (!key) return set_err(BTPS_E_ARG);
-    if (!strcmp(key, "rows")) g_tune.rows = value;
+    if (!strcmp(key, "rows")) {
+#ifndef BTPS_TUNING_VARIANTS
+        // the default build holds the 8 / 16-rows-per-thread kernels only for single-partition plans (n <= 16)
+        if (value == 8 || value == 16) return set_err(BTPS_E_ARG);
+#endif
+        g_tune.rows = value;
+    }
     else if (!strcmp(key, "lanes")) g_tune.lanes = value;
     else if (!strcmp(key, "vec")) g_tune.vec = value;
     else if (!strcmp(key, "tiles_per_cta")) g_tune.tpc = value;
@@ -1696,6 +1716,7 @@ int btps_tune(const char *key, int value)
     else if (!strcmp(key, "one_step_fused")) g_tune.one_step_fused = value;
     else if (!strcmp(key, "host_chunk_kib")) g_tune.host_chunk_kib = value;
     else if (!strcmp(key, "hold_stores")) g_tune.hold_stores = value;
+    else if (!strcmp(key, "blk_pad")) g_tune.blk_pad = value;
     else return set_err(BTPS_E_ARG);
     return set_err(BTPS_OK);
 }

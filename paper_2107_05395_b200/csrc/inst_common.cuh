@@ -62,11 +62,23 @@ static SweepEntry pick_rows(int rows, int single, int tma, int ws, int fuse)
     // the base kinds exist for 8, 16 and 32 rows per thread (small n, tuning); the periodic and
     // Crank-Nicolson kinds only for 32 (other plans run their two-pass form)
     if constexpr (KIND == KIND_TRI || KIND == KIND_PENTA || KIND == KIND_CH) {
+#ifdef BTPS_TUNING_VARIANTS
+        // tuning builds (BTPS_TUNING_VARIANTS=1 python -m paper_2107_05395_b200.build): partitioned plans with 8 / 16 rows per thread
         switch (rows) {
             case 8: return pick_variant<T, V, 8, KIND>(single, tma, ws, fuse);
             case 16: return pick_variant<T, V, 16, KIND>(single, tma, ws, fuse);
             default: break;
         }
+#else
+        // default build: 8 / 16 rows per thread only as the single-partition plans of very short systems (n <= 16)
+        if (single && rows == 8)
+            return fuse ? (tma ? make_entry<T, V, 8, true, KIND, true, false, true>() : SweepEntry{nullptr, nullptr, 0})
+                        : (tma ? make_entry<T, V, 8, true, KIND, true, false>() : make_entry<T, V, 8, true, KIND, false, false>());
+        if (single && rows == 16)
+            return fuse ? (tma ? make_entry<T, V, 16, true, KIND, true, false, true>() : SweepEntry{nullptr, nullptr, 0})
+                        : (tma ? make_entry<T, V, 16, true, KIND, true, false>() : make_entry<T, V, 16, true, KIND, false, false>());
+        if (rows == 8 || rows == 16) return SweepEntry{nullptr, nullptr, 0};
+#endif
     }
     if (rows == 32) return pick_variant<T, V, 32, KIND>(single, tma, ws, fuse);
     SweepEntry none = {nullptr, nullptr, 0};
@@ -86,7 +98,9 @@ template <int KIND>
 static SweepEntry pick_f32(int vec, int rows, int single, int tma, int ws, int fuse)
 {
     if (vec == 1) return pick_rows<float, 1, KIND>(rows, single, tma, ws, fuse);
-    if (vec == 2) return pick_rows<float, 2, KIND>(rows, single, tma, ws, fuse);
+#ifdef BTPS_TUNING_VARIANTS
+    if (vec == 2) return pick_rows<float, 2, KIND>(rows, single, tma, ws, fuse);  // (plans use 4, or 1 for ragged batches)
+#endif
     if (vec == 4) return pick_rows<float, 4, KIND>(rows, single, tma, ws, fuse);
     SweepEntry none = {nullptr, nullptr, 0};
     return none;

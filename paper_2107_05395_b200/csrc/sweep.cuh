@@ -92,6 +92,7 @@ struct SweepArgs {
     int scan_log2_cl;      // log2 of the scan width inside one CTA (smallest power of two >= P / csz)
     unsigned tab_bytes_cl; // bytes of one CTA's scan-table block (csz blocks back to back at offT in the blob)
     unsigned offIn;        // byte offset (shared memory) of the carry inboxes: [forward | backward][NC][W]
+    int blk;               // elements between the coefficient blocks of successive partitions (ELEMS * MR + padding)
 };
 
 template <typename T, int N>
@@ -395,7 +396,7 @@ sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
     if (threadIdx.x == 0) {
         if constexpr (CL) {
             // this CTA's partitions' coefficient blocks, then its own scan-table block behind them
-            const unsigned rows_bytes = (unsigned)(PL * RecLayout<KIND>::ELEMS * MR) * (unsigned)sizeof(T);
+            const unsigned rows_bytes = (unsigned)(PL * a.blk) * (unsigned)sizeof(T);
             mbar_expect_tx(bbar, rows_bytes + a.tab_bytes_cl);
             bulk_load(smem_u32(smem), reinterpret_cast<const unsigned char *>(a.blob) + (size_t)crank * rows_bytes,
                       rows_bytes, bbar);
@@ -419,7 +420,7 @@ sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
 
     // coefficient arrays of this partition's rows (RecLayout): one base address, the arrays at
     // compile-time offsets from it
-    const T *const cb = reinterpret_cast<const T *>(smem) + (size_t)plidx * (RecLayout<KIND>::ELEMS * MR);
+    const T *const cb = reinterpret_cast<const T *>(smem) + (size_t)plidx * a.blk;
     const Pair *const RA = reinterpret_cast<const Pair *>(cb);                             // {inv, nl | nle}
     const T *const RB1 = cb + 2 * MR;                                                      // nch | nlb
     [[maybe_unused]] const Pair *const RBW = reinterpret_cast<const Pair *>(cb + 3 * MR);  // {chi, psi} | {ngam, ndel}
