@@ -562,6 +562,28 @@ def run_ours(args):
     barrier()
     launches = b.btps_launch_count() - launches0
     total_ms = e0.elapsed_time(e1)
+    # ---- the same K steps captured once in a CUDA graph and replayed: what the host's launch gaps cost (context) ------
+    graph_ms = None
+    try:
+        gs = torch.cuda.Stream()
+        gstream = gs.cuda_stream
+        with torch.cuda.stream(gs):
+            g = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(g, stream=gs):
+                for k in range(K):
+                    b.tri_solve_batched(h_tri, dev[0], gstream)
+                    b.penta_solve_batched(h_pen, dev[1], gstream)
+                    b.ch_step_batched(h_ch, dev[2], alpha, 1, gstream)
+            g.replay()
+            torch.cuda.synchronize()
+            g0, g1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            g0.record(gs)
+            g.replay()
+            g1.record(gs)
+            torch.cuda.synchronize()
+            graph_ms = g0.elapsed_time(g1) / K
+    except Exception:
+        graph_ms = None
     # ---- the same K steps again with an event between the kernels: per-kernel durations for the roofline object ----
     evs = [[torch.cuda.Event(enable_timing=True) for _ in range(4)] for _ in range(K)]
     for k in range(K):
@@ -625,7 +647,8 @@ def run_ours(args):
         "dtype": "f64", "data": "synthetic (seeded; DESIGN.md input recipe)",
         "config": {**workload_config(n, batch), "l2": "inputs larger than L2 (3 x 256 MiB buffers per step)",
                    "parallelism": f"dp{world} (independent shards, no collective)"},
-        "unknowns_per_s": value * n, "frac_of_peak_step": round(3 * alg_bytes / ms_per_step / 1e6 / peak, 4),
+        "frac_of_peak_step": round(3 * alg_bytes / ms_per_step / 1e6 / peak, 4),
+        "ms_per_step_in_cuda_graph": None if graph_ms is None else round(graph_ms, 5),
         "roofline": roofline, "kernels": kernels, "inplace_stream_gbs": round(alg_bytes / stream_ms / 1e6, 1),
         "factor_ms": round(factor_ms, 3), "build_id": b.btps_build_id(),
         "gpu_launches": int(launches), "clocks": clocks, "e2e": e2e,

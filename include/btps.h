@@ -174,10 +174,12 @@ BTPS_API int penta_cn_step_batched(penta_handle_t h, double *d_u, int64_t batch,
 /* ------------------------------------------------------------------------------------------
  * (a5) Fused semi-implicit Cahn-Hilliard step.  PAPER.md:365-392 (eq. 24, 25a, 26a-c):
  *   (I + sigma*D4) c^{n+1} = c^n + alpha * D2( (c^n)^3 - c^n ),   alpha = dt/dx^2,
- * truncated (non-periodic) stencils, ghost values zero (BASELINE.json config 5; DESIGN.md
- * C-18, C-21).  `h` is the caller's penta_factor of I + sigma*D4; d_c: DEVICE, n*batch fp64,
- * interleaved, advanced nsteps steps in place.  One kernel per step builds the RHS in
- * registers and sweeps; nothing but c^n in / c^{n+1} out crosses HBM.
+ * `h` is the caller's factor of I + sigma*D4; d_c: DEVICE, n*batch fp64, interleaved, advanced nsteps
+ * steps in place.  With a penta_factor handle both stencils are truncated (non-periodic), ghost values
+ * zero (BASELINE.json config 5; C-18, C-21); with a penta_factor_periodic handle the explicit
+ * D2 and the implicit D4 both wrap around (the paper's own setting: total mass is
+ * conserved, eq. 21-22).  The RHS is built in registers and swept in the same kernel, up to 64 steps per
+ * launch while a tile is on chip (btps_tune "fuse_steps"); nothing but c^n in / c^{n+k} out crosses HBM.
  * ---------------------------------------------------------------------------------------- */
 BTPS_API int ch_step_batched(penta_handle_t h, double *d_c, int64_t batch, double alpha, int nsteps,
                     void *stream);
@@ -260,7 +262,7 @@ BTPS_API int64_t btps_launch_count(void);
  * assumed.  bench.py uses it to check that a committed ncu capture (profiles/) is of the kernels it has just timed. */
 BTPS_API int btps_kernel_tag(int kind, const void *handle, int elem_bytes, int64_t batch, int nsteps, char *buf, int len);
 
-/* Identifier of this build of the library: a hash of the kernel sources, set by the build script. */
+/* Identifier of this build of the library: a hash of the kernel sources (csrc/) and compile flags, set by the build script. */
 BTPS_API const char *btps_build_id(void);
 
 #ifdef __cplusplus

@@ -49,10 +49,10 @@ def _run(cmd):
 
 
 def build_id() -> str:
-    """Hash of the kernel sources (csrc/*.cu, *.cuh, include/btps.h): what btps_build_id() returns."""
+    """Hash of the kernel sources (csrc/*.cu, *.cuh) and the compile flags: what btps_build_id() returns."""
     import hashlib
     h = hashlib.sha1()
-    for name in sorted(UNITS) + HEADERS:
+    for name in sorted(UNITS) + [x for x in HEADERS if not os.path.isabs(x)]:
         with open(name if os.path.isabs(name) else os.path.join(CSRC, name), "rb") as f:
             h.update(f.read())
     h.update(" ".join(NVCC_FLAGS).encode())

@@ -1289,10 +1289,18 @@ sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
         {
             S *ps = p0;
             asm volatile("" : "+l"(ps));  // keep the store addresses from being shared with the loads
+            if (nrow == MR) {  // the common case (whole partition, live columns): no per-row predicate
 #pragma unroll
-            for (int k = 0; k < MR; ++k) {
-                if (k < nrow) st_sys<T, V>(ps, v[k]);
-                ps += batch;
+                for (int k = 0; k < MR; ++k) {
+                    st_sys<T, V>(ps, v[k]);
+                    ps += batch;
+                }
+            } else {
+#pragma unroll
+                for (int k = 0; k < MR; ++k) {
+                    if (k < nrow) st_sys<T, V>(ps, v[k]);
+                    ps += batch;
+                }
             }
         }
     }
