@@ -305,15 +305,22 @@ struct CtaShape {
     static constexpr int MAX_THREADS = WIDE ? 256 : 512;
 };
 
-// Loop over the Kogge-Stone steps.  In fp32 the loop is kept rolled and in fp64 left to the
-// compiler's own choice: measured with ptxas -v, that is what keeps the 255-register wide
-// variants from spilling their tile rows.
-template <bool ROLLED, typename F>
+// Loop over the Kogge-Stone steps.  Measured with ptxas -v, per family, what keeps the 255-register variants from spilling
+// their tile rows and what is fastest in the fused time loops: fp32 keeps the loop rolled (MODE 1); the fp64 tridiagonal kinds
+// unroll it with a compile-time step index (MODE 2: 26.1 -> 25.8 us per fused step at N = 512, 65536 systems); the fp64
+// pentadiagonal kinds leave it to the compiler (MODE 0: unrolled, the fused Cahn-Hilliard step loses 2 %).
+template <int MODE, typename F>
 __device__ __forceinline__ void scan_steps(int n, F &&f)
 {
-    if constexpr (ROLLED) {
+    if constexpr (MODE == 1) {
 #pragma unroll 1
         for (int st = 0; st < n; ++st) f(st);
+    } else if constexpr (MODE == 2) {
+        // unrolled with a compile-time step index (table slots become immediate offsets, the step-4 masks fold away);
+        // steps beyond the scan width are skipped by a warp-uniform branch
+#pragma unroll
+        for (int st = 0; st < SCAN_STEPS; ++st)
+            if (st < n) f(st);
     } else {
         for (int st = 0; st < n; ++st) f(st);
     }
@@ -351,6 +358,7 @@ sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
     constexpr bool PERT = RecLayout<KIND>::PERT;
     constexpr bool WOOD = RecLayout<KIND>::WOOD;
     constexpr int NC = RecLayout<KIND>::NC;
+    [[maybe_unused]] constexpr int SCAN_MODE = sizeof(T) == 4 ? 1 : ((TRI && !PERTF) ? 2 : 0);
     using Pair = Tup<T, 2>;
     extern __shared__ __align__(128) unsigned char smem[];
 
@@ -734,8 +742,10 @@ sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
                     const int spw = 32 >> slog;  // jobs per warp pass
                     const T *tb = TAB + q;
                     if constexpr (FUSE) tb = opaque_shared(tb);
-                    const int mstr = tq;                // elements between matrix entries
-                    const int sstr = NC * NC * tq;      // elements between table slots
+                    // (warp-scan plans have at most 32 partitions, so their table rows always hold SCAN_LANES entries:
+                    //  compile-time strides turn the table addressing into immediate offsets)
+                    constexpr int mstr = SCAN_LANES;            // elements between matrix entries
+                    constexpr int sstr = NC * NC * SCAN_LANES;  // elements between table slots
                     // multipliers of step st: slots 2st (forward) / 2st+1 (backward); step 4 shares
                     // slot 8: its forward entries are nonzero only at q >= 16, its backward ones only
                     // at q < 16, and each reader masks the other half
@@ -765,7 +775,7 @@ sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
                                 fb[c][e] = ok ? xs[c * vstr + ix] : T(0);
                                 bb[c][e] = ok ? xs[(NC + c) * vstr + ix] : T(0);
                             }
-                        scan_steps<sizeof(T) == 4>(slog, [&](int st) {
+                        scan_steps<SCAN_MODE>(slog, [&](int st) {
                             T m[NC * NC];
 #pragma unroll
                             for (int i = 0; i < NC * NC; ++i) m[i] = fwm(st, i);
@@ -873,7 +883,7 @@ sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
                                 }
                             }
                         }
-                        scan_steps<sizeof(T) == 4>(slog, [&](int st) {
+                        scan_steps<SCAN_MODE>(slog, [&](int st) {
                             T m[NC * NC];
 #pragma unroll
                             for (int i = 0; i < NC * NC; ++i) m[i] = bwm(st, i);
