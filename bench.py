@@ -68,6 +68,7 @@ def parse_args():
                     help="time one cell instead of the headline step, e.g. tri,1024,19,f64 (kinds: tri, penta, ch, "
                          "tri_periodic, penta_periodic, ch_periodic); may be repeated")
     ap.add_argument("--tune", action="append", default=[], metavar="KEY=VALUE", help="btps_tune setting applied first")
+    ap.add_argument("--cell-steps", type=int, default=1, help="--cell: time steps per call (tri/penta_solve_steps, ch_step_batched)")
     ap.add_argument("--rotate", type=int, default=0, help="--cell: rotate over this many buffers (default: as many as keep the cell cold)")
     return ap.parse_args()
 
@@ -473,14 +474,15 @@ def run_cells(args):
     for cell in args.cell:
         kind, n, lb, dt = cell.split(",")
         n, batch, elem = int(n), 1 << int(lb), 8 if dt == "f64" else 4
-        h, fn, bufs = make_cell(torch, b, inputs, kind, n, batch, elem, rotate=args.rotate)
+        ks = max(1, args.cell_steps)
+        h, fn, bufs = make_cell(torch, b, inputs, kind, n, batch, elem, steps_per_call=ks, rotate=args.rotate)
         fn(bufs[0])
-        ms = time_launches(torch, fn, bufs, max(4, min(20, len(bufs))) if not args.rotate else 12, repeats=5)
+        ms = time_launches(torch, fn, bufs, (max(4, min(20, len(bufs))) if not args.rotate else 12) if ks == 1 else 2, repeats=5) / ks
         gbs = 2.0 * n * batch * elem / ms / 1e6
         kidx = KIND_INDEX[kind]
-        print(json.dumps({"cell": cell, "tune": args.tune, "ms": round(ms, 5), "hbm_gbs": round(gbs, 1),
+        print(json.dumps({"cell": cell, "tune": args.tune, "steps_per_call": ks, "ms": round(ms, 5), "hbm_gbs": round(gbs, 1),
                           "frac": round(gbs / peak, 4),
-                          "kernel": b.btps_kernel_tag(h, 12 if kind.endswith("f32s") else elem, batch, 1, kind=kidx),
+                          "kernel": b.btps_kernel_tag(h, 12 if kind.endswith("f32s") else elem, batch, ks, kind=kidx),
                           "plan": h.ch_plan(elem) if kind.startswith("ch") else h.plan(elem)}), flush=True)
         del bufs
         torch.cuda.empty_cache()
