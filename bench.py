@@ -618,6 +618,7 @@ def run_ours(args):
     traffic = ncu_traffic(tags[dom], b.btps_build_id())
     roofline = {"bound": "hbm", "kernel": f"{dom}: sweep_kernel<{tags[dom]}>", "achieved": round(alg_bytes / kern_ms[dom] / 1e6, 1),
                 "peak": peak, "unit": "GB/s", "frac": kernels[dom]["frac"], "traffic": traffic,
+                "frac_of_nominal_7700": round(alg_bytes / kern_ms[dom] / 1e6 / 7700.0, 4),
                 "algorithmic_bytes_per_launch": alg_bytes, "peak_source": peak_src,
                 "share_of_step": round(kern_ms[dom] / sum(kern_ms.values()), 4),
                 "timing": "CUDA events around each launch, mean over a second pass of the same K steps"}
