@@ -445,3 +445,70 @@ def test_f32_storage_rejects_what_it_does_not_cover(lib):
     d = torch.zeros(64, 64, dtype=torch.float32, device="cuda")
     with pytest.raises(lib.BtpsError):
         lib.tri_solve_batched_f32s(hp, d)
+
+
+# ---- long systems on thread-block clusters, at the batch bench.py times them on ---------------------------------------------
+
+@pytest.mark.parametrize("kind,n,lb,f32", [("tri", 2048, 16, False), ("penta", 2048, 16, False), ("tri", 4096, 16, False),
+                                           ("penta", 4096, 16, False), ("tri", 1536, 16, False), ("penta", 3072, 15, False),
+                                           ("tri", 4096, 16, True), ("penta", 2048, 17, True)])
+def test_long_systems_full_size_sampled(lib, kind, n, lb, f32):
+    """N > 1024: the rows of a tile are spread over a cluster of 3-8 CTAs (default plan).  Sampled systems (first / last
+    tiles, a stride through the rest) against the oracle, finiteness and the max-norm bound over every element, and the
+    same launch twice gives the same bits (the carry inboxes are reused tile after tile)."""
+    batch = 1 << lb
+    dtype = torch.float32 if f32 else torch.float64
+    elem = 4 if f32 else 8
+    d = torch.empty(n, batch, dtype=dtype, device="cuda")
+    inputs.fill_uniform_device(d, n, seed=31)
+    ids = sample_ids(batch, 1024)
+    gi = torch.from_numpy(ids).cuda()
+    ref = inputs.uniform_rhs(n, len(ids), seed=31, systems=ids.astype(np.uint64))
+    if f32:
+        ref = ref.astype(np.float32).astype(np.float64)
+    if kind == "tri":
+        lhs = inputs.tri_lhs(n, 0.5)
+        h = lib.tri_factor(*lhs)
+        solve = lib.tri_solve_batched_f32 if f32 else lib.tri_solve_batched
+        oracle.tri_solve_interleaved(oracle.tri_factor(*lhs), ref)
+    else:
+        lhs = inputs.penta_lhs(n, 0.5)
+        h = lib.penta_factor(*lhs)
+        solve = lib.penta_solve_batched_f32 if f32 else lib.penta_solve_batched
+        oracle.penta_solve_interleaved(oracle.penta_factor(*lhs), ref)
+    tag = lib.btps_kernel_tag(h, elem, batch)
+    assert tag.split(", ")[8] == "1", tag   # the cluster kernel is the default plan for these sizes
+    d2 = d.clone()
+    solve(h, d)
+    solve(h, d2)
+    assert torch.equal(d, d2)
+    got = d[:, gi].cpu().numpy().astype(np.float64)
+    assert rel_err(got, ref) <= (TOL_F32 if f32 else TOL_SINGLE), (kind, n, batch, tag)
+    assert bool(torch.isfinite(d).all())
+    assert float(d.abs().max()) <= 1.2
+
+
+def test_ragged_batch_at_full_size(lib):
+    """A batch that is neither a multiple of the tile width nor 16-byte aligned in its pitch, at bench size: the direct-load
+    scalar kernels on 2^20 + 17 systems (tail tile with 17 live columns), sampled against the oracle."""
+    n, batch = 256, (1 << 20) + 17
+    d = torch.empty(n, batch, dtype=torch.float64, device="cuda")
+    inputs.fill_uniform_device(d, n, seed=33)
+    ids = sample_ids(batch, 2048)
+    gi = torch.from_numpy(ids).cuda()
+    for kind in ("tri", "penta"):
+        inputs.fill_uniform_device(d, n, seed=33)
+        ref = inputs.uniform_rhs(n, len(ids), seed=33, systems=ids.astype(np.uint64))
+        if kind == "tri":
+            lhs = inputs.tri_lhs(n, 0.5)
+            h = lib.tri_factor(*lhs)
+            lib.tri_solve_batched(h, d)
+            oracle.tri_solve_interleaved(oracle.tri_factor(*lhs), ref)
+        else:
+            lhs = inputs.penta_lhs(n, 0.5)
+            h = lib.penta_factor(*lhs)
+            lib.penta_solve_batched(h, d)
+            oracle.penta_solve_interleaved(oracle.penta_factor(*lhs), ref)
+        assert lib.btps_kernel_tag(h, 8, batch).split(", ")[5] == "0"   # no TMA prefetch: the pitch is not 16-byte aligned
+        assert rel_err(d[:, gi].cpu().numpy(), ref) <= TOL_SINGLE, kind
+        assert bool(torch.isfinite(d).all())
