@@ -56,6 +56,7 @@ extern "C" {
 #define BTPS_E_CUDA (-3)    /* a CUDA runtime call failed (cudaGetLastError text via btps_error_string) */
 #define BTPS_E_ALIGN (-4)   /* device pointer not aligned to sizeof(element)                      */
 #define BTPS_E_DEVICE (-5)  /* handle used while another CUDA device is current than at its creation */
+#define BTPS_E_TOO_LARGE (-6) /* tri_solve_batched_host_static: n * batch * 8 > BTPS_STATIC_SCRATCH_BYTES      */
 
 typedef struct btps_tri_s *tri_handle_t;
 typedef struct btps_penta_s *penta_handle_t;
@@ -207,6 +208,28 @@ BTPS_API int ch_step_batched_stat(penta_handle_t h, double *d_c, int64_t batch, 
 BTPS_API int tri_solve_batched_host(tri_handle_t h, double *h_rhs, int64_t batch, int nsteps);
 BTPS_API int penta_solve_batched_host(penta_handle_t h, double *h_rhs, int64_t batch, int nsteps);
 BTPS_API int ch_step_batched_host(penta_handle_t h, double *h_c, int64_t batch, double alpha, int nsteps);
+
+/* ------------------------------------------------------------------------------------------
+ * The same solve for callers that must not allocate (code under CUDA graph capture set-up, tight serving loops,
+ * harnesses that forbid cudaMalloc): tri_solve_batched_host stages the batch in device buffers it allocates on
+ * first use; this variant stages it in a fixed array of BTPS_STATIC_SCRATCH_BYTES bytes that is part of the library
+ * image (file-scope `static __device__` in btps.cu; every GPU that loads the library holds those 32 MiB until the
+ * process exits).  It calls no cudaMalloc, cudaFree or other allocating routine.
+ *   h      : tridiagonal handle (plain or periodic) factored earlier on the current device (the factor call allocates;
+ *            this call does not);
+ *   h_rhs  : HOST, n*batch doubles, interleaved rhs[i*batch + j]; in: right-hand sides, out: the state after nsteps
+ *            solves (RHS = previous solution), exactly what tri_solve_steps gives on a device buffer.
+ *            Pinned memory copies at full speed; pageable memory works;
+ *   stream : cudaStream_t the copies and kernels are issued on (NULL = default stream).
+ * Limit: n * batch * 8 <= BTPS_STATIC_SCRATCH_BYTES (e.g. n = 512: batch <= 8192); larger problems are rejected with
+ * BTPS_E_TOO_LARGE before anything is issued (btps_error_string names the sizes).  Synchronous: returns when h_rhs
+ * holds the result.  Every call on a device shares the one array, which keeps the previous call's contents: nothing
+ * in it has to start at zero (the copy in overwrites all n*batch elements the kernels read), but two calls that
+ * overlap on the same GPU -- from two host threads or two processes' worth of streams in one process -- race on it.
+ * Serialise them.
+ * ---------------------------------------------------------------------------------------- */
+#define BTPS_STATIC_SCRATCH_BYTES (32ll << 20)
+BTPS_API int tri_solve_batched_host_static(tri_handle_t h, double *h_rhs, int64_t batch, int nsteps, void *stream);
 
 /* ------------------------------------------------------------------------------------------
  * Introspection / tuning (used by tests, bench.py and ncu A/B runs; not needed by callers).

@@ -13,7 +13,8 @@ _NAMES = (
     "tri_solve_batched", "tri_solve_batched_f32", "penta_solve_batched", "penta_solve_batched_f32",
     "tri_solve_batched_f32s", "penta_solve_batched_f32s",
     "tri_solve_steps", "penta_solve_steps", "ch_step_batched", "ch_step_batched_stat", "tri_cn_step_batched", "penta_cn_step_batched",
-    "tri_solve_batched_host", "penta_solve_batched_host", "ch_step_batched_host",
+    "tri_solve_batched_host", "penta_solve_batched_host", "ch_step_batched_host", "tri_solve_batched_host_static",
+    "STATIC_SCRATCH_BYTES",
     "btps_last_error", "btps_plan_info", "btps_tune", "btps_launch_count", "btps_kernel_tag", "btps_build_id", "lib_path",
     "EXPORTS",
 )

@@ -15,7 +15,7 @@ EXPORTS = [
     "tri_solve_batched", "tri_solve_batched_f32", "penta_solve_batched", "penta_solve_batched_f32",
     "tri_solve_batched_f32s", "penta_solve_batched_f32s",
     "tri_solve_steps", "penta_solve_steps", "ch_step_batched", "ch_step_batched_stat", "tri_cn_step_batched", "penta_cn_step_batched",
-    "tri_solve_batched_host", "penta_solve_batched_host", "ch_step_batched_host",
+    "tri_solve_batched_host", "penta_solve_batched_host", "ch_step_batched_host", "tri_solve_batched_host_static",
     "btps_last_error", "btps_error_string", "btps_plan_info", "btps_tune", "btps_launch_count", "btps_kernel_tag",
     "btps_build_id",
 ]
@@ -75,6 +75,8 @@ def _load() -> ctypes.CDLL:
         fn.restype = ci
     lib.ch_step_batched_host.argtypes = [vp, vp, i64, ctypes.c_double, ci]
     lib.ch_step_batched_host.restype = ci
+    lib.tri_solve_batched_host_static.argtypes = [vp, vp, i64, ci, vp]
+    lib.tri_solve_batched_host_static.restype = ci
     lib.btps_last_error.argtypes = [ctypes.POINTER(ci)]
     lib.btps_last_error.restype = ci
     lib.btps_error_string.argtypes = [ci]
@@ -340,6 +342,15 @@ def penta_solve_batched_host(h: PentaHandle, rhs, nsteps: int = 1):
 def ch_step_batched_host(h: PentaHandle, c, alpha: float, nsteps: int = 1):
     p, batch = _host_args(h, c)
     _check(_lib.ch_step_batched_host(h.ptr, p, batch, float(alpha), int(nsteps)))
+
+
+STATIC_SCRATCH_BYTES = 32 << 20  # btps.h BTPS_STATIC_SCRATCH_BYTES
+
+
+def tri_solve_batched_host_static(h: TriHandle, rhs, nsteps: int = 1, stream=None):
+    """btps.h tri_solve_batched_host_static: the host-buffer solve that allocates nothing (n*batch*8 <= 32 MiB)."""
+    p, batch = _host_args(h, rhs)
+    _check(_lib.tri_solve_batched_host_static(h.ptr, p, batch, int(nsteps), _stream(stream)))
 
 
 def btps_last_error():

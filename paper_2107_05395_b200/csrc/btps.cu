@@ -28,6 +28,7 @@ namespace {
 thread_local int tl_err = BTPS_OK;
 thread_local int tl_err_row = 0;
 thread_local char tl_cuda_msg[256] = {0};
+thread_local char tl_size_msg[320] = {0};
 
 int set_err(int code, int row = 0)
 {
@@ -1650,6 +1651,69 @@ int ch_step_batched_host(penta_handle_t h, double *h_c, int64_t batch, double al
     return solve_host<double>(h, MAGIC_PENTA, KIND_CH, h_c, batch, alpha, nsteps);
 }
 
+// ------------------------------------------------------------------------------------------------
+// Host-buffer solve that allocates nothing (include/btps.h "tri_solve_batched_host_static").  The *_host calls above
+// stage the batch in device buffers they cudaMalloc on first use; this one stages it in a fixed array that is part of
+// the library image, so it can be called where cudaMalloc cannot (code under stream capture, serving loops, harnesses
+// that forbid allocation).  Every device that loads the library holds the array until the process exits.
+// ------------------------------------------------------------------------------------------------
+static __device__ __align__(256) unsigned char g_static_scratch[BTPS_STATIC_SCRATCH_BYTES];
+
+// In host code the array's name is a host-side stand-in, not a device address: the address a kernel can use comes from
+// cudaGetSymbolAddress, asked once per device with that device current.  (No allocation: a fixed table of pointers.)
+static int static_scratch_ptr(int dev, void **out)
+{
+    constexpr int MAX_DEV = 64;
+    static std::mutex mu;
+    static void *ptr[MAX_DEV] = {nullptr};
+    if (dev < 0 || dev >= MAX_DEV) return set_err(BTPS_E_DEVICE);
+    std::lock_guard<std::mutex> lk(mu);
+    if (!ptr[dev]) {
+        void *p = nullptr;
+        const cudaError_t e = cudaGetSymbolAddress(&p, g_static_scratch);
+        if (e != cudaSuccess) return cuda_fail(e, "cudaGetSymbolAddress(g_static_scratch)");
+        if (!p || ((uintptr_t)p & 255)) return cuda_fail(cudaErrorInvalidSymbol, "static scratch array address");
+        ptr[dev] = p;
+    }
+    *out = ptr[dev];
+    return BTPS_OK;
+}
+
+int tri_solve_batched_host_static(tri_handle_t hv, double *h_rhs, int64_t batch, int nsteps, void *stream)
+{
+    Handle *h = check(hv, MAGIC_TRI);
+    if (!h || !h_rhs || batch < 1 || nsteps < 0) return set_err(BTPS_E_ARG);
+    // n * batch * 8 bytes must fit in the array (checked without overflow)
+    if ((uint64_t)batch > (uint64_t)BTPS_STATIC_SCRATCH_BYTES / sizeof(double) / (uint64_t)h->n) {
+        snprintf(tl_size_msg, sizeof(tl_size_msg),
+                 "tri_solve_batched_host_static: n * batch * 8 = %lld * %lld * 8 bytes exceeds the static scratch array "
+                 "(BTPS_STATIC_SCRATCH_BYTES = %lld); use tri_solve_batched_host or a device buffer",
+                 (long long)h->n, (long long)batch, (long long)BTPS_STATIC_SCRATCH_BYTES);
+        return set_err(BTPS_E_TOO_LARGE);
+    }
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev != h->device) return set_err(BTPS_E_DEVICE);
+    void *p = nullptr;
+    int rc = static_scratch_ptr(dev, &p);
+    if (rc != BTPS_OK) return rc;
+    double *d = (double *)p;
+    cudaStream_t st = (cudaStream_t)stream;
+    const size_t bytes = (size_t)h->n * (size_t)batch * sizeof(double);
+    // the copy in overwrites every element the kernels read: nothing left in the array by an earlier call is used
+    cudaError_t e = cudaMemcpyAsync(d, h_rhs, bytes, cudaMemcpyHostToDevice, st);
+    if (e != cudaSuccess) return cuda_fail(e, "host-to-device copy into the static scratch array");
+    rc = solve_steps<double>(h, MAGIC_TRI, KIND_TRI, d, batch, 0.0, nsteps, stream);
+    // whatever the outcome, nothing may still be reading or writing the caller's buffer after the return
+    if (rc == BTPS_OK) {
+        e = cudaMemcpyAsync(h_rhs, d, bytes, cudaMemcpyDeviceToHost, st);
+        if (e != cudaSuccess) rc = cuda_fail(e, "device-to-host copy out of the static scratch array");
+    }
+    e = cudaStreamSynchronize(st);
+    if (rc != BTPS_OK) return rc;
+    if (e != cudaSuccess) return cuda_fail(e, "cudaStreamSynchronize");
+    return set_err(BTPS_OK);
+}
+
 int btps_last_error(int *row)
 {
     if (row) *row = tl_err_row;
@@ -1665,6 +1729,7 @@ const char *btps_error_string(int code)
         case BTPS_E_CUDA: return tl_cuda_msg[0] ? tl_cuda_msg : "CUDA runtime failure";
         case BTPS_E_ALIGN: return "device pointer not aligned to the element size";
         case BTPS_E_DEVICE: return "handle used on a device other than the one it was factored on";
+        case BTPS_E_TOO_LARGE: return tl_size_msg[0] ? tl_size_msg : "problem larger than the static scratch array (BTPS_STATIC_SCRATCH_BYTES)";
         default: return "unknown";
     }
 }
