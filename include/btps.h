@@ -269,8 +269,12 @@ BTPS_API int btps_plan_info(int kind, const void *handle, int elem_bytes, int *o
  * and tile sizes where that was measured to win -- tridiagonal kinds and the plain fp64 pentadiagonal solve on full tiles).
  * "blk_pad" (bytes of padding behind every partition's coefficient block in shared memory, a multiple of 16: moves the
  * coefficient reads of the partitions that share a warp onto different banks).
+ * "dedupe" (0: every partition keeps its own coefficient block in shared memory; 1: partitions whose blocks are bitwise
+ * equal -- all interior partitions of a constant-coefficient LHS -- share one, also for the single-step plain pentadiagonal
+ * solve at 32 partitions, which by default keeps an unshared image of its own because it was measured to lose there;
+ * default: share.  Results are bitwise identical either way).
  * value < 0 restores the default.  "pdl", "fuse_steps", "grid", "cluster", "reverse", "one_step_fused",
- * "host_chunk_kib" and "hold_stores" are read at launch time, the others when a handle is built. */
+ * "host_chunk_kib" and "hold_stores" are read at launch time, the others ("dedupe" too) when a handle is built. */
 BTPS_API int btps_tune(const char *key, int value);
 
 /* Number of kernel launches issued by this library in this process (bench.py's gpu_launches). */

@@ -56,7 +56,7 @@ std::atomic<long long> g_launches{0};
 // ------------------------------------------------------------------------------------------------
 struct Tune {
     int rows = -1, lanes = -1, vec = -1, tpc = -1, force_two_pass = -1, reverse = -1, prefetch = -1, pdl = -1,
-        warp_scan = -1, grid = -1, fuse = -1, cluster = -1, blk_pad = -1, cyclic_scan = -1, one_step_fused = -1, host_chunk_kib = -1, hold_stores = -1;
+        warp_scan = -1, grid = -1, fuse = -1, cluster = -1, blk_pad = -1, cyclic_scan = -1, one_step_fused = -1, host_chunk_kib = -1, hold_stores = -1, dedupe = -1;
 };
 Tune g_tune;
 
@@ -107,6 +107,10 @@ struct DtypePlan {
     unsigned tab_bytes_cl = 0;  // bytes of one such block
     unsigned blob_total = 0;    // blob bytes on the device (blob_bytes = what the single-CTA kernels stage)
     int blk_pad = 0;            // bytes of padding behind every partition's coefficient block (blk_stride)
+    // coefficient blocks shared between partitions (dedupe_blocks): the blob holds nuniq distinct blocks, partition p
+    // reads block pmap[p].  nuniq == P: nothing shared, pmap is the identity.
+    int nuniq = 0;
+    unsigned char pmap[MAX_PARTS] = {0};
     Shape cshape;
     KernelSlot ck;
 };
@@ -124,6 +128,10 @@ struct Handle {
     int n;
     int device;
     DtypePlan plan[2];  // 0: fp64, 1: fp32
+    // plain pentadiagonal handles of 32 partitions (N = 993 ... 1024): a second plan whose blob keeps every partition's
+    // own coefficient block, used by the single-step plain solve only (make_penta_handle says why)
+    bool has_alt = false;
+    DtypePlan alt[2];
     std::mutex mu;      // guards lazy occupancy resolution
 };
 
@@ -431,6 +439,58 @@ void put_scan_tables(std::vector<unsigned char> &blob, DtypePlan &pl, int nc, co
     }
 }
 
+// Partitions whose coefficient blocks are bitwise equal share one block.  The factor coefficients of a constant-
+// coefficient LHS (every LHS of the paper: PAPER.md:126, 172, 306, 380) converge to their limit bitwise within 13-28
+// rows, and the per-partition responses (chi, psi) are functions of the block's own rows only, so every interior
+// partition of such a matrix has the same block: N = 1024 keeps 2-3 blocks of 32 (penta fp64: 74 KB -> 7 KB of shared
+// memory).  A general LHS has P distinct blocks and nothing changes.  Called at the very end of build_blob_*: the blob
+// becomes [distinct blocks][everything behind the row records, moved down]; offT / blob_bytes / offTc / blob_total follow.
+// Cluster plans (a CTA stages only its own partitions' blocks) share blocks only when all the distinct ones fit the
+// space of one CTA's share (nuniq <= PLc); otherwise the blob stays whole and each CTA stages its own PLc blocks.
+void dedupe_blocks(DtypePlan &pl, std::vector<unsigned char> &blob, int RT, bool allow)
+{
+    const int P = pl.P;
+    const size_t bb = (size_t)blk_stride(pl, RT) * pl.elem;
+    pl.nuniq = P;
+    for (int p = 0; p < P && p < MAX_PARTS; ++p) pl.pmap[p] = (unsigned char)p;
+    if (!allow || P < 2 || P > MAX_PARTS) return;
+    std::vector<int> first;  // partition index of each distinct block, in order of appearance
+    std::vector<unsigned char> map(P);
+    for (int p = 0; p < P; ++p) {
+        int u = -1;
+        for (size_t k = 0; k < first.size() && u < 0; ++k)
+            if (!memcmp(&blob[(size_t)first[k] * bb], &blob[(size_t)p * bb], bb)) u = (int)k;
+        if (u < 0) {
+            u = (int)first.size();
+            first.push_back(p);
+        }
+        map[p] = (unsigned char)u;
+    }
+    const int U = (int)first.size();
+    if (U == P || (pl.csz && U > pl.PLc)) return;
+    std::vector<unsigned char> out;
+    out.reserve(blob.size());
+    for (int u = 0; u < U; ++u) out.insert(out.end(), blob.begin() + (size_t)first[u] * bb, blob.begin() + (size_t)(first[u] + 1) * bb);
+    const unsigned new_offT = (unsigned)align16((size_t)U * bb);
+    out.resize(new_offT, 0);
+    out.insert(out.end(), blob.begin() + pl.offT, blob.end());
+    const unsigned delta = pl.offT - new_offT;
+    pl.offT = new_offT;
+    pl.blob_bytes -= delta;
+    pl.blob_total -= delta;
+    if (pl.csz) pl.offTc -= delta;
+    blob.swap(out);
+    pl.nuniq = U;
+    for (int p = 0; p < P; ++p) pl.pmap[p] = map[p];
+}
+
+// mode: 1 / 0 = share blocks or not, -1 = as btps_tune("dedupe") says (default: share)
+bool dedupe_wanted(int mode)
+{
+    if (mode >= 0) return mode > 0;
+    return g_tune.dedupe != 0;
+}
+
 size_t scan_table_bytes(const DtypePlan &pl, int nc, size_t elem)
 {
     int slots = pl.ws ? 2 * SCAN_STEPS : 2;  // ws: 8 step slots + merged step 4 + chi
@@ -442,7 +502,7 @@ template <typename T>
 void build_blob_tri(int n, DtypePlan &pl, const std::vector<double> &inv, const std::vector<double> &nl,
                     const std::vector<double> &nch, std::vector<unsigned char> &blob,
                     const std::vector<double> *z = nullptr, const std::vector<double> *zfwd = nullptr, double u0 = 0.0,
-                    double uN = 0.0)
+                    double uN = 0.0, int dedupe_mode = -1)
 {
     const int MR = pl.rows, P = pl.P, Np = P * MR;
     // coefficient values per row: the periodic form carries z = A'^{-1} u as a sixth array
@@ -509,13 +569,14 @@ void build_blob_tri(int n, DtypePlan &pl, const std::vector<double> &inv, const 
                 put<T>(blob, ((size_t)p * blk_stride(pl, RT) + (size_t)5 * MR + k) * sizeof(T), loc[k]);
         }
     }
+    dedupe_blocks(pl, blob, RT, dedupe_wanted(dedupe_mode));
 }
 
 template <typename T>
 void build_blob_penta(int n, DtypePlan &pl, const std::vector<double> &inv, const std::vector<double> &nle,
                       const std::vector<double> &nlb, const std::vector<double> &ngam,
                       const std::vector<double> &ndel, std::vector<unsigned char> &blob,
-                      const std::vector<double> *Z = nullptr)
+                      const std::vector<double> *Z = nullptr, int dedupe_mode = -1)
 {
     const int MR = pl.rows, P = pl.P, Np = P * MR;
     // coefficient values per row: the periodic form carries the rows of Z = A'^{-1} U (n x 4, row-major), or, with the
@@ -626,6 +687,7 @@ void build_blob_penta(int n, DtypePlan &pl, const std::vector<double> &inv, cons
             for (int k = 0; k < MR; ++k) putv(9, r0 + k, m & 1, loc[k]);
         }
     }
+    dedupe_blocks(pl, blob, RT, dedupe_wanted(dedupe_mode));
 }
 
 template <typename T>
@@ -650,6 +712,7 @@ void free_handle(Handle *h)
     for (int t = 0; t < 2; ++t) {
         if (h->plan[t].d_blob) cudaFree(h->plan[t].d_blob);
         if (h->plan[t].d_soa) cudaFree(h->plan[t].d_soa);
+        if (h->alt[t].d_blob) cudaFree(h->alt[t].d_blob);
     }
     h->magic = 0;
     delete h;
@@ -767,7 +830,7 @@ void fill_cluster_slot(Handle *h, DtypePlan &pl)
     sl.xvals = 2 * NC;
     sl.xper = (int)(sl.xvals * PL * W);
     sl.xstride = sl.xper;
-    const size_t rows_bytes = (size_t)PL * blk_stride(pl, elems) * pl.elem;
+    const size_t rows_bytes = (size_t)(pl.nuniq < PL ? pl.nuniq : PL) * blk_stride(pl, elems) * pl.elem;  // shared blocks, or its own PL
     sl.offTl = (unsigned)align16(rows_bytes);
     sl.offX = (unsigned)align16(sl.offTl + pl.tab_bytes_cl);
     sl.offIn = (unsigned)align16(sl.offX + (size_t)sl.xstride * pl.elem);
@@ -798,10 +861,10 @@ void fit_plan(DtypePlan &pl, int handle_kind)
 
 void fill_slots(Handle *h)
 {
-    for (int t = 0; t < 2; ++t) {
-        DtypePlan &pl = h->plan[t];
+    for (int t = 0; t < (h->has_alt ? 4 : 2); ++t) {
+        DtypePlan &pl = t < 2 ? h->plan[t] : h->alt[t - 2];
         fill_cluster_slot(h, pl);
-        if (t == 0 && !h->periodic && !pl.two_pass && (pl.P == 1 || (pl.ws && pl.rows == 32))) {
+        if (pl.elem == 8 && !h->periodic && !pl.two_pass && (pl.P == 1 || (pl.ws && pl.rows == 32))) {
             // fp32 storage, fp64 arithmetic: the plain solve kernels of the fp64 plan with a ring of floats
             const Shape &sh = pl.shape[0];
             for (int s = 0; s < 2; ++s)
@@ -982,7 +1045,9 @@ int launch_one(Handle *h, int kind, S *d_rhs, long long batch, double alpha_x, i
                cudaStream_t st, double *stat = nullptr, const double *ex = nullptr, const char **tag_out = nullptr)
 {
     constexpr bool MIXED = !std::is_same<T, S>::value;  // fp32 in HBM, fp64 arithmetic: plain solves of the fp64 plan
-    DtypePlan &pl = h->plan[sizeof(T) == 8 ? 0 : 1];
+    // (the single-step plain solve of a 32-partition pentadiagonal handle runs on its own unshared blob: make_penta_handle)
+    const bool own_blocks = h->has_alt && kind == KIND_PENTA && ksteps == 1 && !stat;
+    DtypePlan &pl = own_blocks ? h->alt[sizeof(T) == 8 ? 0 : 1] : h->plan[sizeof(T) == 8 ? 0 : 1];
     // a handle's tables live on the device that was current when it was factored
     int dev = -1;
     if (cudaGetDevice(&dev) != cudaSuccess || dev != h->device) return set_err(BTPS_E_DEVICE);
@@ -1110,6 +1175,9 @@ int launch_one(Handle *h, int kind, S *d_rhs, long long batch, double alpha_x, i
     }
     a.blk = blk_stride(pl, h->kind == KIND_TRI ? (h->periodic ? 6 : 5) : (h->periodic ? (pl.wfast ? 11 : 13) : 9));  // = RecLayout<KIND>::ELEMS of the kernel
     a.csz = use_cl ? pl.csz : 1;
+    a.nuniq = pl.nuniq;
+    a.cl_own = (use_cl && pl.nuniq > pl.PLc) ? 1 : 0;  // (then nothing is shared: every CTA stages its own partitions' blocks)
+    memcpy(a.pmap, pl.pmap, sizeof(a.pmap));
     a.scan_log2_cl = pl.scan_log2_cl;
     a.tab_bytes_cl = pl.tab_bytes_cl;
     a.offIn = sl.offIn;
@@ -1476,7 +1544,29 @@ static penta_handle_t make_penta_handle(int n, const std::vector<double> &inv, c
             free_handle(h);
             return nullptr;
         }
+        // Measured on B200 (profiles/r02b_shared_blocks.md): with shared coefficient blocks everything gains or is
+        // indifferent -- N = 1024: periodic solves and CH steps fit their TMA ring (0.51-0.56 -> 0.82-0.91 of the HBM
+        // peak), the CH step fuses its time loop (0.20 -> 0.115 ms per step at 2^16), plain steps in a fused loop gain
+        // 19 % -- except the single-step plain solve at 32 partitions, fp64 and fp32, which LOSES 5-15 % when its sweeps
+        // get shorter (0.87 -> 0.74 at 2^19; also with the blob whole and only the addresses shared, so it is the phasing
+        // of its stores against the next tile's load, not shared-memory size).  That one call keeps a blob of its own.
+        if (!Z && pl.P == 32 && !pl.two_pass && pl.nuniq < pl.P && g_tune.dedupe < 0) {
+            DtypePlan &al = h->alt[t];
+            choose_plan(n, t == 0 ? 8 : 4, h->kind, al);
+            al.wfast = 0;
+            std::vector<unsigned char> blob2;
+            if (t == 0) build_blob_penta<double>(n, al, inv, nle, nlb, ngam, ndel, blob2, nullptr, 0);
+            else build_blob_penta<float>(n, al, inv, nle, nlb, ngam, ndel, blob2, nullptr, 0);
+            al.soa_bytes = 0;
+            fit_plan(al, KIND_PENTA);
+            if (upload(blob2, &al.d_blob) != BTPS_OK) {
+                free_handle(h);
+                return nullptr;
+            }
+            h->has_alt = true;
+        }
     }
+    if (h->has_alt && (!h->alt[0].d_blob || !h->alt[1].d_blob || h->alt[0].two_pass || h->alt[1].two_pass)) h->has_alt = false;
     fill_slots(h);
     set_err(BTPS_OK);
     return (penta_handle_t)h;
@@ -1781,6 +1871,7 @@ int btps_tune(const char *key, int value)
     else if (!strcmp(key, "one_step_fused")) g_tune.one_step_fused = value;
     else if (!strcmp(key, "host_chunk_kib")) g_tune.host_chunk_kib = value;
     else if (!strcmp(key, "hold_stores")) g_tune.hold_stores = value;
+    else if (!strcmp(key, "dedupe")) g_tune.dedupe = value;
     else if (!strcmp(key, "blk_pad")) g_tune.blk_pad = value;
     else return set_err(BTPS_E_ARG);
     return set_err(BTPS_OK);

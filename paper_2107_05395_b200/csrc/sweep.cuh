@@ -48,6 +48,7 @@ enum Kind {
 
 constexpr int SCAN_STEPS = 5;   // Kogge-Stone steps held in the tables (scan width <= 32)
 constexpr int SCAN_LANES = 32;
+constexpr int MAX_PARTS = 128;  // partitions of the largest on-chip plan (8 CTAs x 16)
 
 struct SweepArgs {
     void *rhs;             // device, n*batch elements, interleaved
@@ -93,6 +94,10 @@ struct SweepArgs {
     unsigned tab_bytes_cl; // bytes of one CTA's scan-table block (csz blocks back to back at offT in the blob)
     unsigned offIn;        // byte offset (shared memory) of the carry inboxes: [forward | backward][NC][W]
     int blk;               // elements between the coefficient blocks of successive partitions (ELEMS * MR + padding)
+    // coefficient blocks shared between partitions: shared memory holds nuniq blocks, partition p reads block pmap[p]
+    int nuniq;
+    int cl_own;            // CL: 1 = nothing shared, this CTA stages its own P / csz blocks and indexes them locally
+    unsigned char pmap[MAX_PARTS];
 };
 
 template <typename T, int N>
@@ -404,9 +409,9 @@ sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
     if (threadIdx.x == 0) {
         if constexpr (CL) {
             // this CTA's partitions' coefficient blocks, then its own scan-table block behind them
-            const unsigned rows_bytes = (unsigned)(PL * a.blk) * (unsigned)sizeof(T);
+            const unsigned rows_bytes = (unsigned)((a.cl_own ? PL : a.nuniq) * a.blk) * (unsigned)sizeof(T);
             mbar_expect_tx(bbar, rows_bytes + a.tab_bytes_cl);
-            bulk_load(smem_u32(smem), reinterpret_cast<const unsigned char *>(a.blob) + (size_t)crank * rows_bytes,
+            bulk_load(smem_u32(smem), reinterpret_cast<const unsigned char *>(a.blob) + (a.cl_own ? (size_t)crank * rows_bytes : 0),
                       rows_bytes, bbar);
             bulk_load(smem_u32(smem + a.offTl),
                       reinterpret_cast<const unsigned char *>(a.blob) + a.offT + (size_t)crank * a.tab_bytes_cl,
@@ -428,7 +433,7 @@ sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
 
     // coefficient arrays of this partition's rows (RecLayout): one base address, the arrays at
     // compile-time offsets from it
-    const T *const cb = reinterpret_cast<const T *>(smem) + (size_t)plidx * a.blk;
+    const T *const cb = reinterpret_cast<const T *>(smem) + (size_t)((CL && a.cl_own) ? plidx : (int)a.pmap[part]) * a.blk;
     const Pair *const RA = reinterpret_cast<const Pair *>(cb);                             // {inv, nl | nle}
     const T *const RB1 = cb + 2 * MR;                                                      // nch | nlb
     [[maybe_unused]] const Pair *const RBW = reinterpret_cast<const Pair *>(cb + 3 * MR);  // {chi, psi} | {ngam, ndel}

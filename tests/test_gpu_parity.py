@@ -1077,3 +1077,49 @@ def test_held_stores_are_bitwise_equal(lib):
     ref = rhs.copy()
     oracle.tri_solve_interleaved(oracle.tri_factor(*rand_tri(n, 3)), ref)
     assert rel_err(got[1][0].cpu().numpy(), ref) <= TOL_SINGLE
+
+
+@pytest.mark.parametrize("n", [64, 500, 512, 768, 1024, 2048, 3000])
+def test_shared_coefficient_blocks_are_bitwise_equal(lib, n):
+    """btps_tune('dedupe', 1): partitions whose coefficient blocks are bitwise equal read one shared block (constant-
+    coefficient LHS: all interior partitions).  A storage change only: same bits as with every partition's own block,
+    for every kernel family, on single-CTA and cluster plans; and a general LHS (no equal blocks) is left alone."""
+    batch = 1024 + 32
+    rhs = inputs.uniform_rhs(n, batch, seed=101)
+    _, al = inputs.ch_params(n)
+    x5 = np.array([0.02, -0.08, 0.88, -0.08, 0.02])
+    got, info = {}, {}
+    for mode in (0, 1):
+        try:
+            lib.btps_tune("dedupe", mode)
+            ht, hp, hc = lib.tri_factor(*inputs.tri_lhs(n, 0.5)), lib.penta_factor(*inputs.penta_lhs(n, 0.5)), lib.penta_factor(*inputs.ch_lhs(n))
+            htp = lib.tri_factor_periodic(*inputs.tri_lhs(n, 0.5))
+            hpp, hcp = lib.penta_factor_periodic(*inputs.penta_lhs(n, 0.5)), lib.penta_factor_periodic(*inputs.ch_lhs(n))
+            hg = lib.penta_factor(*rand_penta(n, 4))
+            d = [dev(rhs), dev(rhs), dev(0.1 * rhs), dev(rhs), dev(rhs), dev(0.1 * rhs), dev(rhs.astype(np.float32)),
+                 dev(rhs.astype(np.float32)), dev(rhs), dev(rhs), dev(rhs), dev(rhs)]
+            lib.tri_solve_batched(ht, d[0])
+            lib.penta_solve_batched(hp, d[1])
+            lib.ch_step_batched(hc, d[2], al, 3)
+            lib.tri_solve_batched(htp, d[3])
+            lib.penta_solve_batched(hpp, d[4])
+            lib.ch_step_batched(hcp, d[5], al, 3)
+            lib.tri_solve_batched_f32(ht, d[6])
+            lib.penta_solve_batched_f32(hp, d[7])
+            lib.tri_cn_step_batched(ht, d[8], 0.3, 0.4, 0.3, 2)
+            lib.penta_cn_step_batched(hpp, d[9], x5, 2)
+            lib.penta_solve_steps(hp, d[10], 5)
+            lib.penta_solve_batched(hg, d[11])
+            torch.cuda.synchronize()
+            info[mode] = (lib.btps_plan_info(hp, 8), lib.btps_plan_info(hg, 8))
+        finally:
+            lib.btps_tune("dedupe", -1)
+        got[mode] = d
+    for k, (a, c) in enumerate(zip(got[0], got[1])):
+        assert torch.equal(a, c), k
+    ref = rhs.copy()
+    oracle.penta_solve_interleaved(oracle.penta_factor(*inputs.penta_lhs(n, 0.5)), ref)
+    assert rel_err(got[1][1].cpu().numpy(), ref) <= TOL_SINGLE
+    if info[0][0]["rows_per_thread"] and info[0][0]["partitions"] >= 4:   # on-chip plan, four or more partitions: the image shrank
+        assert info[1][0]["table_bytes"] < info[0][0]["table_bytes"]
+    assert info[1][1]["table_bytes"] == info[0][1]["table_bytes"]         # random LHS: no two blocks are equal
