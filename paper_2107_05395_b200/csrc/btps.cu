@@ -1170,7 +1170,11 @@ int launch_one(Handle *h, int kind, S *d_rhs, long long batch, double alpha_x, i
         const size_t tile_bytes = (size_t)pl.P * pl.rows * sh.lanes * sl.vec * sizeof(S);
         // (and at least 8 tiles per CTA: with 3-4 it loses ~10 %)
         const bool full_tile = (sh.tpc == 1) && !use_cl && tile_bytes >= (112u << 10) && a.num_tiles >= 8ll * sl.max_grid;
-        const bool penta_ok = (kind == KIND_PENTA) && sizeof(T) == 8 && !h->periodic && sh.lanes == 16;
+        // (8-lane tiles, N = 993 ... 1024: held stores cost up to 9 % while the rows of a tile share pages, and win 4-5 % once
+        // every row of the batch is 32 MiB or more -- 2^22 systems in fp64, 2^23 in fp32 -- where they keep 0.69 of the peak
+        // and free-running stores fall to 0.66: profiles/r02b_shared_blocks.md)
+        const bool penta_big = (kind == KIND_PENTA) && !h->periodic && sh.lanes == 8 && (size_t)batch * sizeof(S) >= ((size_t)32 << 20);
+        const bool penta_ok = ((kind == KIND_PENTA) && sizeof(T) == 8 && !h->periodic && sh.lanes == 16) || penta_big;
         a.hold_stores = g_tune.hold_stores >= 0 ? (g_tune.hold_stores > 0) : ((full_tile && (tri_family || penta_ok)) ? 1 : 0);
     }
     a.blk = blk_stride(pl, h->kind == KIND_TRI ? (h->periodic ? 6 : 5) : (h->periodic ? (pl.wfast ? 11 : 13) : 9));  // = RecLayout<KIND>::ELEMS of the kernel

@@ -1123,3 +1123,49 @@ def test_shared_coefficient_blocks_are_bitwise_equal(lib, n):
     if info[0][0]["rows_per_thread"] and info[0][0]["partitions"] >= 4:   # on-chip plan, four or more partitions: the image shrank
         assert info[1][0]["table_bytes"] < info[0][0]["table_bytes"]
     assert info[1][1]["table_bytes"] == info[0][1]["table_bytes"]         # random LHS: no two blocks are equal
+
+
+def two_regime_lhs(n, seed, penta):
+    """Strongly dominant LHS whose coefficients repeat with a period of 32 rows (the rows of one partition), with one
+    random pattern on the first half of the rows and another on the second half.  The factor recurrences contract by
+    more than 10 per row, so they reach their 32-periodic limit bitwise within a partition or two: the partitions of each
+    half then have equal coefficient blocks -- partial sharing, neither the constant-coefficient case nor the general one."""
+    rng = np.random.default_rng(seed)
+    pats = rng.uniform(-1, 1, (2, 4, 32))
+    half = (n // 64) * 32
+    def rows(k):
+        return np.concatenate([np.resize(pats[0, k], half), np.resize(pats[1, k], n - half)])
+    e, a, c, f = (rows(k) for k in range(4))
+    d = 12.0 + np.concatenate([np.zeros(half), np.ones(n - half)])
+    if penta:
+        return e, a, d, c, f
+    return a, d, c
+
+
+@pytest.mark.parametrize("n", [512, 1024, 2048])
+def test_partially_shared_coefficient_blocks_against_oracle(lib, n):
+    batch = 512 + 32
+    rhs = inputs.uniform_rhs(n, batch, seed=103)
+    lt, lp = two_regime_lhs(n, 1, False), two_regime_lhs(n, 2, True)
+    ht, hp = lib.tri_factor(*lt), lib.penta_factor(*lp)
+    full = lib.btps_plan_info(lib.penta_factor(*rand_penta(n, 4)), 8)["table_bytes"]
+    const = lib.btps_plan_info(lib.penta_factor(*inputs.penta_lhs(n, 0.5)), 8)["table_bytes"]
+    part = lib.btps_plan_info(hp, 8)["table_bytes"]
+    assert const < part < full, (const, part, full)   # some blocks shared, more distinct ones than a constant LHS has
+    for h, lhs, solve, steps, fac, osolve in ((ht, lt, lib.tri_solve_batched, lib.tri_solve_steps, oracle.tri_factor, oracle.tri_solve_interleaved),
+                                              (hp, lp, lib.penta_solve_batched, lib.penta_solve_steps, oracle.penta_factor, oracle.penta_solve_interleaved)):
+        d = dev(rhs)
+        solve(h, d)
+        ref = rhs.copy()
+        osolve(fac(*lhs), ref)
+        assert rel_err(d.cpu().numpy(), ref) <= TOL_SINGLE
+        d = dev(rhs)
+        steps(h, d, 3)
+        ref = rhs.copy()
+        osolve(fac(*lhs), ref, nsteps=3)
+        assert rel_err(d.cpu().numpy(), ref) <= TOL_STEPS
+        d32 = dev(rhs.astype(np.float32))
+        (lib.tri_solve_batched_f32 if h is ht else lib.penta_solve_batched_f32)(h, d32)
+        ref = rhs.astype(np.float32).astype(np.float64)
+        osolve(fac(*lhs), ref)
+        assert rel_err(d32.cpu().numpy().astype(np.float64), ref) <= TOL_F32
