@@ -355,15 +355,31 @@ void put_scan_slots(std::vector<unsigned char> &blob, size_t base, int q0, int P
     put_slot(1, Psi);
     if (!ws) return;
     if (chain) {
-        // cluster chain (sweep.cuh, CL): how a carry that enters this block of partitions from the neighbouring CTA reaches
-        // partition q -- slot 10: Phi_q Phi_{q-1} ... Phi_first (forward), slot 11: Psi_q Psi_{q+1} ... Psi_last (backward)
-        std::vector<Mat> Fi(P), Bi(P);
-        Fi[0] = Phi[0];
-        for (int q = 1; q < P; ++q) Fi[q] = matmul(Phi[q], Fi[q - 1], nc);
-        Bi[P - 1] = Psi[P - 1];
-        for (int q = P - 2; q >= 0; --q) Bi[q] = matmul(Psi[q], Bi[q + 1], nc);
-        put_slot(10, Fi);
-        put_slot(11, Bi);
+        // cluster kernels (sweep.cuh, CL): how the carries that enter this CTA's block of partitions -- Gin from the CTA below
+        // into its first partition, Xin from the CTA above into its last -- reach partition q.  With G0 / X0 the carries of the
+        // block solved on its own (Gin = Xin = 0):
+        //   carry into q from below  G_q = G0_q + Pin_q Gin,            Pin_q = Phi_{q-1} ... Phi_first      (slot 10; I at q = 0)
+        //   carry into q from above  X_q = X0_q + Th_{q+1} Gin + Sf_{q+1} Xin   (slots 13 and 11; 0 and I at the last partition)
+        // where Sf_q = Psi_q ... Psi_last and Th_q = Chi0_q Pin_q + Psi_q Th_{q+1} is what Gin adds to the backward sweep's
+        // inclusive value at q through u = x^_first + Chi0 G.
+        const Mat zero;
+        Mat ident;
+        ident.m[0] = 1.0;
+        if (nc == 2) ident.m[3] = 1.0;
+        std::vector<Mat> Pin(P), SfIn(P), ThIn(P);
+        Pin[0] = ident;
+        for (int q = 1; q < P; ++q) Pin[q] = matmul(Phi[q - 1], Pin[q - 1], nc);
+        Mat sf = ident, th = zero;  // Sf_{q+1}, Th_{q+1}
+        for (int q = P - 1; q >= 0; --q) {
+            SfIn[q] = sf;
+            ThIn[q] = th;
+            const Mat cp = matmul(Chi0[q], Pin[q], nc), pt = matmul(Psi[q], th, nc);
+            for (int m = 0; m < ne; ++m) th.m[m] = cp.m[m] + pt.m[m];
+            sf = matmul(Psi[q], sf, nc);
+        }
+        put_slot(10, Pin);
+        put_slot(11, SfIn);
+        put_slot(13, ThIn);
     }
     std::vector<Mat> A = Phi, B = Psi;
     const Mat zero;
@@ -403,37 +419,69 @@ void put_scan_tables(std::vector<unsigned char> &blob, DtypePlan &pl, int nc, co
     if (pl.csz) {
         // one table block per CTA of the cluster chain, behind everything the single-CTA kernels stage
         pl.offTc = pl.blob_bytes;
-        pl.tab_bytes_cl = (unsigned)align16((size_t)13 * nc * nc * SCAN_LANES * sizeof(T));
+        pl.tab_bytes_cl = (unsigned)align16((size_t)14 * nc * nc * SCAN_LANES * sizeof(T));
         pl.blob_total = pl.offTc + (unsigned)pl.csz * pl.tab_bytes_cl;
         blob.resize(pl.blob_total, 0);
         const int k = pl.csz, PL = pl.PLc, ne = nc * nc;
         for (int r = 0; r < k; ++r)
             put_scan_slots<T>(blob, pl.offTc + (size_t)r * pl.tab_bytes_cl, r * PL, PL, SCAN_LANES, nc, true, true, Phi, Psi, Chi0);
-        // slot 12 of CTA r's block: how the other CTAs' contributions reach it.  Entry s < r: C_{r,s} = PhiT_{r-1} ... PhiT_{s+1}
-        // (forward; PhiT_c = product of the Phi of CTA c's partitions, identity for s = r - 1); entry 8 + s, s > r:
-        // D_{r,s} = PsiT_{r+1} ... PsiT_{s-1} (backward, identity for s = r + 1).
-        std::vector<Mat> PhiT(k), PsiT(k);
+        // slot 12 of CTA r's block: how the other CTAs' local carries reach it.  With PhiT_c = Phi_last ... Phi_first,
+        // PsiT_c = Psi_first ... Psi_last and ThT_c = Th_first of CTA c's block (put_scan_slots), the cluster-level recurrences
+        //   Gin_0 = 0, Gin_{c+1} = F_c + PhiT_c Gin_c;   Xin_last = 0, Xin_{c-1} = B_c + ThT_c Gin_c + PsiT_c Xin_c
+        // unroll to  Gin_r = sum_{s<r} C_{r,s} F_s,   Xin_r = sum_{s>r} D_{r,s} B_s + sum_t E_{r,t} F_t  with
+        //   C_{r,s} = PhiT_{r-1} ... PhiT_{s+1}  (entry s;      identity for s = r - 1),
+        //   D_{r,s} = PsiT_{r+1} ... PsiT_{s-1}  (entry 8 + s;  identity for s = r + 1),
+        //   E_{r,t} = sum_{s > max(r,t)} D_{r,s} ThT_s C_{s,t}  (entry 16 + t),
+        // all LHS-only, so every CTA finishes its carries after ONE exchange of (F, B).
+        std::vector<Mat> PhiT(k), PsiT(k), ThT(k);
+        Mat ident;
+        ident.m[0] = 1.0;
+        if (nc == 2) ident.m[3] = 1.0;
         for (int c = 0; c < k; ++c) {
             Mat f = Phi[c * PL], b = Psi[c * PL + PL - 1];
             for (int q = 1; q < PL; ++q) f = matmul(Phi[c * PL + q], f, nc);
             for (int q = PL - 2; q >= 0; --q) b = matmul(Psi[c * PL + q], b, nc);
+            std::vector<Mat> pins(PL);
+            pins[0] = ident;
+            for (int q = 1; q < PL; ++q) pins[q] = matmul(Phi[c * PL + q - 1], pins[q - 1], nc);
+            Mat th;
+            for (int q = PL - 1; q >= 0; --q) {
+                const Mat cp = matmul(Chi0[c * PL + q], pins[q], nc), pt = matmul(Psi[c * PL + q], th, nc);
+                for (int m = 0; m < ne; ++m) th.m[m] = cp.m[m] + pt.m[m];
+            }
             PhiT[c] = f;
             PsiT[c] = b;
+            ThT[c] = th;
         }
-        Mat ident;
-        ident.m[0] = 1.0;
-        if (nc == 2) ident.m[3] = 1.0;
+        // C[r][s], s < r and D[r][s], s > r
+        std::vector<std::vector<Mat>> C(k, std::vector<Mat>(k)), D(k, std::vector<Mat>(k));
         for (int r = 0; r < k; ++r) {
-            const size_t base = pl.offTc + (size_t)r * pl.tab_bytes_cl + (size_t)12 * ne * SCAN_LANES * sizeof(T);
             Mat c = ident;
             for (int sb = r - 1; sb >= 0; --sb) {
                 if (sb < r - 1) c = matmul(c, PhiT[sb + 1], nc);
-                for (int m = 0; m < ne; ++m) put<T>(blob, base + ((size_t)m * SCAN_LANES + sb) * sizeof(T), c.m[m]);
+                C[r][sb] = c;
             }
             Mat d = ident;
             for (int sb = r + 1; sb < k; ++sb) {
                 if (sb > r + 1) d = matmul(d, PsiT[sb - 1], nc);
-                for (int m = 0; m < ne; ++m) put<T>(blob, base + ((size_t)m * SCAN_LANES + 8 + sb) * sizeof(T), d.m[m]);
+                D[r][sb] = d;
+            }
+        }
+        for (int r = 0; r < k; ++r) {
+            const size_t base = pl.offTc + (size_t)r * pl.tab_bytes_cl + (size_t)12 * ne * SCAN_LANES * sizeof(T);
+            for (int sb = 0; sb < k; ++sb) {
+                if (sb < r)
+                    for (int m = 0; m < ne; ++m) put<T>(blob, base + ((size_t)m * SCAN_LANES + sb) * sizeof(T), C[r][sb].m[m]);
+                if (sb > r)
+                    for (int m = 0; m < ne; ++m) put<T>(blob, base + ((size_t)m * SCAN_LANES + 8 + sb) * sizeof(T), D[r][sb].m[m]);
+            }
+            for (int t = 0; t < k; ++t) {
+                Mat e;
+                for (int sb = (r > t ? r : t) + 1; sb < k; ++sb) {
+                    const Mat x = matmul(matmul(D[r][sb], ThT[sb], nc), C[sb][t], nc);
+                    for (int m = 0; m < ne; ++m) e.m[m] += x.m[m];
+                }
+                for (int m = 0; m < ne; ++m) put<T>(blob, base + ((size_t)m * SCAN_LANES + 16 + t) * sizeof(T), e.m[m]);
             }
         }
     }
@@ -805,7 +853,7 @@ SweepEntry find_sweep_cl(int kind, int elem_bytes, int fuse)
     return SweepEntry{nullptr, nullptr, 0};
 }
 
-// Cluster-chain plan (sweep.cuh, CL): a tile's rows are split over csz CTAs of one thread-block cluster (csz SMs), each
+// Cluster plan (sweep.cuh, CL): a tile's rows are split over csz CTAs of one thread-block cluster (csz SMs), each
 // keeping PLc <= 16 partitions on 16 lanes x 16 bytes = 256-byte row segments, which is what HBM and the TLB want
 // (DESIGN.md "Long systems").  Shared memory per CTA: its partitions' coefficient blocks, its own scan-table block, the
 // exchange area of its partitions, the two carry inboxes and the ring of its rows.
@@ -834,7 +882,7 @@ void fill_cluster_slot(Handle *h, DtypePlan &pl)
     sl.offTl = (unsigned)align16(rows_bytes);
     sl.offX = (unsigned)align16(sl.offTl + pl.tab_bytes_cl);
     sl.offIn = (unsigned)align16(sl.offX + (size_t)sl.xstride * pl.elem);
-    sl.offM = (unsigned)align16(sl.offIn + (size_t)2 * 8 * NC * W * pl.elem);  // [forward | backward][8 senders][NC][W]
+    sl.offM = (unsigned)align16(sl.offIn + (size_t)2 * 2 * 8 * NC * W * pl.elem);  // [tile parity][F | B][8 senders][NC][W]
     sl.offR = (unsigned)align_up(sl.offM + 49 * 8, 128);  // 17 barriers as everywhere + 2 x 16 inbox barriers
     int g = 256 / pl.rows < PL ? 256 / pl.rows : PL;
     while (PL % g != 0) --g;

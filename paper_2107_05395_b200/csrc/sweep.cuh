@@ -383,20 +383,22 @@ sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
 
     // ---- stage the coefficient image once per CTA: one asynchronous bulk copy ---------------------
     // mbarrier slots at offM: 0..15 = the groups' prefetch rings, 16 = the coefficient image,
-    // CL: 17 + job / 33 + job = forward / backward carry inbox of scan job `job` (a column of owner threads, 16 per
-    // CTA), filled by the neighbouring CTAs of the cluster.  One barrier per job: a warp that runs two jobs per tile
-    // step must not need its second job's carry from a neighbour that is still waiting for this warp's first job.
+    // CL: 17 + job / 33 + job = carry inbox of scan job `job` (a column of owner threads, 16 per CTA) on even / odd
+    // exchanges, filled by the other CTAs of the cluster.  One barrier per job: a warp that runs two jobs per tile step must
+    // not need its second job's carries from a CTA that is still waiting for this warp's first job.  Two sets (and two
+    // inbox buffers) used in turn: a CTA that runs ahead arrives for exchange t + 1 on the other set, and cannot reach
+    // exchange t + 2 before this CTA has sent its values of t + 1, i.e. has consumed exchange t.
     [[maybe_unused]] const unsigned mbar = smem_u32(smem + a.offM) + 8u * sub;
     const unsigned bbar = smem_u32(smem + a.offM) + 8u * 16u;
     [[maybe_unused]] const unsigned fin_bar = smem_u32(smem + a.offM) + 8u * 17u;
     [[maybe_unused]] const unsigned bin_bar = smem_u32(smem + a.offM) + 8u * 33u;
     if (threadIdx.x == 0) {
         mbar_init(bbar, 1);
-        if constexpr (CL) {  // per tile step one arrival from every CTA below (forward) / above (backward)
-            const unsigned nlo = crank > 0u ? crank : 1u, nhi = (int)crank + 1 < csz ? (unsigned)csz - 1u - crank : 1u;
+        if constexpr (CL) {  // per exchange two arrivals (F and B) from every other CTA of the cluster
+            const unsigned narr = 2u * ((unsigned)csz - 1u);
             for (int jb = 0; jb < a.lanes; ++jb) {
-                mbar_init(fin_bar + 8u * jb, nlo);
-                mbar_init(bin_bar + 8u * jb, nhi);
+                mbar_init(fin_bar + 8u * jb, narr);
+                mbar_init(bin_bar + 8u * jb, narr);
             }
         }
     }
@@ -449,7 +451,7 @@ sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
     // cluster through distributed shared memory
     [[maybe_unused]] T *const inbox = reinterpret_cast<T *>(smem + a.offIn);
     [[maybe_unused]] const unsigned inbox_u32 = smem_u32(smem + a.offIn);
-    [[maybe_unused]] unsigned cphase = 0;  // parity of the inbox barriers: one phase per tile step
+    [[maybe_unused]] unsigned cstep = 0;  // exchanges done: set = cstep & 1, barrier parity = (cstep >> 1) & 1
     [[maybe_unused]] S *const ring = reinterpret_cast<S *>(smem + a.offR + (size_t)sub * ring_bytes);
 
     const int ntiles = (int)a.num_tiles;
@@ -797,60 +799,14 @@ sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
                                 }
                             }
                         });
-                        // CL: carries across the CTAs of the cluster, two exchanges whatever the cluster size.  fb is the inclusive
-                        // scan of this CTA's partitions with zero carry-in; its last value F (this CTA's contribution to every
-                        // carry above it) goes to the inboxes of ALL CTAs above.  The carry into this CTA's first partition is then
-                        // sum over the CTAs s below of C_s F_s with C_s = Phi-products over the CTAs between (table slot 12, LHS
-                        // only), and it reaches partition q through Phi_q ... Phi_first (slot 10).
-                        [[maybe_unused]] T fin[NC][V];
+                        // CL: fb is the inclusive scan of this CTA's partitions with zero carry-in; its last value F is this
+                        // CTA's forward contribution to the cluster-level recurrence (exchanged below, once, together with B)
+                        [[maybe_unused]] T Fown[NC][V];
                         if constexpr (CL) {
-                            if (ok && q == P - 1) {
-                                for (int r = (int)crank + 1; r < csz; ++r) {
-                                    const unsigned rin = cluster_map(inbox_u32, (unsigned)r);
-#pragma unroll
-                                    for (int c = 0; c < NC; ++c)
-#pragma unroll
-                                        for (int e = 0; e < V; ++e)
-                                            st_cluster(rin + (unsigned)((((int)crank * NC + c) * W + sg * V + e) * (int)sizeof(T)), fb[c][e]);
-                                    mbar_arrive_remote(cluster_map(fin_bar, (unsigned)r) + 8u * sg);
-                                }
-                            }
 #pragma unroll
                             for (int c = 0; c < NC; ++c)
 #pragma unroll
-                                for (int e = 0; e < V; ++e) fin[c][e] = T(0);
-                            if (crank > 0u && sg < job1) {
-                                mbar_wait_cluster(fin_bar + 8u * sg, cphase);
-                                for (int sb = 0; sb < (int)crank; ++sb) {
-                                    T cm_[NC * NC];
-#pragma unroll
-                                    for (int i = 0; i < NC * NC; ++i) cm_[i] = TAB[12 * sstr + i * mstr + sb];
-#pragma unroll
-                                    for (int e = 0; e < V; ++e) {
-                                        T f[NC];
-#pragma unroll
-                                        for (int c = 0; c < NC; ++c) f[c] = ok ? inbox[(sb * NC + c) * W + sg * V + e] : T(0);
-                                        if constexpr (TRI) {
-                                            fin[0][e] = fma_t<T>(cm_[0], f[0], fin[0][e]);
-                                        } else {
-                                            fin[0][e] = fma_t<T>(cm_[1], f[1], fma_t<T>(cm_[0], f[0], fin[0][e]));
-                                            fin[1][e] = fma_t<T>(cm_[3], f[1], fma_t<T>(cm_[2], f[0], fin[1][e]));
-                                        }
-                                    }
-                                }
-                                T m[NC * NC];
-#pragma unroll
-                                for (int i = 0; i < NC * NC; ++i) m[i] = tb[10 * sstr + i * mstr];
-#pragma unroll
-                                for (int e = 0; e < V; ++e) {
-                                    if constexpr (TRI) {
-                                        fb[0][e] = fma_t<T>(m[0], fin[0][e], fb[0][e]);
-                                    } else {
-                                        fb[0][e] = fma_t<T>(m[1], fin[1][e], fma_t<T>(m[0], fin[0][e], fb[0][e]));
-                                        fb[1][e] = fma_t<T>(m[3], fin[1][e], fma_t<T>(m[2], fin[0][e], fb[1][e]));
-                                    }
-                                }
-                            }
+                                for (int e = 0; e < V; ++e) Fown[c][e] = __shfl_sync(0xffffffffu, fb[c][e], P - 1, wd);
                         }
                         [[maybe_unused]] T yn1[V], yn2[V];  // cyclic forms: y at rows n-1, n-2 (true g at the last rows)
                         if constexpr (PERTF) {
@@ -877,8 +833,7 @@ sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
 #pragma unroll
                                 for (int c = 0; c < NC; ++c) {
                                     const T g = __shfl_up_sync(0xffffffffu, fb[c][e], 1, wd);
-                                    if constexpr (CL) fb[c][e] = (q == 0) ? fin[c][e] : g;
-                                    else fb[c][e] = (q == 0) ? T(0) : g;
+                                    fb[c][e] = (q == 0) ? T(0) : g;
                                 }
                                 if constexpr (TRI) {
                                     bb[0][e] = fma_t<T>(ch[0], fb[0][e], bb[0][e]);
@@ -905,55 +860,72 @@ sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
                                 }
                             }
                         });
-                        // CL: the backward carries the same way, downwards (bb already holds the true forward carries through u):
-                        // this CTA's first inclusive value goes to ALL CTAs below; the carry into its last partition is the sum
-                        // over the CTAs r above of D_r B_r (slot 12, entries 8 + r) and reaches partition q through slot 11.
-                        [[maybe_unused]] T bin[NC][V];
+                        // CL: the carries across the CTAs of the cluster, ONE exchange per tile step whatever the cluster size.  So
+                        // far this CTA's block of partitions was solved on its own: F = its forward carry out, B = bb at its first
+                        // partition = its backward carry out, both for zero carries in.  Every CTA sends (F, B) to all the others,
+                        // and forms its own carries in from them with the LHS-only matrices of table slot 12 (put_scan_tables in
+                        // btps.cu: the cluster-level recurrences unrolled):  Gin = sum_{s<r} C_s F_s,  Xin = sum_{s>r} D_s B_s +
+                        // sum_t E_t F_t.  They then reach partition q through slots 10 (Pin_q), 13 (Th_{q+1}) and 11 (Sf_{q+1}).
+                        [[maybe_unused]] T gin[NC][V], xin[NC][V];
                         if constexpr (CL) {
-                            if (ok && q == 0) {
-                                for (int r = 0; r < (int)crank; ++r) {
+                            const unsigned set = cstep & 1u;
+                            const unsigned xbar = (set ? bin_bar : fin_bar) + 8u * (unsigned)sg;
+                            const int ibuf = (int)set * (2 * 8 * NC * W);  // this exchange's inbox buffer (elements)
+                            if (ok && (q == P - 1 || q == 0)) {
+                                // lane P-1 sends F (slot crank), lane 0 sends B (slot 8 + crank); one arrival each per receiver
+                                const int slot = (q == 0) ? 8 + (int)crank : (int)crank;
+                                for (int r = 0; r < csz; ++r) {
+                                    if (r == (int)crank) continue;
                                     const unsigned rin = cluster_map(inbox_u32, (unsigned)r);
 #pragma unroll
                                     for (int c = 0; c < NC; ++c)
 #pragma unroll
                                         for (int e = 0; e < V; ++e)
-                                            st_cluster(rin + (unsigned)((((8 + (int)crank) * NC + c) * W + sg * V + e) * (int)sizeof(T)), bb[c][e]);
-                                    mbar_arrive_remote(cluster_map(bin_bar, (unsigned)r) + 8u * sg);
+                                            st_cluster(rin + (unsigned)((ibuf + (slot * NC + c) * W + sg * V + e) * (int)sizeof(T)),
+                                                       (q == 0) ? bb[c][e] : Fown[c][e]);
+                                    mbar_arrive_remote(cluster_map(xbar, (unsigned)r));
                                 }
                             }
 #pragma unroll
                             for (int c = 0; c < NC; ++c)
 #pragma unroll
-                                for (int e = 0; e < V; ++e) bin[c][e] = T(0);
-                            if ((int)crank + 1 < csz && sg < job1) {
-                                mbar_wait_cluster(bin_bar + 8u * sg, cphase);
-                                for (int sb = (int)crank + 1; sb < csz; ++sb) {
-                                    T dm_[NC * NC];
+                                for (int e = 0; e < V; ++e) {
+                                    gin[c][e] = T(0);
+                                    xin[c][e] = T(0);
+                                }
+                            if (sg < job1) {
+                                mbar_wait_cluster(xbar, (cstep >> 1) & 1u);
+                                const T *const ib = inbox + ibuf;
+                                const T *const t12 = TAB + 12 * sstr;
+                                // Gin = sum_{s<r} C_s F_s;  Xin = sum_{s>r} D_s B_s + sum_t E_t F_t  (entries s, 8 + s, 16 + t of slot 12)
+                                for (int cc = 0; cc < csz; ++cc) {
+                                    T cm_[NC * NC], dm_[NC * NC], em_[NC * NC];
 #pragma unroll
-                                    for (int i = 0; i < NC * NC; ++i) dm_[i] = TAB[12 * sstr + i * mstr + 8 + sb];
+                                    for (int i = 0; i < NC * NC; ++i) {
+                                        cm_[i] = t12[i * mstr + cc];        // zero for cc >= r (never written)
+                                        dm_[i] = t12[i * mstr + 8 + cc];    // zero for cc <= r
+                                        em_[i] = t12[i * mstr + 16 + cc];
+                                    }
+                                    const bool own = cc == (int)crank;
 #pragma unroll
                                     for (int e = 0; e < V; ++e) {
-                                        T f[NC];
+                                        T f[NC], b[NC];
 #pragma unroll
-                                        for (int c = 0; c < NC; ++c) f[c] = ok ? inbox[((8 + sb) * NC + c) * W + sg * V + e] : T(0);
-                                        if constexpr (TRI) {
-                                            bin[0][e] = fma_t<T>(dm_[0], f[0], bin[0][e]);
-                                        } else {
-                                            bin[0][e] = fma_t<T>(dm_[1], f[1], fma_t<T>(dm_[0], f[0], bin[0][e]));
-                                            bin[1][e] = fma_t<T>(dm_[3], f[1], fma_t<T>(dm_[2], f[0], bin[1][e]));
+                                        for (int c = 0; c < NC; ++c) {
+                                            f[c] = own ? Fown[c][e] : (ok ? ib[(cc * NC + c) * W + sg * V + e] : T(0));
+                                            b[c] = own ? T(0) : (ok ? ib[((8 + cc) * NC + c) * W + sg * V + e] : T(0));
                                         }
-                                    }
-                                }
-                                T m[NC * NC];
-#pragma unroll
-                                for (int i = 0; i < NC * NC; ++i) m[i] = tb[11 * sstr + i * mstr];
-#pragma unroll
-                                for (int e = 0; e < V; ++e) {
-                                    if constexpr (TRI) {
-                                        bb[0][e] = fma_t<T>(m[0], bin[0][e], bb[0][e]);
-                                    } else {
-                                        bb[0][e] = fma_t<T>(m[1], bin[1][e], fma_t<T>(m[0], bin[0][e], bb[0][e]));
-                                        bb[1][e] = fma_t<T>(m[3], bin[1][e], fma_t<T>(m[2], bin[0][e], bb[1][e]));
+                                        if constexpr (TRI) {
+                                            gin[0][e] = fma_t<T>(cm_[0], f[0], gin[0][e]);
+                                            xin[0][e] = fma_t<T>(em_[0], f[0], fma_t<T>(dm_[0], b[0], xin[0][e]));
+                                        } else {
+                                            gin[0][e] = fma_t<T>(cm_[1], f[1], fma_t<T>(cm_[0], f[0], gin[0][e]));
+                                            gin[1][e] = fma_t<T>(cm_[3], f[1], fma_t<T>(cm_[2], f[0], gin[1][e]));
+                                            xin[0][e] = fma_t<T>(dm_[1], b[1], fma_t<T>(dm_[0], b[0], xin[0][e]));
+                                            xin[1][e] = fma_t<T>(dm_[3], b[1], fma_t<T>(dm_[2], b[0], xin[1][e]));
+                                            xin[0][e] = fma_t<T>(em_[1], f[1], fma_t<T>(em_[0], f[0], xin[0][e]));
+                                            xin[1][e] = fma_t<T>(em_[3], f[1], fma_t<T>(em_[2], f[0], xin[1][e]));
+                                        }
                                     }
                                 }
                             }
@@ -992,8 +964,21 @@ sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
                             for (int e = 0; e < V; ++e) {
                                 T x = __shfl_down_sync(0xffffffffu, bb[c][e], 1, wd);
                                 const int ix = (sg * V + e) ^ qsw;
-                                if constexpr (CL) x = (q + 1 < P) ? x : bin[c][e];
-                                else x = (q + 1 < P) ? x : T(0);
+                                x = (q + 1 < P) ? x : T(0);
+                                if constexpr (CL) {
+                                    // G_q = G0_q + Pin_q Gin;  X_q = X0_q + Th_{q+1} Gin + Sf_{q+1} Xin  (row c of each matrix)
+                                    if constexpr (TRI) {
+                                        fb[c][e] = fma_t<T>(tb[10 * sstr], gin[0][e], fb[c][e]);
+                                        x = fma_t<T>(tb[11 * sstr], xin[0][e], fma_t<T>(tb[13 * sstr], gin[0][e], x));
+                                    } else {
+                                        fb[c][e] = fma_t<T>(tb[10 * sstr + (2 * c + 1) * mstr], gin[1][e],
+                                                            fma_t<T>(tb[10 * sstr + (2 * c) * mstr], gin[0][e], fb[c][e]));
+                                        x = fma_t<T>(tb[13 * sstr + (2 * c + 1) * mstr], gin[1][e],
+                                                     fma_t<T>(tb[13 * sstr + (2 * c) * mstr], gin[0][e], x));
+                                        x = fma_t<T>(tb[11 * sstr + (2 * c + 1) * mstr], xin[1][e],
+                                                     fma_t<T>(tb[11 * sstr + (2 * c) * mstr], xin[0][e], x));
+                                    }
+                                }
                                 if constexpr (PERTF) {
                                     fb[c][e] = fma_t<T>(tb[10 * sstr], nw[0][e], fb[c][e]);
                                     x = fma_t<T>(tb[11 * sstr], nw[0][e], x);
@@ -1019,7 +1004,7 @@ sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
                             }
                     }
                 }
-                if constexpr (CL) cphase ^= 1u;  // both inbox barriers have completed one phase (or are unused at the chain's ends)
+                if constexpr (CL) ++cstep;
                 group_sync(a.tpc, sub, tpt);
 #pragma unroll
                 for (int e = 0; e < V; ++e) {
