@@ -1081,10 +1081,13 @@ int make_tmap(CUtensorMap *tm, T *d_rhs, long long batch, int n, int W, unsigned
 template <typename T>
 bool cl_pays(int kind, const DtypePlan &pl, long long batch)
 {
-    // measured on B200 (profiles/r02_long_systems.md): the pair's two carry exchanges per tile cost ~1.5 us, which only
-    // pays where the single CTA's 128-byte segments are at their worst -- tridiagonal, 32 partitions (N = 992 / 1024),
-    // batches of >= 2^22 systems: 0.72 / 0.71 (fp64 / fp32) against 0.69 / 0.69.  Pentadiagonal: the pair loses everywhere.
-    return kind == KIND_TRI && pl.P == 32 && pl.csz == 2 && batch >= (1ll << 22);
+    // measured on B200 (profiles/r02b_long_systems.md, one carry exchange per tile): the tridiagonal pair at 32 partitions
+    // (N = 992 / 1024) holds 0.84-0.87 whatever the batch, the single CTA's 128-byte segments fall from 0.90 (2^17 systems)
+    // to 0.69 (2^22) -- the pair wins once a row of the batch reaches the 2 MiB page size (2^18 systems fp64, 2^19 fp32).
+    // 28-30 partitions: only from 32 MiB rows (0.73 against 0.68).  Pentadiagonal: the pair loses everywhere (0.63-0.67).
+    if (kind != KIND_TRI || pl.csz != 2) return false;
+    const size_t pitch = (size_t)batch * (size_t)pl.elem;
+    return (pl.P == 32 && pitch >= ((size_t)2 << 20)) || (pl.P >= 28 && pitch >= ((size_t)32 << 20));
 }
 
 // one sweep launch (kind = KIND_TRI / KIND_PENTA / KIND_CH) on a device buffer

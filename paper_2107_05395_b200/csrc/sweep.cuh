@@ -253,12 +253,6 @@ __device__ __forceinline__ unsigned cluster_nctarank()
     asm volatile("mov.u32 %0, %%cluster_nctarank;" : "=r"(r));
     return r;
 }
-// arrive (release at cluster scope) on an mbarrier in another CTA of the cluster: orders this thread's earlier
-// st.shared::cluster writes before the arrival
-__device__ __forceinline__ void mbar_arrive_remote(unsigned remote_bar)
-{
-    asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" ::"r"(remote_bar) : "memory");
-}
 // wait on a local mbarrier whose arrivals come from another CTA (acquire at cluster scope).  A neighbour that never
 // arrives would otherwise hang the device: after ~4 s without progress the kernel traps (the launch then fails with
 // an error instead of spinning forever).
@@ -282,13 +276,16 @@ __device__ __forceinline__ void mbar_wait_cluster(unsigned bar, unsigned parity)
         }
     }
 }
-__device__ __forceinline__ void st_cluster(unsigned addr, double v)
+// Store into another CTA's shared memory that signals the receiver's mbarrier itself (complete_tx of its own bytes): no
+// arrive and so no release fence on the sender.  (A separate mbarrier.arrive.release.cluster compiles to MEMBAR.ALL + ERRBAR,
+// which also waits for the sender's global stores of the previous tile: 18 % of all stall samples of the cluster kernels.)
+__device__ __forceinline__ void st_async_cluster(unsigned addr, double v, unsigned remote_bar)
 {
-    asm volatile("st.shared::cluster.f64 [%0], %1;" ::"r"(addr), "d"(v) : "memory");
+    asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.f64 [%0], %1, [%2];" ::"r"(addr), "d"(v), "r"(remote_bar) : "memory");
 }
-__device__ __forceinline__ void st_cluster(unsigned addr, float v)
+__device__ __forceinline__ void st_async_cluster(unsigned addr, float v, unsigned remote_bar)
 {
-    asm volatile("st.shared::cluster.f32 [%0], %1;" ::"r"(addr), "f"(v) : "memory");
+    asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.f32 [%0], %1, [%2];" ::"r"(addr), "f"(v), "r"(remote_bar) : "memory");
 }
 
 // Barrier over the threads of one tile group.  A CTA hosts `tpc` groups that walk their tiles
@@ -394,11 +391,10 @@ sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
     [[maybe_unused]] const unsigned bin_bar = smem_u32(smem + a.offM) + 8u * 33u;
     if (threadIdx.x == 0) {
         mbar_init(bbar, 1);
-        if constexpr (CL) {  // per exchange two arrivals (F and B) from every other CTA of the cluster
-            const unsigned narr = 2u * ((unsigned)csz - 1u);
+        if constexpr (CL) {  // per exchange one local arrival that states the bytes to expect (F and B from every other CTA)
             for (int jb = 0; jb < a.lanes; ++jb) {
-                mbar_init(fin_bar + 8u * jb, narr);
-                mbar_init(bin_bar + 8u * jb, narr);
+                mbar_init(fin_bar + 8u * jb, 1);
+                mbar_init(bin_bar + 8u * jb, 1);
             }
         }
     }
@@ -872,18 +868,21 @@ sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
                             const unsigned xbar = (set ? bin_bar : fin_bar) + 8u * (unsigned)sg;
                             const int ibuf = (int)set * (2 * 8 * NC * W);  // this exchange's inbox buffer (elements)
                             if (ok && (q == P - 1 || q == 0)) {
-                                // lane P-1 sends F (slot crank), lane 0 sends B (slot 8 + crank); one arrival each per receiver
+                                // lane 0 arms this CTA's barrier for the bytes the others will send (its own arrival; it has waited
+                                // for this barrier's previous phase itself), then lane P-1 sends F (slot crank) and lane 0 sends B
+                                // (slot 8 + crank): every store completes its own bytes on the receiver's barrier
+                                if (q == 0) mbar_expect_tx(xbar, (unsigned)((csz - 1) * 2 * NC * V) * (unsigned)sizeof(T));
                                 const int slot = (q == 0) ? 8 + (int)crank : (int)crank;
                                 for (int r = 0; r < csz; ++r) {
                                     if (r == (int)crank) continue;
                                     const unsigned rin = cluster_map(inbox_u32, (unsigned)r);
+                                    const unsigned rbar = cluster_map(xbar, (unsigned)r);
 #pragma unroll
                                     for (int c = 0; c < NC; ++c)
 #pragma unroll
                                         for (int e = 0; e < V; ++e)
-                                            st_cluster(rin + (unsigned)((ibuf + (slot * NC + c) * W + sg * V + e) * (int)sizeof(T)),
-                                                       (q == 0) ? bb[c][e] : Fown[c][e]);
-                                    mbar_arrive_remote(cluster_map(xbar, (unsigned)r));
+                                            st_async_cluster(rin + (unsigned)((ibuf + (slot * NC + c) * W + sg * V + e) * (int)sizeof(T)),
+                                                             (q == 0) ? bb[c][e] : Fown[c][e], rbar);
                                 }
                             }
 #pragma unroll
