@@ -1081,13 +1081,16 @@ int make_tmap(CUtensorMap *tm, T *d_rhs, long long batch, int n, int W, unsigned
 template <typename T>
 bool cl_pays(int kind, const DtypePlan &pl, long long batch)
 {
-    // measured on B200 (profiles/r02b_long_systems.md, one carry exchange per tile): the tridiagonal pair at 32 partitions
-    // (N = 992 / 1024) holds 0.84-0.87 whatever the batch, the single CTA's 128-byte segments fall from 0.90 (2^17 systems)
-    // to 0.69 (2^22) -- the pair wins once a row of the batch reaches the 2 MiB page size (2^18 systems fp64, 2^19 fp32).
-    // 28-30 partitions: only from 32 MiB rows (0.73 against 0.68).  Pentadiagonal: the pair loses everywhere (0.63-0.67).
-    if (kind != KIND_TRI || pl.csz != 2) return false;
+    // measured on B200 (profiles/r02b_long_systems.md; one carry exchange per tile, sent with st.async): the pair keeps
+    // 0.82-0.91 (tri) / 0.78-0.87 (penta, 32 partitions) of the HBM peak whatever the batch, while the single CTA's 128-byte
+    // segments fall from 0.85-0.91 to 0.69 as a row of the batch grows from 1 MiB to 32 MiB.  Crossovers by row pitch:
+    //   tri,   24-32 partitions (N > 736): pair from 4 MiB rows;  18-23 partitions: from 32 MiB rows (0.74-0.82 against 0.71)
+    //   penta, 31-32 partitions (N > 960): pair from 8 MiB rows (0.87 / 0.78 against 0.78 / 0.69);  fewer: the pair loses
+    if (pl.csz != 2) return false;
     const size_t pitch = (size_t)batch * (size_t)pl.elem;
-    return (pl.P == 32 && pitch >= ((size_t)2 << 20)) || (pl.P >= 28 && pitch >= ((size_t)32 << 20));
+    if (kind == KIND_TRI) return (pl.P >= 24 && pitch >= ((size_t)4 << 20)) || pitch >= ((size_t)32 << 20);
+    if (kind == KIND_PENTA) return pl.P >= 31 && pitch >= ((size_t)8 << 20);
+    return false;
 }
 
 // one sweep launch (kind = KIND_TRI / KIND_PENTA / KIND_CH) on a device buffer
