@@ -287,6 +287,21 @@ __device__ __forceinline__ void st_async_cluster(unsigned addr, float v, unsigne
 {
     asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.f32 [%0], %1, [%2];" ::"r"(addr), "f"(v), "r"(remote_bar) : "memory");
 }
+// the V adjacent values of one owner thread as one 16-byte store where they are 16 bytes (V = 2 doubles / 4 floats)
+template <typename T, int V>
+__device__ __forceinline__ void st_async_cluster_vec(unsigned addr, const T (&v)[V], unsigned remote_bar)
+{
+    if constexpr (sizeof(T) == 8 && V == 2) {
+        asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.v2.f64 [%0], {%1, %2}, [%3];" ::"r"(addr), "d"(v[0]),
+                     "d"(v[1]), "r"(remote_bar) : "memory");
+    } else if constexpr (sizeof(T) == 4 && V == 4) {
+        asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.v4.f32 [%0], {%1, %2, %3, %4}, [%5];" ::"r"(addr),
+                     "f"(v[0]), "f"(v[1]), "f"(v[2]), "f"(v[3]), "r"(remote_bar) : "memory");
+    } else {
+#pragma unroll
+        for (int e = 0; e < V; ++e) st_async_cluster(addr + (unsigned)(e * (int)sizeof(T)), v[e], remote_bar);
+    }
+}
 
 // Barrier over the threads of one tile group.  A CTA hosts `tpc` groups that walk their tiles
 // independently of one another (so one group's arithmetic overlaps another group's waits); a
@@ -878,11 +893,12 @@ sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
                                     const unsigned rin = cluster_map(inbox_u32, (unsigned)r);
                                     const unsigned rbar = cluster_map(xbar, (unsigned)r);
 #pragma unroll
-                                    for (int c = 0; c < NC; ++c)
+                                    for (int c = 0; c < NC; ++c) {
+                                        T pay[V];
 #pragma unroll
-                                        for (int e = 0; e < V; ++e)
-                                            st_async_cluster(rin + (unsigned)((ibuf + (slot * NC + c) * W + sg * V + e) * (int)sizeof(T)),
-                                                             (q == 0) ? bb[c][e] : Fown[c][e], rbar);
+                                        for (int e = 0; e < V; ++e) pay[e] = (q == 0) ? bb[c][e] : Fown[c][e];
+                                        st_async_cluster_vec<T, V>(rin + (unsigned)((ibuf + (slot * NC + c) * W + sg * V) * (int)sizeof(T)), pay, rbar);
+                                    }
                                 }
                             }
 #pragma unroll
