@@ -1088,7 +1088,9 @@ bool cl_pays(int kind, const DtypePlan &pl, long long batch)
     //   penta, 31-32 partitions (N > 960): pair from 8 MiB rows (0.87 / 0.78 against 0.78 / 0.69);  fewer: the pair loses
     if (pl.csz != 2) return false;
     const size_t pitch = (size_t)batch * (size_t)pl.elem;
-    if (kind == KIND_TRI) return (pl.P >= 24 && pitch >= ((size_t)4 << 20)) || pitch >= ((size_t)32 << 20);
+    // (tri at 32 partitions: the pair's CTAs keep full 128 KB shares and hold their stores, launch_one -- 0.88-0.93 from 2^16
+    //  systems on, never behind the single CTA's 0.87-0.91)
+    if (kind == KIND_TRI) return (pl.PLc == 16 && pitch >= ((size_t)512 << 10)) || (pl.P >= 24 && pitch >= ((size_t)4 << 20)) || pitch >= ((size_t)32 << 20);
     if (kind == KIND_PENTA) return pl.P >= 31 && pitch >= ((size_t)8 << 20);
     return false;
 }
@@ -1229,7 +1231,11 @@ int launch_one(Handle *h, int kind, S *d_rhs, long long batch, double alpha_x, i
         // and free-running stores fall to 0.66: profiles/r02b_shared_blocks.md)
         const bool penta_big = (kind == KIND_PENTA) && !h->periodic && sh.lanes == 8 && (size_t)batch * sizeof(S) >= ((size_t)32 << 20);
         const bool penta_ok = ((kind == KIND_PENTA) && sizeof(T) == 8 && !h->periodic && sh.lanes == 16) || penta_big;
-        a.hold_stores = g_tune.hold_stores >= 0 ? (g_tune.hold_stores > 0) : ((full_tile && (tri_family || penta_ok)) ? 1 : 0);
+        // cluster kernels: only the tridiagonal pair whose CTAs keep a full 128 KB share (32 partitions, N = 993 ... 1024) gains
+        // -- 0.84 -> 0.90-0.93 from 2^19 systems, fp32 0.84 -> 0.92; shares of 96-112 KB (N = 768 / 896) lose 0-3 %, clusters of
+        // 3 / 4 / 8 are indifferent or lose up to 10 %, the pentadiagonal pair is indifferent (profiles/r02b_long_systems.md)
+        const bool pair_tile = use_cl && kind == KIND_TRI && pl.csz == 2 && pl.PLc == 16 && a.num_tiles >= 8ll * (sl.max_grid / 2);
+        a.hold_stores = g_tune.hold_stores >= 0 ? (g_tune.hold_stores > 0) : (((full_tile && (tri_family || penta_ok)) || pair_tile) ? 1 : 0);
     }
     a.blk = blk_stride(pl, h->kind == KIND_TRI ? (h->periodic ? 6 : 5) : (h->periodic ? (pl.wfast ? 11 : 13) : 9));  // = RecLayout<KIND>::ELEMS of the kernel
     a.csz = use_cl ? pl.csz : 1;
