@@ -396,16 +396,11 @@ def extra_table(torch, b, inputs, peak):
         torch.cuda.empty_cache()
 
     entry("1 (latency-bound: 512 KiB)", "tri", 64, 1024, 8, launches=64, graph=True)
-    entry("2 (100 steps per call)", "tri", 512, 65536, 8, steps_per_call=100, launches=2)
-    entry("3 (100 steps per call)", "penta", 512, 65536, 8, steps_per_call=100, launches=2)
-    entry("5 (1000 steps per call)", "ch", 256, 1 << 20, 8, steps_per_call=1000, launches=1)
     # periodic BCs, the form the paper's own benchmarks solve
     for n in (512, 1024):
         entry("f1 periodic (single solve)", "tri_periodic", n, 65536, 8)
         entry("f1 periodic (single solve)", "penta_periodic", n, 65536, 8)
         entry("f1 periodic (single step)", "ch_periodic", n, 65536, 8)
-    entry("f1 periodic CH, 2^20 runs (1000 steps per call)", "ch_periodic", 256, 1 << 20, 8, steps_per_call=1000,
-          launches=1)
     # fp32 in HBM, fp64 arithmetic (algorithmic bytes = 2 * N * M * 4)
     for kind in ("tri_f32s", "penta_f32s"):
         for n, lb in ((512, 16), (64, 20), (256, 20), (1024, 19)):
@@ -421,7 +416,16 @@ def extra_table(torch, b, inputs, peak):
                     # cells of a few microseconds are bound by the host's launch path: also replayed from a CUDA graph
                     entry("4 sweep", kind, n, 1 << lb, elem, launches=10 if lb < 22 else 4,
                           graph=(n * (1 << lb) * elem <= (32 << 20)))
-    return out
+    # The time loops last: seconds of fp64-pipe-bound work at the board's power cap, after which the SM clock stays low for
+    # a while -- single-solve cells timed right behind them read 8-20 % low (seen on the periodic cells when they followed
+    # config 5).  Listed in the side file right after config 1, as BASELINE.json numbers them.
+    head = len(out)
+    entry("2 (100 steps per call)", "tri", 512, 65536, 8, steps_per_call=100, launches=2)
+    entry("3 (100 steps per call)", "penta", 512, 65536, 8, steps_per_call=100, launches=2)
+    entry("5 (1000 steps per call)", "ch", 256, 1 << 20, 8, steps_per_call=1000, launches=1)
+    entry("f1 periodic CH, 2^20 runs (1000 steps per call)", "ch_periodic", 256, 1 << 20, 8, steps_per_call=1000,
+          launches=1)
+    return out[:1] + out[head:] + out[1:head]
 
 
 # The paper's own benchmarks (Table 1; 302-335 Table 2): periodic Crank-Nicolson diffusion /
