@@ -1169,3 +1169,53 @@ def test_partially_shared_coefficient_blocks_against_oracle(lib, n):
         ref = rhs.astype(np.float32).astype(np.float64)
         osolve(fac(*lhs), ref)
         assert rel_err(d32.cpu().numpy().astype(np.float64), ref) <= TOL_F32
+
+
+def test_default_cluster_policy_by_row_pitch(lib):
+    """Which kernel a call launches by default (btps_kernel_tag, nothing is launched): the cluster pair where a row of the
+    batch is long enough for 256-byte segments to pay, one CTA per tile below that, clusters
+    always above 1024 rows."""
+    def cl(h, elem, batch):
+        return lib.btps_kernel_tag(h, elem, batch).split(", ")[8] == "1"
+    ht, hp = lib.tri_factor(*inputs.tri_lhs(1024, 0.5)), lib.penta_factor(*inputs.penta_lhs(1024, 0.5))
+    assert not cl(ht, 8, 1 << 13) and cl(ht, 8, 1 << 16) and cl(ht, 8, 1 << 22)       # tri, 32 partitions: from 512 KiB rows
+    assert not cl(ht, 4, 1 << 16) and cl(ht, 4, 1 << 17)
+    assert not cl(hp, 8, 1 << 19) and cl(hp, 8, 1 << 20) and cl(hp, 4, 1 << 21)       # penta, 32 partitions: from 8 MiB rows
+    h768, h640 = lib.tri_factor(*inputs.tri_lhs(768, 0.5)), lib.tri_factor(*inputs.tri_lhs(640, 0.5))
+    assert not cl(h768, 8, 1 << 18) and cl(h768, 8, 1 << 19)                          # 24 partitions: from 4 MiB rows
+    assert not cl(h640, 8, 1 << 21) and cl(h640, 8, 1 << 22)                          # 20 partitions: from 32 MiB rows
+    assert not cl(lib.penta_factor(*inputs.penta_lhs(768, 0.5)), 8, 1 << 22)
+    assert not cl(lib.tri_factor(*inputs.tri_lhs(512, 0.5)), 8, 1 << 22)              # 16 partitions: never
+    for n in (1100, 2048, 4096):
+        assert cl(lib.tri_factor(*inputs.tri_lhs(n, 0.5)), 8, 1 << 10) and cl(lib.penta_factor(*inputs.penta_lhs(n, 0.5)), 4, 1 << 10)
+    assert not cl(ht, 8, (1 << 16) + 1)                                               # unaligned pitch: no TMA, no cluster
+
+
+def test_cluster_pair_held_stores_bitwise_equal_and_against_oracle(lib):
+    """The tridiagonal pair at 32 partitions holds its stores by default once a cluster has 8 tiles to walk: same bits as
+    with free-running stores, equal to the oracle, over enough tiles for the default to be on (148 / 2 clusters x 8 x 32)."""
+    n, batch = 1024, 32 * 74 * 9 + 64
+    lhs = inputs.tri_lhs(n, 0.5)
+    rhs = inputs.uniform_rhs(n, batch, seed=107)
+    got = {}
+    for mode in (-1, 0, 1):
+        try:
+            lib.btps_tune("hold_stores", mode)
+            lib.btps_tune("cluster", 1)       # (the default takes the pair from 512 KiB rows; this batch has 167 KiB ones)
+            h = lib.tri_factor(*lhs)
+            assert lib.btps_kernel_tag(h, 8, batch).split(", ")[8] == "1"
+            d, d32 = dev(rhs), dev(rhs.astype(np.float32))
+            lib.tri_solve_batched(h, d)
+            lib.tri_solve_steps(h, d, 3)
+            lib.tri_solve_batched_f32(h, d32)
+            torch.cuda.synchronize()
+        finally:
+            lib.btps_tune("hold_stores", -1)
+            lib.btps_tune("cluster", -1)
+        got[mode] = (d, d32)
+    for mode in (0, 1):
+        assert torch.equal(got[-1][0], got[mode][0]) and torch.equal(got[-1][1], got[mode][1])
+    ids = np.unique(np.concatenate([np.arange(0, 128), np.arange(batch - 128, batch), np.arange(128, batch - 128, 97)]))
+    ref = rhs[:, ids].copy()
+    oracle.tri_solve_interleaved(oracle.tri_factor(*lhs), ref, nsteps=4)
+    assert rel_err(got[-1][0].cpu().numpy()[:, ids], ref) <= TOL_STEPS
