@@ -135,7 +135,8 @@ BTPS_API int penta_solve_batched_f32(penta_handle_t h, float *d_rhs, int64_t bat
  * with the handle's fp64 tables (eq. 3-6 / Sec. 4.1 as above), and rounded to float once when it is stored.  HBM moves
  * half the bytes of the fp64 calls; the result is the fp64 solution of the (exactly representable) float right-hand
  * side, rounded to nearest float -- about 6e-8 relative to each entry, against ~1e-6 for the all-fp32 *_f32 calls.
- * Non-periodic handles with n <= 1024 (the register-resident plans); other handles fail with BTPS_E_ARG.
+ * Non-periodic handles with n <= 4096 (the register-resident plans; above 1024 rows, on thread-block clusters, the batch needs
+ * 16-byte aligned rows: batch a multiple of 4 and a 16-byte aligned pointer); other handles fail with BTPS_E_ARG.
  * ---------------------------------------------------------------------------------------- */
 BTPS_API int tri_solve_batched_f32s(tri_handle_t h, float *d_rhs, int64_t batch, void *stream);
 BTPS_API int penta_solve_batched_f32s(penta_handle_t h, float *d_rhs, int64_t batch, void *stream);

@@ -113,6 +113,7 @@ struct DtypePlan {
     unsigned char pmap[MAX_PARTS] = {0};
     Shape cshape;
     KernelSlot ck;
+    KernelSlot ck32;  // fp64 plan only: the cluster kernels on fp32 storage (the *_f32s calls); same shape, a ring of floats
 };
 
 constexpr int MAGIC_TRI = 0x74726931;    // "tri1"
@@ -857,9 +858,11 @@ SweepEntry find_sweep_cl(int kind, int elem_bytes, int fuse)
 // keeping PLc <= 16 partitions on 16 lanes x 16 bytes = 256-byte row segments, which is what HBM and the TLB want
 // (DESIGN.md "Long systems").  Shared memory per CTA: its partitions' coefficient blocks, its own scan-table block, the
 // exchange area of its partitions, the two carry inboxes and the ring of its rows.
-void fill_cluster_slot(Handle *h, DtypePlan &pl)
+void fill_cluster_slot(Handle *h, DtypePlan &pl, bool f32s = false)
 {
-    pl.ck = KernelSlot();
+    KernelSlot &sl = f32s ? pl.ck32 : pl.ck;
+    sl = KernelSlot();
+    const size_t selem = f32s ? 4 : (size_t)pl.elem;  // bytes per element of the batch in global memory / in the ring
     if (!pl.csz || h->periodic || g_tune.cluster == 0 || g_tune.prefetch == 0 || pl.rows != 32) return;
     const int kind = h->kind;  // KIND_TRI / KIND_PENTA
     const int NC = (kind == KIND_TRI) ? 1 : 2;
@@ -871,7 +874,6 @@ void fill_cluster_slot(Handle *h, DtypePlan &pl)
     sh.tpc = 1;
     const int PL = pl.PLc;
     sh.threads = PL * sh.lanes;
-    KernelSlot &sl = pl.ck;
     sl.vec = sh.vec;
     sl.tma = 1;
     const size_t W = (size_t)sh.lanes * sl.vec;
@@ -888,10 +890,14 @@ void fill_cluster_slot(Handle *h, DtypePlan &pl)
     while (PL % g != 0) --g;
     sl.box_rows = (unsigned)(g * pl.rows);
     sl.nboxes = (unsigned)(PL / g);
-    sl.smem = sl.offR + (size_t)PL * pl.rows * W * pl.elem;
+    sl.smem = sl.offR + (size_t)PL * pl.rows * W * selem;
     if (sl.smem > SMEM_LIMIT) return;
-    sl.ent = find_sweep_cl(kind, pl.elem, 0);
-    sl.fused = find_sweep_cl(kind, pl.elem, 1);
+    if (f32s) {
+        sl.ent = find_sweep_cl_f32s(kind);  // single-step launches only, as the other *_f32s kernels
+    } else {
+        sl.ent = find_sweep_cl(kind, pl.elem, 0);
+        sl.fused = find_sweep_cl(kind, pl.elem, 1);
+    }
     if (sl.ent.func && sl.ent.max_threads < sh.threads) sl.ent = SweepEntry{nullptr, nullptr, 0};
 }
 
@@ -912,6 +918,7 @@ void fill_slots(Handle *h)
     for (int t = 0; t < (h->has_alt ? 4 : 2); ++t) {
         DtypePlan &pl = t < 2 ? h->plan[t] : h->alt[t - 2];
         fill_cluster_slot(h, pl);
+        if (pl.elem == 8) fill_cluster_slot(h, pl, true);
         if (pl.elem == 8 && !h->periodic && !pl.two_pass && (pl.P == 1 || (pl.ws && pl.rows == 32))) {
             // fp32 storage, fp64 arithmetic: the plain solve kernels of the fp64 plan with a ring of floats
             const Shape &sh = pl.shape[0];
@@ -1079,7 +1086,7 @@ int make_tmap(CUtensorMap *tm, T *d_rhs, long long batch, int n, int W, unsigned
 // 17..32 partitions (512 < N <= 1024): one CTA keeps such a tile on 8 lanes = 128-byte row segments, the chain of two
 // CTAs on 256-byte ones.  Where the pair wins by default (measured on B200).
 template <typename T>
-bool cl_pays(int kind, const DtypePlan &pl, long long batch)
+bool cl_pays(int kind, const DtypePlan &pl, long long batch, size_t selem)
 {
     // measured on B200 (profiles/r02b_long_systems.md; one carry exchange per tile, sent with st.async): the pair keeps
     // 0.82-0.91 (tri) / 0.78-0.87 (penta, 32 partitions) of the HBM peak whatever the batch, while the single CTA's 128-byte
@@ -1087,7 +1094,10 @@ bool cl_pays(int kind, const DtypePlan &pl, long long batch)
     //   tri,   24-32 partitions (N > 736): pair from 4 MiB rows;  18-23 partitions: from 32 MiB rows (0.74-0.82 against 0.71)
     //   penta, 31-32 partitions (N > 960): pair from 8 MiB rows (0.87 / 0.78 against 0.78 / 0.69);  fewer: the pair loses
     if (pl.csz != 2) return false;
-    const size_t pitch = (size_t)batch * (size_t)pl.elem;
+    const size_t pitch = (size_t)batch * selem;
+    // fp32 storage with fp64 sweeps (*_f32s): the pair turns 64-byte segments into 128-byte ones -- at 32 partitions tri 0.57 -> 0.72
+    // at 2^19 systems, 0.36 -> 0.68 at 2^22, penta 0.46 -> 0.50, 0.36 -> 0.51; with fewer partitions it loses (N = 768: 0.57 -> 0.49)
+    if (selem != (size_t)pl.elem) return pl.PLc == 16 && pitch >= ((size_t)(kind == KIND_TRI ? 1 : 2) << 20);
     // (tri at 32 partitions: the pair's CTAs keep full 128 KB shares and hold their stores, launch_one -- 0.88-0.93 from 2^16
     //  systems on, never behind the single CTA's 0.87-0.91)
     if (kind == KIND_TRI) return (pl.PLc == 16 && pitch >= ((size_t)512 << 10)) || (pl.P >= 24 && pitch >= ((size_t)4 << 20)) || pitch >= ((size_t)32 << 20);
@@ -1115,7 +1125,7 @@ int launch_one(Handle *h, int kind, S *d_rhs, long long batch, double alpha_x, i
             return BTPS_OK;
         }
         if (MIXED) {  // the two-pass form writes g to global memory: in fp32 storage that would not be an fp64 solve
-            snprintf(tl_cuda_msg, sizeof(tl_cuda_msg), "fp32-storage solves need the on-chip plan (n <= 1024)");
+            snprintf(tl_cuda_msg, sizeof(tl_cuda_msg), "fp32-storage solves need an on-chip plan (n <= 4096, 16-byte aligned rows above 1024)");
             return set_err(BTPS_E_ARG);
         }
         T *const dr = (T *)(void *)d_rhs;  // (same type unless MIXED, which has returned above)
@@ -1162,10 +1172,11 @@ int launch_one(Handle *h, int kind, S *d_rhs, long long batch, double alpha_x, i
     // More than 32 partitions (N > 1024) have no other on-chip plan; for 17..32 partitions the default comes from
     // measurements on B200; btps_tune("cluster", 1) forces the chain for every eligible plan,
     // 0 switches it off.
-    const bool cl_default = (pl.P > 32) || cl_pays<T>(kind, pl, batch);
+    KernelSlot &clslot = MIXED ? pl.ck32 : pl.ck;
+    const bool cl_default = (pl.P > 32) || cl_pays<T>(kind, pl, batch, sizeof(S));
     const bool cl_wanted = (g_tune.cluster > 0) || (g_tune.cluster < 0 && cl_default);
-    const bool use_cl = !MIXED && (ks == 0) && (kind == KIND_TRI || kind == KIND_PENTA) && cl_wanted && pl.ck.ent.func && tma_ok &&
-                        (batch % pl.cshape.vec == 0);
+    const bool use_cl = (ks == 0) && (kind == KIND_TRI || kind == KIND_PENTA) && cl_wanted && clslot.ent.func && tma_ok &&
+                        (batch % pl.cshape.vec == 0) && !(MIXED && h->periodic);
     if (!use_cl && pl.two_pass) return two_pass();
     const Shape &sh = use_cl ? pl.cshape : pl.shape[ks];
     // the vectorised kernels need whole vectors: batch % vec == 0 and an aligned base pointer;
@@ -1180,7 +1191,7 @@ int launch_one(Handle *h, int kind, S *d_rhs, long long batch, double alpha_x, i
     int d = (tma_ok && slot_at(s, 0).ent.func) ? 0 : 1;
     if (!slot_at(s, d).ent.func && s == 0) s = 1;  // e.g. the wide variant has no direct-load twin that fits
     if (!slot_at(s, d).ent.func) d = 1;
-    KernelSlot &sl = use_cl ? pl.ck : slot_at(s, d);
+    KernelSlot &sl = use_cl ? clslot : slot_at(s, d);
     if (!sl.ent.func) return two_pass();
     {
         // takes the handle's lock: max_grid / prefer_fused are written by the first launch of this slot
@@ -1234,7 +1245,8 @@ int launch_one(Handle *h, int kind, S *d_rhs, long long batch, double alpha_x, i
         // cluster kernels: only the tridiagonal pair whose CTAs keep a full 128 KB share (32 partitions, N = 993 ... 1024) gains
         // -- 0.84 -> 0.90-0.93 from 2^19 systems, fp32 0.84 -> 0.92; shares of 96-112 KB (N = 768 / 896) lose 0-3 %, clusters of
         // 3 / 4 / 8 are indifferent or lose up to 10 %, the pentadiagonal pair is indifferent (profiles/r02b_long_systems.md)
-        const bool pair_tile = use_cl && kind == KIND_TRI && pl.csz == 2 && pl.PLc == 16 && a.num_tiles >= 8ll * (sl.max_grid / 2);
+        // (not with fp32 storage: its shares are 64 KB and held stores lose 6-17 % there)
+        const bool pair_tile = use_cl && !MIXED && kind == KIND_TRI && pl.csz == 2 && pl.PLc == 16 && a.num_tiles >= 8ll * (sl.max_grid / 2);
         a.hold_stores = g_tune.hold_stores >= 0 ? (g_tune.hold_stores > 0) : (((full_tile && (tri_family || penta_ok)) || pair_tile) ? 1 : 0);
     }
     a.blk = blk_stride(pl, h->kind == KIND_TRI ? (h->periodic ? 6 : 5) : (h->periodic ? (pl.wfast ? 11 : 13) : 9));  // = RecLayout<KIND>::ELEMS of the kernel

@@ -115,6 +115,7 @@ static SweepEntry pick_cl(int fuse)
 }
 SweepEntry find_sweep_cl(int kind, int elem_bytes, int fuse);
 SweepEntry find_sweep_f32s(int kind, int vec, int rows, int single, int tma, int ws);
+SweepEntry find_sweep_cl_f32s(int kind);
 SweepEntry find_sweep_cl_tri_f64(int fuse);
 SweepEntry find_sweep_cl_tri_f32(int fuse);
 SweepEntry find_sweep_cl_penta_f64(int fuse);

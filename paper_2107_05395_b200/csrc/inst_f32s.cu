@@ -1,5 +1,5 @@
 // inst_f32s.cu -- instantiations of sweep_kernel for fp32 storage with fp64 arithmetic (the *_f32s calls):
-// KIND_TRI / KIND_PENTA, 32 rows per thread, one or two systems per thread, single-step launches.
+// KIND_TRI / KIND_PENTA, 32 rows per thread, one or two systems per thread, single-step launches; also on clusters.
 #include "inst_common.cuh"
 
 namespace btps {
@@ -33,6 +33,14 @@ SweepEntry find_sweep_f32s(int kind, int vec, int rows, int single, int tma, int
         return vec == 2 ? pick_f32s_rows<2, KIND_TRI>(rows, single, tma, ws) : pick_f32s_rows<1, KIND_TRI>(rows, single, tma, ws);
     if (kind == KIND_PENTA)
         return vec == 2 ? pick_f32s_rows<2, KIND_PENTA>(rows, single, tma, ws) : pick_f32s_rows<1, KIND_PENTA>(rows, single, tma, ws);
+    return SweepEntry{nullptr, nullptr, 0};
+}
+
+// cluster-split variants (rows of a tile over 2 ... 8 CTAs): two systems per thread, 16 lanes = 128-byte row segments of floats
+SweepEntry find_sweep_cl_f32s(int kind)
+{
+    if (kind == KIND_TRI) return make_entry<double, 2, 32, false, KIND_TRI, true, true, false, true, float>();
+    if (kind == KIND_PENTA) return make_entry<double, 2, 32, false, KIND_PENTA, true, true, false, true, float>();
     return SweepEntry{nullptr, nullptr, 0};
 }
 

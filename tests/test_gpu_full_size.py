@@ -435,12 +435,44 @@ def test_f32_storage_full_size_sampled(lib, kind, n, lb):
     assert bool(torch.isfinite(d).all())
 
 
+@pytest.mark.parametrize("n", [1024, 1100, 1536, 2048, 3000, 4096])
+def test_f32_storage_on_clusters(lib, n):
+    """*_f32s on the cluster kernels: N > 1024 (default) and the pair at N = 1024 (forced), a ring of floats, fp64 sweeps and
+    fp64 carries across the CTAs.  Same bar as the single-CTA form: within one float ulp of the rounded fp64 solution."""
+    batch = 1024 + 32
+    lt, lp = inputs.tri_lhs(n, 0.5), inputs.penta_lhs(n, 0.5)
+    r32 = inputs.uniform_rhs(n, batch, seed=80 + n).astype(np.float32)
+    try:
+        if n <= 1024:
+            lib.btps_tune("cluster", 1)
+        ht, hp = lib.tri_factor(*lt), lib.penta_factor(*lp)
+        for kind in ("tri", "penta"):
+            ref = r32.astype(np.float64)
+            if kind == "tri":
+                oracle.tri_solve_interleaved(oracle.tri_factor(*lt), ref)
+            else:
+                oracle.penta_solve_interleaved(oracle.penta_factor(*lp), ref)
+            ref32 = ref.astype(np.float32).astype(np.float64)
+            h = ht if kind == "tri" else hp
+            tag = lib.btps_kernel_tag(h, 12, batch).split(", ")
+            assert tag[0] == "double" and tag[8] == "1" and tag[9] == "float", tag
+            d = torch.from_numpy(r32).cuda()
+            (lib.tri_solve_batched_f32s if kind == "tri" else lib.penta_solve_batched_f32s)(h, d)
+            got = d.cpu().numpy().astype(np.float64)
+            ulp = np.spacing(np.abs(ref32).astype(np.float32)).astype(np.float64)
+            assert np.all(np.abs(got - ref32) <= ulp + 1e-300), (n, kind)
+            assert rel_err(got, ref) <= TOL_F32S, (n, kind)
+    finally:
+        lib.btps_tune("cluster", -1)
+
+
 def test_f32_storage_rejects_what_it_does_not_cover(lib):
-    n = 2048
-    h = lib.tri_factor(*inputs.tri_lhs(n, 0.5))
-    d = torch.zeros(n, 64, dtype=torch.float32, device="cuda")
-    with pytest.raises(lib.BtpsError):
-        lib.tri_solve_batched_f32s(h, d)
+    # beyond the on-chip plans (N > 4096), and long systems whose row pitch TMA cannot take (not a multiple of 16 bytes)
+    for n, batch in ((5000, 64), (2048, 63)):
+        h = lib.tri_factor(*inputs.tri_lhs(n, 0.5))
+        d = torch.zeros(n, batch, dtype=torch.float32, device="cuda")
+        with pytest.raises(lib.BtpsError):
+            lib.tri_solve_batched_f32s(h, d)
     hp = lib.tri_factor_periodic(*inputs.tri_lhs(64, 0.5))
     d = torch.zeros(64, 64, dtype=torch.float32, device="cuda")
     with pytest.raises(lib.BtpsError):
