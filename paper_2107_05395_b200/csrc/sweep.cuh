@@ -550,14 +550,15 @@ sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
                 // c^n: nobody stores before the barriers below).
 #pragma unroll
                 for (int e = 0; e < V; ++e) cm[e] = cp[e] = T(0);
-                if (act && r0 > 0) ld_sys<T, V>(cm, p0 - batch);
+                // (r0 <= n: partitions that lie wholly beyond row n -- plans padded to whole cluster CTAs -- have no row r0-1)
+                if (act && r0 > 0 && r0 <= a.n) ld_sys<T, V>(cm, p0 - batch);
                 else if (WRAP && act) ld_sys<T, V>(cm, p0 + (long long)(a.n - 1) * batch);   // r0 == 0: row n-1
                 if (act && (r0 + MR < a.n)) ld_sys<T, V>(cp, p0 + (long long)MR * batch);
                 else if (WRAP && act) ld_sys<T, V>(cp, p0 - (long long)r0 * batch);          // row 0
                 if constexpr (HALO2) {
 #pragma unroll
                     for (int e = 0; e < V; ++e) cm2[e] = cp2[e] = T(0);
-                    if (act && r0 > 1) ld_sys<T, V>(cm2, p0 - 2 * batch);
+                    if (act && r0 > 1 && r0 <= a.n + 1) ld_sys<T, V>(cm2, p0 - 2 * batch);
                     else if (WRAP && act) ld_sys<T, V>(cm2, p0 + (long long)(a.n - 2) * batch);      // r0 == 0: row n-2
                     if (act && (r0 + MR + 1 < a.n)) ld_sys<T, V>(cp2, p0 + (long long)(MR + 1) * batch);
                     else if (WRAP && act) ld_sys<T, V>(cp2, p0 - (long long)(r0 - 1) * batch);       // row 1

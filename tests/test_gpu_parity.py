@@ -1219,3 +1219,30 @@ def test_cluster_pair_held_stores_bitwise_equal_and_against_oracle(lib):
     ref = rhs[:, ids].copy()
     oracle.tri_solve_interleaved(oracle.tri_factor(*lhs), ref, nsteps=4)
     assert rel_err(got[-1][0].cpu().numpy()[:, ids], ref) <= TOL_STEPS
+
+
+@pytest.mark.parametrize("n,batch", [(1056, 2344), (1835, 2276), (2048, 1027), (4000, 515)])
+def test_explicit_halves_on_plans_padded_to_whole_cluster_ctas(lib, n, batch):
+    """Above 1024 rows the partition count is padded to whole cluster CTAs (N = 1056: 33 -> 36 partitions).  The kinds with
+    an explicit half have no cluster form there and walk the carries serially with direct loads; their halo loads must not
+    reach for row r0 - 1 of a partition that lies wholly beyond row N (an out-of-bounds read that faulted at these sizes:
+    found by a randomised sweep of sizes against the oracle, fixed in sweep.cuh)."""
+    rhs = inputs.uniform_rhs(n, batch, seed=109)
+    _, al = inputs.ch_params(n)
+    x5 = np.array([-0.5, 2.0, -2.0, 2.0, -0.5])
+    lt, lp, lc = inputs.tri_lhs(n, 0.5), inputs.penta_lhs(n, 0.5), inputs.ch_lhs(n)
+    d = dev(0.1 * rhs)
+    lib.ch_step_batched(lib.penta_factor(*lc), d, al, 2)
+    ref = 0.1 * rhs
+    oracle.ch_step_interleaved(oracle.penta_factor(*lc), ref, al, nsteps=2)
+    assert rel_err(d.cpu().numpy(), ref) <= TOL_STEPS
+    d = dev(rhs)
+    lib.tri_cn_step_batched(lib.tri_factor(*lt), d, 0.5, 0.0, 0.5, 2)
+    ref = rhs.copy()
+    oracle.tri_cn_step_interleaved(oracle.tri_factor(*lt), ref, 0.5, 0.0, 0.5, nsteps=2)
+    assert rel_err(d.cpu().numpy(), ref) <= TOL_STEPS
+    d = dev(rhs)
+    lib.penta_cn_step_batched(lib.penta_factor(*lp), d, x5, 2)
+    ref = rhs.copy()
+    oracle.penta_cn_step_interleaved(oracle.penta_factor(*lp), ref, x5, nsteps=2)
+    assert rel_err(d.cpu().numpy(), ref) <= TOL_STEPS
