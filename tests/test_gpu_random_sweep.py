@@ -1,0 +1,156 @@
+"""Randomised sweep of the whole C-ABI against the oracle: sizes 1 ... 5000 (every plan: single partition, warp scan, cluster
+pair, clusters of 3-8 CTAs, serial walk, two-pass), batches 1 ... 3000 (aligned, ragged, unaligned), every call family,
+constant and general LHS, and the btps_tune keys that change which kernel or which storage of the tables is used.  Seeded
+(numpy Generator), so every run draws the same cases.  The same sweep run for ~21 000 cases found the out-of-bounds halo
+load that test_explicit_halves_on_plans_padded_to_whole_cluster_ctas pins.  Tolerances are BASELINE.json's (x 50 for the
+random, worse conditioned LHS)."""
+import numpy as np
+import pytest
+
+import inputs
+import oracle
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+
+KINDS = ["tri", "penta", "trip", "pentap", "ch", "chp", "tri32", "penta32", "tri32s", "penta32s", "tristeps", "pentasteps",
+         "tricn", "pentacn", "tricnp", "pentacnp", "chstat"]
+
+
+@pytest.fixture(scope="module")
+def lib():
+    if not torch.cuda.is_available():
+        pytest.fail("gpu tests need a CUDA device")
+    import paper_2107_05395_b200 as b
+    return b
+
+
+def rel(got, ref):
+    return float(np.max(np.abs(got - ref)) / max(np.max(np.abs(ref)), 1e-300))
+
+
+def rand_tri(n, rs):
+    a, c = rs.uniform(-1, 1, n), rs.uniform(-1, 1, n)
+    return a, (np.abs(a) + np.abs(c) + rs.uniform(0.5, 1.5, n)) * rs.choice([-1.0, 1.0], n), c
+
+
+def rand_penta(n, rs):
+    e, a, c, f = (rs.uniform(-1, 1, n) for _ in range(4))
+    d = np.abs(e) + np.abs(a) + np.abs(c) + np.abs(f) + rs.uniform(0.5, 1.5, n)
+    return e, a, d * rs.choice([-1.0, 1.0], n), c, f
+
+
+def one_case(b, rng):
+    """Draws one case, runs it on the GPU and in the oracle; returns (description, error, tolerance) or None if skipped."""
+    n = int(rng.choice([rng.integers(1, 70), rng.integers(70, 1100), rng.integers(1100, 4200),
+                        rng.choice([32, 64, 512, 544, 992, 1024, 1056, 2048, 4096, 4097, 5000])]))
+    batch = int(rng.choice([rng.integers(1, 40), rng.integers(40, 3000), 32 * rng.integers(1, 80), 4 * rng.integers(1, 600)]))
+    kind = str(rng.choice(KINDS))
+    const = bool(rng.random() < 0.6)
+    seed = int(rng.integers(1, 1 << 30))
+    tunes = {}
+    if rng.random() < 0.3:
+        tunes["cluster"] = int(rng.integers(0, 2))
+    if rng.random() < 0.2:
+        tunes["dedupe"] = int(rng.integers(0, 2))
+    if rng.random() < 0.2:
+        tunes["hold_stores"] = int(rng.integers(0, 2))
+    if (kind in ("trip", "tricnp") and n < 3) or (kind in ("pentap", "chp", "pentacnp", "chstat") and n < 5) or (kind == "ch" and n < 3):
+        return None
+    rs = np.random.default_rng(seed)
+    desc = (kind, n, batch, const, seed, tunes)
+    try:
+        for k, v in tunes.items():
+            b.btps_tune(k, v)
+        rhs = inputs.uniform_rhs(n, batch, seed=seed % 1000)
+        ref, tol = rhs.copy(), 1e-12
+        tri_l = inputs.tri_lhs(n, 0.5) if const else rand_tri(n, rs)
+        pen_l = inputs.penta_lhs(n, 0.5) if const else rand_penta(n, rs)
+        if kind == "tri":
+            d = torch.from_numpy(rhs).cuda()
+            b.tri_solve_batched(b.tri_factor(*tri_l), d)
+            oracle.tri_solve_interleaved(oracle.tri_factor(*tri_l), ref)
+        elif kind == "penta":
+            d = torch.from_numpy(rhs).cuda()
+            b.penta_solve_batched(b.penta_factor(*pen_l), d)
+            oracle.penta_solve_interleaved(oracle.penta_factor(*pen_l), ref)
+        elif kind == "trip":
+            d, tol = torch.from_numpy(rhs).cuda(), 1e-11
+            b.tri_solve_batched(b.tri_factor_periodic(*tri_l), d)
+            oracle.tri_periodic_solve_interleaved(oracle.tri_periodic_factor(*tri_l), ref)
+        elif kind == "pentap":
+            d, tol = torch.from_numpy(rhs).cuda(), 1e-11
+            b.penta_solve_batched(b.penta_factor_periodic(*pen_l), d)
+            oracle.penta_periodic_solve_interleaved(oracle.penta_periodic_factor(*pen_l), ref)
+        elif kind in ("ch", "chp", "chstat"):
+            lhs, (_, al) = inputs.ch_lhs(n), inputs.ch_params(n)
+            ref, ns, tol, const = 0.1 * rhs, int(rng.integers(1, 5)), 1e-10, True
+            d = torch.from_numpy(ref.copy()).cuda()
+            if kind == "ch":
+                b.ch_step_batched(b.penta_factor(*lhs), d, al, ns)
+                oracle.ch_step_interleaved(oracle.penta_factor(*lhs), ref, al, nsteps=ns)
+            elif kind == "chp":
+                b.ch_step_batched(b.penta_factor_periodic(*lhs), d, al, ns)
+                oracle.ch_periodic_step_interleaved(oracle.penta_periodic_factor(*lhs), ref, al, nsteps=ns)
+            else:
+                lb = torch.zeros(ns, dtype=torch.float64, device="cuda")
+                b.ch_step_batched_stat(b.penta_factor_periodic(*lhs), d, al, ns, lb)
+                want = oracle.ch_steps_with_lbar(oracle.penta_periodic_factor(*lhs), ref, al, ns, periodic=True)
+                assert rel(lb.cpu().numpy(), np.asarray(want)) <= 1e-10, desc
+        elif kind in ("tri32", "penta32", "tri32s", "penta32s"):
+            r32 = rhs.astype(np.float32)
+            ref, d = r32.astype(np.float64), torch.from_numpy(r32).cuda()
+            tol = 2e-5 if kind.endswith("32") else 1.2e-7
+            tri = kind.startswith("tri")
+            h = b.tri_factor(*tri_l) if tri else b.penta_factor(*pen_l)
+            fn = {"tri32": b.tri_solve_batched_f32, "penta32": b.penta_solve_batched_f32, "tri32s": b.tri_solve_batched_f32s,
+                  "penta32s": b.penta_solve_batched_f32s}[kind]
+            try:
+                fn(h, d)
+            except b.BtpsError:
+                assert kind.endswith("32s") and n > 1024, desc   # documented limits of the *_f32s calls
+                return None
+            if tri:
+                oracle.tri_solve_interleaved(oracle.tri_factor(*tri_l), ref)
+            else:
+                oracle.penta_solve_interleaved(oracle.penta_factor(*pen_l), ref)
+        elif kind in ("tricn", "tricnp"):
+            lhs, ns, tol, const = inputs.tri_lhs(n, 0.5), int(rng.integers(1, 6)), 1e-10, True
+            per = kind == "tricnp"
+            d = torch.from_numpy(rhs).cuda()
+            b.tri_cn_step_batched((b.tri_factor_periodic if per else b.tri_factor)(*lhs), d, 0.5, 0.0, 0.5, ns)
+            oracle.tri_cn_step_interleaved((oracle.tri_periodic_factor if per else oracle.tri_factor)(*lhs), ref, 0.5, 0.0, 0.5, nsteps=ns)
+        elif kind in ("pentacn", "pentacnp"):
+            lhs, ns, tol, const = inputs.penta_lhs(n, 0.5), int(rng.integers(1, 6)), 1e-10, True
+            per, x5 = kind == "pentacnp", np.array([-0.5, 2.0, -2.0, 2.0, -0.5])
+            d = torch.from_numpy(rhs).cuda()
+            b.penta_cn_step_batched((b.penta_factor_periodic if per else b.penta_factor)(*lhs), d, x5, ns)
+            oracle.penta_cn_step_interleaved((oracle.penta_periodic_factor if per else oracle.penta_factor)(*lhs), ref, x5, nsteps=ns)
+        else:
+            ns, tol = int(rng.integers(2, 70)), 1e-10
+            d = torch.from_numpy(rhs).cuda()
+            if kind == "tristeps":
+                b.tri_solve_steps(b.tri_factor(*tri_l), d, ns)
+                oracle.tri_solve_interleaved(oracle.tri_factor(*tri_l), ref, nsteps=ns)
+            else:
+                b.penta_solve_steps(b.penta_factor(*pen_l), d, ns)
+                oracle.penta_solve_interleaved(oracle.penta_factor(*pen_l), ref, nsteps=ns)
+        torch.cuda.synchronize()
+        return desc, rel(d.cpu().numpy().astype(np.float64), ref), tol * (1 if const else 50)
+    finally:
+        for k in tunes:
+            b.btps_tune(k, -1)
+
+
+@pytest.mark.parametrize("seed", [1, 2, 3])
+def test_random_sweep_against_oracle(lib, seed):
+    rng = np.random.default_rng(seed)
+    done, bad = 0, []
+    while done < 160:
+        r = one_case(lib, rng)
+        if r is None:
+            continue
+        done += 1
+        if not r[1] <= r[2]:
+            bad.append(r)
+    assert not bad, bad
