@@ -529,6 +529,12 @@ sweep_kernel(const SweepArgs a, const __grid_constant__ CUtensorMap tmap)
                     }
                 }
             }
+            // The ring is about to be overwritten by the TMA unit (async proxy) while these loads went through the generic
+            // proxy: every thread orders its own reads before that write with a proxy fence, then the group meets.  Without
+            // it a one-warp group (__syncwarp does not wait for outstanding shared-memory loads) could have loads of this
+            // tile still queued behind seven other groups' when the next tile arrived from L2: wrong tiles now and then on
+            // L2-resident batches with eight groups per CTA (N = 64, found by the randomised sweep against the oracle).
+            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
             group_sync(a.tpc, sub, tpt);  // every thread has drained the ring
             if (lt == 0 && t + stride_tiles < ntiles) tma_issue(t + stride_tiles);
         } else {

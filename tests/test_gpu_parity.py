@@ -1246,3 +1246,29 @@ def test_explicit_halves_on_plans_padded_to_whole_cluster_ctas(lib, n, batch):
     ref = rhs.copy()
     oracle.penta_cn_step_interleaved(oracle.penta_factor(*lp), ref, x5, nsteps=2)
     assert rel_err(d.cpu().numpy(), ref) <= TOL_STEPS
+
+
+@pytest.mark.parametrize("n", [64, 58, 40])
+def test_one_warp_groups_reuse_their_ring_on_an_l2_resident_batch(lib, n):
+    """N <= 64 runs eight one-warp tile groups per CTA, each with its own one-tile TMA ring.  On few CTAs every group walks
+    many tiles, and on a batch that stays in L2 the next tile can arrive within a microsecond of being asked for -- while
+    this tile's shared-memory loads (generic proxy) are still queued behind the other groups'.  The kernels order those
+    reads before the TMA write with fence.proxy.async; without it this test failed in nearly every repetition (wrong
+    tiles now and then, found by a randomised sweep against the oracle)."""
+    batch, steps = 13632, 40
+    lhs = inputs.tri_lhs(n, 0.5)
+    rhs = inputs.uniform_rhs(n, batch, seed=383)
+    ref = rhs.copy()
+    oracle.tri_solve_interleaved(oracle.tri_factor(*lhs), ref, nsteps=steps)
+    try:
+        lib.btps_tune("grid", 3)
+        lib.btps_tune("fuse_steps", 1)      # one launch per step: 40 launches over the same 7 MB
+        h = lib.tri_factor(*lhs)
+        assert lib.btps_plan_info(h, 8)["tma_prefetch"] == 1 and lib.btps_plan_info(h, 8)["tiles_per_cta"] >= 4
+        for rep in range(4):
+            d = dev(rhs)
+            lib.tri_solve_steps(h, d, steps)
+            assert rel_err(d.cpu().numpy(), ref) <= TOL_STEPS, rep
+    finally:
+        lib.btps_tune("grid", -1)
+        lib.btps_tune("fuse_steps", -1)
