@@ -56,7 +56,7 @@ std::atomic<long long> g_launches{0};
 // ------------------------------------------------------------------------------------------------
 struct Tune {
     int rows = -1, lanes = -1, vec = -1, tpc = -1, force_two_pass = -1, reverse = -1, prefetch = -1, pdl = -1,
-        warp_scan = -1, grid = -1, fuse = -1, cluster = -1, blk_pad = -1, cyclic_scan = -1, one_step_fused = -1, host_chunk_kib = -1, hold_stores = -1, dedupe = -1;
+        warp_scan = -1, grid = -1, fuse = -1, cluster = -1, blk_pad = -1, cyclic_scan = -1, one_step_fused = -1, host_chunk_kib = -1, hold_stores = -1, dedupe = -1, narrow = -1;
 };
 Tune g_tune;
 
@@ -113,6 +113,10 @@ struct DtypePlan {
     unsigned char pmap[MAX_PARTS] = {0};
     Shape cshape;
     KernelSlot ck;
+    // long fused time loops of plans whose partitions share coefficient blocks (fp64): half-width tiles (8 lanes), so that a
+    // CTA hosts two or four tile groups whose phases overlap (fill_slots, launch_one); kn[ks].fused.func == nullptr: none
+    Shape nshape[3];
+    KernelSlot kn[3];
     KernelSlot ck32;  // fp64 plan only: the cluster kernels on fp32 storage (the *_f32s calls); same shape, a ring of floats
 };
 
@@ -980,6 +984,29 @@ void fill_slots(Handle *h)
                     if (sl.ent.func && sl.tma && can_fuse) sl.fused = find_sweep(kind, pl.elem, sl.vec, pl.rows, single, 1, pl.ws, 1);
                 }
             }
+            // Half-width tiles for long fused loops (same kernels, lanes = 8): with shared coefficient blocks the four
+            // partitions of a warp read one address, and two (four) half-size groups per CTA overlap one group's carry scan
+            // and barriers with the other's sweeps.  Which calls use it: launch_one (narrow_pays).
+            pl.kn[ks] = KernelSlot();
+            {
+                const KernelSlot &base = pl.k[ks][0][0];
+                if (pl.elem == 8 && pl.ws && pl.rows == 32 && pl.nuniq < pl.P && base.fused.func && sh.lanes == 16 && sh.vec == 2 &&
+                    (pl.P * 8) % 32 == 0 && g_tune.lanes < 0 && g_tune.tpc < 0) {
+                    Shape &nsh = pl.nshape[ks];
+                    nsh = sh;
+                    nsh.lanes = 8;
+                    nsh.lanes_log2 = 3;
+                    finish_shape(pl.elem, pl.rows, pl.P, nsh);
+                    KernelSlot &nk = pl.kn[ks];
+                    nk.vec = base.vec;
+                    nk.tma = 1;
+                    layout_slot(pl, nsh, kind, nk);
+                    if (nsh.tpc >= 2 && nk.smem <= SMEM_LIMIT && base.fused.max_threads >= nsh.threads) {
+                        nk.ent = base.ent;
+                        nk.fused = base.fused;
+                    }
+                }
+            }
         }
     }
 }
@@ -1105,11 +1132,16 @@ bool cl_pays(int kind, const DtypePlan &pl, long long batch, size_t selem)
     return false;
 }
 
+// calls that advance at least this many time steps keep 17..32 partitions on one CTA (launch_one)
+constexpr int LOOP_STEPS_SINGLE_CTA = 4;
+
 // one sweep launch (kind = KIND_TRI / KIND_PENTA / KIND_CH) on a device buffer
 template <typename T, typename S = T>
 int launch_one(Handle *h, int kind, S *d_rhs, long long batch, double alpha_x, int reverse, int ksteps,
-               cudaStream_t st, double *stat = nullptr, const double *ex = nullptr, const char **tag_out = nullptr)
+               cudaStream_t st, double *stat = nullptr, const double *ex = nullptr, const char **tag_out = nullptr,
+               int call_steps = 0)
 {
+    if (call_steps < ksteps) call_steps = ksteps;  // time steps of the whole call this launch belongs to
     constexpr bool MIXED = !std::is_same<T, S>::value;  // fp32 in HBM, fp64 arithmetic: plain solves of the fp64 plan
     // (the single-step plain solve of a 32-partition pentadiagonal handle runs on its own unshared blob: make_penta_handle)
     const bool own_blocks = h->has_alt && kind == KIND_PENTA && ksteps == 1 && !stat;
@@ -1173,17 +1205,21 @@ int launch_one(Handle *h, int kind, S *d_rhs, long long batch, double alpha_x, i
     // measurements on B200; btps_tune("cluster", 1) forces the chain for every eligible plan,
     // 0 switches it off.
     KernelSlot &clslot = MIXED ? pl.ck32 : pl.ck;
-    const bool cl_default = (pl.P > 32) || cl_pays<T>(kind, pl, batch, sizeof(S));
+    // (time loops: a tile that stays on chip for several steps is read and written once per launch, so the width of its row
+    //  segments no longer decides, and per step the single CTA is the faster one -- N = 1024, 128 steps per call, us per step:
+    //  tri 53.3 against the pair's 64.3 at 2^16 systems, 838 against 1013 at 2^20; penta 1465 against 1811 at 2^20.  Decided
+    //  per CALL, not per launch, so that every launch of one loop runs the same kernel whatever the steps per launch.)
+    const bool cl_default = (pl.P > 32) || (call_steps < LOOP_STEPS_SINGLE_CTA && cl_pays<T>(kind, pl, batch, sizeof(S)));
     const bool cl_wanted = (g_tune.cluster > 0) || (g_tune.cluster < 0 && cl_default);
     const bool use_cl = (ks == 0) && (kind == KIND_TRI || kind == KIND_PENTA) && cl_wanted && clslot.ent.func && tma_ok &&
                         (batch % pl.cshape.vec == 0) && !(MIXED && h->periodic);
     if (!use_cl && pl.two_pass) return two_pass();
-    const Shape &sh = use_cl ? pl.cshape : pl.shape[ks];
+    const Shape &sh0 = use_cl ? pl.cshape : pl.shape[ks];
     // the vectorised kernels need whole vectors: batch % vec == 0 and an aligned base pointer;
     // TMA needs a 16-byte aligned base and row pitch
     int s = 0;
-    if (sh.vec > 1) {
-        const bool ok = (batch % sh.vec == 0) && (((uintptr_t)d_rhs % (sizeof(S) * sh.vec)) == 0);
+    if (sh0.vec > 1) {
+        const bool ok = (batch % sh0.vec == 0) && (((uintptr_t)d_rhs % (sizeof(S) * sh0.vec)) == 0);
         if (!ok) s = 1;
     }
     auto slot_at = [&](int sv, int dv) -> KernelSlot & { return MIXED ? pl.ks32[sv][dv] : pl.k[ks][sv][dv]; };
@@ -1191,7 +1227,16 @@ int launch_one(Handle *h, int kind, S *d_rhs, long long batch, double alpha_x, i
     int d = (tma_ok && slot_at(s, 0).ent.func) ? 0 : 1;
     if (!slot_at(s, d).ent.func && s == 0) s = 1;  // e.g. the wide variant has no direct-load twin that fits
     if (!slot_at(s, d).ent.func) d = 1;
-    KernelSlot &sl = use_cl ? clslot : slot_at(s, d);
+    // Long fused loops on half-width tiles (fill_slots).  Measured on B200 (128 steps per call, us per step, 16 -> 8 lanes):
+    // tri N = 512 / 256 at 2^16 systems 25.5 -> 24.5 / 12.2 -> 11.9, N = 256 at 2^20 191 -> 184; Cahn-Hilliard N = 256 at 2^16 /
+    // 2^20 26.9 -> 25.6 / 424 -> 404, periodic 540 -> 527; everything else within +-1 % or slower (N = 128: + 5-17 %, plain
+    // and periodic penta + 0-3 %, periodic tri N = 512 + 5 %), so only those.  A launch's load and store are slower on the
+    // 128-byte segments, hence only launches of 16 or more steps.  Same arithmetic per system: the results are bitwise equal.
+    const bool narrow_pays = (kind == KIND_TRI && !h->periodic && pl.P >= 8 && pl.P <= 16) || (kind == KIND_CH && pl.P >= 8 && pl.P <= 12);
+    const bool narrow = !use_cl && !MIXED && s == 0 && d == 0 && ksteps >= 16 && narrow_pays && pl.kn[ks].fused.func &&
+                        g_tune.lanes < 0 && g_tune.tpc < 0 && g_tune.narrow != 0;
+    const Shape &sh = narrow ? pl.nshape[ks] : sh0;
+    KernelSlot &sl = use_cl ? clslot : (narrow ? pl.kn[ks] : slot_at(s, d));
     if (!sl.ent.func) return two_pass();
     {
         // takes the handle's lock: max_grid / prefer_fused are written by the first launch of this slot
@@ -1345,7 +1390,7 @@ int solve_steps(const void *hv, int magic, int kind, S *d_rhs, int64_t batch, do
     for (int s = 0, l = 0; s < nsteps; ++l) {
         const int k = (nsteps - s < kmax) ? (nsteps - s) : kmax;
         const int rc = launch_one<T, S>(h, kind, d_rhs, batch, alpha_x, rev ? (l & 1) : 0, k, (cudaStream_t)stream,
-                                        d_stat ? d_stat + s : nullptr, ex);
+                                        d_stat ? d_stat + s : nullptr, ex, nullptr, nsteps);
         if (rc != BTPS_OK) return rc;
         s += k;
     }
@@ -1450,7 +1495,7 @@ int solve_host(const void *hv, int magic, int kind, T *h_rhs, int64_t batch, dou
         const int kmax = fuse_limit(h->plan[sizeof(T) == 8 ? 0 : 1]);
         for (int s = 0, l = 0; s < nsteps && rc == BTPS_OK; ++l) {
             const int k = (nsteps - s < kmax) ? (nsteps - s) : kmax;
-            rc = launch_one<T>(h, kind, d, w, alpha_x, rev ? (l & 1) : 0, k, st);
+            rc = launch_one<T>(h, kind, d, w, alpha_x, rev ? (l & 1) : 0, k, st, nullptr, nullptr, nullptr, nsteps);
             s += k;
         }
         if (rc != BTPS_OK) break;
@@ -1949,6 +1994,7 @@ int btps_tune(const char *key, int value)
     else if (!strcmp(key, "hold_stores")) g_tune.hold_stores = value;
     else if (!strcmp(key, "dedupe")) g_tune.dedupe = value;
     else if (!strcmp(key, "blk_pad")) g_tune.blk_pad = value;
+    else if (!strcmp(key, "narrow_loops")) g_tune.narrow = value;
     else return set_err(BTPS_E_ARG);
     return set_err(BTPS_OK);
 }

@@ -546,6 +546,44 @@ def test_fused_steps_equal_single_step_launches(lib, n, batch):
     assert rel_err(outs[-1][2], ref) <= TOL_STEPS
 
 
+@pytest.mark.parametrize("n,batch", [(512, 148 * 16 * 3 + 48), (256, 9000), (384, 4100)])
+def test_long_fused_loops_on_half_width_tiles(lib, n, batch):
+    """Launches of 16 or more fused steps of the plain tridiagonal loop and of the Cahn-Hilliard step run on half-width
+    tiles (8 lanes, two or four tile groups per CTA) when the partitions share their coefficient blocks
+    (btps_tune narrow_loops = 0 keeps the full-width tiles).  Same arithmetic per system: bitwise equal results, several
+    tiles per group, a ragged last tile; and both match the oracle's loop.  40 steps: one launch; 70 steps: 64 on
+    half-width tiles + 6 on full-width ones."""
+    lt, lc = inputs.tri_lhs(n, 0.5), inputs.ch_lhs(n)
+    _, al = inputs.ch_params(n)
+    rhs = inputs.uniform_rhs(n, batch, seed=91)
+    c0 = 0.1 * rhs
+    for steps in (40, 70):
+        outs = {}
+        for narrow in (-1, 0):
+            try:
+                lib.btps_tune("narrow_loops", narrow)
+                ht, hc, hcp = lib.tri_factor(*lt), lib.penta_factor(*lc), lib.penta_factor_periodic(*lc)
+                a, b_, c = dev(rhs), dev(c0), dev(c0)
+                lib.tri_solve_steps(ht, a, steps)
+                lib.ch_step_batched(hc, b_, al, steps)
+                lib.ch_step_batched(hcp, c, al, steps)
+                outs[narrow] = [x.cpu().numpy() for x in (a, b_, c)]
+            finally:
+                lib.btps_tune("narrow_loops", -1)
+        for x, y in zip(outs[-1], outs[0]):
+            assert np.array_equal(x, y)
+        if steps == 40:
+            ref = rhs.copy()
+            oracle.tri_solve_interleaved(oracle.tri_factor(*lt), ref, nsteps=steps)
+            assert rel_err(outs[-1][0], ref) <= TOL_STEPS
+            ref = c0.copy()
+            oracle.ch_step_interleaved(oracle.penta_factor(*lc), ref, al, nsteps=steps)
+            assert rel_err(outs[-1][1], ref) <= TOL_STEPS
+            ref = c0.copy()
+            oracle.ch_periodic_step_interleaved(oracle.penta_periodic_factor(*lc), ref, al, nsteps=steps)
+            assert rel_err(outs[-1][2], ref) <= TOL_STEPS
+
+
 # ---- periodic tridiagonal (Sherman-Morrison, PAPER.md:140-164) ---------------------------------------
 
 def rand_cyclic(n, seed):
@@ -1189,6 +1227,38 @@ def test_default_cluster_policy_by_row_pitch(lib):
     for n in (1100, 2048, 4096):
         assert cl(lib.tri_factor(*inputs.tri_lhs(n, 0.5)), 8, 1 << 10) and cl(lib.penta_factor(*inputs.penta_lhs(n, 0.5)), 4, 1 << 10)
     assert not cl(ht, 8, (1 << 16) + 1)                                               # unaligned pitch: no TMA, no cluster
+    # time loops (calls of 4 or more steps) keep up to 32 partitions on one CTA; above 1024 rows there is only the cluster plan
+    def cl_steps(h, batch, nsteps):
+        return lib.btps_kernel_tag(h, 8, batch, nsteps).split(", ")[8] == "1"
+    assert cl_steps(ht, 1 << 22, 3) and not cl_steps(ht, 1 << 22, 4) and not cl_steps(ht, 1 << 16, 100)
+    assert cl_steps(hp, 1 << 20, 2) and not cl_steps(hp, 1 << 20, 64)
+    assert cl_steps(lib.tri_factor(*inputs.tri_lhs(2048, 0.5)), 1 << 12, 100)
+
+
+def test_time_loops_of_long_rows_stay_on_one_cta(lib):
+    """N = 1024 at 2^16 systems: a single solve runs on the cluster pair (256-byte row segments), a time loop on one CTA per
+    tile (faster per step once the tile stays on chip).  The choice is made per call: every launch of one loop runs the same
+    kernel, so fused and per-step launches stay bitwise equal, and the loop matches the oracle's."""
+    n, batch, steps = 1024, 1 << 16, 5
+    lt = inputs.tri_lhs(n, 0.5)
+    rhs = inputs.uniform_rhs(n, batch, seed=77)
+    h = lib.tri_factor(*lt)
+    assert lib.btps_kernel_tag(h, 8, batch, 1).split(", ")[8] == "1"
+    assert lib.btps_kernel_tag(h, 8, batch, steps).split(", ")[8] == "0"
+    outs = []
+    for fuse in (-1, 1):
+        try:
+            lib.btps_tune("fuse_steps", fuse)
+            d = dev(rhs)
+            lib.tri_solve_steps(h, d, steps)
+            outs.append(d.cpu().numpy())
+            del d
+        finally:
+            lib.btps_tune("fuse_steps", -1)
+    assert np.array_equal(outs[0], outs[1])
+    ref = rhs.copy()
+    oracle.tri_solve_interleaved(oracle.tri_factor(*lt), ref, nsteps=steps)
+    assert rel_err(outs[0], ref) <= TOL_STEPS
 
 
 def test_cluster_pair_held_stores_bitwise_equal_and_against_oracle(lib):
