@@ -55,6 +55,8 @@ def one_case(b, rng):
         tunes["dedupe"] = int(rng.integers(0, 2))
     if rng.random() < 0.2:
         tunes["hold_stores"] = int(rng.integers(0, 2))
+    if rng.random() < 0.15:
+        tunes["grid"] = int(rng.integers(1, 9))   # few CTAs: many tiles per tile group
     if (kind in ("trip", "tricnp") and n < 3) or (kind in ("pentap", "chp", "pentacnp", "chstat") and n < 5) or (kind == "ch" and n < 3):
         return None
     rs = np.random.default_rng(seed)
@@ -83,8 +85,12 @@ def one_case(b, rng):
             b.penta_solve_batched(b.penta_factor_periodic(*pen_l), d)
             oracle.penta_periodic_solve_interleaved(oracle.penta_periodic_factor(*pen_l), ref)
         elif kind in ("ch", "chp", "chstat"):
-            lhs, (_, al) = inputs.ch_lhs(n), inputs.ch_params(n)
-            ref, ns, tol, const = 0.1 * rhs, int(rng.integers(1, 5)), 1e-10, True
+            lhs, (sig, al) = inputs.ch_lhs(n), inputs.ch_params(n)
+            # (1-4 steps, or a launch long enough for the half-width tiles of long fused loops)
+            ref, ns, tol, const = 0.1 * rhs, int(rng.choice([rng.integers(1, 5), rng.integers(16, 40)])), 1e-10, True
+            # the CH matrix I + sigma D4 has sigma = g dt / dx^4 ~ N^4 (cond ~ 1 + 16 sigma: 5.6e3 at N = 1024, 1.6e6 at N = 4172):
+            # beyond BASELINE's sizes the bound is rounding x cond (reading C-33)
+            tol = max(tol, 16 * 2.2e-16 * (1 + 16 * sig))
             d = torch.from_numpy(ref.copy()).cuda()
             if kind == "ch":
                 b.ch_step_batched(b.penta_factor(*lhs), d, al, ns)
@@ -96,7 +102,7 @@ def one_case(b, rng):
                 lb = torch.zeros(ns, dtype=torch.float64, device="cuda")
                 b.ch_step_batched_stat(b.penta_factor_periodic(*lhs), d, al, ns, lb)
                 want = oracle.ch_steps_with_lbar(oracle.penta_periodic_factor(*lhs), ref, al, ns, periodic=True)
-                assert rel(lb.cpu().numpy(), np.asarray(want)) <= 1e-10, desc
+                assert rel(lb.cpu().numpy(), np.asarray(want)) <= tol, desc
         elif kind in ("tri32", "penta32", "tri32s", "penta32s"):
             r32 = rhs.astype(np.float32)
             ref, d = r32.astype(np.float64), torch.from_numpy(r32).cuda()
