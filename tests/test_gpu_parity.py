@@ -567,11 +567,19 @@ def test_long_fused_loops_on_half_width_tiles(lib, n, batch):
                 lib.tri_solve_steps(ht, a, steps)
                 lib.ch_step_batched(hc, b_, al, steps)
                 lib.ch_step_batched(hcp, c, al, steps)
-                outs[narrow] = [x.cpu().numpy() for x in (a, b_, c)]
+                # the same loop with the coarsening statistic of eq. 30 recorded inside the kernel
+                e, lb = dev(c0), torch.zeros(steps, dtype=torch.float64, device="cuda")
+                lib.ch_step_batched_stat(hcp, e, al, steps, lb)
+                outs[narrow] = [x.cpu().numpy() for x in (a, b_, c, e, lb)]
             finally:
                 lib.btps_tune("narrow_loops", -1)
-        for x, y in zip(outs[-1], outs[0]):
+        for x, y in zip(outs[-1][:4], outs[0][:4]):
             assert np.array_equal(x, y)
+        assert np.array_equal(outs[-1][2], outs[-1][3])
+        assert rel_err(outs[-1][4], outs[0][4]) <= 1e-12  # (the order of the sum over the runs is not fixed)
+        if steps == 40:
+            want = oracle.ch_steps_with_lbar(oracle.penta_periodic_factor(*lc), c0.copy(), al, steps, periodic=True)
+            assert rel_err(outs[-1][4], np.asarray(want)) <= TOL_STEPS
         if steps == 40:
             ref = rhs.copy()
             oracle.tri_solve_interleaved(oracle.tri_factor(*lt), ref, nsteps=steps)
