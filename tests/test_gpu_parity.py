@@ -548,12 +548,14 @@ def test_fused_steps_equal_single_step_launches(lib, n, batch):
 
 @pytest.mark.parametrize("n,batch", [(512, 148 * 16 * 3 + 48), (256, 9000), (384, 4100)])
 def test_long_fused_loops_on_half_width_tiles(lib, n, batch):
-    """Launches of 16 or more fused steps of the plain tridiagonal loop and of the Cahn-Hilliard step run on half-width
+    """Launches of 16 or more fused steps of the plain tridiagonal loop, of the Cahn-Hilliard step and of the Crank-Nicolson
+    steps run on half-width
     tiles (8 lanes, two or four tile groups per CTA) when the partitions share their coefficient blocks
     (btps_tune narrow_loops = 0 keeps the full-width tiles).  Same arithmetic per system: bitwise equal results, several
     tiles per group, a ragged last tile; and both match the oracle's loop.  40 steps: one launch; 70 steps: 64 on
     half-width tiles + 6 on full-width ones."""
-    lt, lc = inputs.tri_lhs(n, 0.5), inputs.ch_lhs(n)
+    lt, lc, lp = inputs.tri_lhs(n, 0.5), inputs.ch_lhs(n), inputs.penta_lhs(n, 0.5)
+    x5 = np.array([-0.5, 2.0, -2.0, 2.0, -0.5])
     _, al = inputs.ch_params(n)
     rhs = inputs.uniform_rhs(n, batch, seed=91)
     c0 = 0.1 * rhs
@@ -570,11 +572,26 @@ def test_long_fused_loops_on_half_width_tiles(lib, n, batch):
                 # the same loop with the coarsening statistic of eq. 30 recorded inside the kernel
                 e, lb = dev(c0), torch.zeros(steps, dtype=torch.float64, device="cuda")
                 lib.ch_step_batched_stat(hcp, e, al, steps, lb)
-                outs[narrow] = [x.cpu().numpy() for x in (a, b_, c, e, lb)]
+                # Crank-Nicolson diffusion / hyperdiffusion steps (eq. 9-11, 17-19), truncated and periodic
+                cn = []
+                for per in (False, True):
+                    f, g = dev(rhs), dev(rhs)
+                    lib.tri_cn_step_batched((lib.tri_factor_periodic if per else lib.tri_factor)(*lt), f, 0.5, 0.0, 0.5, steps)
+                    lib.penta_cn_step_batched((lib.penta_factor_periodic if per else lib.penta_factor)(*lp), g, x5, steps)
+                    cn += [f.cpu().numpy(), g.cpu().numpy()]
+                outs[narrow] = [x.cpu().numpy() for x in (a, b_, c, e, lb)] + cn
             finally:
                 lib.btps_tune("narrow_loops", -1)
-        for x, y in zip(outs[-1][:4], outs[0][:4]):
+        for x, y in zip(outs[-1][:4] + outs[-1][5:], outs[0][:4] + outs[0][5:]):
             assert np.array_equal(x, y)
+        if steps == 40:
+            for per in (False, True):
+                ref = rhs.copy()
+                oracle.tri_cn_step_interleaved((oracle.tri_periodic_factor if per else oracle.tri_factor)(*lt), ref, 0.5, 0.0, 0.5, nsteps=steps)
+                assert rel_err(outs[-1][5 + 2 * per], ref) <= TOL_STEPS
+                ref = rhs.copy()
+                oracle.penta_cn_step_interleaved((oracle.penta_periodic_factor if per else oracle.penta_factor)(*lp), ref, x5, nsteps=steps)
+                assert rel_err(outs[-1][6 + 2 * per], ref) <= TOL_STEPS
         assert np.array_equal(outs[-1][2], outs[-1][3])
         assert rel_err(outs[-1][4], outs[0][4]) <= 1e-12  # (the order of the sum over the runs is not fixed)
         if steps == 40:

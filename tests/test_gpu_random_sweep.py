@@ -121,13 +121,13 @@ def one_case(b, rng):
             else:
                 oracle.penta_solve_interleaved(oracle.penta_factor(*pen_l), ref)
         elif kind in ("tricn", "tricnp"):
-            lhs, ns, tol, const = inputs.tri_lhs(n, 0.5), int(rng.integers(1, 6)), 1e-10, True
+            lhs, ns, tol, const = inputs.tri_lhs(n, 0.5), int(rng.choice([rng.integers(1, 6), rng.integers(16, 40)])), 1e-10, True
             per = kind == "tricnp"
             d = torch.from_numpy(rhs).cuda()
             b.tri_cn_step_batched((b.tri_factor_periodic if per else b.tri_factor)(*lhs), d, 0.5, 0.0, 0.5, ns)
             oracle.tri_cn_step_interleaved((oracle.tri_periodic_factor if per else oracle.tri_factor)(*lhs), ref, 0.5, 0.0, 0.5, nsteps=ns)
         elif kind in ("pentacn", "pentacnp"):
-            lhs, ns, tol, const = inputs.penta_lhs(n, 0.5), int(rng.integers(1, 6)), 1e-10, True
+            lhs, ns, tol, const = inputs.penta_lhs(n, 0.5), int(rng.choice([rng.integers(1, 6), rng.integers(16, 40)])), 1e-10, True
             per, x5 = kind == "pentacnp", np.array([-0.5, 2.0, -2.0, 2.0, -0.5])
             d = torch.from_numpy(rhs).cuda()
             b.penta_cn_step_batched((b.penta_factor_periodic if per else b.penta_factor)(*lhs), d, x5, ns)
