@@ -66,7 +66,8 @@ def parse_args():
     ap.add_argument("--side-file", default=os.path.join(ROOT, SIDE_FILE))
     ap.add_argument("--cell", action="append", default=[], metavar="KIND,N,LOG2BATCH,DTYPE",
                     help="time one cell instead of the headline step, e.g. tri,1024,19,f64 (kinds: tri, penta, ch, "
-                         "tri_periodic, penta_periodic, ch_periodic); may be repeated")
+                         "tri_periodic, penta_periodic, ch_periodic, tri_f32s, penta_f32s, tri_cn[_periodic], penta_cn[_periodic]); "
+                         "may be repeated")
     ap.add_argument("--tune", action="append", default=[], metavar="KEY=VALUE", help="btps_tune setting applied first")
     ap.add_argument("--cell-steps", type=int, default=1, help="--cell: time steps per call (tri/penta_solve_steps, ch_step_batched)")
     ap.add_argument("--rotate", type=int, default=0, help="--cell: rotate over this many buffers (default: as many as keep the cell cold)")
@@ -320,7 +321,7 @@ def time_in_graph(torch, fn_of_buf, bufs, launches, repeats=3):
 
 
 KIND_INDEX = {"tri": 0, "tri_periodic": 0, "tri_f32s": 0, "penta": 1, "penta_periodic": 1, "penta_f32s": 1, "ch": 2,
-              "ch_periodic": 2}
+              "ch_periodic": 2, "tri_cn": 3, "tri_cn_periodic": 3, "penta_cn": 4, "penta_cn_periodic": 4}
 
 
 def make_cell(torch, b, inputs, kind, n, batch, elem, steps_per_call=1, rotate=0):
@@ -351,6 +352,15 @@ def make_cell(torch, b, inputs, kind, n, batch, elem, steps_per_call=1, rotate=0
         one = b.penta_solve_batched if elem == 8 else b.penta_solve_batched_f32
         fn = (lambda t, s=None: one(h, t, s)) if steps_per_call == 1 else \
             (lambda t, s=None: b.penta_solve_steps(h, t, steps_per_call, s))
+    elif kind in ("tri_cn", "tri_cn_periodic"):
+        # Crank-Nicolson diffusion step (eq. 9-11; periodic: the scheme of the paper's Table 1), sigma = 0.5
+        h = (b.tri_factor if kind == "tri_cn" else b.tri_factor_periodic)(*inputs.tri_lhs(n, 0.5))
+        fn = lambda t, s=None: b.tri_cn_step_batched(h, t, 0.5, 0.0, 0.5, steps_per_call, s)
+    elif kind in ("penta_cn", "penta_cn_periodic"):
+        # Crank-Nicolson hyperdiffusion step (eq. 17-19; periodic: Table 2's scheme), sigma = 0.5
+        h = (b.penta_factor if kind == "penta_cn" else b.penta_factor_periodic)(*inputs.penta_lhs(n, 0.5))
+        x5 = [-0.5, 2.0, -2.0, 2.0, -0.5]
+        fn = lambda t, s=None: b.penta_cn_step_batched(h, t, x5, steps_per_call, s)
     else:
         h = b.penta_factor(*inputs.ch_lhs(n)) if kind == "ch" else b.penta_factor_periodic(*inputs.ch_lhs(n))
         _, alpha = inputs.ch_params(n)
@@ -487,7 +497,8 @@ def run_cells(args):
         print(json.dumps({"cell": cell, "tune": args.tune, "steps_per_call": ks, "ms": round(ms, 5), "hbm_gbs": round(gbs, 1),
                           "frac": round(gbs / peak, 4),
                           "kernel": b.btps_kernel_tag(h, 12 if kind.endswith("f32s") else elem, batch, ks, kind=kidx),
-                          "plan": h.ch_plan(elem) if kind.startswith("ch") else h.plan(elem)}), flush=True)
+                          "plan": h.ch_plan(elem) if kind.startswith("ch") else (h.cn_plan(elem) if kind.startswith("penta_cn") else h.plan(elem))}),
+              flush=True)
         del bufs
         torch.cuda.empty_cache()
 

@@ -148,7 +148,18 @@ def one_case(b, rng):
             b.btps_tune(k, -1)
 
 
-@pytest.mark.parametrize("seed", [1, 2, 3])
+# BTPS_SWEEP_SEEDS=first:last runs those seeds instead (160 cases each): how the longer builder runs recorded in
+# profiles/r02c_ab_notes.md are repeated
+def _seeds():
+    import os
+    spec = os.environ.get("BTPS_SWEEP_SEEDS", "")
+    if ":" in spec:
+        lo, hi = (int(x) for x in spec.split(":"))
+        return list(range(lo, hi + 1))
+    return [1, 2, 3]
+
+
+@pytest.mark.parametrize("seed", _seeds())
 def test_random_sweep_against_oracle(lib, seed):
     rng = np.random.default_rng(seed)
     done, bad = 0, []
