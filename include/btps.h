@@ -263,7 +263,7 @@ BTPS_API int btps_plan_info(int kind, const void *handle, int elem_bytes, int *o
  * that split the rows of a tile, 0: never use cluster kernels -- systems longer than 1024 rows then run the serial carry walk or the
  * two-pass form; default: by the length of a row of the batch in bytes -- tridiagonal with 32 partitions from 512 KiB, 24-31
  * partitions from 4 MiB, 18-23 from 32 MiB; pentadiagonal with 31-32 partitions from 8 MiB; always above 1024 rows; calls that
- * advance 4 or more time steps keep up to 32 partitions on one CTA, which is the faster one per step once the tile stays on chip), "reverse"
+ * advance 3 or more time steps keep up to 32 partitions on one CTA, which is the faster one per step once the tile stays on chip), "reverse"
  * (0/1: alternate the tile order on successive steps of *_solve_steps / ch_step_batched so a
  * step starts on the data the previous one left in L2), "one_step_fused" (1: one-step calls run the multi-step
  * instantiation of their kernel, 0: the single-step one; default: whichever keeps the smaller local-memory frame),

@@ -1133,7 +1133,7 @@ bool cl_pays(int kind, const DtypePlan &pl, long long batch, size_t selem)
 }
 
 // calls that advance at least this many time steps keep 17..32 partitions on one CTA (launch_one)
-constexpr int LOOP_STEPS_SINGLE_CTA = 4;
+constexpr int LOOP_STEPS_SINGLE_CTA = 3;
 
 // one sweep launch (kind = KIND_TRI / KIND_PENTA / KIND_CH) on a device buffer
 template <typename T, typename S = T>
@@ -1208,7 +1208,8 @@ int launch_one(Handle *h, int kind, S *d_rhs, long long batch, double alpha_x, i
     // (time loops: a tile that stays on chip for several steps is read and written once per launch, so the width of its row
     //  segments no longer decides, and per step the single CTA is the faster one -- N = 1024, 128 steps per call, us per step:
     //  tri 53.3 against the pair's 64.3 at 2^16 systems, 838 against 1013 at 2^20; penta 1465 against 1811 at 2^20.  Decided
-    //  per CALL, not per launch, so that every launch of one loop runs the same kernel whatever the steps per launch.)
+    //  per CALL, not per launch, so that every launch of one loop runs the same kernel whatever the steps per launch.  Crossover,
+    //  ms per call, one CTA / pair: 2 steps 15.2 / 13.0 at 2^22 systems, 0.251 / 0.246 at 2^16; 3 steps 16.6 / 17.0, 0.257 / 0.288.)
     const bool cl_default = (pl.P > 32) || (call_steps < LOOP_STEPS_SINGLE_CTA && cl_pays<T>(kind, pl, batch, sizeof(S)));
     const bool cl_wanted = (g_tune.cluster > 0) || (g_tune.cluster < 0 && cl_default);
     const bool use_cl = (ks == 0) && (kind == KIND_TRI || kind == KIND_PENTA) && cl_wanted && clslot.ent.func && tma_ok &&

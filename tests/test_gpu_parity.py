@@ -1252,10 +1252,10 @@ def test_default_cluster_policy_by_row_pitch(lib):
     for n in (1100, 2048, 4096):
         assert cl(lib.tri_factor(*inputs.tri_lhs(n, 0.5)), 8, 1 << 10) and cl(lib.penta_factor(*inputs.penta_lhs(n, 0.5)), 4, 1 << 10)
     assert not cl(ht, 8, (1 << 16) + 1)                                               # unaligned pitch: no TMA, no cluster
-    # time loops (calls of 4 or more steps) keep up to 32 partitions on one CTA; above 1024 rows there is only the cluster plan
+    # time loops (calls of 3 or more steps) keep up to 32 partitions on one CTA; above 1024 rows there is only the cluster plan
     def cl_steps(h, batch, nsteps):
         return lib.btps_kernel_tag(h, 8, batch, nsteps).split(", ")[8] == "1"
-    assert cl_steps(ht, 1 << 22, 3) and not cl_steps(ht, 1 << 22, 4) and not cl_steps(ht, 1 << 16, 100)
+    assert cl_steps(ht, 1 << 22, 2) and not cl_steps(ht, 1 << 22, 3) and not cl_steps(ht, 1 << 16, 100)
     assert cl_steps(hp, 1 << 20, 2) and not cl_steps(hp, 1 << 20, 64)
     assert cl_steps(lib.tri_factor(*inputs.tri_lhs(2048, 0.5)), 1 << 12, 100)
 
