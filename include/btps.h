@@ -267,7 +267,7 @@ BTPS_API int btps_plan_info(int kind, const void *handle, int elem_bytes, int *o
  * (0/1: alternate the tile order on successive steps of *_solve_steps / ch_step_batched so a
  * step starts on the data the previous one left in L2), "one_step_fused" (1: one-step calls run the multi-step
  * instantiation of their kernel, 0: the single-step one; default: whichever keeps the smaller local-memory frame),
- * "narrow_loops" (0: fused time loops never switch to half-width tiles; default: launches of 16 or more steps of the plain
+ * "narrow_loops" (0: fused time loops never switch to half-width tiles; default: launches of 4 or more steps of the plain
  * tridiagonal loop and of the Crank-Nicolson steps with 8-16 partitions and of the Cahn-Hilliard step with 8-12 partitions do, when
  * the partitions share their coefficient blocks -- 2-11 % faster per step, bitwise the same results),
  * "host_chunk_kib" (size in KiB of the column chunks the *_host calls pipeline through the device; default 32768:

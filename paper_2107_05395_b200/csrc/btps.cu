@@ -1232,12 +1232,14 @@ int launch_one(Handle *h, int kind, S *d_rhs, long long batch, double alpha_x, i
     // tri N = 512 / 256 at 2^16 systems 25.5 -> 24.5 / 12.2 -> 11.9, N = 256 at 2^20 191 -> 184; Cahn-Hilliard N = 256 at 2^16 /
     // 2^20 26.9 -> 25.6 / 424 -> 404, periodic 540 -> 527; everything else within +-1 % or slower (N = 128: + 5-17 %, plain
     // and periodic penta + 0-3 %, periodic tri N = 512 + 5 %), so only those.  A launch's load and store are slower on the
-    // 128-byte segments, hence only launches of 16 or more steps.  Same arithmetic per system: the results are bitwise equal.
+    // 128-byte segments, hence only launches of 4 or more steps (ms per call, 16 / 8 lanes: tri N = 512 at 2^16 systems 0.107 /
+    // 0.115 with 2 steps, 0.132 / 0.128 with 3, 0.157 / 0.150 with 4; the Cahn-Hilliard and Crank-Nicolson steps gain 4-9 % from 2
+    // steps on).  Same arithmetic per system: the results are bitwise equal.
     // The Crank-Nicolson steps (tri_cn_step_batched, penta_cn_step_batched; plain and periodic handles) gain throughout 8-16
     // partitions: N = 256 3-5 %, N = 384 6-11 %, N = 512 4 % (periodic 1 %).
     const bool narrow_pays = (kind == KIND_TRI && !h->periodic && pl.P >= 8 && pl.P <= 16) || (kind == KIND_CH && pl.P >= 8 && pl.P <= 12) ||
                              ((kind == KIND_TRICN || kind == KIND_PENTACN) && pl.P >= 8 && pl.P <= 16);
-    const bool narrow = !use_cl && !MIXED && s == 0 && d == 0 && ksteps >= 16 && narrow_pays && pl.kn[ks].fused.func &&
+    const bool narrow = !use_cl && !MIXED && s == 0 && d == 0 && ksteps >= 4 && narrow_pays && pl.kn[ks].fused.func &&
                         g_tune.lanes < 0 && g_tune.tpc < 0 && g_tune.narrow != 0;
     const Shape &sh = narrow ? pl.nshape[ks] : sh0;
     KernelSlot &sl = use_cl ? clslot : (narrow ? pl.kn[ks] : slot_at(s, d));

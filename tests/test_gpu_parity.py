@@ -548,18 +548,18 @@ def test_fused_steps_equal_single_step_launches(lib, n, batch):
 
 @pytest.mark.parametrize("n,batch", [(512, 148 * 16 * 3 + 48), (256, 9000), (384, 4100)])
 def test_long_fused_loops_on_half_width_tiles(lib, n, batch):
-    """Launches of 16 or more fused steps of the plain tridiagonal loop, of the Cahn-Hilliard step and of the Crank-Nicolson
+    """Launches of 4 or more fused steps of the plain tridiagonal loop, of the Cahn-Hilliard step and of the Crank-Nicolson
     steps run on half-width
     tiles (8 lanes, two or four tile groups per CTA) when the partitions share their coefficient blocks
     (btps_tune narrow_loops = 0 keeps the full-width tiles).  Same arithmetic per system: bitwise equal results, several
-    tiles per group, a ragged last tile; and both match the oracle's loop.  40 steps: one launch; 70 steps: 64 on
-    half-width tiles + 6 on full-width ones."""
+    tiles per group, a ragged last tile; and both match the oracle's loop.  40 steps: one launch; 70 steps: 64 + 6, both
+    on half-width tiles; 3 steps: full-width tiles either way."""
     lt, lc, lp = inputs.tri_lhs(n, 0.5), inputs.ch_lhs(n), inputs.penta_lhs(n, 0.5)
     x5 = np.array([-0.5, 2.0, -2.0, 2.0, -0.5])
     _, al = inputs.ch_params(n)
     rhs = inputs.uniform_rhs(n, batch, seed=91)
     c0 = 0.1 * rhs
-    for steps in (40, 70):
+    for steps in (40, 70, 3):
         outs = {}
         for narrow in (-1, 0):
             try:
